@@ -1,0 +1,167 @@
+/*
+ * msas.h — C ABI of libmsas: the Modality Activation Sparsity (MAS) pass of MSAO
+ * (arxiv/paper_2604_02945, §4.1 "Lightweight Heterogeneous Modality-Aware via Fine-Grained Sparsity",
+ * PAPER.md:81-124, Eq. 3-7), B200 / sm_100a.
+ *
+ * What the pass computes (normative definitions: SPEC.md S0-S5):
+ *   spatial     per-token RMS activation, per-segment standardise, sigmoid  -> M_spatial, rho_spatial  (Eq. 3-4)
+ *   temporal    per-patch relative L2 change against the previous frame     -> gamma, gamma_avg       (Eq. 5,   PAPER.md:100-105)
+ *   crossmodal  max-over-query cosine relevance (X·Q^T on tensor cores)      -> rel, alpha, beta       (Eq. 6,   PAPER.md:107-116)
+ *   fuse        per-token and per-modality MAS                               -> mas_tok, MAS_m         (Eq. 7,   PAPER.md:118-124)
+ *   select      top-k (ties -> lower index) or threshold, stream compaction  -> keep_mask, kept_idx, Y
+ *
+ * Conventions
+ *   - Plain C ABI. Every call returns an int status (MAS_OK = 0). No exceptions, no printing, no global mutable state
+ *     (the last CUDA error code is kept per thread).
+ *   - Pointers named h_* are HOST pointers, read during the call. All other data pointers are DEVICE pointers.
+ *   - The caller owns every buffer. The library never allocates or frees device memory. Device entry points never
+ *     synchronise: all work is enqueued on the caller's stream (`mas_stream_t` is a `cudaStream_t`) and outputs are
+ *     valid once the caller has synchronised that stream. Only `mas_forward_host` blocks (documented there).
+ *   - Inputs are never modified. Inputs must be finite; NaN/Inf give unspecified scores but no out-of-bounds access.
+ *   - X is [N, d] row-major (bf16 or fp32), row stride d, base pointer 16-byte aligned, rows of all segments packed in
+ *     segment order. Q is [sum L_r, d] row-major, same dtype, 16-byte aligned; request r owns rows q_off[r]..q_off[r+1].
+ *   - Limits: d % 8 == 0 (bf16) or d % 4 == 0 (fp32), 8 <= d <= 65536; 1 <= L_r <= MAS_MAX_QUERY_TOKENS; T, P >= 1.
+ *     Anything else returns MAS_ERR_UNSUPPORTED (never a silent fallback; there is no CPU path).
+ */
+#ifndef MSAS_H_
+#define MSAS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MAS_VERSION 100              /* 0.1.0 */
+#define MAS_MAX_QUERY_TOKENS 128     /* per request */
+
+enum { MAS_OK = 0, MAS_ERR_INVALID_ARG = 1, MAS_ERR_UNSUPPORTED = 2, MAS_ERR_WORKSPACE = 3, MAS_ERR_CUDA = 4 };
+
+typedef enum { MAS_F32 = 0, MAS_BF16 = 1 } mas_dtype;
+typedef enum { MAS_MOD_IMAGE = 1, MAS_MOD_VIDEO = 2, MAS_MOD_AUDIO = 3 } mas_modality;   /* text is the query, never a segment */
+typedef enum { MAS_SELECT_TOPK = 0, MAS_SELECT_THRESHOLD = 1 } mas_select_mode;
+
+typedef void* mas_stream_t;          /* a cudaStream_t (0 = the legacy default stream) */
+
+/* One per (request, modality). Segments of one request are contiguous and in request order; segments tile X
+ * in order without gaps: row0[0] = 0, row0[s+1] = row0[s] + n_frames[s]*n_patches[s].  (SPEC.md "Data model") */
+typedef struct {
+  int32_t request;          /* 0..R-1, non-decreasing */
+  int32_t modality;         /* mas_modality, informational: n_frames > 1 decides temporal applicability (G11) */
+  int64_t row0;             /* first row in X */
+  int32_t n_frames;         /* T >= 1 */
+  int32_t n_patches;        /* P >= 1, N_s = T*P */
+  int32_t keep_k;           /* top-k mode: 1..N_s (see mas_keep_count); ignored in threshold mode */
+  int32_t reserved_;        /* must be 0 */
+} mas_segment;              /* 32 bytes */
+
+typedef struct {
+  float lambda_spatial;     /* 0.6 */
+  float lambda_temp;        /* 0.4   PAPER.md:255 ; both >= 0, lambda_spatial + lambda_temp <= 1 */
+  float tau_s;              /* 0.3   PAPER.md:255, Eq. 4 */
+  float kappa;              /* 10.0  softmax temperature on the mean cosine (SPEC G20) */
+  float spatial_gain;       /* 1     the 1x1 conv on the one-channel statistic (SPEC G2) */
+  float spatial_bias;       /* 0 */
+  float rel_gain;           /* 1 */
+  float rel_bias;           /* 0 */
+  float cut;                /* 0.5   threshold mode: keep iff MAS_i <= cut (SPEC G17) */
+  int32_t select_mode;      /* mas_select_mode */
+} mas_params;               /* 40 bytes */
+
+/* Per-segment result (device). 36 bytes. */
+typedef struct {
+  float rho_spatial;        /* Eq. 4 */
+  float gamma_avg;          /* S2: mean frame change over t = 1..T-1 (0 if T = 1) */
+  float alpha_mean;         /* S3: mean_i max_j cos */
+  float beta;               /* softmax over the request's segments */
+  float mas;                /* Eq. 7 (redundancy reading G8) */
+  float mean_s, std_s;      /* standardisation statistics of s (diagnostic) */
+  int32_t n_tokens;
+  int32_t n_kept;
+} mas_segment_out;
+
+/* Output bundle used by mas_forward_host; any member may be NULL (that output is skipped). */
+typedef struct {
+  float* m_spatial;         /* [N] */
+  float* gamma;             /* [N] */
+  float* rel;               /* [N] */
+  float* mas_tok;           /* [N] */
+  mas_segment_out* seg_out; /* [n_segs] */
+  uint8_t* keep_mask;       /* [N] */
+  int32_t* kept_idx;        /* [cap_rows] */
+  int64_t* kept_off;        /* [n_segs+1] */
+  void* Y;                  /* [cap_rows, d] */
+  int64_t cap_rows;
+} mas_outputs;
+
+typedef struct mas_plan mas_plan;    /* opaque host object */
+
+/* ---- host helpers (no GPU needed) ---- */
+int         mas_version(void);
+int         mas_last_cuda_error(void);                   /* cudaError_t of the last MAS_ERR_CUDA on this thread */
+const char* mas_status_string(int status);
+void        mas_params_default(mas_params* p);           /* the values in the comments above, MAS_SELECT_TOPK */
+int32_t     mas_keep_count(int64_t n, double ratio);     /* SPEC S5/G16: min(n, max(1, ceil(ratio*n - 1e-9))) */
+
+/* ---- plan: validates the tables, lays out the device workspace, builds the tile schedule ----
+ * h_segs[n_segs], h_q_off[n_requests+1] are host arrays read during the call only.
+ * mas_plan_workspace_bytes: bytes of device workspace the plan needs (256-byte aligned base expected).
+ * mas_plan_create: copies the tables into d_workspace asynchronously on `stream` (from a pinned staging area owned
+ * by the plan) and returns a host object; the workspace must stay alive and untouched until mas_plan_destroy.
+ * One plan may be used by one stream at a time (the workspace holds per-call scratch).
+ * Errors: INVALID_ARG (NULL, negative sizes, tables not tiling / not ordered, keep_k out of range in top-k mode,
+ * bad params), UNSUPPORTED (limits above), WORKSPACE (too small), CUDA. */
+int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
+                             int32_t d, int32_t dtype, size_t* out_bytes);
+int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off,
+                    int32_t n_requests, int32_t d, int32_t dtype, const mas_params* params,
+                    void* d_workspace, size_t workspace_bytes, mas_stream_t stream);
+int mas_plan_destroy(mas_plan* plan);                    /* frees the host object and its pinned staging only */
+
+/* plan queries (host) */
+int64_t mas_plan_n_tokens(const mas_plan* plan);         /* N */
+int64_t mas_plan_n_queries(const mas_plan* plan);        /* sum L_r */
+int64_t mas_plan_kept_capacity(const mas_plan* plan);    /* top-k: sum keep_k ; threshold: N (worst case) */
+int32_t mas_plan_forward_launches(const mas_plan* plan); /* number of kernels one mas_forward enqueues */
+
+/* ---- staged entry points (device pointers; each usable alone; outputs fp32 unless noted) ---- */
+
+/* S1 (Eq. 3-4): s_i = RMS of row i; m_spatial = sigmoid of the per-segment standardised s. Either output may be NULL. */
+int mas_spatial(const mas_plan* plan, const void* X, float* s /*[N]*/, float* m_spatial /*[N]*/, mas_stream_t stream);
+
+/* S2 (Eq. 5 exact form): gamma[N]; 0 for T = 1 segments, 1 on keyframe rows. */
+int mas_temporal(const mas_plan* plan, const void* X, float* gamma /*[N]*/, mas_stream_t stream);
+
+/* S3 (Eq. 6 training-free): rel[N] = max_j cos(x_i, q_j). S_opt (may be NULL) receives the raw dot products
+ * S_ij, row-major [N, MAS_MAX_QUERY_TOKENS] with columns >= L_r left untouched (tests only). */
+int mas_crossmodal(const mas_plan* plan, const void* X, const void* Q, float* rel /*[N]*/, float* S_opt, mas_stream_t stream);
+
+/* S1 stats + S3 stats + S4 (Eq. 7): per-token m_spatial, mas_tok; per-segment record (n_kept left 0). */
+int mas_fuse(const mas_plan* plan, const float* s, const float* gamma, const float* rel,
+             float* m_spatial /*[N] or NULL*/, float* mas_tok /*[N]*/, mas_segment_out* seg_out /*[n_segs]*/, mas_stream_t stream);
+
+/* S5: selection on mas_tok, index compaction, row gather. Y may be NULL (indices only). cap_rows >= sum keep_k
+ * (top-k) or any value >= 0 (threshold): nothing is written past cap_rows and kept_off[n_segs] still holds the
+ * true total so the caller detects overflow. seg_out (may be NULL): only n_kept is written. */
+int mas_select_compact(const mas_plan* plan, const void* X, const float* mas_tok,
+                       uint8_t* keep_mask /*[N]*/, int32_t* kept_idx /*[cap_rows]*/, int64_t* kept_off /*[n_segs+1]*/,
+                       void* Y /*[cap_rows, d] or NULL*/, int64_t cap_rows, mas_segment_out* seg_out, mas_stream_t stream);
+
+/* ---- fused entry point: one streaming score pass over X (a1+a2+a3), one segment kernel (a4+a5), one gather (a6).
+ * Same outputs as the staged calls; any output may be NULL except kept_idx/kept_off when Y is requested. */
+int mas_forward(const mas_plan* plan, const void* X, const void* Q,
+                float* m_spatial, float* gamma, float* rel, float* mas_tok, mas_segment_out* seg_out,
+                uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows, mas_stream_t stream);
+
+/* ---- end-to-end convenience: HOST inputs -> HOST outputs.
+ * Copies h_X -> d_X and h_Q -> d_Q (cudaMemcpyAsync; pinned host memory recommended), runs mas_forward into d_out,
+ * copies every non-NULL member of h_out back (Y/kept_idx: only the rows actually kept) and SYNCHRONISES the stream
+ * before returning. d_out members needed by the requested h_out members must be non-NULL. */
+int mas_forward_host(const mas_plan* plan, const void* h_X, const void* h_Q, void* d_X, void* d_Q,
+                     const mas_outputs* d_out, const mas_outputs* h_out, mas_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSAS_H_ */

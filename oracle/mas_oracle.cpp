@@ -1,0 +1,301 @@
+// mas_oracle.cpp — the CPU ORACLE of the MAS pass.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load this library.
+// It shares no code, header, table or helper with the CUDA path (paper_2604_02945_b200/csrc): the structs below are
+// re-declared here on purpose.
+//
+// What it is: the plain definition of SPEC.md S0-S5 (paper: MSAO, arxiv/paper_2604_02945, §4.1, PAPER.md:81-124,
+// Eq. 3-7; constants PAPER.md:255), written out step by step, single thread, every sum a `double` accumulated in
+// index order, inputs converted exactly (bf16 -> double, fp32 -> double). No blocking, fusion or reordering.
+//
+// Pins (tests/test_oracle_pins.py, `-m "not gpu"`): explicit hand-expanded dot products, closed forms
+// (sigma(+-1), 1/sqrt2, 1/3, sin(theta/2)), invariances (query permutation, power-of-two scaling, duplicate query),
+// softmax identities, Eq. 7 special cases, brute-force sort/count for selection, numpy float64 cross-checks,
+// AR(1) statistical law.  Free conventions shared by both sides and therefore not pinnable by mathematics:
+// kappa = 10 (G20) and the standardisation floors 1e-6 (G18).
+//
+// Build: g++ -O2 -shared -fPIC (no -ffast-math, no OpenMP).  See oracle/build_oracle.py.
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+extern "C" {
+
+typedef struct {
+  int32_t request;
+  int32_t modality;
+  int64_t row0;
+  int32_t n_frames;   // T
+  int32_t n_patches;  // P
+  int32_t keep_k;
+  int32_t reserved_;
+} mas_ref_segment;
+
+typedef struct {
+  double lambda_spatial, lambda_temp, tau_s, kappa;
+  double spatial_gain, spatial_bias, rel_gain, rel_bias;
+  double cut;
+  int32_t select_mode;  // 0 = top-k, 1 = threshold
+  int32_t pad_;
+} mas_ref_params;
+
+typedef struct {
+  double rho_spatial, gamma_avg, alpha_mean, beta, mas, mean_s, std_s, mean_r, std_r;
+  int64_t n_tokens, n_kept;
+} mas_ref_segment_out;
+
+enum { REF_F32 = 0, REF_BF16 = 1 };
+
+}  // extern "C"
+
+namespace {
+
+// exact element -> double
+inline double elem(const void* base, int dtype, int64_t idx) {
+  if (dtype == REF_BF16) {
+    uint16_t h = static_cast<const uint16_t*>(base)[idx];
+    uint32_t u = static_cast<uint32_t>(h) << 16;
+    float f;
+    std::memcpy(&f, &u, 4);
+    return static_cast<double>(f);
+  }
+  return static_cast<double>(static_cast<const float*>(base)[idx]);
+}
+
+inline int64_t elem_bytes(int dtype) { return dtype == REF_BF16 ? 2 : 4; }
+
+inline double sigmoid(double u) { return 1.0 / (1.0 + std::exp(-u)); }
+
+// S0: n2_i = sum_c x_ic^2
+double row_n2(const void* X, int dtype, int64_t row, int64_t d) {
+  double acc = 0.0;
+  for (int64_t c = 0; c < d; ++c) {
+    double v = elem(X, dtype, row * d + c);
+    acc += v * v;
+  }
+  return acc;
+}
+
+}  // namespace
+
+extern "C" {
+
+void mas_ref_params_default(mas_ref_params* p) {
+  p->lambda_spatial = 0.6;
+  p->lambda_temp = 0.4;
+  p->tau_s = 0.3;
+  p->kappa = 10.0;          // SPEC G20
+  p->spatial_gain = 1.0;
+  p->spatial_bias = 0.0;
+  p->rel_gain = 1.0;
+  p->rel_bias = 0.0;
+  p->cut = 0.5;
+  p->select_mode = 0;
+  p->pad_ = 0;
+}
+
+// SPEC S5 / G16
+int32_t mas_ref_keep_count(int64_t n, double ratio) {
+  double c = std::ceil(ratio * static_cast<double>(n) - 1e-9);
+  int64_t k = static_cast<int64_t>(c);
+  if (k < 1) k = 1;
+  if (k > n) k = n;
+  return static_cast<int32_t>(k);
+}
+
+// S1 first half (Eq. 3's pooled statistic, G1): s_i = sqrt(n2_i / d) for every row of every segment.
+int mas_ref_rms(const mas_ref_segment* segs, int32_t n_segs, int64_t d, int dtype, const void* X, double* s) {
+  for (int32_t k = 0; k < n_segs; ++k) {
+    int64_t n = static_cast<int64_t>(segs[k].n_frames) * segs[k].n_patches;
+    for (int64_t i = segs[k].row0; i < segs[k].row0 + n; ++i) s[i] = std::sqrt(row_n2(X, dtype, i, d) / static_cast<double>(d));
+  }
+  return 0;
+}
+
+// S2 (Eq. 5 in exact form; G4-G6): per-patch relative L2 change against the previous frame.
+int mas_ref_temporal(const mas_ref_segment* segs, int32_t n_segs, int64_t d, int dtype, const void* X, double* gamma) {
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const int64_t T = segs[k].n_frames, P = segs[k].n_patches, r0 = segs[k].row0;
+    for (int64_t t = 0; t < T; ++t) {
+      for (int64_t p = 0; p < P; ++p) {
+        const int64_t i = r0 + t * P + p;
+        if (T == 1) { gamma[i] = 0.0; continue; }   // temporal term not applicable
+        if (t == 0) { gamma[i] = 1.0; continue; }   // keyframe rule G6
+        const int64_t j = i - P;                    // same patch, previous frame
+        double D = 0.0;
+        for (int64_t c = 0; c < d; ++c) {
+          double diff = elem(X, dtype, i * d + c) - elem(X, dtype, j * d + c);
+          D += diff * diff;
+        }
+        double den = std::sqrt(row_n2(X, dtype, i, d)) + std::sqrt(row_n2(X, dtype, j, d));
+        gamma[i] = den > 0.0 ? std::sqrt(D) / den : 0.0;
+      }
+    }
+  }
+  return 0;
+}
+
+// S3 (Eq. 6, training-free form G9): S_ij = x_i . q_j ; c_ij = S_ij / (|x_i||q_j|) ; r_i = max_j c_ij.
+// S_opt (may be NULL): raw dot products, row-major [N, S_stride], columns >= L_r untouched.
+int mas_ref_crossmodal(const mas_ref_segment* segs, int32_t n_segs, const int64_t* q_off, int32_t n_requests,
+                       int64_t d, int dtype, const void* X, const void* Q, double* rel, double* S_opt, int64_t S_stride) {
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const int32_t r = segs[k].request;
+    if (r < 0 || r >= n_requests) return 1;
+    const int64_t q0 = q_off[r], q1 = q_off[r + 1];
+    const int64_t n = static_cast<int64_t>(segs[k].n_frames) * segs[k].n_patches;
+    std::vector<double> qn(static_cast<size_t>(q1 - q0));
+    for (int64_t j = q0; j < q1; ++j) qn[static_cast<size_t>(j - q0)] = std::sqrt(row_n2(Q, dtype, j, d));
+    for (int64_t i = segs[k].row0; i < segs[k].row0 + n; ++i) {
+      const double xn = std::sqrt(row_n2(X, dtype, i, d));
+      double best = 0.0;
+      bool first = true;
+      for (int64_t j = q0; j < q1; ++j) {
+        double S = 0.0;
+        for (int64_t c = 0; c < d; ++c) S += elem(X, dtype, i * d + c) * elem(Q, dtype, j * d + c);
+        if (S_opt) S_opt[i * S_stride + (j - q0)] = S;
+        const double qnj = qn[static_cast<size_t>(j - q0)];
+        const double cosv = (xn > 0.0 && qnj > 0.0) ? S / (xn * qnj) : 0.0;
+        if (first || cosv > best) { best = cosv; first = false; }
+      }
+      rel[i] = best;
+    }
+  }
+  return 0;
+}
+
+// S1 statistics + S3 statistics + S4 (Eq. 3, 4, 6-softmax, 7).
+int mas_ref_fuse(const mas_ref_segment* segs, int32_t n_segs, const mas_ref_params* prm,
+                 const double* s, const double* gamma, const double* rel,
+                 double* m_spatial, double* mas_tok, mas_ref_segment_out* out) {
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const int64_t T = segs[k].n_frames, P = segs[k].n_patches, r0 = segs[k].row0, n = T * P;
+    const double a = T > 1 ? 1.0 : 0.0;  // temporal applicability
+    // S1: population mean / std of s
+    double mu_s = 0.0;
+    for (int64_t i = r0; i < r0 + n; ++i) mu_s += s[i];
+    mu_s /= static_cast<double>(n);
+    double var_s = 0.0;
+    for (int64_t i = r0; i < r0 + n; ++i) var_s += (s[i] - mu_s) * (s[i] - mu_s);
+    const double sd_s = std::sqrt(var_s / static_cast<double>(n));
+    const double den_s = std::max(sd_s, 1e-6 * mu_s);
+    // S3: population mean / std of rel
+    double mu_r = 0.0;
+    for (int64_t i = r0; i < r0 + n; ++i) mu_r += rel[i];
+    mu_r /= static_cast<double>(n);
+    double var_r = 0.0;
+    for (int64_t i = r0; i < r0 + n; ++i) var_r += (rel[i] - mu_r) * (rel[i] - mu_r);
+    const double sd_r = std::sqrt(var_r / static_cast<double>(n));
+    const double den_r = std::max(sd_r, 1e-6);
+    int64_t below = 0;
+    for (int64_t i = r0; i < r0 + n; ++i) {
+      const double z = den_s > 0.0 ? (s[i] - mu_s) / den_s : 0.0;
+      const double M = sigmoid(prm->spatial_gain * z + prm->spatial_bias);          // Eq. 3
+      if (M < prm->tau_s) ++below;                                                   // Eq. 4, strict <
+      const double g = sigmoid(prm->rel_gain * (rel[i] - mu_r) / den_r + prm->rel_bias);
+      const double mas = 1.0 - g * (1.0 - prm->lambda_spatial * (1.0 - M) - a * prm->lambda_temp * (1.0 - gamma[i]));  // S4 per token
+      if (m_spatial) m_spatial[i] = M;
+      mas_tok[i] = mas;
+    }
+    // S2 aggregate: gamma_avg = mean over t = 1..T-1 of the per-frame patch means
+    double gavg = 0.0;
+    if (T > 1) {
+      for (int64_t t = 1; t < T; ++t) {
+        double gt = 0.0;
+        for (int64_t p = 0; p < P; ++p) gt += gamma[r0 + t * P + p];
+        gavg += gt / static_cast<double>(P);
+      }
+      gavg /= static_cast<double>(T - 1);
+    }
+    out[k].rho_spatial = static_cast<double>(below) / static_cast<double>(n);
+    out[k].gamma_avg = gavg;
+    out[k].alpha_mean = mu_r;
+    out[k].mean_s = mu_s;
+    out[k].std_s = sd_s;
+    out[k].mean_r = mu_r;
+    out[k].std_r = sd_r;
+    out[k].n_tokens = n;
+    out[k].n_kept = 0;
+    out[k].beta = 0.0;
+    out[k].mas = 0.0;
+  }
+  // softmax over the segments of each request, then Eq. 7 per segment
+  int32_t k0 = 0;
+  while (k0 < n_segs) {
+    int32_t k1 = k0;
+    while (k1 < n_segs && segs[k1].request == segs[k0].request) ++k1;
+    double mx = prm->kappa * out[k0].alpha_mean;
+    for (int32_t k = k0; k < k1; ++k) mx = std::max(mx, prm->kappa * out[k].alpha_mean);
+    double z = 0.0;
+    for (int32_t k = k0; k < k1; ++k) z += std::exp(prm->kappa * out[k].alpha_mean - mx);
+    for (int32_t k = k0; k < k1; ++k) {
+      const double a = segs[k].n_frames > 1 ? 1.0 : 0.0;
+      out[k].beta = std::exp(prm->kappa * out[k].alpha_mean - mx) / z;
+      out[k].mas = 1.0 - out[k].beta * (1.0 - prm->lambda_spatial * out[k].rho_spatial - a * prm->lambda_temp * (1.0 - out[k].gamma_avg));  // Eq. 7, G8
+    }
+    k0 = k1;
+  }
+  return 0;
+}
+
+// S5: selection + compaction.  Y may be NULL.  Nothing is written past cap_rows;
+// kept_off[n_segs] is always the true total.
+int mas_ref_select_compact(const mas_ref_segment* segs, int32_t n_segs, int64_t d, int dtype, const mas_ref_params* prm,
+                           const void* X, const double* mas_tok, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off,
+                           void* Y, int64_t cap_rows, mas_ref_segment_out* out) {
+  int64_t total = 0;
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const int64_t r0 = segs[k].row0, n = static_cast<int64_t>(segs[k].n_frames) * segs[k].n_patches;
+    for (int64_t i = r0; i < r0 + n; ++i) keep_mask[i] = 0;
+    if (prm->select_mode == 0) {
+      // the keep_k smallest under the strict total order (MAS_i, i): stable sort by value keeps lower index first
+      std::vector<int64_t> order(static_cast<size_t>(n));
+      for (int64_t i = 0; i < n; ++i) order[static_cast<size_t>(i)] = r0 + i;
+      std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return mas_tok[a] < mas_tok[b]; });
+      int64_t kk = segs[k].keep_k;
+      if (kk < 0 || kk > n) return 1;
+      for (int64_t j = 0; j < kk; ++j) keep_mask[order[static_cast<size_t>(j)]] = 1;
+    } else {
+      for (int64_t i = r0; i < r0 + n; ++i) keep_mask[i] = mas_tok[i] <= prm->cut ? 1 : 0;   // G17
+    }
+    kept_off[k] = total;
+    for (int64_t i = r0; i < r0 + n; ++i) {
+      if (!keep_mask[i]) continue;
+      if (total < cap_rows) {
+        if (kept_idx) kept_idx[total] = static_cast<int32_t>(i);
+        if (Y) std::memcpy(static_cast<char*>(Y) + total * d * elem_bytes(dtype),
+                           static_cast<const char*>(X) + i * d * elem_bytes(dtype), static_cast<size_t>(d * elem_bytes(dtype)));
+      }
+      ++total;
+    }
+    if (out) out[k].n_kept = total - kept_off[k];
+  }
+  kept_off[n_segs] = total;
+  return 0;
+}
+
+// Whole pass = the staged definitions in order.  Any of m_spatial/gamma/rel may be NULL (scratch is used).
+int mas_ref_forward(const mas_ref_segment* segs, int32_t n_segs, const int64_t* q_off, int32_t n_requests,
+                    int64_t d, int dtype, const mas_ref_params* prm, const void* X, const void* Q,
+                    double* s, double* m_spatial, double* gamma, double* rel, double* mas_tok, mas_ref_segment_out* out,
+                    uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows) {
+  if (n_segs <= 0) { if (kept_off) kept_off[0] = 0; return 0; }
+  const int64_t N = segs[n_segs - 1].row0 + static_cast<int64_t>(segs[n_segs - 1].n_frames) * segs[n_segs - 1].n_patches;
+  std::vector<double> s_buf, g_buf, r_buf;
+  if (!s) { s_buf.resize(static_cast<size_t>(N)); s = s_buf.data(); }
+  if (!gamma) { g_buf.resize(static_cast<size_t>(N)); gamma = g_buf.data(); }
+  if (!rel) { r_buf.resize(static_cast<size_t>(N)); rel = r_buf.data(); }
+  int rc;
+  if ((rc = mas_ref_rms(segs, n_segs, d, dtype, X, s))) return rc;
+  if ((rc = mas_ref_temporal(segs, n_segs, d, dtype, X, gamma))) return rc;
+  if ((rc = mas_ref_crossmodal(segs, n_segs, q_off, n_requests, d, dtype, X, Q, rel, nullptr, 0))) return rc;
+  if ((rc = mas_ref_fuse(segs, n_segs, prm, s, gamma, rel, m_spatial, mas_tok, out))) return rc;
+  if (keep_mask && kept_off)
+    if ((rc = mas_ref_select_compact(segs, n_segs, d, dtype, prm, X, mas_tok, keep_mask, kept_idx, kept_off, Y, cap_rows, out))) return rc;
+  return 0;
+}
+
+}  // extern "C"

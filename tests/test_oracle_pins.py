@@ -1,0 +1,382 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (SPEC.md, SURVEY.md §8(c) "Pins").
+No GPU.  Each test is chosen so that a plausible mistake in oracle/mas_oracle.cpp (dropped term, wrong sign or index,
+transposed operand, wrong normalisation) fails it.  Expected values come from tests/golden/closed_forms.txt (hand
+expansions of the paper's equations), from brute force written independently here, or from numpy float64."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import mas_ref as O
+from paper_2604_02945_b200 import synth
+
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")) as fh:
+    for line in fh:
+        line = line.split("#")[0].strip()
+        if "=" in line:
+            k, v = line.split("=")
+            GOLD[k.strip()] = float(v)
+
+
+def seg1(T, P, k=1, req=0, mod=1):
+    return O.make_segments([(req, mod, T, P, k)])[0]
+
+
+def f32(a):
+    return np.ascontiguousarray(a, np.float32)
+
+
+# ---------------------------------------------------------------- S0 / S3: dot products, norms, cosine
+def test_dot_products_hand_expanded():
+    X = f32([[1, 2, 3, 4], [0, -1, 2, -3]])
+    Q = f32([[1, 0, -1, 2], [2, 2, 2, 2], [-1, 3, 0, 1]])
+    rel, S = O.crossmodal(seg1(1, 2), [0, 3], X, Q, want_S=True)
+    exp = np.array([[GOLD["S_00"], GOLD["S_01"], GOLD["S_02"]], [GOLD["S_10"], GOLD["S_11"], GOLD["S_12"]]])
+    assert np.array_equal(S, exp)          # a transposed operand or wrong stride breaks this
+    xn = np.array([math.sqrt(30), math.sqrt(14)])
+    qn = np.array([math.sqrt(6), 4.0, math.sqrt(11)])
+    cos = exp / xn[:, None] / qn[None, :]
+    assert np.allclose(rel, cos.max(axis=1), rtol=0, atol=1e-15)
+    assert rel[1] < 0                       # max of all-negative cosines stays negative (no clamp at 0)
+
+
+def test_cosine_closed_forms_and_zero_rows():
+    X = f32([[1, 0], [1, 1], [0, 0]])
+    Q = f32([[1, 0], [0, 1]])
+    rel = O.crossmodal(seg1(1, 3), [0, 2], X, Q)
+    assert rel[0] == 1.0
+    assert abs(rel[1] - GOLD["cos_11_vs_axes"]) < 1e-15
+    assert rel[2] == 0.0                    # G18: zero row -> cos := 0
+    rel = O.crossmodal(seg1(1, 3), [0, 2], X, f32([[0, 0], [0, -1]]))
+    assert rel[0] == 0.0 and rel[1] == 0.0  # zero query contributes cos 0, which beats -1/sqrt2
+
+
+def test_crossmodal_matches_numpy_float64_and_bf16_decoding():
+    rng = np.random.default_rng(7)
+    N, L, d = 12, 5, 40
+    Xf = rng.standard_normal((N, d)).astype(np.float32)
+    Qf = rng.standard_normal((2 * L, d)).astype(np.float32)
+    Xb, Qb = synth.f32_to_bf16_bits(Xf), synth.f32_to_bf16_bits(Qf)
+    segs, _ = O.make_segments([(0, 1, 1, 7, 1), (1, 1, 1, 5, 1)])
+    rel, S = O.crossmodal(segs, [0, L, 2 * L], Xb, Qb, want_S=True)
+    X64 = synth.bf16_bits_to_f32(Xb).astype(np.float64)
+    Q64 = synth.bf16_bits_to_f32(Qb).astype(np.float64)
+    for (lo, hi, q0) in [(0, 7, 0), (7, 12, L)]:      # each request uses only its own queries
+        Sx = X64[lo:hi] @ Q64[q0:q0 + L].T
+        assert np.allclose(S[lo:hi, :L], Sx, rtol=1e-13, atol=1e-13)
+        cos = Sx / np.linalg.norm(X64[lo:hi], axis=1)[:, None] / np.linalg.norm(Q64[q0:q0 + L], axis=1)[None, :]
+        assert np.allclose(rel[lo:hi], cos.max(axis=1), rtol=1e-13)
+
+
+def test_query_permutation_and_duplicate_query_are_bit_invariant():
+    w = synth.batched_images(seed=11, R=2, d=64, L_lo=6, L_hi=6)
+    segs, _ = O.make_segments(w.segments)
+    prm = O.default_params()
+    a = O.forward(segs, w.q_off, prm, w.X, w.Q, want_Y=False)
+    perm = np.concatenate([np.random.default_rng(1).permutation(6), 6 + np.random.default_rng(2).permutation(6)])
+    b = O.forward(segs, w.q_off, prm, w.X, w.Q[perm], want_Y=False)
+    for k in ("rel", "mas_tok", "m_spatial", "keep_mask", "kept_idx"):
+        assert np.array_equal(a[k], b[k]), k
+    # appending a duplicate query to every request changes nothing
+    Q2 = np.concatenate([w.Q[0:6], w.Q[0:1], w.Q[6:12], w.Q[7:8]])
+    c = O.forward(segs, np.array([0, 7, 14]), prm, w.X, Q2, want_Y=False)
+    for k in ("rel", "mas_tok", "keep_mask"):
+        assert np.array_equal(a[k], c[k]), k
+
+
+# ---------------------------------------------------------------- S1: RMS, standardise, sigmoid, rho
+def test_spatial_two_rows_closed_form():
+    X = f32([[1, -1, 1, -1], [3, 3, -3, -3]])       # RMS 1 and 3
+    s = O.rms(seg1(1, 2), X)
+    assert np.array_equal(s, [1.0, 3.0])
+    m, mas, out = O.fuse(seg1(1, 2), O.default_params(), s, np.zeros(2), np.zeros(2))
+    assert abs(m[0] - GOLD["sigmoid_minus1"]) < 1e-15 and abs(m[1] - GOLD["sigmoid_plus1"]) < 1e-15
+    assert out[0].rho_spatial == GOLD["rho_two_rows"]
+    assert out[0].mean_s == 2.0 and out[0].std_s == 1.0
+
+
+def test_spatial_constant_segment_and_strict_threshold():
+    s = np.full(5, 2.5)
+    m, _, out = O.fuse(seg1(1, 5), O.default_params(), s, np.zeros(5), np.zeros(5))
+    assert np.all(m == 0.5) and out[0].rho_spatial == 0.0           # G18: den_s floor, z -> 0
+    m, _, out = O.fuse(seg1(1, 5), O.default_params(tau_s=0.5), s, np.zeros(5), np.zeros(5))
+    assert out[0].rho_spatial == 0.0                                 # strict '<' (G12): M == tau is not below
+    s0 = np.zeros(4)
+    m, _, out = O.fuse(seg1(1, 4), O.default_params(), s0, np.zeros(4), np.zeros(4))
+    assert np.all(m == 0.5)                                          # den_s = 0 -> z = 0
+
+
+def test_spatial_statistics_bruteforce():
+    rng = np.random.default_rng(3)
+    s = np.abs(rng.standard_normal(257)) + 0.1
+    prm = O.default_params()
+    m, _, out = O.fuse(seg1(1, 257), prm, s, np.zeros(257), rng.standard_normal(257))
+    z = (s - s.mean()) / s.std()
+    assert abs(z.mean()) < 1e-12 and abs(z.var() - 1) < 1e-12
+    assert np.allclose(m, 1 / (1 + np.exp(-z)), rtol=1e-13)
+    assert np.all((m > 0) & (m < 1))
+    assert out[0].rho_spatial == np.count_nonzero(m < 0.3) / 257
+    assert 0 < out[0].rho_spatial < 1
+    # RMS itself against numpy on random bf16 data
+    Xb = synth.f32_to_bf16_bits(rng.standard_normal((9, 24)).astype(np.float32))
+    x64 = synth.bf16_bits_to_f32(Xb).astype(np.float64)
+    assert np.allclose(O.rms(seg1(1, 9), Xb), np.sqrt((x64 ** 2).mean(axis=1)), rtol=1e-14)
+
+
+# ---------------------------------------------------------------- S2: temporal change
+def test_temporal_closed_forms():
+    a = [1.0, 2.0, -3.0, 0.5]
+    rows = [a, a,                       # identical -> 0 exactly
+            [-v for v in a],            # opposite of previous -> 1
+            [-2 * v for v in a],        # doubled -> 1/3
+            [0, 0, 0, 0],               # one zero row -> 1
+            [0, 0, 0, 0],               # both zero -> 0 (G18)
+            [3, 0, 0, 0], [0, 3, 0, 0]]  # orthogonal equal norm -> 1/sqrt2
+    g = O.temporal(seg1(8, 1), f32(rows))
+    assert g[0] == 1.0                                   # keyframe G6
+    assert g[1] == 0.0
+    assert g[2] == GOLD["gamma_opposite"]
+    assert abs(g[3] - GOLD["gamma_doubled"]) < 1e-15
+    assert g[4] == 1.0 and g[5] == 0.0
+    assert g[6] == 1.0                                   # previous row is zero
+    assert abs(g[7] - GOLD["gamma_orthogonal_equal_norm"]) < 1e-15
+
+
+def test_temporal_indexing_frame_major_and_single_frame():
+    # T=3 frames x P=2 patches: row (t,p) compares with (t-1,p), not with the adjacent row
+    X = f32([[1, 0], [0, 1],      # t=0
+             [1, 0], [0, -1],     # t=1: p0 identical, p1 opposite
+             [2, 0], [0, -1]])    # t=2: p0 doubled, p1 identical
+    g = O.temporal(seg1(3, 2), X)
+    assert list(g[:2]) == [1.0, 1.0]
+    assert g[2] == 0.0 and g[3] == 1.0
+    assert abs(g[4] - 1 / 3) < 1e-15 and g[5] == 0.0
+    assert np.all(O.temporal(seg1(1, 6), X) == 0.0)      # T = 1: not applicable
+    # two segments: the second must not look into the first
+    segs, _ = O.make_segments([(0, 1, 1, 2, 1), (0, 2, 2, 2, 1)])
+    g = O.temporal(segs, X)
+    assert list(g) == [0, 0, 1, 1, g[4], g[5]] and abs(g[4] - 1 / 3) < 1e-15 and g[5] == 0.0
+
+
+def test_temporal_equal_norm_is_sin_half_angle_and_range():
+    rng = np.random.default_rng(5)
+    d = 6
+    for _ in range(20):
+        u = rng.standard_normal(d); u /= np.linalg.norm(u)
+        v = rng.standard_normal(d); v /= np.linalg.norm(v)
+        X = np.stack([u, v]).astype(np.float32)
+        x64 = X.astype(np.float64)
+        g = O.temporal(seg1(2, 1), X)[1]
+        # general definition in float64 (norms are equal only up to fp32 rounding, so use the full formula) ...
+        exp = np.linalg.norm(x64[1] - x64[0]) / (np.linalg.norm(x64[1]) + np.linalg.norm(x64[0]))
+        assert abs(g - exp) < 1e-14 and 0 <= g <= 1
+        # ... and the closed form sin(theta/2) for (nearly) equal norms
+        cos = x64[0] @ x64[1] / np.linalg.norm(x64[0]) / np.linalg.norm(x64[1])
+        assert abs(g - math.sqrt((1 - cos) / 2)) < 1e-6
+
+
+def test_temporal_ar1_statistical_law():
+    # AR(1) x_t = rho x_{t-1} + sqrt(1-rho^2) n: E|x_t - x_{t-1}|^2 = 2(1-rho)|x|^2 -> gamma ~ sqrt(2(1-rho))/2
+    rng = np.random.default_rng(9)
+    for rho, expect in ((0.95, 0.158), (0.9, 0.224)):
+        d, T = 512, 200
+        x = np.empty((T, d), np.float32)
+        x[0] = rng.standard_normal(d)
+        for t in range(1, T):
+            x[t] = rho * x[t - 1] + math.sqrt(1 - rho * rho) * rng.standard_normal(d)
+        g = O.temporal(seg1(T, 1), x)[1:]
+        assert abs(g.mean() - expect) < 0.05 * expect
+
+
+# ---------------------------------------------------------------- softmax / Eq. 7
+def _fuse_segments(rows, s, gamma, rel, **kw):
+    segs, n = O.make_segments(rows)
+    return O.fuse(segs, O.default_params(**kw), s, gamma, rel)
+
+
+def test_softmax_identities():
+    rng = np.random.default_rng(2)
+    rows = [(0, 1, 1, 4, 1), (0, 3, 3, 2, 1), (0, 2, 2, 3, 1), (1, 1, 1, 5, 1)]
+    n = 4 + 6 + 6 + 5
+    s, gam, rel = rng.random(n) + 0.5, rng.random(n), rng.standard_normal(n) * 0.1
+    _, _, out = _fuse_segments(rows, s, gam, rel)
+    beta = O.seg_out_array(out, "beta")
+    assert abs(beta[:3].sum() - 1) < 1e-15 and beta[3] == 1.0      # one segment -> beta = 1
+    alpha = np.array([rel[0:4].mean(), rel[4:10].mean(), rel[10:16].mean()])
+    e = np.exp(10 * alpha)
+    assert np.allclose(beta[:3], e / e.sum(), rtol=1e-13)          # kappa = 10 (G20)
+    assert np.allclose(O.seg_out_array(out, "alpha_mean")[:3], alpha, rtol=1e-14)
+    # shift invariance: adding a constant to every rel leaves beta unchanged; equal alpha -> 1/n
+    _, _, out2 = _fuse_segments(rows, s, gam, rel + 0.25)
+    assert np.allclose(O.seg_out_array(out2, "beta"), beta, rtol=1e-12)
+    _, _, out3 = _fuse_segments(rows, s, gam, np.full(n, 0.3))
+    assert np.allclose(O.seg_out_array(out3, "beta")[:3], 1 / 3, rtol=1e-15)
+
+
+def test_eq7_special_cases():
+    # single image segment: beta = 1, a = 0 -> MAS = lambda_sp * rho
+    s = np.array([1.0, 3.0])
+    _, _, out = _fuse_segments([(0, 1, 1, 2, 1)], s, np.zeros(2), np.zeros(2))
+    assert abs(out[0].mas - GOLD["mas_single_image_rho_half"]) < 1e-15
+    # single video segment, all frames identical (gamma = 0 beyond the keyframe) -> lambda_sp*rho + lambda_t
+    s = np.array([1.0, 3.0, 1.0, 3.0, 1.0, 3.0])
+    gam = np.array([1, 1, 0, 0, 0, 0.0])
+    _, _, out = _fuse_segments([(0, 2, 3, 2, 1)], s, gam, np.zeros(6))
+    assert out[0].gamma_avg == 0.0                                  # keyframe excluded (G6/G7)
+    assert abs(out[0].mas - GOLD["mas_static_video_rho_half"]) < 1e-15
+    # gamma_avg is the mean over frames t>=1 of per-frame patch means
+    gam = np.array([1, 1, 0.2, 0.4, 0.6, 1.0])
+    _, _, out = _fuse_segments([(0, 2, 3, 2, 1)], s, gam, np.zeros(6))
+    assert abs(out[0].gamma_avg - 0.55) < 1e-15
+    assert abs(out[0].mas - (1 - (1 - 0.6 * 0.5 - 0.4 * (1 - 0.55)))) < 1e-15
+    # lambda weights are not swapped
+    _, _, out = _fuse_segments([(0, 2, 3, 2, 1)], s, gam, np.zeros(6), lambda_spatial=0.9, lambda_temp=0.1)
+    assert abs(out[0].mas - (0.9 * 0.5 + 0.1 * 0.45)) < 1e-15
+
+
+def test_per_token_mas_formula_ranges_and_monotonicity():
+    rng = np.random.default_rng(4)
+    n = 64
+    s, gam, rel = rng.random(n) + 0.2, rng.random(n), rng.standard_normal(n)
+    gam[:8] = 1.0
+    rows = [(0, 2, 8, 8, 1)]
+    m, mas, out = _fuse_segments(rows, s, gam, rel)
+    g = 1 / (1 + np.exp(-(rel - rel.mean()) / rel.std()))
+    exp = 1 - g * (1 - 0.6 * (1 - m) - 0.4 * (1 - gam))
+    assert np.allclose(mas, exp, rtol=1e-13)
+    assert np.all((mas >= 0) & (mas <= 1)) and 0 <= out[0].mas <= 1
+    # T = 1: temporal term dropped even if a gamma array is supplied
+    m1, mas1, _ = _fuse_segments([(0, 1, 1, 64, 1)], s, gam, rel)
+    assert np.allclose(mas1, 1 - g * (1 - 0.6 * (1 - m1)), rtol=1e-13)
+    # raising gamma_i (more change) never raises MAS_i; extreme token -> MAS near 0
+    gam2 = gam.copy(); gam2[20] = min(1.0, gam[20] + 0.3)
+    _, mas2, _ = _fuse_segments(rows, s, gam2, rel)
+    assert mas2[20] <= mas[20] and np.array_equal(np.delete(mas2, 20), np.delete(mas, 20))
+    s3, rel3 = s.copy(), rel.copy()
+    s3[5] = 100.0; rel3[5] = 100.0
+    g3 = gam.copy(); g3[5] = 1.0
+    _, mas3, _ = _fuse_segments(rows, s3, g3, rel3)
+    assert mas3[5] < 1e-3 and mas3[5] == mas3.min()
+
+
+# ---------------------------------------------------------------- S5: selection and compaction
+def test_keep_count_rule():
+    assert O.keep_count(576, 0.25) == 144 and O.keep_count(18432, 0.15) == 2765 and O.keep_count(1500, 0.40) == 600
+    assert O.keep_count(10, 0.0) == 1 and O.keep_count(10, 2.0) == 10 and O.keep_count(7, 0.5) == 4
+    for n in (1, 5, 144, 577, 2880):
+        for r in (0.1, 0.15, 0.25, 0.4, 1.0):
+            assert O.keep_count(n, r) == synth.keep_count(n, r)
+
+
+def test_topk_bruteforce_with_ties():
+    rng = np.random.default_rng(8)
+    rows = [(0, 1, 1, 9, 4), (0, 1, 1, 1, 1), (1, 2, 2, 5, 10), (2, 1, 1, 7, 3)]
+    segs, n = O.make_segments(rows)
+    vals = rng.integers(0, 4, n).astype(np.float64) / 4          # heavy ties
+    X = rng.standard_normal((n, 8)).astype(np.float32)
+    prm = O.default_params()
+    mask, idx, off, Y, out = O.select_compact(segs, prm, X, vals)
+    r0 = 0
+    exp_idx = []
+    for (_, _, T, P, k) in rows:
+        ns = T * P
+        order = sorted(range(r0, r0 + ns), key=lambda i: (vals[i], i))[:k]   # brute force: (MAS, index) order
+        exp_idx += sorted(order)
+        r0 += ns
+    total = len(exp_idx)
+    assert list(idx[:total]) == exp_idx
+    assert list(off) == [0, 4, 5, 15, 18]
+    assert [o.n_kept for o in out] == [4, 1, 10, 3]
+    exp_mask = np.zeros(n, np.uint8); exp_mask[exp_idx] = 1
+    assert np.array_equal(mask, exp_mask)
+    assert np.array_equal(Y[:total], X[exp_idx])                  # byte-exact rows
+    # explicit tie case: equal scores -> lower index wins
+    segs, _ = O.make_segments([(0, 1, 1, 5, 2)])
+    mask, idx, off, _, _ = O.select_compact(segs, prm, X[:5], np.array([0.5, 0.2, 0.5, 0.2, 0.2]))
+    assert list(idx[:2]) == [1, 3] and list(mask) == [0, 1, 0, 1, 0]
+
+
+def test_threshold_mode_and_cap_overflow():
+    rng = np.random.default_rng(10)
+    rows = [(0, 1, 1, 6, 6), (1, 1, 1, 5, 5), (2, 1, 1, 4, 4)]
+    segs, n = O.make_segments(rows)
+    vals = np.array([0.5, 0.50001, 0.1, 0.9, 0.5, 0.0, 0.9, 0.8, 0.7, 0.6, 0.51, 0.3, 0.5, 0.2, 1.0])
+    Xb = synth.f32_to_bf16_bits(rng.standard_normal((n, 16)).astype(np.float32))
+    prm = O.default_params(select_mode=1, cut=0.5)
+    mask, idx, off, Y, out = O.select_compact(segs, prm, Xb, vals)
+    exp = [i for i in range(n) if vals[i] <= 0.5]                 # inclusive (G17)
+    assert exp == [0, 2, 4, 5, 11, 12, 13]
+    assert list(idx[:len(exp)]) == exp and list(off) == [0, 4, 4, 7]   # a segment may keep 0 tokens
+    assert np.array_equal(Y[:len(exp)], Xb[exp])
+    # cap smaller than the total: nothing past the cap, true total still reported
+    mask2, idx2, off2, Y2, _ = O.select_compact(segs, prm, Xb, vals, cap_rows=5)
+    assert list(idx2) == exp[:5] and off2[-1] == 7 and np.array_equal(mask2, mask)
+
+
+# ---------------------------------------------------------------- whole-pass invariances
+def test_power_of_two_scaling_is_bit_invariant():
+    w = synth.video(seed=21, R=2, T=4, P=12, d=64, L=5)
+    segs, _ = O.make_segments(w.segments)
+    prm = O.default_params()
+    a = O.forward(segs, w.q_off, prm, w.X, w.Q, want_Y=False)
+    Xs = synth.f32_to_bf16_bits(synth.bf16_bits_to_f32(w.X) * np.float32(4.0))
+    Qs = synth.f32_to_bf16_bits(synth.bf16_bits_to_f32(w.Q) * np.float32(0.25))
+    b = O.forward(segs, w.q_off, prm, Xs, Qs, want_Y=False)
+    for k in ("m_spatial", "gamma", "rel", "mas_tok", "keep_mask", "kept_idx"):
+        assert np.array_equal(a[k], b[k]), k
+    assert np.array_equal(O.seg_out_array(a["seg_out"], "mas"), O.seg_out_array(b["seg_out"], "mas"))
+
+
+def test_row_permutation_of_image_segment():
+    w = synth.batched_images(seed=22, R=1, d=48, L_lo=4, L_hi=4)
+    segs, n = O.make_segments(w.segments)
+    prm = O.default_params()
+    a = O.forward(segs, w.q_off, prm, w.X, w.Q, want_Y=False)
+    perm = np.random.default_rng(0).permutation(n)
+    b = O.forward(segs, w.q_off, prm, w.X[perm], w.Q, want_Y=False)
+    for k in ("m_spatial", "rel", "mas_tok"):
+        assert np.allclose(a[k][perm], b[k], rtol=1e-11, atol=1e-13), k
+    for f in ("rho_spatial", "alpha_mean", "beta", "mas"):
+        assert np.allclose(O.seg_out_array(a["seg_out"], f), O.seg_out_array(b["seg_out"], f), rtol=1e-11), f
+
+
+def test_forward_equals_staged_composition_and_static_patches_are_zero():
+    w = synth.video(seed=23, R=2, T=5, P=576, d=32, L=6)
+    segs, n = O.make_segments(w.segments)
+    prm = O.default_params()
+    full = O.forward(segs, w.q_off, prm, w.X, w.Q)
+    gam = O.temporal(segs, w.X)
+    assert np.array_equal(full["gamma"], gam)
+    # static background patches are bit copies (unless the salient block touched them in either frame) -> gamma == 0
+    P = 576
+    for r in range(2):
+        static = w.meta["static"][r]
+        base = r * 5 * P
+        for t in range(1, 5):
+            rows = base + t * P + np.nonzero(static)[0]
+            same = np.all(w.X[rows] == w.X[rows - P], axis=1)
+            assert same.sum() > 0.4 * P
+            assert np.all(gam[rows[same]] == 0.0)
+            assert np.all(gam[rows[~same]] > 0.0)
+    m, mas, out = O.fuse(segs, prm, O.rms(segs, w.X), gam, O.crossmodal(segs, w.q_off, w.X, w.Q))
+    assert np.array_equal(mas, full["mas_tok"]) and np.array_equal(m, full["m_spatial"])
+    mask, idx, off, Y, _ = O.select_compact(segs, prm, w.X, mas)
+    assert np.array_equal(mask, full["keep_mask"]) and np.array_equal(idx, full["kept_idx"]) and np.array_equal(Y, full["Y"])
+    # structural checks on the selection
+    for k, (_, _, T, Pn, kk) in enumerate(w.segments):
+        sl = idx[off[k]:off[k + 1]]
+        assert len(sl) == kk and np.all(np.diff(sl) > 0)
+        assert sl.min() >= segs[k].row0 and sl.max() < segs[k].row0 + T * Pn
+    assert mask.sum() == off[-1]
+
+
+def test_planted_salient_tokens_are_preferentially_kept():
+    # sanity of the instantiation (not parity): salient, query-aligned rows should mostly survive the 25 % top-k
+    w = synth.batched_images(seed=24, R=3, d=256)
+    segs, _ = O.make_segments(w.segments)
+    r = O.forward(segs, w.q_off, O.default_params(), w.X, w.Q, want_Y=False)
+    kept = r["keep_mask"].astype(bool)
+    recall = (kept & w.salient).sum() / max(1, min(w.salient.sum(), kept.sum()))
+    assert recall > 0.6
