@@ -125,6 +125,14 @@ int64_t mas_plan_n_queries(const mas_plan* plan);        /* sum L_r */
 int64_t mas_plan_kept_capacity(const mas_plan* plan);    /* top-k: sum keep_k ; threshold: N (worst case) */
 int32_t mas_plan_forward_launches(const mas_plan* plan); /* number of kernels one mas_forward enqueues */
 
+/* Profiling aid (bench.py's roofline leg).  After mas_plan_enable_profiling(plan, max_calls > 0) every mas_forward
+ * records CUDA events on the caller's stream at its stage boundaries (score | segment+select | gather) into a ring of
+ * max_calls slots; max_calls = 0 switches it off again.  mas_plan_stage_times reads the slot of call number `call`
+ * (counted from the enable, modulo the ring) once the caller has synchronised the stream: ms[0..2] = stage durations.
+ * The events are host-side driver objects owned by the plan; no device memory is allocated. */
+int mas_plan_enable_profiling(mas_plan* plan, int32_t max_calls);
+int mas_plan_stage_times(const mas_plan* plan, int32_t call, float* ms /*[3]*/);
+
 /* ---- staged entry points (device pointers; each usable alone; outputs fp32 unless noted) ---- */
 
 /* S1 (Eq. 3-4): s_i = RMS of row i; m_spatial = sigmoid of the per-segment standardised s. Either output may be NULL. */

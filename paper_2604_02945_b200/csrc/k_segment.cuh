@@ -1,0 +1,330 @@
+// k_segment.cuh — K2: per-segment statistics, fusion and selection over the per-token scalars only
+// and K3: the row gather (row a6).
+//   a4  mean / population std of s and rel, M_i = sigma(z) (Eq. 3), rho (Eq. 4), gamma_avg, alpha, per-token MAS (SPEC S4),
+//       then per request softmax -> beta and Eq. 7.
+//   a5  exact k-th smallest (MAS_i, i) by 4 x 8-bit radix select on order-preserving keys, ties -> lower index;
+//       or threshold MAS_i <= cut; warp ballot + block prefix scan -> kept_idx (ascending row ids).
+//   a6  Y[j,:] = X[kept_idx[j],:], 16-byte copies, bit exact.
+// All reductions are fixed-order (no floating-point atomics): runs are bit-reproducible.
+#pragma once
+#include "../../include/msas.h"
+#include "msas_internal.cuh"
+
+namespace msas {
+
+struct SegArgs {
+  const DevSeg* segs;
+  const int32_t* req_seg_off;   // [R+1] first segment of each request
+  int n_segs, n_requests;
+  DevParams prm;
+  const float* s;
+  const float* gamma;
+  const float* rel;
+  float* m_spatial;             // may be NULL
+  float* mas_tok;               // FUSE: output; SELECT only: input
+  mas_segment_out* seg_out;     // may be NULL
+  uint8_t* keep_mask;           // may be NULL
+  int32_t* kept_idx;            // may be NULL
+  int64_t* kept_off;            // may be NULL
+  int64_t cap_rows;
+  int32_t* seg_nkept;           // workspace [n_segs]
+  unsigned int* done_counter;   // workspace, zero between launches
+};
+
+constexpr int kSegThreads = 1024;
+
+struct SegSmem {
+  double red[3][32];
+  int ired[2][32];
+  unsigned int hist[256];
+  int bcast[4];
+};
+
+// fixed-order block sum of up to three doubles; result broadcast to every thread
+__device__ __forceinline__ void block_sum3(SegSmem& sm, double& a, double& b, double& c) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+  __syncthreads();
+  if (lane == 0) { sm.red[0][warp] = a; sm.red[1][warp] = b; sm.red[2][warp] = c; }
+  __syncthreads();
+  double x = sm.red[0][lane], y = sm.red[1][lane], z = sm.red[2][lane];   // 32 warps
+  a = warp_sum(x); b = warp_sum(y); c = warp_sum(z);
+}
+
+// exclusive prefix over the block of two small counts; also returns block totals
+__device__ __forceinline__ void block_scan2(SegSmem& sm, int fa, int fb, int& pa, int& pb, int& ta, int& tb) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned ba = __ballot_sync(0xffffffffu, fa), bb = __ballot_sync(0xffffffffu, fb);
+  const unsigned lt = (1u << lane) - 1u;
+  __syncthreads();
+  if (lane == 0) { sm.ired[0][warp] = __popc(ba); sm.ired[1][warp] = __popc(bb); }
+  __syncthreads();
+  int wa = sm.ired[0][lane], wb = sm.ired[1][lane];
+  int ia = wa, ib = wb;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int ua = __shfl_up_sync(0xffffffffu, ia, o), ub = __shfl_up_sync(0xffffffffu, ib, o);
+    if (lane >= o) { ia += ua; ib += ub; }
+  }
+  ta = __shfl_sync(0xffffffffu, ia, 31);
+  tb = __shfl_sync(0xffffffffu, ib, 31);
+  const int ea = __shfl_sync(0xffffffffu, ia - wa, warp), eb = __shfl_sync(0xffffffffu, ib - wb, warp);
+  pa = ea + __popc(ba & lt);
+  pb = eb + __popc(bb & lt);
+}
+
+template <bool FUSE, bool SELECT>
+__global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
+  __shared__ SegSmem sm;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int sidx = blockIdx.x;
+  const DevSeg seg = a.segs[sidx];
+  const int n = seg.n_rows;
+  const int64_t base = seg.row0;
+  const DevParams& p = a.prm;
+
+  if (FUSE) {
+    const bool temporal = seg.n_frames > 1;
+    double ss = 0, sr = 0, sg = 0;
+    for (int i = tid; i < n; i += kSegThreads) {
+      ss += (double)a.s[base + i];
+      sr += (double)a.rel[base + i];
+      if (temporal && i >= seg.n_patches) sg += (double)a.gamma[base + i];
+    }
+    block_sum3(sm, ss, sr, sg);
+    const double mu_s = ss / n, mu_r = sr / n;
+    const double gavg = temporal ? sg / ((double)(seg.n_frames - 1) * seg.n_patches) : 0.0;
+    double vs = 0, vr = 0, dummy = 0;
+    for (int i = tid; i < n; i += kSegThreads) {
+      const double ds = (double)a.s[base + i] - mu_s, dr = (double)a.rel[base + i] - mu_r;
+      vs += ds * ds; vr += dr * dr;
+    }
+    block_sum3(sm, vs, vr, dummy);
+    const double sd_s = sqrt(vs / n), sd_r = sqrt(vr / n);
+    const double den_s = fmax(sd_s, 1e-6 * mu_s), den_r = fmax(sd_r, 1e-6);
+    const float inv_s = den_s > 0.0 ? (float)(1.0 / den_s) : 0.f, inv_r = (float)(1.0 / den_r);
+    const float at = temporal ? p.lambda_temp : 0.f;
+    int below = 0;
+    for (int i = tid; i < n; i += kSegThreads) {
+      // differences in double (s, rel are fp32 values; the means are not representable in fp32)
+      const float z = (float)(((double)a.s[base + i] - mu_s)) * inv_s;
+      const float M = sigmoidf_acc(p.spatial_gain * z + p.spatial_bias);
+      const float zr = (float)(((double)a.rel[base + i] - mu_r)) * inv_r;
+      const float g = sigmoidf_acc(p.rel_gain * zr + p.rel_bias);
+      const float gam = temporal ? a.gamma[base + i] : 0.f;
+      const float mas = 1.0f - g * (1.0f - p.lambda_spatial * (1.0f - M) - at * (1.0f - gam));
+      if (a.m_spatial) a.m_spatial[base + i] = M;
+      a.mas_tok[base + i] = mas;
+      below += M < p.tau_s ? 1 : 0;
+    }
+    double db = below, d1 = 0, d2 = 0;
+    block_sum3(sm, db, d1, d2);
+    if (tid == 0 && a.seg_out) {
+      mas_segment_out o;
+      o.rho_spatial = (float)(db / n);
+      o.gamma_avg = (float)gavg;
+      o.alpha_mean = (float)mu_r;
+      o.beta = 0.f; o.mas = 0.f;
+      o.mean_s = (float)mu_s; o.std_s = (float)sd_s;
+      o.n_tokens = n; o.n_kept = 0;
+      a.seg_out[sidx] = o;
+    }
+    __syncthreads();   // mas_tok of this segment is re-read below by other threads
+  }
+
+  if (SELECT) {
+    const float* mas = a.mas_tok + base;
+    if (p.select_mode == MAS_SELECT_TOPK) {
+      int kk = seg.keep_k < n ? seg.keep_k : n;
+      const int k_total = kk;
+      unsigned prefix = 0, maskbits = 0;
+#pragma unroll 1
+      for (int pass = 0; pass < 4; ++pass) {
+        const int shift = 24 - 8 * pass;
+        if (tid < 256) sm.hist[tid] = 0;
+        __syncthreads();
+        for (int i = tid; i < n; i += kSegThreads) {
+          const unsigned key = float_key(mas[i]);
+          if ((key & maskbits) == prefix) atomicAdd(&sm.hist[(key >> shift) & 255u], 1u);
+        }
+        __syncthreads();
+        if (warp == 0) {   // find the bin where the cumulative count reaches kk
+          unsigned loc[8], tot = 0;
+#pragma unroll
+          for (int b = 0; b < 8; ++b) { loc[b] = sm.hist[lane * 8 + b]; tot += loc[b]; }
+          unsigned inc = tot;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) { unsigned u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
+          unsigned exc = inc - tot;
+          const bool mine = exc < (unsigned)kk && (unsigned)kk <= inc;   // exactly one lane
+          if (mine) {
+            unsigned run = exc;
+            int bin = 0;
+#pragma unroll
+            for (int b = 0; b < 8; ++b) { if (run < (unsigned)kk && (unsigned)kk <= run + loc[b]) { bin = b; break; } run += loc[b]; }
+            sm.bcast[0] = lane * 8 + bin;
+            sm.bcast[1] = (int)run;   // elements strictly below the chosen bin
+          }
+        }
+        __syncthreads();
+        prefix |= (unsigned)sm.bcast[0] << shift;
+        maskbits |= 255u << shift;
+        kk -= sm.bcast[1];
+        __syncthreads();
+      }
+      // prefix = key of the k-th smallest; keep every key < prefix and the first kk keys == prefix (index order)
+      const int64_t off = seg.kept_off_static;
+      int run_less = 0, run_eq = 0;
+      for (int c0 = 0; c0 < n; c0 += kSegThreads) {
+        const int i = c0 + tid;
+        unsigned key = 0xffffffffu;
+        bool valid = i < n;
+        if (valid) key = float_key(mas[i]);
+        const int fl = valid && key < prefix, fe = valid && key == prefix;
+        int pl, pe, tl, te;
+        block_scan2(sm, fl, fe, pl, pe, tl, te);
+        const int eq_before = run_eq + pe;
+        const bool keep = fl || (fe && eq_before < kk);
+        if (valid) {
+          if (a.keep_mask) a.keep_mask[base + i] = keep ? 1 : 0;
+          if (keep && a.kept_idx) {
+            const int64_t pos = off + run_less + pl + (eq_before < kk ? eq_before : kk);
+            if (pos < a.cap_rows) a.kept_idx[pos] = (int32_t)(base + i);
+          }
+        }
+        run_less += tl; run_eq += te;
+      }
+      if (tid == 0) {
+        a.seg_nkept[sidx] = k_total;
+        if (a.seg_out) a.seg_out[sidx].n_kept = k_total;
+      }
+    } else {
+      int cnt = 0;
+      for (int i = tid; i < n; i += kSegThreads) {
+        const bool keep = mas[i] <= p.cut;
+        if (a.keep_mask) a.keep_mask[base + i] = keep ? 1 : 0;
+        cnt += keep;
+      }
+      double dc = cnt, d1 = 0, d2 = 0;
+      block_sum3(sm, dc, d1, d2);
+      if (tid == 0) {
+        a.seg_nkept[sidx] = (int)dc;
+        if (a.seg_out) a.seg_out[sidx].n_kept = (int)dc;
+      }
+    }
+  }
+
+  // ---- last block: per-request softmax + Eq. 7, and the kept_off table
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) sm.bcast[2] = (atomicAdd(a.done_counter, 1u) == gridDim.x - 1) ? 1 : 0;
+  __syncthreads();
+  if (!sm.bcast[2]) return;
+  __threadfence();
+  if (FUSE && a.seg_out) {
+    volatile mas_segment_out* so = a.seg_out;
+    for (int r = tid; r < a.n_requests; r += kSegThreads) {
+      const int k0 = a.req_seg_off[r], k1 = a.req_seg_off[r + 1];
+      float mx = -INFINITY;
+      for (int k = k0; k < k1; ++k) mx = fmaxf(mx, p.kappa * so[k].alpha_mean);
+      float zsum = 0.f;
+      for (int k = k0; k < k1; ++k) zsum += expf(p.kappa * so[k].alpha_mean - mx);
+      for (int k = k0; k < k1; ++k) {
+        const float beta = expf(p.kappa * so[k].alpha_mean - mx) / zsum;
+        const float at = a.segs[k].n_frames > 1 ? p.lambda_temp : 0.f;
+        so[k].beta = beta;
+        so[k].mas = 1.0f - beta * (1.0f - p.lambda_spatial * so[k].rho_spatial - at * (1.0f - so[k].gamma_avg));
+      }
+    }
+  }
+  if (SELECT && a.kept_off) {
+    if (p.select_mode == MAS_SELECT_TOPK) {
+      for (int k = tid; k < a.n_segs; k += kSegThreads) a.kept_off[k] = a.segs[k].kept_off_static;
+      if (tid == 0) a.kept_off[a.n_segs] = a.segs[a.n_segs - 1].kept_off_static + a.segs[a.n_segs - 1].keep_k;
+    } else {
+      volatile int32_t* nk = a.seg_nkept;
+      long long run = 0;
+      for (int c0 = 0; c0 < a.n_segs; c0 += kSegThreads) {
+        const int k = c0 + tid;
+        const int v = k < a.n_segs ? nk[k] : 0;
+        // inclusive scan of v over the block (values up to 2^31 in total fit a long long running sum)
+        int inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
+        __syncthreads();
+        if (lane == 31) sm.ired[0][warp] = inc;
+        __syncthreads();
+        int wv = sm.ired[0][lane], winc = wv;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += u; }
+        const int wexc = __shfl_sync(0xffffffffu, winc - wv, warp);
+        const int tot = __shfl_sync(0xffffffffu, winc, 31);
+        if (k < a.n_segs) a.kept_off[k] = run + wexc + inc - v;
+        run += tot;
+      }
+      if (tid == 0) a.kept_off[a.n_segs] = run;
+    }
+  }
+  if (tid == 0) *a.done_counter = 0u;
+}
+
+// Threshold mode only: index compaction once kept_off is known (one CTA per segment, ordered ballot + scan).
+__global__ void __launch_bounds__(kSegThreads) k_compact_idx(const DevSeg* segs, const uint8_t* keep_mask, const int64_t* kept_off,
+                                                             int32_t* kept_idx, int64_t cap_rows) {
+  __shared__ SegSmem sm;
+  const DevSeg seg = segs[blockIdx.x];
+  const int64_t off = kept_off[blockIdx.x];
+  int run = 0;
+  for (int c0 = 0; c0 < seg.n_rows; c0 += kSegThreads) {
+    const int i = c0 + threadIdx.x;
+    const int f = i < seg.n_rows && keep_mask[seg.row0 + i];
+    int pf, pz, tf, tz;
+    block_scan2(sm, f, 0, pf, pz, tf, tz);
+    if (f) {
+      const int64_t pos = off + run + pf;
+      if (pos < cap_rows) kept_idx[pos] = (int32_t)(seg.row0 + i);
+    }
+    run += tf;
+  }
+}
+
+// K3 (a6): one warp per kept row, 16-byte copies, four in flight per lane.
+__global__ void __launch_bounds__(256) k_gather(const char* __restrict__ X, char* __restrict__ Y, const int32_t* __restrict__ kept_idx,
+                                                const int64_t* __restrict__ total_ptr, int64_t cap_rows, int row_bytes) {
+  const int lane = threadIdx.x & 31;
+  const int64_t total = *total_ptr < cap_rows ? *total_ptr : cap_rows;
+  const int64_t n_warps = (int64_t)gridDim.x * 8;
+  const int n16 = row_bytes >> 4;
+  for (int64_t j = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5); j < total; j += n_warps) {
+    const uint4* src = reinterpret_cast<const uint4*>(X + (int64_t)kept_idx[j] * row_bytes);
+    uint4* dst = reinterpret_cast<uint4*>(Y + j * row_bytes);
+    int i = lane;
+    for (; i + 96 < n16; i += 128) {
+      uint4 v0 = ld_nc16(src + i), v1 = ld_nc16(src + i + 32), v2 = ld_nc16(src + i + 64), v3 = ld_nc16(src + i + 96);
+      st_na16(dst + i, v0); st_na16(dst + i + 32, v1); st_na16(dst + i + 64, v2); st_na16(dst + i + 96, v3);
+    }
+    for (; i < n16; i += 32) st_na16(dst + i, ld_nc16(src + i));
+  }
+}
+
+// staged mas_spatial second phase: m_spatial from s (per-segment standardise + sigmoid, Eq. 3)
+__global__ void __launch_bounds__(kSegThreads) k_spatial_finish(const DevSeg* segs, DevParams p, const float* s, float* m_spatial) {
+  __shared__ SegSmem sm;
+  const DevSeg seg = segs[blockIdx.x];
+  const int n = seg.n_rows;
+  const int64_t base = seg.row0;
+  double ss = 0, d1 = 0, d2 = 0;
+  for (int i = threadIdx.x; i < n; i += kSegThreads) ss += (double)s[base + i];
+  block_sum3(sm, ss, d1, d2);
+  const double mu = ss / n;
+  double vs = 0;
+  for (int i = threadIdx.x; i < n; i += kSegThreads) { const double e = (double)s[base + i] - mu; vs += e * e; }
+  d1 = d2 = 0;
+  block_sum3(sm, vs, d1, d2);
+  const double den = fmax(sqrt(vs / n), 1e-6 * mu);
+  const float inv = den > 0.0 ? (float)(1.0 / den) : 0.f;
+  for (int i = threadIdx.x; i < n; i += kSegThreads)
+    m_spatial[base + i] = sigmoidf_acc(p.spatial_gain * ((float)((double)s[base + i] - mu) * inv) + p.spatial_bias);
+}
+
+}  // namespace msas

@@ -1,0 +1,479 @@
+// msas_api.cu — the C ABI of libmsas (include/msas.h): plan construction, argument validation and kernel launches.
+// Every step of the pass runs in the CUDA kernels of this directory; there is no CPU path.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <vector>
+
+#include "../../include/msas.h"
+#include "k_score_simple.cuh"
+#include "k_score_tc.cuh"
+#include "k_segment.cuh"
+
+using namespace msas;
+
+static thread_local int g_last_cuda = 0;
+#define CK(x)                                             \
+  do {                                                    \
+    cudaError_t e_ = (x);                                 \
+    if (e_ != cudaSuccess) { g_last_cuda = (int)e_; (void)cudaGetLastError(); return MAS_ERR_CUDA; } \
+  } while (0)
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+  size_t segs, tiles, req, tc_sched, tables_end;   // uploaded tables (contiguous from 0)
+  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, total;
+};
+
+struct mas_plan {
+  int32_t n_segs = 0, n_requests = 0, d = 0, dtype = 0;
+  int64_t N = 0, nQ = 0, kept_cap = 0;
+  int32_t n_tiles = 0;
+  int32_t max_L = 0;
+  DevParams prm{};
+  Layout lay{};
+  char* ws = nullptr;
+  void* pinned = nullptr;
+  size_t pinned_bytes = 0;
+  int sm_count = 148;
+  TcSchedule tc{};            // tcgen05 fast-path schedule (tc.enabled == false -> generic kernels)
+  mutable std::vector<cudaEvent_t> prof_ev;   // profiling ring: 4 events per slot
+  mutable int64_t prof_calls = 0;
+  int32_t prof_slots = 0;
+  template <class T> T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
+};
+
+// ------------------------------------------------------------------------------------------------ host helpers
+extern "C" int mas_version(void) { return MAS_VERSION; }
+extern "C" int mas_last_cuda_error(void) { return g_last_cuda; }
+extern "C" const char* mas_status_string(int st) {
+  switch (st) {
+    case MAS_OK: return "ok";
+    case MAS_ERR_INVALID_ARG: return "invalid argument";
+    case MAS_ERR_UNSUPPORTED: return "unsupported shape, dtype or alignment";
+    case MAS_ERR_WORKSPACE: return "workspace too small";
+    case MAS_ERR_CUDA: return "CUDA error (see mas_last_cuda_error)";
+    default: return "unknown status";
+  }
+}
+extern "C" void mas_params_default(mas_params* p) {
+  if (!p) return;
+  p->lambda_spatial = 0.6f; p->lambda_temp = 0.4f; p->tau_s = 0.3f; p->kappa = 10.0f;
+  p->spatial_gain = 1.0f; p->spatial_bias = 0.0f; p->rel_gain = 1.0f; p->rel_bias = 0.0f;
+  p->cut = 0.5f; p->select_mode = MAS_SELECT_TOPK;
+}
+extern "C" int32_t mas_keep_count(int64_t n, double ratio) {
+  if (n <= 0) return 0;
+  int64_t k = (int64_t)std::ceil(ratio * (double)n - 1e-9);
+  if (k < 1) k = 1;
+  if (k > n) k = n;
+  return (int32_t)k;
+}
+
+// ------------------------------------------------------------------------------------------------ validation + layout
+static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_off, int32_t n_req, int32_t d, int32_t dtype,
+                    const mas_params* prm, int64_t* N_out, int64_t* nQ_out, int32_t* n_tiles_out, int32_t* maxL_out) {
+  if (!segs || !q_off || n_segs <= 0 || n_req <= 0) return MAS_ERR_INVALID_ARG;
+  if (dtype != MAS_F32 && dtype != MAS_BF16) return MAS_ERR_INVALID_ARG;
+  if (d < 8 || d > 65536) return MAS_ERR_UNSUPPORTED;
+  if (dtype == MAS_BF16 ? (d % 8 != 0) : (d % 4 != 0)) return MAS_ERR_UNSUPPORTED;
+  if (q_off[0] != 0) return MAS_ERR_INVALID_ARG;
+  int32_t maxL = 0;
+  for (int32_t r = 0; r < n_req; ++r) {
+    const int64_t L = q_off[r + 1] - q_off[r];
+    if (L < 0) return MAS_ERR_INVALID_ARG;
+    if (L < 1 || L > MAS_MAX_QUERY_TOKENS) return MAS_ERR_UNSUPPORTED;
+    if (L > maxL) maxL = (int32_t)L;
+  }
+  if (q_off[n_req] > (int64_t)0x7fffffff) return MAS_ERR_UNSUPPORTED;
+  int64_t row = 0, tiles = 0;
+  int32_t prev_req = -1;
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const mas_segment& s = segs[k];
+    if (s.n_frames < 1 || s.n_patches < 1) return MAS_ERR_INVALID_ARG;
+    if (s.request < 0 || s.request >= n_req || s.request < prev_req) return MAS_ERR_INVALID_ARG;
+    if (s.row0 != row) return MAS_ERR_INVALID_ARG;
+    const int64_t n = (int64_t)s.n_frames * s.n_patches;
+    if (n > (int64_t)0x7fffffff) return MAS_ERR_UNSUPPORTED;
+    if (prm && prm->select_mode == MAS_SELECT_TOPK && (s.keep_k < 1 || s.keep_k > n)) return MAS_ERR_INVALID_ARG;
+    prev_req = s.request;
+    row += n;
+    tiles += (n + kTileRows - 1) / kTileRows;
+  }
+  if (row > (int64_t)0x7fffffff - kTileRows) return MAS_ERR_UNSUPPORTED;   // kept_idx is int32
+  if (prm) {
+    if (prm->select_mode != MAS_SELECT_TOPK && prm->select_mode != MAS_SELECT_THRESHOLD) return MAS_ERR_INVALID_ARG;
+    if (!(prm->lambda_spatial >= 0.f) || !(prm->lambda_temp >= 0.f) || !(prm->lambda_spatial + prm->lambda_temp <= 1.0f + 1e-6f))
+      return MAS_ERR_INVALID_ARG;
+  }
+  *N_out = row; *nQ_out = q_off[n_req]; *n_tiles_out = (int32_t)tiles; *maxL_out = maxL;
+  return MAS_OK;
+}
+
+static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes) {
+  Layout l{};
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
+  l.segs = take(sizeof(DevSeg) * n_segs);
+  l.tiles = take(sizeof(DevTile) * n_tiles);
+  l.req = take(sizeof(int32_t) * (n_req + 1));
+  l.tc_sched = take(tc_bytes);
+  l.tables_end = o;
+  l.qinv = take(sizeof(float) * nQ);
+  l.s = take(sizeof(float) * N);
+  l.gamma = take(sizeof(float) * N);
+  l.rel = take(sizeof(float) * N);
+  l.mas = take(sizeof(float) * N);
+  l.mask = take(N);
+  l.segout = take(sizeof(mas_segment_out) * n_segs);
+  l.nkept = take(sizeof(int32_t) * n_segs);
+  l.keptoff = take(sizeof(int64_t) * (n_segs + 1));
+  l.counter = take(256);
+  l.total = o;
+  return l;
+}
+
+extern "C" int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
+                                        int32_t d, int32_t dtype, size_t* out_bytes) {
+  if (!out_bytes) return MAS_ERR_INVALID_ARG;
+  int64_t N, nQ; int32_t nt, maxL;
+  int st = validate(h_segs, n_segs, h_q_off, n_requests, d, dtype, nullptr, &N, &nQ, &nt, &maxL);
+  if (st != MAS_OK) return st;
+  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs)).total;
+  return MAS_OK;
+}
+
+static std::once_flag g_attr_once;
+static void set_kernel_attrs() {
+  cudaFuncSetAttribute(k_score_mma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
+  cudaFuncSetAttribute(k_score_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
+  tc_set_kernel_attrs();
+  (void)cudaGetLastError();
+}
+
+extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off,
+                               int32_t n_requests, int32_t d, int32_t dtype, const mas_params* params,
+                               void* d_workspace, size_t workspace_bytes, mas_stream_t stream_) {
+  if (!out || !params || !d_workspace) return MAS_ERR_INVALID_ARG;
+  *out = nullptr;
+  cudaStream_t stream = (cudaStream_t)stream_;
+  int64_t N, nQ; int32_t nt, maxL;
+  int st = validate(h_segs, n_segs, h_q_off, n_requests, d, dtype, params, &N, &nQ, &nt, &maxL);
+  if (st != MAS_OK) return st;
+  if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0) return MAS_ERR_UNSUPPORTED;
+  const size_t tc_bytes = tc_schedule_bytes(h_segs, n_segs);
+  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes);
+  if (workspace_bytes < lay.total) return MAS_ERR_WORKSPACE;
+
+  mas_plan* p = new (std::nothrow) mas_plan();
+  if (!p) return MAS_ERR_INVALID_ARG;
+  p->n_segs = n_segs; p->n_requests = n_requests; p->d = d; p->dtype = dtype;
+  p->N = N; p->nQ = nQ; p->n_tiles = nt; p->max_L = maxL; p->lay = lay; p->ws = static_cast<char*>(d_workspace);
+  p->prm.lambda_spatial = params->lambda_spatial; p->prm.lambda_temp = params->lambda_temp; p->prm.tau_s = params->tau_s;
+  p->prm.kappa = params->kappa; p->prm.spatial_gain = params->spatial_gain; p->prm.spatial_bias = params->spatial_bias;
+  p->prm.rel_gain = params->rel_gain; p->prm.rel_bias = params->rel_bias; p->prm.cut = params->cut;
+  p->prm.select_mode = params->select_mode;
+
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) { p->pinned_bytes = lay.tables_end + 256; e = cudaHostAlloc(&p->pinned, p->pinned_bytes, cudaHostAllocDefault); }
+  if (e != cudaSuccess) { g_last_cuda = (int)e; (void)cudaGetLastError(); delete p; return MAS_ERR_CUDA; }
+  std::call_once(g_attr_once, set_kernel_attrs);
+
+  char* h = static_cast<char*>(p->pinned);
+  std::memset(h, 0, p->pinned_bytes);
+  DevSeg* hs = reinterpret_cast<DevSeg*>(h + lay.segs);
+  DevTile* ht = reinterpret_cast<DevTile*>(h + lay.tiles);
+  int32_t* hr = reinterpret_cast<int32_t*>(h + lay.req);
+  int64_t kept = 0;
+  int32_t ti = 0;
+  for (int32_t r = 0; r <= n_requests; ++r) hr[r] = n_segs;
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const mas_segment& s = h_segs[k];
+    DevSeg& ds = hs[k];
+    ds.row0 = s.row0;
+    ds.kept_off_static = kept;
+    ds.n_rows = s.n_frames * s.n_patches;
+    ds.n_patches = s.n_patches;
+    ds.n_frames = s.n_frames;
+    ds.request = s.request;
+    ds.q0 = (int32_t)h_q_off[s.request];
+    ds.L = (int32_t)(h_q_off[s.request + 1] - h_q_off[s.request]);
+    ds.keep_k = params->select_mode == MAS_SELECT_TOPK ? s.keep_k : ds.n_rows;
+    kept += params->select_mode == MAS_SELECT_TOPK ? s.keep_k : 0;
+    if (hr[s.request] > k) hr[s.request] = k;
+    for (int32_t r0 = 0; r0 < ds.n_rows; r0 += kTileRows) {
+      ht[ti].row_start = (int32_t)(s.row0 + r0);
+      ht[ti].n_rows = ds.n_rows - r0 < kTileRows ? ds.n_rows - r0 : kTileRows;
+      ht[ti].seg = k;
+      ++ti;
+    }
+  }
+  for (int32_t r = n_requests - 1; r >= 0; --r)   // requests without segments get an empty range
+    if (hr[r] > hr[r + 1]) hr[r] = hr[r + 1];
+  p->kept_cap = params->select_mode == MAS_SELECT_TOPK ? kept : N;
+  tc_build_schedule(p->tc, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched, p->ws + lay.tc_sched);
+
+  e = cudaMemcpyAsync(p->ws, p->pinned, lay.tables_end, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(p->ws + lay.counter, 0, 256, stream);
+  if (e != cudaSuccess) { g_last_cuda = (int)e; (void)cudaGetLastError(); cudaFreeHost(p->pinned); delete p; return MAS_ERR_CUDA; }
+  *out = p;
+  return MAS_OK;
+}
+
+extern "C" int mas_plan_enable_profiling(mas_plan* p, int32_t max_calls) {
+  if (!p || max_calls < 0) return MAS_ERR_INVALID_ARG;
+  for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
+  p->prof_ev.clear();
+  p->prof_slots = 0;
+  p->prof_calls = 0;
+  for (int32_t i = 0; i < max_calls * 4; ++i) {
+    cudaEvent_t e;
+    CK(cudaEventCreate(&e));
+    p->prof_ev.push_back(e);
+  }
+  p->prof_slots = max_calls;
+  return MAS_OK;
+}
+extern "C" int mas_plan_stage_times(const mas_plan* p, int32_t call, float* ms) {
+  if (!p || !ms || p->prof_slots <= 0 || call < 0 || call >= p->prof_calls) return MAS_ERR_INVALID_ARG;
+  const cudaEvent_t* e = &p->prof_ev[(size_t)(call % p->prof_slots) * 4];
+  for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&ms[i], e[i], e[i + 1]));
+  return MAS_OK;
+}
+
+extern "C" int mas_plan_destroy(mas_plan* p) {
+  if (!p) return MAS_OK;
+  for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
+  if (p->pinned) cudaFreeHost(p->pinned);
+  delete p;
+  return MAS_OK;
+}
+extern "C" int64_t mas_plan_n_tokens(const mas_plan* p) { return p ? p->N : -1; }
+extern "C" int64_t mas_plan_n_queries(const mas_plan* p) { return p ? p->nQ : -1; }
+extern "C" int64_t mas_plan_kept_capacity(const mas_plan* p) { return p ? p->kept_cap : -1; }
+
+// ------------------------------------------------------------------------------------------------ launches
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int launch_qprep(const mas_plan* p, const void* Q, cudaStream_t st) {
+  const unsigned grid = (unsigned)((p->nQ + 7) / 8);
+  if (p->dtype == MAS_BF16) k_qprep<1><<<grid, 256, 0, st>>>(Q, p->at<float>(p->lay.qinv), p->nQ, p->d);
+  else k_qprep<0><<<grid, 256, 0, st>>>(Q, p->at<float>(p->lay.qinv), p->nQ, p->d);
+  CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+static ScoreArgs score_args(const mas_plan* p, const void* X, const void* Q, float* s, float* gamma, float* rel, float* S_opt) {
+  ScoreArgs a;
+  a.X = X; a.Q = Q; a.qinv = p->at<float>(p->lay.qinv);
+  a.segs = p->at<DevSeg>(p->lay.segs); a.tiles = p->at<DevTile>(p->lay.tiles);
+  a.s = s; a.gamma = gamma; a.rel = rel; a.S_opt = S_opt; a.d = p->d;
+  return a;
+}
+
+static int launch_rowstats(const mas_plan* p, const void* X, float* s, float* gamma, cudaStream_t st) {
+  ScoreArgs a = score_args(p, X, nullptr, s, gamma, nullptr, nullptr);
+  if (p->dtype == MAS_BF16) k_rowstats<1><<<p->n_tiles, 256, 0, st>>>(a);
+  else k_rowstats<0><<<p->n_tiles, 256, 0, st>>>(a);
+  CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+static int launch_score_mma(const mas_plan* p, const void* X, const void* Q, float* s, float* gamma, float* rel, float* S_opt, cudaStream_t st) {
+  ScoreArgs a = score_args(p, X, Q, s, gamma, rel, S_opt);
+  if (p->dtype == MAS_BF16) k_score_mma<1><<<p->n_tiles, 256, score_mma_smem_bytes(1), st>>>(a);
+  else k_score_mma<0><<<p->n_tiles, 256, score_mma_smem_bytes(0), st>>>(a);
+  CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+static SegArgs seg_args(const mas_plan* p, const float* s, const float* gamma, const float* rel, float* m_spatial, float* mas_tok,
+                        mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, int64_t cap_rows) {
+  SegArgs a;
+  a.segs = p->at<DevSeg>(p->lay.segs); a.req_seg_off = p->at<int32_t>(p->lay.req);
+  a.n_segs = p->n_segs; a.n_requests = p->n_requests; a.prm = p->prm;
+  a.s = s; a.gamma = gamma; a.rel = rel; a.m_spatial = m_spatial; a.mas_tok = mas_tok; a.seg_out = seg_out;
+  a.keep_mask = keep_mask; a.kept_idx = kept_idx; a.kept_off = kept_off; a.cap_rows = cap_rows;
+  a.seg_nkept = p->at<int32_t>(p->lay.nkept);
+  a.done_counter = p->at<unsigned int>(p->lay.counter);
+  return a;
+}
+
+static int launch_gather(const mas_plan* p, const void* X, const int32_t* kept_idx, const int64_t* kept_off, void* Y, int64_t cap_rows,
+                         cudaStream_t st) {
+  if (Y && cap_rows > 0) {
+    const int64_t rows = cap_rows < p->kept_cap ? cap_rows : p->kept_cap;
+    int64_t grid = (rows + 7) / 8;
+    const int64_t gmax = (int64_t)p->sm_count * 16;
+    if (grid > gmax) grid = gmax;
+    if (grid < 1) grid = 1;
+    const int esz = p->dtype == MAS_BF16 ? 2 : 4;
+    k_gather<<<(unsigned)grid, 256, 0, st>>>(static_cast<const char*>(X), static_cast<char*>(Y), kept_idx, kept_off + p->n_segs,
+                                            cap_rows, p->d * esz);
+    CK(cudaGetLastError());
+  }
+  return MAS_OK;
+}
+
+static int launch_select_tail(const mas_plan* p, const void* X, const uint8_t* mask, int32_t* kept_idx, const int64_t* kept_off,
+                              void* Y, int64_t cap_rows, cudaStream_t st) {
+  if (p->prm.select_mode == MAS_SELECT_THRESHOLD && kept_idx) {
+    k_compact_idx<<<p->n_segs, kSegThreads, 0, st>>>(p->at<DevSeg>(p->lay.segs), mask, kept_off, kept_idx, cap_rows);
+    CK(cudaGetLastError());
+  }
+  return launch_gather(p, X, kept_idx, kept_off, Y, cap_rows, st);
+}
+
+extern "C" int32_t mas_plan_forward_launches(const mas_plan* p) {
+  if (!p) return -1;
+  // [qprep +] score + segment (+ index compaction in threshold mode) + gather
+  return (p->tc.enabled ? 3 : 4) + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
+}
+
+// ------------------------------------------------------------------------------------------------ staged entry points
+extern "C" int mas_spatial(const mas_plan* p, const void* X, float* s, float* m_spatial, mas_stream_t stream) {
+  if (!p || !X || (!s && !m_spatial)) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X)) return MAS_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  float* sb = s ? s : p->at<float>(p->lay.s);
+  int rc = launch_rowstats(p, X, sb, nullptr, st);
+  if (rc != MAS_OK) return rc;
+  if (m_spatial) {
+    k_spatial_finish<<<p->n_segs, kSegThreads, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->prm, sb, m_spatial);
+    CK(cudaGetLastError());
+  }
+  return MAS_OK;
+}
+
+extern "C" int mas_temporal(const mas_plan* p, const void* X, float* gamma, mas_stream_t stream) {
+  if (!p || !X || !gamma) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X)) return MAS_ERR_UNSUPPORTED;
+  return launch_rowstats(p, X, nullptr, gamma, (cudaStream_t)stream);
+}
+
+extern "C" int mas_crossmodal(const mas_plan* p, const void* X, const void* Q, float* rel, float* S_opt, mas_stream_t stream) {
+  if (!p || !X || !Q || (!rel && !S_opt)) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(Q)) return MAS_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc = launch_qprep(p, Q, st);
+  if (rc != MAS_OK) return rc;
+  return launch_score_mma(p, X, Q, nullptr, nullptr, rel ? rel : p->at<float>(p->lay.rel), S_opt, st);
+}
+
+extern "C" int mas_fuse(const mas_plan* p, const float* s, const float* gamma, const float* rel, float* m_spatial, float* mas_tok,
+                        mas_segment_out* seg_out, mas_stream_t stream) {
+  if (!p || !s || !gamma || !rel || !mas_tok) return MAS_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  SegArgs a = seg_args(p, s, gamma, rel, m_spatial, mas_tok, seg_out ? seg_out : p->at<mas_segment_out>(p->lay.segout), nullptr, nullptr,
+                       nullptr, 0);
+  k_segment<true, false><<<p->n_segs, kSegThreads, 0, st>>>(a);
+  CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+extern "C" int mas_select_compact(const mas_plan* p, const void* X, const float* mas_tok, uint8_t* keep_mask, int32_t* kept_idx,
+                                  int64_t* kept_off, void* Y, int64_t cap_rows, mas_segment_out* seg_out, mas_stream_t stream) {
+  if (!p || !mas_tok || cap_rows < 0) return MAS_ERR_INVALID_ARG;
+  if (Y && (!X || !kept_idx)) return MAS_ERR_INVALID_ARG;
+  if (Y && !aligned16(X)) return MAS_ERR_UNSUPPORTED;
+  if (Y && !aligned16(Y)) return MAS_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  uint8_t* mask = keep_mask ? keep_mask : p->at<uint8_t>(p->lay.mask);
+  int64_t* koff = kept_off ? kept_off : p->at<int64_t>(p->lay.keptoff);
+  SegArgs a = seg_args(p, nullptr, nullptr, nullptr, nullptr, const_cast<float*>(mas_tok), seg_out, mask, kept_idx, koff, cap_rows);
+  k_segment<false, true><<<p->n_segs, kSegThreads, 0, st>>>(a);
+  CK(cudaGetLastError());
+  return launch_select_tail(p, X, mask, kept_idx, koff, Y, cap_rows, st);
+}
+
+// ------------------------------------------------------------------------------------------------ fused entry point
+extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, float* m_spatial, float* gamma, float* rel, float* mas_tok,
+                           mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows,
+                           mas_stream_t stream) {
+  if (!p || !X || !Q || cap_rows < 0) return MAS_ERR_INVALID_ARG;
+  if (Y && !kept_idx) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(Q) || (Y && !aligned16(Y))) return MAS_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  float* sb = p->at<float>(p->lay.s);
+  float* gb = gamma ? gamma : p->at<float>(p->lay.gamma);
+  float* rb = rel ? rel : p->at<float>(p->lay.rel);
+  float* mb = mas_tok ? mas_tok : p->at<float>(p->lay.mas);
+  mas_segment_out* so = seg_out ? seg_out : p->at<mas_segment_out>(p->lay.segout);
+  uint8_t* mask = keep_mask ? keep_mask : p->at<uint8_t>(p->lay.mask);
+  int64_t* koff = kept_off ? kept_off : p->at<int64_t>(p->lay.keptoff);
+
+  const cudaEvent_t* pev = p->prof_slots > 0 ? &p->prof_ev[(size_t)(p->prof_calls++ % p->prof_slots) * 4] : nullptr;
+  if (pev) CK(cudaEventRecord(pev[0], st));
+  int rc;
+  if (p->tc.enabled) {
+    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->N, p->nQ, p->d, st);   // a0-a3 in one kernel
+    if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
+  } else {
+    if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
+    if ((rc = launch_score_mma(p, X, Q, sb, gb, rb, nullptr, st)) != MAS_OK) return rc;
+  }
+  SegArgs a = seg_args(p, sb, gb, rb, m_spatial, mb, so, mask, kept_idx, koff, cap_rows);
+  if (pev) CK(cudaEventRecord(pev[1], st));
+  k_segment<true, true><<<p->n_segs, kSegThreads, 0, st>>>(a);
+  CK(cudaGetLastError());
+  if (p->prm.select_mode == MAS_SELECT_THRESHOLD && kept_idx) {
+    k_compact_idx<<<p->n_segs, kSegThreads, 0, st>>>(p->at<DevSeg>(p->lay.segs), mask, koff, kept_idx, cap_rows);
+    CK(cudaGetLastError());
+  }
+  if (pev) CK(cudaEventRecord(pev[2], st));
+  rc = launch_gather(p, X, kept_idx, koff, Y, cap_rows, st);
+  if (pev) CK(cudaEventRecord(pev[3], st));
+  return rc;
+}
+
+// ------------------------------------------------------------------------------------------------ host-buffer convenience
+extern "C" int mas_forward_host(const mas_plan* p, const void* h_X, const void* h_Q, void* d_X, void* d_Q, const mas_outputs* d_out,
+                                const mas_outputs* h_out, mas_stream_t stream) {
+  if (!p || !h_X || !h_Q || !d_X || !d_Q || !d_out) return MAS_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t esz = p->dtype == MAS_BF16 ? 2 : 4;
+  CK(cudaMemcpyAsync(d_X, h_X, (size_t)p->N * p->d * esz, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(d_Q, h_Q, (size_t)p->nQ * p->d * esz, cudaMemcpyHostToDevice, st));
+  int64_t* koff = d_out->kept_off ? d_out->kept_off : p->at<int64_t>(p->lay.keptoff);
+  int rc = mas_forward(p, d_X, d_Q, d_out->m_spatial, d_out->gamma, d_out->rel, d_out->mas_tok, d_out->seg_out, d_out->keep_mask,
+                       d_out->kept_idx, koff, d_out->Y, d_out->cap_rows, stream);
+  if (rc != MAS_OK) return rc;
+  if (h_out) {
+    const size_t N = (size_t)p->N;
+    auto back = [&](void* h, const void* d, size_t bytes) -> cudaError_t {
+      if (!h) return cudaSuccess;
+      if (!d) return cudaErrorInvalidValue;
+      return cudaMemcpyAsync(h, d, bytes, cudaMemcpyDeviceToHost, st);
+    };
+    CK(back(h_out->m_spatial, d_out->m_spatial, N * 4));
+    CK(back(h_out->gamma, d_out->gamma, N * 4));
+    CK(back(h_out->rel, d_out->rel, N * 4));
+    CK(back(h_out->mas_tok, d_out->mas_tok, N * 4));
+    CK(back(h_out->seg_out, d_out->seg_out, sizeof(mas_segment_out) * p->n_segs));
+    CK(back(h_out->keep_mask, d_out->keep_mask, N));
+    CK(back(h_out->kept_off, koff, sizeof(int64_t) * (p->n_segs + 1)));
+    if (h_out->kept_idx || h_out->Y) {
+      int64_t* total_h = reinterpret_cast<int64_t*>(static_cast<char*>(p->pinned) + p->lay.tables_end);
+      int64_t total = p->kept_cap;
+      if (p->prm.select_mode == MAS_SELECT_THRESHOLD) {   // the kept count is data dependent: read it before sizing the copies
+        CK(cudaMemcpyAsync(total_h, koff + p->n_segs, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        total = *total_h;
+      }
+      if (total > d_out->cap_rows) total = d_out->cap_rows;
+      if (total > h_out->cap_rows) total = h_out->cap_rows;
+      if (total > 0) {
+        CK(back(h_out->kept_idx, d_out->kept_idx, sizeof(int32_t) * (size_t)total));
+        CK(back(h_out->Y, d_out->Y, (size_t)total * p->d * esz));
+      }
+    }
+  }
+  CK(cudaStreamSynchronize(st));
+  return MAS_OK;
+}

@@ -1,0 +1,63 @@
+"""Shared helpers of the GPU parity tests: run the CUDA path through the C-ABI binding and the oracle on the same seeded
+host arrays and compare under SPEC.md "Parity rules"."""
+import numpy as np
+
+RTOL, ATOL = 1e-3, 1e-6          # north_star: relative error 1e-3 (bf16 inputs, fp32 accumulation)
+SEL_BAND = 1e-3                  # selection must agree wherever the oracle score is further than this from the cut
+
+
+def assert_close(gpu, ref, name):
+    gpu = np.asarray(gpu, np.float64)
+    ref = np.asarray(ref, np.float64)
+    assert gpu.shape == ref.shape, (name, gpu.shape, ref.shape)
+    err = np.abs(gpu - ref)
+    tol = RTOL * np.abs(ref) + ATOL
+    bad = np.nonzero(err > tol)[0]
+    assert bad.size == 0, "%s: %d/%d outside tolerance; worst idx %d gpu=%r ref=%r" % (
+        name, bad.size, ref.size, bad[np.argmax(err[bad] - tol[bad])], gpu[bad[0]], ref[bad[0]])
+
+
+def check_selection(rows, select_mode, cut, ref_mas, gpu_mask, gpu_idx, gpu_off, row_base=0):
+    """rows: (request, modality, T, P, keep_k) of the compared segments; arrays cover exactly these segments
+    (gpu_idx holds global ids: subtract row_base).  SPEC.md parity rules for selection."""
+    gpu_mask = np.asarray(gpu_mask).astype(bool)
+    r0 = 0
+    for k, (_, _, T, P, kk) in enumerate(rows):
+        n = T * P
+        mas = np.asarray(ref_mas[r0:r0 + n], np.float64)
+        if select_mode == 0:
+            order = np.sort(mas)
+            c = order[kk - 1] if kk >= n else 0.5 * (order[kk - 1] + order[kk])
+            ref_keep = np.zeros(n, bool)
+            ref_keep[np.lexsort((np.arange(n), mas))[:kk]] = True       # (MAS, index) order
+            assert gpu_off[k + 1] - gpu_off[k] == kk, "segment %d: n_kept %d != keep_k %d" % (k, gpu_off[k + 1] - gpu_off[k], kk)
+        else:
+            c = cut
+            ref_keep = mas <= cut
+        decided = np.abs(mas - c) > SEL_BAND
+        gm = gpu_mask[r0:r0 + n]
+        diff = np.nonzero(decided & (gm != ref_keep))[0]
+        assert diff.size == 0, "segment %d: %d decided tokens with a different mask bit (first %d, mas %r, cut %r)" % (
+            k, diff.size, diff[0], mas[diff[0]], c)
+        idx = np.asarray(gpu_idx[gpu_off[k]:gpu_off[k + 1]], np.int64) - row_base - r0
+        assert np.all(np.diff(idx) > 0), "segment %d: kept_idx not strictly ascending" % k
+        assert idx.size == 0 or (idx.min() >= 0 and idx.max() < n), "segment %d: kept_idx outside the segment" % k
+        assert np.array_equal(np.nonzero(gm)[0], idx), "segment %d: mask and kept_idx disagree" % k
+        assert np.array_equal(idx[decided[idx]], np.nonzero(ref_keep & decided)[0]), "segment %d: decided kept lists differ" % k
+        r0 += n
+
+
+def check_seg_out(rows, gpu_so, ref_so, ref_m, tau_s=0.3, lambda_spatial=0.6):
+    """Per-segment records.  rho may differ by the tokens whose M_i sits within 1e-3*tau_s of tau_s (SPEC)."""
+    r0 = 0
+    for k, (_, _, T, P, _) in enumerate(rows):
+        n = T * P
+        g, r = gpu_so[k], ref_so[k]
+        for f in ("gamma_avg", "alpha_mean", "beta", "mean_s", "std_s"):
+            assert abs(float(g[f]) - getattr(r, f)) <= RTOL * abs(getattr(r, f)) + ATOL, (k, f, float(g[f]), getattr(r, f))
+        near = np.count_nonzero(np.abs(np.asarray(ref_m[r0:r0 + n]) - tau_s) <= 1e-3 * tau_s)
+        assert abs(float(g["rho_spatial"]) - r.rho_spatial) <= near / n + 1e-6, (k, "rho", float(g["rho_spatial"]), r.rho_spatial, near)
+        slack = lambda_spatial * near / n
+        assert abs(float(g["mas"]) - r.mas) <= RTOL * abs(r.mas) + ATOL + slack, (k, "mas", float(g["mas"]), r.mas)
+        assert int(g["n_tokens"]) == n
+        r0 += n

@@ -1,0 +1,271 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances: SPEC.md "Parity rules" (north_star: 1e-3 relative for scores, bit-exact masks / indices
+wherever the oracle score is more than 1e-3 from the cut, bit-exact compacted rows)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import mas_ref as O
+from paper_2604_02945_b200 import synth
+from tests import parity as P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2604_02945_b200 import binding
+    return binding
+
+
+def _dt(B, w):
+    return B.MAS_BF16 if w.dtype == "bf16" else B.MAS_F32
+
+
+def _plan(B, w, **prm):
+    return B.Plan(w.segments, w.q_off, w.d, _dt(B, w), B.default_params(select_mode=w.select_mode, cut=w.cut, **prm))
+
+
+def _oracle_params(w, **prm):
+    return O.default_params(select_mode=w.select_mode, cut=w.cut, **prm)
+
+
+def small_workloads():
+    """Shrunken versions of the five BASELINE.json configs: several 128-row tiles plus ragged tails."""
+    return [
+        synth.single_image(seed=0, d=1024, dtype="f32"),                                    # config 1 at full size
+        synth.single_image(seed=5, d=200, dtype="f32", L=7),                                # fp32, d % 8 != 0
+        synth.batched_images(seed=1, R=5, d=512, L_lo=3, L_hi=70, P=333),                   # ragged tile tails, mixed L
+        synth.video(seed=2, R=2, T=4, P=576, d=256, L=48),
+        synth.video(seed=6, R=2, T=7, P=50, d=264, L=17, static_frac=0.5),                  # P < tile rows, d % 64 != 0
+        synth.audio_vision(seed=3, R=2, d=256, L=64, P_img=576, T_aud=300),
+        synth.ragged(seed=4, R=9, d=128, n_lo=20, n_hi=700, L_lo=1, L_hi=128),
+    ]
+
+
+IDS = ["cfg1_image_f32", "image_f32_d200", "batched_images", "video", "video_smallP", "audio_vision", "ragged_threshold"]
+
+
+@pytest.mark.parametrize("w", small_workloads(), ids=IDS)
+def test_staged_scores(B, w):
+    segs, n = O.make_segments(w.segments)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    s, m = plan.spatial(X)
+    gam = plan.temporal(X)
+    rel, S = plan.crossmodal(X, Q, want_S=True)
+    torch.cuda.synchronize()
+    ref_s = O.rms(segs, w.X)
+    ref_g = O.temporal(segs, w.X)
+    ref_rel, ref_S = O.crossmodal(segs, w.q_off, w.X, w.Q, want_S=True)
+    P.assert_close(s.cpu().numpy(), ref_s, "s")
+    P.assert_close(gam.cpu().numpy(), ref_g, "gamma")
+    assert np.array_equal(gam.cpu().numpy() == 0.0, ref_g == 0.0)          # bit-identical rows give exactly 0.0f
+    P.assert_close(rel.cpu().numpy(), ref_rel, "rel")
+    # raw dot products: error relative to |x||q| (the scale of the accumulation), not to a possibly tiny S_ij
+    Sg = S.cpu().numpy()
+    r0 = 0
+    xn = ref_s * np.sqrt(w.d)
+    for (req, _, T, Pn, _) in w.segments:
+        L = int(w.q_off[req + 1] - w.q_off[req])
+        qseg = O.make_segments([(0, 1, 1, L, 1)])[0]
+        qn = O.rms(qseg, w.Q[w.q_off[req]:w.q_off[req + 1]]) * np.sqrt(w.d)
+        sl = slice(r0, r0 + T * Pn)
+        err = np.abs(Sg[sl, :L] - ref_S[sl, :L])
+        assert np.all(err <= 1e-4 * xn[sl, None] * qn[None, :] + 1e-6), "S"
+        assert np.all(np.isnan(Sg[sl, L:]))                                  # columns >= L untouched
+        r0 += T * Pn
+    m_ref, _, _ = O.fuse(segs, _oracle_params(w), ref_s, ref_g, ref_rel)
+    P.assert_close(m.cpu().numpy(), m_ref, "m_spatial")
+    plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_staged_fuse_and_select_on_shared_scalars(B, mode):
+    """mas_fuse / mas_select_compact in isolation: both sides get the same fp32 scalars, selection must be bit-exact."""
+    rng = np.random.default_rng(40 + mode)
+    rows = [(0, 1, 1, 576, 144), (0, 3, 1500, 1, 600), (1, 2, 5, 300, 225), (2, 1, 1, 1, 1), (3, 2, 33, 555, 2000), (3, 1, 1, 130, 130)]
+    segs, n = O.make_segments(rows)
+    s = (np.abs(rng.standard_normal(n)) + 0.3).astype(np.float32)
+    gam = rng.random(n).astype(np.float32)
+    rel = (0.05 * rng.standard_normal(n)).astype(np.float32)
+    w_d = 64
+    X = rng.standard_normal((n, w_d)).astype(np.float32)
+    plan = B.Plan(rows, [0, 4, 8, 12, 16], w_d, B.MAS_F32, B.default_params(select_mode=mode, cut=0.45))
+    prm = O.default_params(select_mode=mode, cut=0.45)
+    m, mas, so = plan.fuse(torch.from_numpy(s).cuda(), torch.from_numpy(gam).cuda(), torch.from_numpy(rel).cuda())
+    m_ref, mas_ref_, so_ref = O.fuse(segs, prm, s, gam, rel)
+    P.assert_close(m.cpu().numpy(), m_ref, "m_spatial")
+    P.assert_close(mas.cpu().numpy(), mas_ref_, "mas_tok")
+    P.check_seg_out(rows, B.seg_out_numpy(so), so_ref, m_ref)
+    # selection on scores with heavy ties, quantised so that both sides see identical fp32 values
+    vals = (rng.integers(0, 64, n) / 64.0).astype(np.float32)
+    o = plan.select_compact(torch.from_numpy(X).cuda(), torch.from_numpy(vals).cuda())
+    mask_r, idx_r, off_r, Y_r, so_r = O.select_compact(segs, prm, X, vals)
+    off = o["kept_off"].cpu().numpy()
+    assert np.array_equal(off, off_r)
+    assert np.array_equal(o["keep_mask"].cpu().numpy(), mask_r)
+    tot = int(off[-1])
+    assert np.array_equal(o["kept_idx"].cpu().numpy()[:tot], idx_r[:tot])
+    assert np.array_equal(o["Y"].cpu().numpy()[:tot], Y_r[:tot])
+    assert [int(v) for v in B.seg_out_numpy(o["seg_out"])["n_kept"]] == [x.n_kept for x in so_r]
+    plan.close()
+
+
+def _forward_and_compare(B, w, sample_requests=None, **prm):
+    """Run mas_forward on the whole workload; compare the sampled requests (default: all) against the oracle."""
+    plan = _plan(B, w, **prm)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    o = plan.forward(X, Q)
+    torch.cuda.synchronize()
+    host = {k: (v.cpu().numpy() if isinstance(v, torch.Tensor) and k not in ("Y", "seg_out") else v) for k, v in o.items()}
+    so = B.seg_out_numpy(o["seg_out"])
+    seg_req = np.array([s[0] for s in w.segments])
+    seg_rows = np.array([s[2] * s[3] for s in w.segments])
+    seg_row0 = np.concatenate([[0], np.cumsum(seg_rows)])
+    reqs = range(w.n_requests) if sample_requests is None else sample_requests
+    oprm = _oracle_params(w, **prm)
+    for r in reqs:
+        ks = np.nonzero(seg_req == r)[0]
+        rows = [(0,) + tuple(w.segments[k][1:]) for k in ks]
+        lo, hi = int(seg_row0[ks[0]]), int(seg_row0[ks[-1] + 1])
+        segs, n = O.make_segments(rows)
+        ref = O.forward(segs, [0, int(w.q_off[r + 1] - w.q_off[r])], oprm, w.X[lo:hi], w.Q[w.q_off[r]:w.q_off[r + 1]], want_Y=False)
+        for name in ("m_spatial", "gamma", "rel", "mas_tok"):
+            P.assert_close(host[name][lo:hi], ref[name], "%s[req %d]" % (name, r))
+        assert np.array_equal(host["gamma"][lo:hi] == 0.0, ref["gamma"] == 0.0)
+        P.check_seg_out(rows, so[ks[0]:ks[-1] + 1], ref["seg_out"], ref["m_spatial"])
+        off = host["kept_off"][ks[0]:ks[-1] + 2]
+        P.check_selection(rows, w.select_mode, w.cut, ref["mas_tok"], host["keep_mask"][lo:hi], host["kept_idx"], off, row_base=lo)
+    # whole-batch structural properties (hold at any size)
+    total = int(host["kept_off"][-1])
+    assert host["keep_mask"].sum() == total
+    assert np.array_equal(np.nonzero(host["keep_mask"])[0], host["kept_idx"][:total])
+    assert [int(v) for v in so["n_kept"]] == list(np.diff(host["kept_off"]))
+    idx = o["kept_idx"][:total].long()
+    assert torch.equal(o["Y"][:total].view(torch.uint8), X[idx].view(torch.uint8))       # bit-exact compacted rows
+    g = host["gamma"]
+    assert np.all((g >= 0) & (g <= 1 + 1e-6)) and np.all((host["mas_tok"] >= -1e-6) & (host["mas_tok"] <= 1 + 1e-6))
+    plan.close()
+    return host, so
+
+
+@pytest.mark.parametrize("w", small_workloads(), ids=IDS)
+def test_forward_small(B, w):
+    _forward_and_compare(B, w)
+
+
+def test_forward_nondefault_params(B):
+    w = synth.video(seed=8, R=2, T=3, P=200, d=128, L=9)
+    _forward_and_compare(B, w, lambda_spatial=0.3, lambda_temp=0.5, tau_s=0.45, kappa=3.0, spatial_gain=2.0, spatial_bias=-0.5,
+                         rel_gain=0.5, rel_bias=0.25)
+
+
+def test_edge_cases(B):
+    rng = np.random.default_rng(77)
+    d = 64
+    # zero rows, identical rows, a one-token segment, L = 1 and L = 128, minimum d
+    rows = [(0, 2, 3, 4, 5), (1, 1, 1, 1, 1), (2, 3, 6, 1, 2)]
+    n = 12 + 1 + 6
+    X = rng.standard_normal((n, d)).astype(np.float32)
+    X[5] = X[1]            # frame 1 patch 1 identical to frame 0
+    X[6] = 0               # zero row against non-zero previous -> gamma 1
+    X[10] = 0              # zero row, previous (6) also zero -> gamma 0
+    X[14] = X[13]
+    Xb = synth.f32_to_bf16_bits(X)
+    Q = synth.f32_to_bf16_bits(rng.standard_normal((1 + 128 + 2, d)).astype(np.float32))
+    Q[129] = 0             # zero query
+    w = synth.Workload("edge", d, "bf16", rows, np.array([0, 1, 129, 131]), Xb, Q, salient=np.zeros(n, bool))
+    host, so = _forward_and_compare(B, w)
+    assert host["gamma"][5] == 0.0 and host["gamma"][6] == 1.0 and host["gamma"][10] == 0.0 and host["gamma"][14] == 0.0
+    assert host["rel"][6] == 0.0
+    # minimum width d = 8 (bf16) and d = 4... the documented floor is 8
+    w8 = synth.batched_images(seed=12, R=2, d=8, L_lo=2, L_hi=5, P=40)
+    _forward_and_compare(B, w8)
+
+
+def test_threshold_cap_overflow_and_empty_segments(B):
+    w = synth.ragged(seed=14, R=4, d=64, n_lo=100, n_hi=300, L_lo=4, L_hi=9, cut=0.2)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    full = plan.forward(X, Q)
+    total = int(full["kept_off"][-1].item())
+    assert 0 < total < w.n_tokens
+    cap = max(1, total // 2)
+    o = plan.alloc_outputs(cap_rows=cap + 3)
+    o["kept_idx"][cap:] = -7
+    o["Y"][cap:] = 123.0
+    o["cap_rows"] = cap
+    plan.forward(X, Q, out=o)
+    torch.cuda.synchronize()
+    assert int(o["kept_off"][-1].item()) == total                                     # true total still reported
+    assert torch.equal(o["kept_idx"][:cap], full["kept_idx"][:cap])
+    assert torch.all(o["kept_idx"][cap:] == -7) and torch.all(o["Y"][cap:] == 123.0)   # nothing written past the cap
+    plan.close()
+    # a cut below every score keeps nothing anywhere
+    w0 = synth.ragged(seed=14, R=3, d=64, n_lo=100, n_hi=300, L_lo=4, L_hi=9, cut=-1.0)
+    plan = _plan(B, w0)
+    o = plan.forward(B.to_device(w0.X), B.to_device(w0.Q))
+    assert int(o["kept_off"][-1].item()) == 0 and int(o["keep_mask"].sum().item()) == 0
+    plan.close()
+
+
+def test_invariances_on_gpu(B):
+    w = synth.video(seed=31, R=2, T=4, P=150, d=128, L=12)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    a = plan.forward(X, Q)
+    b = plan.forward(X, Q)                                                            # bit-reproducible
+    for k in ("m_spatial", "gamma", "rel", "mas_tok", "keep_mask", "kept_idx", "kept_off", "seg_out", "Y"):
+        assert torch.equal(a[k].view(torch.uint8), b[k].view(torch.uint8)), k
+    c = plan.forward(X * 4.0, Q * 0.25)                                               # power-of-two scaling
+    for k in ("m_spatial", "gamma", "rel", "mas_tok"):
+        P.assert_close(c[k].cpu().numpy(), a[k].cpu().numpy(), k)
+    assert torch.equal(a["keep_mask"], c["keep_mask"])
+    perm = torch.cat([torch.randperm(12), 12 + torch.randperm(12)]).cuda()            # query order is irrelevant
+    e = plan.forward(X, Q[perm])
+    P.assert_close(e["rel"].cpu().numpy(), a["rel"].cpu().numpy(), "rel under query permutation")
+    plan.close()
+
+
+def test_forward_host_matches_device_path(B):
+    w = synth.batched_images(seed=33, R=3, d=256, L_lo=5, L_hi=20)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    dev = plan.forward(X, Q)
+    hX = torch.from_numpy(w.X).view(torch.bfloat16).pin_memory()
+    hQ = torch.from_numpy(w.Q).view(torch.bfloat16).pin_memory()
+    dX, dQ = torch.empty_like(X), torch.empty_like(Q)
+    d_out = plan.alloc_outputs()
+    h_out = {k: (torch.zeros_like(v, device="cpu").pin_memory() if isinstance(v, torch.Tensor) else v) for k, v in d_out.items()}
+    plan.forward_host(hX, hQ, dX, dQ, d_out, h_out)
+    for k in ("m_spatial", "gamma", "rel", "mas_tok", "keep_mask", "kept_idx", "kept_off", "seg_out", "Y"):
+        assert torch.equal(h_out[k].view(torch.uint8), dev[k].cpu().view(torch.uint8)), k
+    plan.close()
+
+
+def test_unsupported_inputs_fail_loudly(B):
+    w = synth.batched_images(seed=34, R=1, d=64, L_lo=4, L_hi=4, P=32)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    Xmis = torch.empty(w.n_tokens * 64 + 8, dtype=torch.bfloat16, device="cuda")[1:1 + w.n_tokens * 64].view(w.n_tokens, 64)
+    with pytest.raises(B.MasError) as ei:
+        plan.forward(Xmis, Q)
+    assert ei.value.status == B.MAS_ERR_UNSUPPORTED
+    o = plan.alloc_outputs()
+    o["kept_idx"] = None
+    with pytest.raises(B.MasError):
+        plan.forward(X, Q, out=o)                                                     # Y without kept_idx
+    plan.close()
+
+
+# ---------------------------------------------------------------- full BASELINE.json sizes, bench launch configuration
+FULL = [("batched_images", {}, [0, 31, 63]), ("video", {}, [5]), ("audio_vision", {}, [7]), ("ragged", {}, [3, 100, 255])]
+
+
+@pytest.mark.parametrize("name,kw,sample", FULL, ids=[f[0] for f in FULL])
+def test_forward_full_size_sampled(B, name, kw, sample):
+    w = synth.make(name, **kw)
+    _forward_and_compare(B, w, sample_requests=sample)
