@@ -333,7 +333,7 @@ static int launch_select_tail(const mas_plan* p, const void* X, const uint8_t* m
 extern "C" int32_t mas_plan_forward_launches(const mas_plan* p) {
   if (!p) return -1;
   // [qprep +] score + segment (+ index compaction in threshold mode) + gather
-  return (p->tc.enabled ? 3 : 4) + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
+  return 4 + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
 }
 
 // ------------------------------------------------------------------------------------------------ staged entry points
@@ -412,7 +412,8 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   if (pev) CK(cudaEventRecord(pev[0], st));
   int rc;
   if (p->tc.enabled) {
-    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->N, p->nQ, p->d, st);   // a0-a3 in one kernel
+    if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
+    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->N, p->nQ, p->d, st);   // a1-a3: TMA + tcgen05
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else {
     if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
