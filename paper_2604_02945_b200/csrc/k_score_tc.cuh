@@ -6,10 +6,12 @@
 //   query chunk Q[L, kc] into a multi-stage shared-memory ring.
 //   One elected thread issues tcgen05.mma (kind::f16, bf16 x bf16 -> fp32, M = 128, N = pad16(L), K = 16) accumulating
 //   S = X·Q^T in TMEM (two accumulators: the epilogue of tile i overlaps the MMAs of tile i+1).          (Eq. 6)
-//   Eight CUDA-core warps read the same shared-memory tiles (conflict-free thanks to the hardware swizzle) and
-//   accumulate sum x^2, sum (x - x_prev)^2, sum x_prev^2 in fp32.                                        (Eq. 3, Eq. 5)
+//   Sixteen CUDA-core warps (four threads per token row) read the same shared-memory tiles — conflict-free thanks to
+//   the hardware swizzle — and accumulate sum x^2 and sum (x - x_prev)^2 with packed fp32x2 FMAs.    (Eq. 3, Eq. 5)
 //   Four epilogue warps read the accumulator rows with tcgen05.ld (one token row per thread, so the max over query
-//   tokens needs no shuffles), scale by 1/|q_j| and 1/|x_i| and write s, gamma, rel: 12 B per token.
+//   tokens needs no shuffles), scale by 1/|q_j| and 1/|x_i| and write s, sqrt(D), rel: 12 B per token.
+//   The temporal ratio gamma = sqrt(D) / (|x_t| + |x_{t-1}|) is finished by the segment kernel, which has both norms
+//   from s; the previous row's norm is therefore never recomputed here.
 //
 // Persistent: one CTA per SM walks a host-built, cost-balanced (LPT) tile list.  Tiles never straddle a segment.
 #pragma once
@@ -17,6 +19,8 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <queue>
 #include <vector>
@@ -28,24 +32,24 @@ namespace msas {
 
 struct TcTile {            // 32 bytes
   int32_t row_start;       // global row id of the first row
-  int32_t n_rows;          // valid rows, <= box rows
-  int32_t box_kind;        // 0: 128-row TMA box, 1: 64, 2: 32, 3: 16
+  int32_t n_rows;          // valid rows, 1..128
   int32_t q_row0;          // first query row of the request
   int32_t L;               // query tokens of the request
   int32_t prev_delta;      // P if the segment is temporal (T > 1), else 0
-  int32_t key_rows;        // leading rows of the tile that belong to frame 0 (gamma = 1)
-  int32_t pad_;
+  int32_t key_rows;        // leading rows of the tile that belong to frame 0 (no previous frame)
+  int32_t pad_[2];
 };
 
-constexpr int kTcThreads = 512;
-constexpr int kTcMaxStages = 10;
-constexpr int kTcBoxBytes = 128 * 128;    // 128 rows x 64 bf16 columns
+constexpr int kTcAluWarps = 4;                       // one token row per thread
+constexpr int kTcThreads = 256 + 32 * kTcAluWarps;   // warps 0-7: TMA (X), MMA, TMEM, TMA (Q), 4 x epilogue; then the ALU warps
+constexpr int kTcSlots = 16;                         // mbarrier pairs of the chunk ring (slots are variable-sized)
+constexpr int kTcBoxBytes = 128 * 128;               // 128 rows x 64 bf16 columns
+constexpr int kTcCtrlBytes = 4096;
+constexpr int kTcRingBytes = (227 * 1024 - kTcCtrlBytes - 1024 - kTcBoxBytes) & ~1023;   // 1 KB alignment slack, 16 KB MMA over-read pad
 
 struct TcSchedule {
   bool enabled = false;
-  bool any_temporal = false;
-  int n_ctas = 0, n_tiles = 0, stages = 0, lmax_pad = 16;
-  int stage_bytes = 0, smem_bytes = 0;
+  int n_ctas = 0, n_tiles = 0, smem_bytes = 0;
   const TcTile* d_tiles = nullptr;
   const int32_t* d_cta_off = nullptr;
 };
@@ -55,15 +59,57 @@ struct TcParams {
   const int32_t* cta_off;
   const float* qinv;
   float* s;
-  float* gamma;
+  float* dnorm;       // sqrt(sum (x - x_prev)^2) for rows that have a previous frame
   float* rel;
   int d;
   int n_kchunks;
-  int stages;
-  int stage_bytes;
-  int prev_off;       // byte offset of the previous-frame tile inside a stage (0 = no such region)
-  int q_off;          // byte offset of the query chunk inside a stage
+#ifdef MSAS_ABLATE
+  int dbg;            // development only: bit0 no ALU math, bit1 no MMA, bit2 no Q loads, bit3 no prev loads
+  unsigned long long* dbg_t;
+#endif
 };
+
+// The chunk ring.  One chunk = one 64-column K-slice of a tile: [x rows16 x 128 B][previous-frame rows, same size,
+// temporal tiles only][query rows pad16(L) x 128 B].  Chunks are packed back to back in a circular byte buffer, so a
+// short tile (few rows) still leaves the same number of BYTES in flight; every role replays the same deterministic
+// offset sequence from the tile list, only the producer tracks which bytes are still in use.
+struct TcRing {
+  uint32_t off = 0;     // physical byte offset of the next chunk
+  uint32_t vhead = 0;   // virtual offset of the next chunk (monotonic mod 2^32, counts wrap padding): only differences are used
+  uint32_t k = 0;       // chunk counter -> barrier slot k % kTcSlots, parity (k / kTcSlots) & 1
+  __device__ __forceinline__ uint32_t place(uint32_t need) {   // physical offset of the next chunk; advances the ring
+    if (off + need > (uint32_t)kTcRingBytes) { vhead += (uint32_t)kTcRingBytes - off; off = 0; }
+    const uint32_t r = off;
+    off += need; vhead += need;
+    return r;
+  }
+  __device__ __forceinline__ uint32_t slot() const { return k % (uint32_t)kTcSlots; }
+  __device__ __forceinline__ uint32_t parity() const { return (k / (uint32_t)kTcSlots) & 1u; }
+};
+// Geometry of one tile's chunks.  A chunk carries kw consecutive 64-column K-slices so that it holds about 16 KB of
+// token rows whatever the tile height (128 rows x 1 slice ... 16 rows x 8 slices): per-chunk costs (barrier round
+// trip, producer instructions) are then paid per byte, not per row.  Layout of a chunk:
+//   [kw x token slice (xbytes each)] [kw x previous-frame slice, temporal tiles only] [kw x query slice (qbytes each)]
+struct TcGeom {
+  uint32_t xbytes, xall, qbytes, need;
+  int kw, nch, nqb;
+  bool has_prev;
+};
+__device__ __forceinline__ TcGeom tc_geom(const TcTile& t, int nk, int dbg) {
+  TcGeom g;
+  const int rows16 = (t.n_rows + 15) & ~15;
+  g.xbytes = (uint32_t)rows16 * 128u;
+  g.has_prev = t.prev_delta > 0 && t.key_rows < t.n_rows && !(dbg & 8);
+  g.nqb = (dbg & 4) ? 0 : (t.L + 15) >> 4;
+  int kw = rows16 <= 16 ? 8 : rows16 <= 32 ? 4 : rows16 <= 64 ? 2 : 1;
+  while (kw > 1 && (kw * g.nqb > 16 || nk % kw != 0)) kw >>= 1;   // <= 32 KB of query rows per chunk; kw divides d / 64
+  g.kw = kw;
+  g.nch = nk / kw;
+  g.xall = g.xbytes * (g.has_prev ? 2u : 1u);
+  g.qbytes = (uint32_t)g.nqb * 2048u;
+  g.need = (uint32_t)kw * (g.xall + g.qbytes);
+  return g;
+}
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -118,6 +164,26 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16]) {
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// packed fp32 pairs (Blackwell FFMA2 / FADD2): two lanes of fp32 per 64-bit register
+__device__ __forceinline__ uint64_t bf16x2_to_f32x2(uint32_t w) {   // exact: low half -> .x, high half -> .y
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(w << 16), "r"(w & 0xffff0000u));
+  return r;
+}
+__device__ __forceinline__ uint64_t sub_f32x2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ void fma_sq_f32x2(uint64_t& acc, uint64_t a) {   // acc += a * a (per lane)
+  asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(acc) : "l"(a));
+}
+__device__ __forceinline__ float sum_f32x2(uint64_t a) {
+  float lo, hi;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+  return lo + hi;
+}
+
 // shared-memory matrix descriptor: K-major, SWIZZLE_128B, 8-row groups 1024 B apart (sm_100 descriptor version 1)
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
   const uint32_t lo = ((saddr & 0x3FFFFu) >> 4) | (1u << 16);             // start address | LBO (unused for swizzled K-major)
@@ -129,39 +195,48 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
 }
 
+
 // ------------------------------------------------------------------------------------------------ the kernel
 struct TcCtrl {                      // lives at the (1024-aligned) start of dynamic shared memory
-  uint64_t full[kTcMaxStages];       // TMA -> consumers           (1 arrival + transaction bytes)
-  uint64_t empty[kTcMaxStages];      // consumers -> TMA           (1 MMA commit + 8 ALU warps)
+  uint64_t full[kTcSlots];           // TMA -> consumers           (1 arrival + transaction bytes)
+  uint64_t empty[kTcSlots];          // consumers -> TMA           (1 MMA commit + the ALU warps)
   uint64_t tmem_full[2];             // MMA -> epilogue            (1 commit)
   uint64_t tmem_empty[2];            // epilogue -> MMA            (4 warps)
-  uint64_t stat_full[2];             // ALU -> epilogue            (8 warps)
+  uint64_t stat_full[2];             // ALU -> epilogue            (ALU warps)
   uint64_t stat_empty[2];            // epilogue -> ALU            (4 warps)
   uint32_t tmem_base;
+  uint32_t vstart[kTcSlots];         // X producer only: virtual start offset of the chunk in each barrier slot
+  uint32_t vstart_q[kTcSlots];       // Q producer only: its own copy
   uint32_t pad_[31];
-  float rowstat[2][3][128];          // n2, D, n2_prev per tile row, double buffered
+  float rowstat[2][2][128];          // partial sum x^2, sum (x - x_prev)^2 per (K-slice, tile row), double buffered
 };
-constexpr int kTcCtrlBytes = 4096;
 static_assert(sizeof(TcCtrl) <= kTcCtrlBytes, "control block too large");
-
-__device__ __forceinline__ int tc_box_rows(int kind) { return 128 >> kind; }
 
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CUtensorMap mx64, const __grid_constant__ CUtensorMap mx32,
-           const __grid_constant__ CUtensorMap mx16, const __grid_constant__ CUtensorMap mq, const TcParams p) {
+           const __grid_constant__ CUtensorMap mx16, const __grid_constant__ CUtensorMap mq64, const __grid_constant__ CUtensorMap mq32,
+           const __grid_constant__ CUtensorMap mq16, const TcParams p) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   TcCtrl* ctrl = reinterpret_cast<TcCtrl*>(smem);
-  unsigned char* stage0 = smem + kTcCtrlBytes;
+  unsigned char* ring0 = smem + kTcCtrlBytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int tile_lo = p.cta_off[blockIdx.x], tile_hi = p.cta_off[blockIdx.x + 1];
-  const int S = p.stages, nk = p.n_kchunks;
+  const int nk = p.n_kchunks;
+#ifdef MSAS_ABLATE
+  const int dbg = p.dbg;
+  auto gtime = [] { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; };
+  if (tid == 0 && p.dbg_t) { p.dbg_t[blockIdx.x * 8 + 0] = gtime(); unsigned sm; asm volatile("mov.u32 %0, %smid;" : "=r"(sm)); p.dbg_t[blockIdx.x * 8 + 1] = sm; }
+#else
+  constexpr int dbg = 0;
+#endif
 
+  pdl_launch_dependents();   // the segment kernel may be scheduled as SMs free up; it waits for this grid to complete
   if (warp == 1 && lane == 0) {
-    for (int i = 0; i < S; ++i) { mbar_init(smem_u32(&ctrl->full[i]), 1); mbar_init(smem_u32(&ctrl->empty[i]), 9); }
+    for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), 2); mbar_init(smem_u32(&ctrl->empty[i]), 1 + kTcAluWarps); }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&ctrl->tmem_full[i]), 1); mbar_init(smem_u32(&ctrl->tmem_empty[i]), 4);
-      mbar_init(smem_u32(&ctrl->stat_full[i]), 8); mbar_init(smem_u32(&ctrl->stat_empty[i]), 4);
+      mbar_init(smem_u32(&ctrl->stat_full[i]), kTcAluWarps); mbar_init(smem_u32(&ctrl->stat_empty[i]), 4);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -171,62 +246,123 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
   }
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&mx128) : "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&mx64) : "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&mq) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&mq64) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&mq16) : "memory");
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = ctrl->tmem_base;
 
-  if (warp == 0) {
-    // ===================================================================== TMA producer (one thread)
+  if (warp == 0 || warp == 3) {
+    // ===================================================================== TMA producers (one thread each)
+    // warp 0 streams the token rows (and the previous-frame rows), warp 3 the query rows.  A single thread issues about
+    // one instruction every few cycles, so the per-chunk loop is kept to a few dozen instructions per producer.
     if (lane == 0) {
-      int stage = 0; uint32_t phase = 0;
+      const bool xprod = warp == 0;
+      TcRing ring;
+#ifdef MSAS_ABLATE
+      long long wait_clk = 0; const long long cstart = clock64();
+#endif
+      uint32_t rel = 0;                    // oldest chunk not yet known to be released
+      uint32_t v_oldest = 0;               // virtual start offset of chunk `rel` (valid while rel < ring.k)
+      uint32_t* vstart = xprod ? ctrl->vstart : ctrl->vstart_q;     // virtual start offset of chunk j, at j % kTcSlots
       for (int t = tile_lo; t < tile_hi; ++t) {
         const TcTile tile = p.tiles[t];
-        const CUtensorMap* mx = tile.box_kind == 0 ? &mx128 : tile.box_kind == 1 ? &mx64 : tile.box_kind == 2 ? &mx32 : &mx16;
-        const bool has_prev = tile.prev_delta > 0 && tile.key_rows < tile.n_rows;
-        const int nqb = (tile.L + 15) >> 4;
-        const uint32_t box_bytes = (uint32_t)tc_box_rows(tile.box_kind) * 128u;
-        const uint32_t tx = box_bytes * (has_prev ? 2u : 1u) + (uint32_t)nqb * 2048u;
-        for (int kc = 0; kc < nk; ++kc) {
-          mbar_wait(smem_u32(&ctrl->empty[stage]), phase ^ 1u);
-          const uint32_t bar = smem_u32(&ctrl->full[stage]);
-          unsigned char* st = stage0 + (size_t)stage * p.stage_bytes;
-          mbar_expect_tx(bar, tx);
-          tma_load_2d(smem_u32(st), mx, bar, kc * 64, tile.row_start);
-          if (has_prev) tma_load_2d(smem_u32(st + p.prev_off), mx, bar, kc * 64, tile.row_start - tile.prev_delta);
-          for (int j = 0; j < nqb; ++j) tma_load_2d(smem_u32(st + p.q_off + j * 2048), &mq, bar, kc * 64, tile.q_row0 + 16 * j);
-          if (++stage == S) { stage = 0; phase ^= 1u; }
+        const TcGeom g = tc_geom(tile, nk, dbg);
+        const int r16 = (int)(g.xbytes >> 11);                      // 16-row groups: 8 -> one 128-row box, else its bits
+        const int row = tile.row_start, prow = tile.row_start - tile.prev_delta;
+        const uint32_t poff = (uint32_t)g.kw * g.xbytes;            // previous-frame slices follow the token slices
+        for (int ch = 0; ch < g.nch; ++ch) {
+          const uint32_t off = ring.place(g.need);
+          const uint32_t vbeg = ring.vhead - g.need;
+          // wait until the barrier slot is free and the bytes [vbeg, vbeg + need) no longer overlap an unreleased chunk
+          while (rel < ring.k && (ring.k - rel >= (uint32_t)kTcSlots || ring.vhead - v_oldest > (uint32_t)kTcRingBytes)) {
+#ifdef MSAS_ABLATE
+            const long long c0 = clock64();
+#endif
+            mbar_wait(smem_u32(&ctrl->empty[rel % kTcSlots]), (rel / kTcSlots) & 1u);
+#ifdef MSAS_ABLATE
+            wait_clk += clock64() - c0;
+#endif
+            ++rel;
+            v_oldest = vstart[rel % kTcSlots];
+          }
+          vstart[ring.slot()] = vbeg;
+          if (rel == ring.k) v_oldest = vbeg;
+          const uint32_t bar = smem_u32(&ctrl->full[ring.slot()]);
+          const uint32_t base = smem_u32(ring0 + off);
+          if (xprod) {
+            mbar_expect_tx(bar, (uint32_t)g.kw * g.xall);
+            for (int j = 0; j < g.kw; ++j) {
+              const int c0 = (ch * g.kw + j) * 64;
+              const uint32_t dst = base + (uint32_t)j * g.xbytes;
+              if (r16 == 8) {
+                tma_load_2d(dst, &mx128, bar, c0, row);
+                if (g.has_prev) tma_load_2d(dst + poff, &mx128, bar, c0, prow);
+              } else {   // rows past the end of X are zero-filled by the TMA unit
+                int o = 0;
+                if (r16 & 4) { tma_load_2d(dst, &mx64, bar, c0, row); if (g.has_prev) tma_load_2d(dst + poff, &mx64, bar, c0, prow); o = 64; }
+                if (r16 & 2) {
+                  tma_load_2d(dst + o * 128, &mx32, bar, c0, row + o);
+                  if (g.has_prev) tma_load_2d(dst + poff + o * 128, &mx32, bar, c0, prow + o);
+                  o += 32;
+                }
+                if (r16 & 1) {
+                  tma_load_2d(dst + o * 128, &mx16, bar, c0, row + o);
+                  if (g.has_prev) tma_load_2d(dst + poff + o * 128, &mx16, bar, c0, prow + o);
+                }
+              }
+            }
+          } else {
+            mbar_expect_tx(bar, (uint32_t)g.kw * g.qbytes);
+            uint32_t sq = base + (uint32_t)g.kw * g.xall;
+            for (int j = 0; j < g.kw; ++j) {
+              const int c0 = (ch * g.kw + j) * 64;
+              int qr = tile.q_row0;
+              for (int i = 0; i < (g.nqb >> 2); ++i) { tma_load_2d(sq, &mq64, bar, c0, qr); sq += 8192; qr += 64; }
+              if (g.nqb & 2) { tma_load_2d(sq, &mq32, bar, c0, qr); sq += 4096; qr += 32; }
+              if (g.nqb & 1) { tma_load_2d(sq, &mq16, bar, c0, qr); sq += 2048; }
+            }
+          }
+          ++ring.k;
         }
       }
+#ifdef MSAS_ABLATE
+      if (p.dbg_t && xprod) { p.dbg_t[blockIdx.x * 8 + 4] = wait_clk; p.dbg_t[blockIdx.x * 8 + 7] = clock64() - cstart; }
+#endif
     }
   } else if (warp == 1) {
     // ===================================================================== MMA issuer (one thread)
     if (lane == 0) {
-      int stage = 0; uint32_t phase = 0;
+      TcRing ring;
       int it = 0;
       for (int t = tile_lo; t < tile_hi; ++t, ++it) {
-        const int L = p.tiles[t].L;
-        const int npad = ((L + 15) >> 4) << 4;
-        const uint32_t idesc = umma_idesc_bf16(npad);
+        const TcTile tile = p.tiles[t];
+        const TcGeom g = tc_geom(tile, nk, dbg);
+        const uint32_t idesc = umma_idesc_bf16(((tile.L + 15) >> 4) << 4);
         const int acc = it & 1;
         const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
         mbar_wait(smem_u32(&ctrl->tmem_empty[acc]), acc_phase ^ 1u);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)acc * 128u;
-        for (int kc = 0; kc < nk; ++kc) {
-          mbar_wait(smem_u32(&ctrl->full[stage]), phase);
+        for (int ch = 0; ch < g.nch; ++ch) {
+          const uint32_t off = ring.place(g.need);
+          mbar_wait(smem_u32(&ctrl->full[ring.slot()]), ring.parity());
           tc_fence_after();
-          unsigned char* st = stage0 + (size_t)stage * p.stage_bytes;
-          const uint64_t adesc = umma_desc_sw128(smem_u32(st));
-          const uint64_t bdesc = umma_desc_sw128(smem_u32(st + p.q_off));
+          const uint32_t base = smem_u32(ring0 + off);
+          if (!(dbg & 2)) {
+            for (int j = 0; j < g.kw; ++j) {
+              // M = 128: rows past the tile read whatever follows in the ring (their accumulator rows are never used)
+              const uint64_t adesc = umma_desc_sw128(base + (uint32_t)j * g.xbytes);
+              const uint64_t bdesc = umma_desc_sw128(base + (uint32_t)g.kw * g.xall + (uint32_t)j * g.qbytes);
 #pragma unroll
-          for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
-            tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(kc | k));
-          tc_commit(smem_u32(&ctrl->empty[stage]));
-          if (++stage == S) { stage = 0; phase ^= 1u; }
+              for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
+                tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(ch | j | k));
+            }
+          }
+          tc_commit(smem_u32(&ctrl->empty[ring.slot()]));
+          ++ring.k;
         }
         tc_commit(smem_u32(&ctrl->tmem_full[acc]));
       }
@@ -235,9 +371,12 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
     // ===================================================================== epilogue: one accumulator row per thread
     const int q = warp - 4;                  // TMEM lane quarter this warp may access (warp % 4)
     const int r = q * 32 + lane;             // tile row
+    const float inv_d = 1.0f / (float)p.d;
+    pdl_wait();                              // qinv comes from the query-prep kernel launched just before this one
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
+      const TcGeom g = tc_geom(tile, nk, dbg);
       const int acc = it & 1;
       const uint32_t ph = (uint32_t)(it >> 1) & 1u;
       const int nqb = (tile.L + 15) >> 4;
@@ -259,81 +398,98 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->tmem_empty[acc]));
       mbar_wait(smem_u32(&ctrl->stat_full[acc]), ph);
-      const float n2 = ctrl->rowstat[acc][0][r], D = ctrl->rowstat[acc][1][r], n2p = ctrl->rowstat[acc][2][r];
+      float n2 = 0.f, D = 0.f;               // the ALU threads hold one partial per (row, K-slice of the chunk)
+      if (r < tile.n_rows) {
+        const int rp2 = 128 / g.kw;
+        for (int j = 0; j < g.kw; ++j) { n2 += ctrl->rowstat[acc][0][r + j * rp2]; D += ctrl->rowstat[acc][1][r + j * rp2]; }
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_empty[acc]));
       if (r < tile.n_rows) {
         const int64_t row = (int64_t)tile.row_start + r;
-        p.s[row] = sqrtf(n2 / (float)p.d);
-        float g = 0.f;
-        if (tile.prev_delta > 0) {
-          if (r < tile.key_rows) g = 1.0f;
-          else { const float den = sqrtf(n2) + sqrtf(n2p); g = den > 0.f ? sqrtf(D) / den : 0.f; }
-        }
-        p.gamma[row] = g;
+        p.s[row] = sqrtf(n2 * inv_d);
+        p.dnorm[row] = sqrtf(D);
         p.rel[row] = n2 > 0.f ? m / sqrtf(n2) : 0.f;
       }
     }
   } else if (warp >= 8) {
-    // ===================================================================== CUDA-core statistics: two threads per tile row
+    // ===================================================================== CUDA-core statistics: one thread per (row, K-slice)
     const int a = tid - 256;
-    const int r = a >> 1, half = a & 1;
-    int stage = 0; uint32_t phase = 0;
+    TcRing ring;
+#ifdef MSAS_ABLATE
+    long long alu_wait = 0;
+#endif
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
-      const bool has_prev = tile.prev_delta > 0 && tile.key_rows < tile.n_rows;
-      const bool active = r < tc_box_rows(tile.box_kind);
-      float n2a = 0.f, n2b = 0.f, Da = 0.f, Db = 0.f, pa = 0.f, pb = 0.f;
-      const uint32_t row_off = (uint32_t)r * 128u;
-      for (int kc = 0; kc < nk; ++kc) {
-        mbar_wait(smem_u32(&ctrl->full[stage]), phase);
+      const TcGeom g = tc_geom(tile, nk, dbg);
+      const int rp2 = 128 / g.kw;
+      const int r = a & (rp2 - 1), j = a / rp2;
+      const bool active = r < tile.n_rows && !(dbg & 1);
+      // hardware 128-byte swizzle: 16-byte unit u of row r sits at unit u ^ (r & 7)
+      const uint32_t my_off = (uint32_t)j * g.xbytes + (uint32_t)r * 128u;
+      const uint32_t sw = (uint32_t)(r & 7);
+      const uint32_t poff = (uint32_t)g.kw * g.xbytes;
+      uint64_t n2a = 0, n2b = 0, Da = 0, Db = 0;     // packed fp32 pairs, all zero bits = (0.f, 0.f)
+      for (int ch = 0; ch < g.nch; ++ch) {
+        const uint32_t off = ring.place(g.need);
+#ifdef MSAS_ABLATE
+        const long long c0 = clock64();
+#endif
+        mbar_wait(smem_u32(&ctrl->full[ring.slot()]), ring.parity());
+#ifdef MSAS_ABLATE
+        alu_wait += clock64() - c0;
+        if (tid == 256 && p.dbg_t && t == tile_lo && ch == 0) p.dbg_t[blockIdx.x * 8 + 2] = gtime();
+#endif
         if (active) {
-          const unsigned char* st = stage0 + (size_t)stage * p.stage_bytes;
+          const unsigned char* sx = ring0 + off + my_off;
+          uint4 x[8];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const uint32_t off = row_off + ((uint32_t)((half * 4 + j) ^ (r & 7)) << 4);   // hardware 128-byte swizzle
-            const uint4 x = *reinterpret_cast<const uint4*>(st + off);
-            const uint32_t xw[4] = {x.x, x.y, x.z, x.w};
-            if (has_prev) {
-              const uint4 u = *reinterpret_cast<const uint4*>(st + p.prev_off + off);
-              const uint32_t uw[4] = {u.x, u.y, u.z, u.w};
+          for (int u = 0; u < 8; ++u) x[u] = *reinterpret_cast<const uint4*>(sx + (((uint32_t)u ^ sw) << 4));
+          if (g.has_prev) {
+            const unsigned char* su = sx + poff;
+            uint4 v[8];
 #pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const float x0 = bf_lo(xw[k]), x1 = bf_hi(xw[k]), u0 = bf_lo(uw[k]), u1 = bf_hi(uw[k]);
-                n2a = fmaf(x0, x0, n2a); n2b = fmaf(x1, x1, n2b);
-                pa = fmaf(u0, u0, pa); pb = fmaf(u1, u1, pb);
-                const float e0 = x0 - u0, e1 = x1 - u1;
-                Da = fmaf(e0, e0, Da); Db = fmaf(e1, e1, Db);
-              }
-            } else {
+            for (int u = 0; u < 8; ++u) v[u] = *reinterpret_cast<const uint4*>(su + (((uint32_t)u ^ sw) << 4));
 #pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const float x0 = bf_lo(xw[k]), x1 = bf_hi(xw[k]);
-                n2a = fmaf(x0, x0, n2a); n2b = fmaf(x1, x1, n2b);
-              }
+            for (int u = 0; u < 8; ++u) {
+              const uint64_t x0 = bf16x2_to_f32x2(x[u].x), x1 = bf16x2_to_f32x2(x[u].y), x2 = bf16x2_to_f32x2(x[u].z), x3 = bf16x2_to_f32x2(x[u].w);
+              const uint64_t e0 = sub_f32x2(x0, bf16x2_to_f32x2(v[u].x)), e1 = sub_f32x2(x1, bf16x2_to_f32x2(v[u].y));
+              const uint64_t e2 = sub_f32x2(x2, bf16x2_to_f32x2(v[u].z)), e3 = sub_f32x2(x3, bf16x2_to_f32x2(v[u].w));
+              fma_sq_f32x2(n2a, x0); fma_sq_f32x2(n2b, x1); fma_sq_f32x2(n2a, x2); fma_sq_f32x2(n2b, x3);
+              fma_sq_f32x2(Da, e0); fma_sq_f32x2(Db, e1); fma_sq_f32x2(Da, e2); fma_sq_f32x2(Db, e3);
+            }
+          } else {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].x)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].y));
+              fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].z)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].w));
             }
           }
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctrl->empty[stage]));
-        if (++stage == S) { stage = 0; phase ^= 1u; }
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl->empty[ring.slot()]));
+        ++ring.k;
       }
-      float n2 = n2a + n2b, D = Da + Db, n2p = pa + pb;
-      n2 += __shfl_xor_sync(0xffffffffu, n2, 1);
-      D += __shfl_xor_sync(0xffffffffu, D, 1);
-      n2p += __shfl_xor_sync(0xffffffffu, n2p, 1);
+      const float n2 = sum_f32x2(n2a) + sum_f32x2(n2b);
+      const float D = sum_f32x2(Da) + sum_f32x2(Db);
       const int buf = it & 1;
       const uint32_t ph = (uint32_t)(it >> 1) & 1u;
       mbar_wait(smem_u32(&ctrl->stat_empty[buf]), ph ^ 1u);
-      if (half == 0) { ctrl->rowstat[buf][0][r] = n2; ctrl->rowstat[buf][1][r] = D; ctrl->rowstat[buf][2][r] = n2p; }
+      ctrl->rowstat[buf][0][a] = n2; ctrl->rowstat[buf][1][a] = D;      // slot a = j * rp2 + r
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_full[buf]));
     }
+#ifdef MSAS_ABLATE
+    if (tid == 256 && p.dbg_t) p.dbg_t[blockIdx.x * 8 + 6] = alu_wait;
+#endif
   }
 
   tc_fence_before();
   __syncthreads();
+#ifdef MSAS_ABLATE
+  if (tid == 0 && p.dbg_t) p.dbg_t[blockIdx.x * 8 + 3] = gtime();
+#endif
   if (warp == 2) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(256) : "memory");
@@ -341,16 +497,27 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
 }
 
 // ------------------------------------------------------------------------------------------------ host side
-// Tile decomposition of one segment: greedy TMA boxes of 128/64/32/16 rows (a last partial box of <16 valid rows).
-inline int tc_count_tiles(int64_t n) {
-  int c = 0;
-  while (n >= 128) { n -= 128; ++c; }
-  for (int b = 64; b >= 16; b >>= 1) if (n >= b) { n -= b; ++c; }
-  return c + (n > 0 ? 1 : 0);
-}
+// Schedule.  Cost of a tile = bytes it pulls into the SM in units of 128-byte rows: rows16 from HBM, the previous-frame
+// rows and the query rows from L2 at a fraction of that.  Two phases:
+//   bulk: 128-row tiles dealt round-robin in row order, as many complete rounds as fit under the per-CTA target
+//         (neighbouring CTAs sweep neighbouring rows at the same time, so previous-frame tiles are still in L2);
+//   fill: the remaining rows are cut into tiles sized to each CTA's remaining gap (largest gap first, multiples of 16
+//         rows, at least 32 unless a segment ends), which levels the CTAs to about one 16-row box.
+// Short tiles keep the same bytes in flight (variable-size chunk ring) but re-stream the query chunks more often,
+// which is why only the fill phase uses them.
+struct TcCost {
+  double w_prev = 0.12, w_q = 0.20, c_tile = 2.0;
+  TcCost() {
+#ifdef MSAS_ABLATE
+    if (getenv("MSAS_WPREV")) w_prev = atof(getenv("MSAS_WPREV"));
+    if (getenv("MSAS_WQ")) w_q = atof(getenv("MSAS_WQ"));
+    if (getenv("MSAS_CTILE")) c_tile = atof(getenv("MSAS_CTILE"));
+#endif
+  }
+};
 inline size_t tc_schedule_bytes(const mas_segment* segs, int32_t n_segs) {
-  size_t tiles = 0;
-  for (int32_t k = 0; k < n_segs; ++k) tiles += (size_t)tc_count_tiles((int64_t)segs[k].n_frames * segs[k].n_patches);
+  size_t tiles = 0;   // upper bound: every segment in 32-row tiles plus one remainder each
+  for (int32_t k = 0; k < n_segs; ++k) tiles += (size_t)(((int64_t)segs[k].n_frames * segs[k].n_patches + 31) / 32) + 1;
   return tiles * sizeof(TcTile) + 1024 * sizeof(int32_t) + 256;
 }
 
@@ -359,70 +526,104 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
                               int sm_count, char* h_dst, char* d_dst) {
   sc = TcSchedule();
   if (dtype != MAS_BF16 || d % 64 != 0 || sm_count < 1 || sm_count > 1000) return;
-  std::vector<TcTile> tiles;
-  int lmax = 1;
-  bool any_temporal = false;
+  const TcCost cw;
+  struct SegInfo { double w_row, c_fix; int L, P; };
+  std::vector<SegInfo> si(n_segs);
+  double total = 0.0;
+  int64_t n_full = 0;
   for (int32_t k = 0; k < n_segs; ++k) {
     const mas_segment& s = segs[k];
     const int64_t n = (int64_t)s.n_frames * s.n_patches;
-    const int L = (int)(q_off[s.request + 1] - q_off[s.request]);
-    lmax = std::max(lmax, L);
-    const int P = s.n_frames > 1 ? s.n_patches : 0;
-    any_temporal |= P > 0;
-    int64_t r = 0;
-    auto push = [&](int kind, int rows_valid) {
-      TcTile t{};
-      t.row_start = (int32_t)(s.row0 + r);
-      t.n_rows = rows_valid;
-      t.box_kind = kind;
-      t.q_row0 = (int32_t)q_off[s.request];
-      t.L = L;
-      t.prev_delta = P;
-      t.key_rows = P > 0 ? (int32_t)std::min<int64_t>(std::max<int64_t>(P - r, 0), rows_valid) : 0;
-      tiles.push_back(t);
-      r += rows_valid;
-    };
-    while (n - r >= 128) push(0, 128);
-    for (int kind = 1; kind <= 3; ++kind) if (n - r >= (128 >> kind)) push(kind, 128 >> kind);
-    if (n - r > 0) push(3, (int)(n - r));
+    si[k].L = (int)(q_off[s.request + 1] - q_off[s.request]);
+    si[k].P = s.n_frames > 1 ? s.n_patches : 0;
+    si[k].w_row = 1.0 + (si[k].P > 0 ? cw.w_prev : 0.0);
+    si[k].c_fix = cw.w_q * (((si[k].L + 15) / 16) * 16) + cw.c_tile;
+    total += (double)n * si[k].w_row + (double)((n + 127) / 128) * si[k].c_fix;
+    n_full += n / 128;
   }
-  const int n_tiles = (int)tiles.size();
-  const int n_ctas = std::min(sm_count, n_tiles);
-  // LPT: heaviest tile first onto the least-loaded CTA (ties -> lowest CTA id, which makes equal-cost tiles round-robin
-  // in row order: neighbouring CTAs sweep neighbouring rows, so previous-frame tiles are still in L2).
-  auto cost = [&](const TcTile& t) {
-    const bool has_prev = t.prev_delta > 0 && t.key_rows < t.n_rows;
-    return (int64_t)(128 >> t.box_kind) * (has_prev ? 2 : 1) + ((t.L + 15) / 16) * 16 + 8;
+  const int n_ctas = (int)std::min<int64_t>(sm_count, std::max<int64_t>(1, (int64_t)(total / 64.0)));
+
+  std::vector<TcTile> tiles;
+  std::vector<std::vector<int>> per;
+  auto make_tile = [&](int32_t k, int64_t r, int h) {
+    const mas_segment& s = segs[k];
+    TcTile t{};
+    t.row_start = (int32_t)(s.row0 + r);
+    t.n_rows = h;
+    t.q_row0 = (int32_t)q_off[s.request];
+    t.L = si[k].L;
+    t.prev_delta = si[k].P;
+    t.key_rows = si[k].P > 0 ? (int32_t)std::min<int64_t>(std::max<int64_t>(si[k].P - r, 0), h) : 0;
+    tiles.push_back(t);
+    return (int)tiles.size() - 1;
   };
-  std::vector<int> order(n_tiles);
-  for (int i = 0; i < n_tiles; ++i) order[i] = i;
-  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost(tiles[a]) > cost(tiles[b]); });
-  typedef std::pair<int64_t, int> Load;   // (load, cta)
-  std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-  for (int c = 0; c < n_ctas; ++c) heap.push(Load(0, c));
-  std::vector<std::vector<int>> per(n_ctas);
-  for (int i : order) {
-    Load l = heap.top(); heap.pop();
-    per[l.second].push_back(i);
-    heap.push(Load(l.first + cost(tiles[i]), l.second));
+  double cost128_max = 0.0;
+  for (int32_t k = 0; k < n_segs; ++k) cost128_max = std::max(cost128_max, 128.0 * si[k].w_row + si[k].c_fix);
+  struct Piece { int32_t seg; int64_t r0, r1; };
+  // one attempt at per-CTA target `target`; returns the heaviest CTA's load
+  auto attempt = [&](double target) {
+    tiles.clear();
+    per.assign(n_ctas, std::vector<int>());
+    std::vector<double> load(n_ctas, 0.0);
+    // ---- bulk: complete round-robin rounds of 128-row tiles that keep every CTA under target - reserve
+    const double reserve = 48.0;
+    int64_t rounds = (int64_t)((target - reserve) / cost128_max);
+    if (rounds < 0) rounds = 0;
+    const int64_t n_bulk = std::min<int64_t>(n_full, rounds * n_ctas) / n_ctas * n_ctas;
+    std::vector<Piece> pieces;
+    int64_t dealt = 0;
+    for (int32_t k = 0; k < n_segs; ++k) {
+      const int64_t n = (int64_t)segs[k].n_frames * segs[k].n_patches;
+      int64_t r = 0;
+      while (n - r >= 128 && dealt < n_bulk) {
+        const int c = (int)(dealt % n_ctas);
+        per[c].push_back(make_tile(k, r, 128));
+        load[c] += 128.0 * si[k].w_row + si[k].c_fix;
+        r += 128; ++dealt;
+      }
+      if (r < n) pieces.push_back(Piece{k, r, n});
+    }
+    // ---- fill: cut the remaining rows to the CTAs' gaps, largest gap first
+    typedef std::pair<double, int> Gap;   // (gap, -cta) : max-heap, ties -> lowest CTA id
+    std::priority_queue<Gap> heap;
+    for (int c = 0; c < n_ctas; ++c) heap.push(Gap(target - load[c], -c));
+    for (const Piece& pc : pieces) {
+      const SegInfo& g = si[pc.seg];
+      int64_t r = pc.r0;
+      while (r < pc.r1) {
+        const Gap top = heap.top(); heap.pop();
+        const int c = -top.second;
+        const int64_t left = pc.r1 - r;
+        int64_t h = (int64_t)((top.first - g.c_fix) / g.w_row) / 16 * 16;
+        h = std::max<int64_t>(32, std::min<int64_t>(128, h));
+        if (h >= left || left - h < 32) h = std::min<int64_t>(left, 128);
+        per[c].push_back(make_tile(pc.seg, r, (int)h));
+        load[c] += (double)((h + 15) / 16 * 16) * g.w_row + g.c_fix;
+        heap.push(Gap(target - load[c], -c));
+        r += h;
+      }
+    }
+    return *std::max_element(load.begin(), load.end());
+  };
+  // the fill phase spends a per-tile cost the estimate above cannot know: raise the target until no CTA overshoots
+  double best_t = total / n_ctas, best_max = 1e300;
+  for (int i = 0; i < 40; ++i) {
+    const double t = total / n_ctas * (1.0 + 0.005 * i);
+    const double m = attempt(t);
+    if (m < best_max - 1e-9) { best_max = m; best_t = t; }
   }
+  attempt(best_t);
+  const int n_tiles = (int)tiles.size();
   TcTile* ht = reinterpret_cast<TcTile*>(h_dst);
   int32_t* hoff = reinterpret_cast<int32_t*>(h_dst + (size_t)n_tiles * sizeof(TcTile));
   int w = 0;
   for (int c = 0; c < n_ctas; ++c) {
-    std::sort(per[c].begin(), per[c].end());   // ascending rows inside a CTA
+    std::sort(per[c].begin(), per[c].end(), [&](int a, int b) { return tiles[a].row_start < tiles[b].row_start; });
     hoff[c] = w;
     for (int i : per[c]) ht[w++] = tiles[i];
   }
   hoff[n_ctas] = w;
-  const int lmax_pad = ((lmax + 15) / 16) * 16;
-  sc.any_temporal = any_temporal;
-  sc.lmax_pad = lmax_pad;
-  sc.stage_bytes = kTcBoxBytes * (any_temporal ? 2 : 1) + lmax_pad * 128;
-  const int budget = 227 * 1024 - kTcCtrlBytes - 1024;
-  sc.stages = std::min(kTcMaxStages, budget / sc.stage_bytes);
-  if (sc.stages < 2) return;
-  sc.smem_bytes = kTcCtrlBytes + 1024 + sc.stages * sc.stage_bytes;
+  sc.smem_bytes = kTcCtrlBytes + 1024 + kTcRingBytes + kTcBoxBytes;
   sc.n_ctas = n_ctas;
   sc.n_tiles = n_tiles;
   sc.d_tiles = reinterpret_cast<const TcTile*>(d_dst);
@@ -458,19 +659,50 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// returns 0 on success, -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error)
-inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, const float* qinv, float* s, float* gamma, float* rel,
-                           int64_t N, int64_t nQ, int d, cudaStream_t st) {
-  CUtensorMap mx[4], mq;
+// returns 0 on success, -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error).
+// `pdl`: launch with programmatic stream serialization behind the query-prep kernel (the kernel waits for it itself).
+inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, const float* qinv, float* s, float* dnorm, float* rel,
+                           int64_t N, int64_t nQ, int d, bool pdl, cudaStream_t st) {
+  CUtensorMap mx[4], mq[3];
   for (int k = 0; k < 4; ++k)
     if (!tc_make_map(&mx[k], X, N, d, 128 >> k)) return -1;
-  if (!tc_make_map(&mq, Q, nQ, d, 16)) return -1;
+  for (int k = 0; k < 3; ++k)
+    if (!tc_make_map(&mq[k], Q, nQ, d, 64 >> k)) return -1;
   TcParams p;
-  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.s = s; p.gamma = gamma; p.rel = rel;
-  p.d = d; p.n_kchunks = d / 64; p.stages = sc.stages; p.stage_bytes = sc.stage_bytes;
-  p.prev_off = sc.any_temporal ? kTcBoxBytes : 0;
-  p.q_off = kTcBoxBytes * (sc.any_temporal ? 2 : 1);
-  k_score_tc<<<sc.n_ctas, kTcThreads, sc.smem_bytes, st>>>(mx[0], mx[1], mx[2], mx[3], mq, p);
+  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.s = s; p.dnorm = dnorm; p.rel = rel;
+  p.d = d; p.n_kchunks = d / 64;
+#ifdef MSAS_ABLATE
+  p.dbg = getenv("MSAS_ABLATE") ? atoi(getenv("MSAS_ABLATE")) : 0;
+  static unsigned long long* dbuf = nullptr;
+  if (!dbuf) cudaMalloc(&dbuf, 1024 * 8 * 8);
+  p.dbg_t = dbuf;
+#endif
+  if (launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl, mx[0], mx[1], mx[2], mx[3], mq[0], mq[1], mq[2], p) !=
+      cudaSuccess)
+    return -1;
+#ifdef MSAS_ABLATE
+  if (getenv("MSAS_TIMES")) {
+    cudaStreamSynchronize(st);
+    std::vector<unsigned long long> h(sc.n_ctas * 8);
+    cudaMemcpy(h.data(), dbuf, h.size() * 8, cudaMemcpyDeviceToHost);
+    unsigned long long t0 = ~0ull;
+    for (int c = 0; c < sc.n_ctas; ++c) t0 = std::min(t0, h[c * 8]);
+    if (getenv("MSAS_TIMES")[0] == '2')
+      for (int c = 0; c < sc.n_ctas; ++c) fprintf(stderr, "cta %d sm %d end %.1f\n", c, (int)h[c * 8 + 1], (double)(h[c * 8 + 3] - t0) * 1e-3);
+    {
+      double pw = 0, aw = 0, tot = 0;
+      for (int c = 0; c < sc.n_ctas; ++c) { pw += (double)h[c * 8 + 4]; aw += (double)h[c * 8 + 6]; tot += (double)h[c * 8 + 7]; }
+      fprintf(stderr, "producer waits on empty %.1f%% of its time, ALU warp waits on full %.1f%%\n", 100 * pw / tot, 100 * aw / tot);
+    }
+    for (int k = 2; k < 4; ++k) {
+      std::vector<double> v;
+      for (int c = 0; c < sc.n_ctas; ++c) v.push_back((double)(h[c * 8 + k] - t0) * 1e-3);
+      std::sort(v.begin(), v.end());
+      fprintf(stderr, "stamp%d us: min %.1f p10 %.1f p50 %.1f p90 %.1f max %.1f\n", k, v[0], v[v.size() / 10], v[v.size() / 2],
+              v[v.size() * 9 / 10], v.back());
+    }
+  }
+#endif
   return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }
 

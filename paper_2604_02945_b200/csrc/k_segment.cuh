@@ -18,7 +18,7 @@ struct SegArgs {
   int n_segs, n_requests;
   DevParams prm;
   const float* s;
-  const float* gamma;
+  float* gamma;                 // FUSE: final gamma, or (gamma_raw) sqrt(D) from the tcgen05 score kernel, finished in place
   const float* rel;
   float* m_spatial;             // may be NULL
   float* mas_tok;               // FUSE: output; SELECT only: input
@@ -29,6 +29,8 @@ struct SegArgs {
   int64_t cap_rows;
   int32_t* seg_nkept;           // workspace [n_segs]
   unsigned int* done_counter;   // workspace, zero between launches
+  int gamma_raw;                // 1: gamma holds sqrt(sum (x_t - x_{t-1})^2); gamma = that / (|x_t| + |x_{t-1}|) (SPEC S2)
+  float sqrt_d;                 // |x_i| = s_i * sqrt(d)
 };
 
 constexpr int kSegThreads = 1024;
@@ -82,14 +84,25 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
   const int n = seg.n_rows;
   const int64_t base = seg.row0;
   const DevParams& p = a.prm;
+  pdl_launch_dependents();
+  pdl_wait();
 
   if (FUSE) {
     const bool temporal = seg.n_frames > 1;
     double ss = 0, sr = 0, sg = 0;
     for (int i = tid; i < n; i += kSegThreads) {
-      ss += (double)a.s[base + i];
+      const float si = a.s[base + i];
+      ss += (double)si;
       sr += (double)a.rel[base + i];
-      if (temporal && i >= seg.n_patches) sg += (double)a.gamma[base + i];
+      if (a.gamma_raw) {   // finish Eq. 5's exact form: both norms are available here (same thread re-reads gamma below)
+        float g = 0.f;
+        if (temporal) {
+          if (i < seg.n_patches) g = 1.0f;
+          else { const float den = (si + a.s[base + i - seg.n_patches]) * a.sqrt_d; g = den > 0.f ? a.gamma[base + i] / den : 0.f; }
+        }
+        a.gamma[base + i] = g;
+        if (temporal && i >= seg.n_patches) sg += (double)g;
+      } else if (temporal && i >= seg.n_patches) sg += (double)a.gamma[base + i];
     }
     block_sum3(sm, ss, sr, sg);
     const double mu_s = ss / n, mu_r = sr / n;
@@ -272,6 +285,8 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
 __global__ void __launch_bounds__(kSegThreads) k_compact_idx(const DevSeg* segs, const uint8_t* keep_mask, const int64_t* kept_off,
                                                              int32_t* kept_idx, int64_t cap_rows) {
   __shared__ SegSmem sm;
+  pdl_launch_dependents();
+  pdl_wait();
   const DevSeg seg = segs[blockIdx.x];
   const int64_t off = kept_off[blockIdx.x];
   int run = 0;
@@ -292,6 +307,7 @@ __global__ void __launch_bounds__(kSegThreads) k_compact_idx(const DevSeg* segs,
 __global__ void __launch_bounds__(256) k_gather(const char* __restrict__ X, char* __restrict__ Y, const int32_t* __restrict__ kept_idx,
                                                 const int64_t* __restrict__ total_ptr, int64_t cap_rows, int row_bytes) {
   const int lane = threadIdx.x & 31;
+  pdl_wait();
   const int64_t total = *total_ptr < cap_rows ? *total_ptr : cap_rows;
   const int64_t n_warps = (int64_t)gridDim.x * 8;
   const int n16 = row_bytes >> 4;

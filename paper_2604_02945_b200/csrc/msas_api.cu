@@ -293,8 +293,9 @@ static int launch_score_mma(const mas_plan* p, const void* X, const void* Q, flo
   return MAS_OK;
 }
 
-static SegArgs seg_args(const mas_plan* p, const float* s, const float* gamma, const float* rel, float* m_spatial, float* mas_tok,
-                        mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, int64_t cap_rows) {
+static SegArgs seg_args(const mas_plan* p, const float* s, float* gamma, const float* rel, float* m_spatial, float* mas_tok,
+                        mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, int64_t cap_rows,
+                        bool gamma_raw = false) {
   SegArgs a;
   a.segs = p->at<DevSeg>(p->lay.segs); a.req_seg_off = p->at<int32_t>(p->lay.req);
   a.n_segs = p->n_segs; a.n_requests = p->n_requests; a.prm = p->prm;
@@ -302,11 +303,13 @@ static SegArgs seg_args(const mas_plan* p, const float* s, const float* gamma, c
   a.keep_mask = keep_mask; a.kept_idx = kept_idx; a.kept_off = kept_off; a.cap_rows = cap_rows;
   a.seg_nkept = p->at<int32_t>(p->lay.nkept);
   a.done_counter = p->at<unsigned int>(p->lay.counter);
+  a.gamma_raw = gamma_raw ? 1 : 0;
+  a.sqrt_d = sqrtf((float)p->d);
   return a;
 }
 
 static int launch_gather(const mas_plan* p, const void* X, const int32_t* kept_idx, const int64_t* kept_off, void* Y, int64_t cap_rows,
-                         cudaStream_t st) {
+                         cudaStream_t st, bool pdl = false) {
   if (Y && cap_rows > 0) {
     const int64_t rows = cap_rows < p->kept_cap ? cap_rows : p->kept_cap;
     int64_t grid = (rows + 7) / 8;
@@ -314,9 +317,8 @@ static int launch_gather(const mas_plan* p, const void* X, const int32_t* kept_i
     if (grid > gmax) grid = gmax;
     if (grid < 1) grid = 1;
     const int esz = p->dtype == MAS_BF16 ? 2 : 4;
-    k_gather<<<(unsigned)grid, 256, 0, st>>>(static_cast<const char*>(X), static_cast<char*>(Y), kept_idx, kept_off + p->n_segs,
-                                            cap_rows, p->d * esz);
-    CK(cudaGetLastError());
+    CK(launch_k(k_gather, dim3((unsigned)grid), dim3(256), 0, st, pdl, static_cast<const char*>(X), static_cast<char*>(Y), kept_idx,
+                kept_off + p->n_segs, cap_rows, p->d * esz));
   }
   return MAS_OK;
 }
@@ -370,8 +372,8 @@ extern "C" int mas_fuse(const mas_plan* p, const float* s, const float* gamma, c
                         mas_segment_out* seg_out, mas_stream_t stream) {
   if (!p || !s || !gamma || !rel || !mas_tok) return MAS_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  SegArgs a = seg_args(p, s, gamma, rel, m_spatial, mas_tok, seg_out ? seg_out : p->at<mas_segment_out>(p->lay.segout), nullptr, nullptr,
-                       nullptr, 0);
+  SegArgs a = seg_args(p, s, const_cast<float*>(gamma), rel, m_spatial, mas_tok, seg_out ? seg_out : p->at<mas_segment_out>(p->lay.segout),
+                       nullptr, nullptr, nullptr, 0);
   k_segment<true, false><<<p->n_segs, kSegThreads, 0, st>>>(a);
   CK(cudaGetLastError());
   return MAS_OK;
@@ -411,24 +413,24 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   const cudaEvent_t* pev = p->prof_slots > 0 ? &p->prof_ev[(size_t)(p->prof_calls++ % p->prof_slots) * 4] : nullptr;
   if (pev) CK(cudaEventRecord(pev[0], st));
   int rc;
+  const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
+  if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
   if (p->tc.enabled) {
-    if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
-    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->N, p->nQ, p->d, st);   // a1-a3: TMA + tcgen05
+    // a1-a3: TMA + tcgen05; gb receives sqrt(D), finished into gamma by the segment kernel
+    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->N, p->nQ, p->d, pdl, st);
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else {
-    if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
     if ((rc = launch_score_mma(p, X, Q, sb, gb, rb, nullptr, st)) != MAS_OK) return rc;
   }
-  SegArgs a = seg_args(p, sb, gb, rb, m_spatial, mb, so, mask, kept_idx, koff, cap_rows);
+  SegArgs a = seg_args(p, sb, gb, rb, m_spatial, mb, so, mask, kept_idx, koff, cap_rows, p->tc.enabled);
   if (pev) CK(cudaEventRecord(pev[1], st));
-  k_segment<true, true><<<p->n_segs, kSegThreads, 0, st>>>(a);
-  CK(cudaGetLastError());
+  CK(launch_k(k_segment<true, true>, dim3((unsigned)p->n_segs), dim3(kSegThreads), 0, st, pdl, a));
   if (p->prm.select_mode == MAS_SELECT_THRESHOLD && kept_idx) {
-    k_compact_idx<<<p->n_segs, kSegThreads, 0, st>>>(p->at<DevSeg>(p->lay.segs), mask, koff, kept_idx, cap_rows);
-    CK(cudaGetLastError());
+    CK(launch_k(k_compact_idx, dim3((unsigned)p->n_segs), dim3(kSegThreads), 0, st, pdl, (const DevSeg*)p->at<DevSeg>(p->lay.segs),
+                (const uint8_t*)mask, (const int64_t*)koff, kept_idx, cap_rows));
   }
   if (pev) CK(cudaEventRecord(pev[2], st));
-  rc = launch_gather(p, X, kept_idx, koff, Y, cap_rows, st);
+  rc = launch_gather(p, X, kept_idx, koff, Y, cap_rows, st, pdl);
   if (pev) CK(cudaEventRecord(pev[3], st));
   return rc;
 }
