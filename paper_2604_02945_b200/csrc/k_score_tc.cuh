@@ -40,12 +40,18 @@ struct TcTile {            // 32 bytes
   int32_t pad_[2];
 };
 
-constexpr int kTcAluWarps = 4;                       // one token row per thread
+constexpr int kTcAluSets = 2;                        // ALU warp sets taking alternate chunks
+constexpr int kTcAluWarps = 4 * kTcAluSets;          // per set: one (token row, K-slice) per thread
 constexpr int kTcThreads = 256 + 32 * kTcAluWarps;   // warps 0-7: TMA (X), MMA, TMEM, TMA (Q), 4 x epilogue; then the ALU warps
 constexpr int kTcSlots = 16;                         // mbarrier pairs of the chunk ring (slots are variable-sized)
 constexpr int kTcBoxBytes = 128 * 128;               // 128 rows x 64 bf16 columns
-constexpr int kTcCtrlBytes = 4096;
+constexpr int kTcCtrlBytes = 8192;
 constexpr int kTcRingBytes = (227 * 1024 - kTcCtrlBytes - 1024 - kTcBoxBytes) & ~1023;   // 1 KB alignment slack, 16 KB MMA over-read pad
+
+struct TcMaps {
+  CUtensorMap x[8];    // token rows: box = (16 * (i + 1)) rows x 64 columns
+  CUtensorMap q[3];    // query rows: box = 64 / 32 / 16 rows x 64 columns
+};
 
 struct TcSchedule {
   bool enabled = false;
@@ -66,6 +72,7 @@ struct TcParams {
 #ifdef MSAS_ABLATE
   int dbg;            // development only: bit0 no ALU math, bit1 no MMA, bit2 no Q loads, bit3 no prev loads
   unsigned long long* dbg_t;
+  int dbg_rows;
 #endif
 };
 
@@ -205,17 +212,17 @@ struct TcCtrl {                      // lives at the (1024-aligned) start of dyn
   uint64_t stat_full[2];             // ALU -> epilogue            (ALU warps)
   uint64_t stat_empty[2];            // epilogue -> ALU            (4 warps)
   uint32_t tmem_base;
-  uint32_t vstart[kTcSlots];         // X producer only: virtual start offset of the chunk in each barrier slot
-  uint32_t vstart_q[kTcSlots];       // Q producer only: its own copy
   uint32_t pad_[31];
-  float rowstat[2][2][128];          // partial sum x^2, sum (x - x_prev)^2 per (K-slice, tile row), double buffered
+  float rowstat[2][kTcAluSets][2][128];   // partial sum x^2, sum (x - x_prev)^2 per (ALU set, K-slice, tile row), double buffered
 };
 static_assert(sizeof(TcCtrl) <= kTcCtrlBytes, "control block too large");
 
 __global__ void __launch_bounds__(kTcThreads, 1)
-k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CUtensorMap mx64, const __grid_constant__ CUtensorMap mx32,
-           const __grid_constant__ CUtensorMap mx16, const __grid_constant__ CUtensorMap mq64, const __grid_constant__ CUtensorMap mq32,
-           const __grid_constant__ CUtensorMap mq16, const TcParams p) {
+k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
+  const CUtensorMap& mx128 = maps.x[7];
+  const CUtensorMap& mq64 = maps.q[0];
+  const CUtensorMap& mq32 = maps.q[1];
+  const CUtensorMap& mq16 = maps.q[2];
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   TcCtrl* ctrl = reinterpret_cast<TcCtrl*>(smem);
@@ -231,9 +238,60 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
   constexpr int dbg = 0;
 #endif
 
+#ifdef MSAS_ABLATE
+  if (dbg & 64) {   // probe mode: the bare streaming loop of _work/probe/tmabw.cu inside this kernel and harness
+    uint64_t* full = ctrl->full; uint64_t* empty = ctrl->empty;
+    if (tid == 0) { for (int i = 0; i < 12; ++i) { mbar_init(smem_u32(&full[i]), 1); mbar_init(smem_u32(&empty[i]), 1); } asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+    __syncthreads();
+    const int n_tiles = p.dbg_rows / 128;
+    if (tid == 0 && (dbg & 1024)) {   // the real tile list, one 128-row box per tile and K-slice
+      int stage = 0; uint32_t ph = 0;
+      for (int t = tile_lo; t < tile_hi; ++t) {
+        const int row = p.tiles[t].row_start;
+        for (int cg = 0; cg < nk; ++cg) {
+          mbar_wait(smem_u32(&empty[stage]), ph ^ 1u);
+          uint32_t bar = smem_u32(&full[stage]);
+          mbar_expect_tx(bar, 16384);
+          tma_load_2d(smem_u32(ring0 + stage * 16384), &mx128, bar, cg * 64, row);
+          if (++stage == 12) { stage = 0; ph ^= 1u; }
+        }
+      }
+    } else if (tid == 32 && (dbg & 1024)) {
+      int stage = 0; uint32_t ph = 0;
+      for (int t = tile_lo; t < tile_hi; ++t)
+        for (int cg = 0; cg < nk; ++cg) {
+          mbar_wait(smem_u32(&full[stage]), ph);
+          mbar_arrive(smem_u32(&empty[stage]));
+          if (++stage == 12) { stage = 0; ph ^= 1u; }
+        }
+    } else if (dbg & 1024) {
+    } else if (tid == 0) {
+      int stage = 0; uint32_t ph = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x)
+        for (int cg = 0; cg < nk; ++cg) {
+          mbar_wait(smem_u32(&empty[stage]), ph ^ 1u);
+          uint32_t bar = smem_u32(&full[stage]);
+          mbar_expect_tx(bar, 16384);
+          tma_load_2d(smem_u32(ring0 + stage * 16384), &mx128, bar, cg * 64, t * 128);
+          if (++stage == 12) { stage = 0; ph ^= 1u; }
+        }
+    } else if (tid == 32) {
+      int stage = 0; uint32_t ph = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x)
+        for (int cg = 0; cg < nk; ++cg) {
+          mbar_wait(smem_u32(&full[stage]), ph);
+          mbar_arrive(smem_u32(&empty[stage]));
+          if (++stage == 12) { stage = 0; ph ^= 1u; }
+        }
+    }
+    __syncthreads();
+    if (tid == 0 && p.dbg_t) p.dbg_t[blockIdx.x * 8 + 3] = gtime();
+    return;
+  }
+#endif
   pdl_launch_dependents();   // the segment kernel may be scheduled as SMs free up; it waits for this grid to complete
   if (warp == 1 && lane == 0) {
-    for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), 2); mbar_init(smem_u32(&ctrl->empty[i]), 1 + kTcAluWarps); }
+    for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), (dbg & 32) ? 1 : 2); mbar_init(smem_u32(&ctrl->empty[i]), ((dbg & 512) ? 0 : 1) + ((dbg & 256) ? 0 : 4)); }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&ctrl->tmem_full[i]), 1); mbar_init(smem_u32(&ctrl->tmem_empty[i]), 4);
       mbar_init(smem_u32(&ctrl->stat_full[i]), kTcAluWarps); mbar_init(smem_u32(&ctrl->stat_empty[i]), 4);
@@ -254,65 +312,46 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
   tc_fence_after();
   const uint32_t tmem_base = ctrl->tmem_base;
 
-  if (warp == 0 || warp == 3) {
+  if (warp == 0 || (warp == 3 && !(dbg & 32))) {
     // ===================================================================== TMA producers (one thread each)
     // warp 0 streams the token rows (and the previous-frame rows), warp 3 the query rows.  A single thread issues about
     // one instruction every few cycles, so the per-chunk loop is kept to a few dozen instructions per producer.
     if (lane == 0) {
       const bool xprod = warp == 0;
       TcRing ring;
-#ifdef MSAS_ABLATE
-      long long wait_clk = 0; const long long cstart = clock64();
-#endif
-      uint32_t rel = 0;                    // oldest chunk not yet known to be released
-      uint32_t v_oldest = 0;               // virtual start offset of chunk `rel` (valid while rel < ring.k)
-      uint32_t* vstart = xprod ? ctrl->vstart : ctrl->vstart_q;     // virtual start offset of chunk j, at j % kTcSlots
+      // `tail` replays the same placement sequence one released chunk at a time: tail.vhead is (a lower bound of) the
+      // virtual start of the oldest chunk whose release has not been observed yet, tail.k its index.  Registers only.
+      TcRing tail;
+      int tail_t = tile_lo, tail_ch = 0;
+      TcGeom tg = tc_geom(p.tiles[tile_lo], nk, dbg);
       for (int t = tile_lo; t < tile_hi; ++t) {
         const TcTile tile = p.tiles[t];
         const TcGeom g = tc_geom(tile, nk, dbg);
-        const int r16 = (int)(g.xbytes >> 11);                      // 16-row groups: 8 -> one 128-row box, else its bits
+        const CUtensorMap* mx = &maps.x[(g.xbytes >> 11) - 1];      // one box of rows16 rows per K-slice
         const int row = tile.row_start, prow = tile.row_start - tile.prev_delta;
         const uint32_t poff = (uint32_t)g.kw * g.xbytes;            // previous-frame slices follow the token slices
+#ifdef MSAS_ABLATE
+        if (xprod && (blockIdx.x == 0 || blockIdx.x == 77) && p.dbg_t) p.dbg_t[2048 + (blockIdx.x ? 64 : 0) + (t - tile_lo)] = gtime();
+#endif
         for (int ch = 0; ch < g.nch; ++ch) {
           const uint32_t off = ring.place(g.need);
-          const uint32_t vbeg = ring.vhead - g.need;
-          // wait until the barrier slot is free and the bytes [vbeg, vbeg + need) no longer overlap an unreleased chunk
-          while (rel < ring.k && (ring.k - rel >= (uint32_t)kTcSlots || ring.vhead - v_oldest > (uint32_t)kTcRingBytes)) {
-#ifdef MSAS_ABLATE
-            const long long c0 = clock64();
-#endif
-            mbar_wait(smem_u32(&ctrl->empty[rel % kTcSlots]), (rel / kTcSlots) & 1u);
-#ifdef MSAS_ABLATE
-            wait_clk += clock64() - c0;
-#endif
-            ++rel;
-            v_oldest = vstart[rel % kTcSlots];
+          // wait until the barrier slot is free and the bytes of this chunk no longer overlap an unreleased chunk
+          while (tail.k < ring.k && (ring.k - tail.k >= (uint32_t)kTcSlots || ring.vhead - tail.vhead > (uint32_t)kTcRingBytes)) {
+            mbar_wait(smem_u32(&ctrl->empty[tail.slot()]), tail.parity());
+            tail.place(tg.need);
+            ++tail.k;
+            if (++tail_ch == tg.nch && tail_t + 1 < tile_hi) { tail_ch = 0; tg = tc_geom(p.tiles[++tail_t], nk, dbg); }
           }
-          vstart[ring.slot()] = vbeg;
-          if (rel == ring.k) v_oldest = vbeg;
           const uint32_t bar = smem_u32(&ctrl->full[ring.slot()]);
           const uint32_t base = smem_u32(ring0 + off);
           if (xprod) {
-            mbar_expect_tx(bar, (uint32_t)g.kw * g.xall);
+            const bool ld_prev = g.has_prev && !(dbg & 4096);
+            mbar_expect_tx(bar, (uint32_t)g.kw * (ld_prev ? g.xall : g.xbytes));
             for (int j = 0; j < g.kw; ++j) {
               const int c0 = (ch * g.kw + j) * 64;
               const uint32_t dst = base + (uint32_t)j * g.xbytes;
-              if (r16 == 8) {
-                tma_load_2d(dst, &mx128, bar, c0, row);
-                if (g.has_prev) tma_load_2d(dst + poff, &mx128, bar, c0, prow);
-              } else {   // rows past the end of X are zero-filled by the TMA unit
-                int o = 0;
-                if (r16 & 4) { tma_load_2d(dst, &mx64, bar, c0, row); if (g.has_prev) tma_load_2d(dst + poff, &mx64, bar, c0, prow); o = 64; }
-                if (r16 & 2) {
-                  tma_load_2d(dst + o * 128, &mx32, bar, c0, row + o);
-                  if (g.has_prev) tma_load_2d(dst + poff + o * 128, &mx32, bar, c0, prow + o);
-                  o += 32;
-                }
-                if (r16 & 1) {
-                  tma_load_2d(dst + o * 128, &mx16, bar, c0, row + o);
-                  if (g.has_prev) tma_load_2d(dst + poff + o * 128, &mx16, bar, c0, prow + o);
-                }
-              }
+              tma_load_2d(dst, mx, bar, c0, row);      // rows past the end of X are zero-filled by the TMA unit
+              if (ld_prev) tma_load_2d(dst + poff, mx, bar, c0, prow);
             }
           } else {
             mbar_expect_tx(bar, (uint32_t)g.kw * g.qbytes);
@@ -328,13 +367,10 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
           ++ring.k;
         }
       }
-#ifdef MSAS_ABLATE
-      if (p.dbg_t && xprod) { p.dbg_t[blockIdx.x * 8 + 4] = wait_clk; p.dbg_t[blockIdx.x * 8 + 7] = clock64() - cstart; }
-#endif
     }
   } else if (warp == 1) {
     // ===================================================================== MMA issuer (one thread)
-    if (lane == 0) {
+    if (lane == 0 && !(dbg & 512)) {
       TcRing ring;
       int it = 0;
       for (int t = tile_lo; t < tile_hi; ++t, ++it) {
@@ -343,7 +379,7 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
         const uint32_t idesc = umma_idesc_bf16(((tile.L + 15) >> 4) << 4);
         const int acc = it & 1;
         const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
-        mbar_wait(smem_u32(&ctrl->tmem_empty[acc]), acc_phase ^ 1u);
+        if (!(dbg & 128)) mbar_wait(smem_u32(&ctrl->tmem_empty[acc]), acc_phase ^ 1u);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)acc * 128u;
         for (int ch = 0; ch < g.nch; ++ch) {
@@ -364,7 +400,7 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
           tc_commit(smem_u32(&ctrl->empty[ring.slot()]));
           ++ring.k;
         }
-        tc_commit(smem_u32(&ctrl->tmem_full[acc]));
+        if (!(dbg & 128)) tc_commit(smem_u32(&ctrl->tmem_full[acc]));
       }
     }
   } else if (warp >= 4 && warp < 8) {
@@ -374,7 +410,7 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
     const float inv_d = 1.0f / (float)p.d;
     pdl_wait();                              // qinv comes from the query-prep kernel launched just before this one
     int it = 0;
-    for (int t = tile_lo; t < tile_hi; ++t, ++it) {
+    for (int t = tile_lo; t < ((dbg & 128) ? tile_lo : tile_hi); ++t, ++it) {
       const TcTile tile = p.tiles[t];
       const TcGeom g = tc_geom(tile, nk, dbg);
       const int acc = it & 1;
@@ -401,7 +437,9 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
       float n2 = 0.f, D = 0.f;               // the ALU threads hold one partial per (row, K-slice of the chunk)
       if (r < tile.n_rows) {
         const int rp2 = 128 / g.kw;
-        for (int j = 0; j < g.kw; ++j) { n2 += ctrl->rowstat[acc][0][r + j * rp2]; D += ctrl->rowstat[acc][1][r + j * rp2]; }
+        for (int j = 0; j < g.kw; ++j)
+#pragma unroll
+          for (int st = 0; st < kTcAluSets; ++st) { n2 += ctrl->rowstat[acc][st][0][r + j * rp2]; D += ctrl->rowstat[acc][st][1][r + j * rp2]; }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_empty[acc]));
@@ -414,13 +452,14 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
     }
   } else if (warp >= 8) {
     // ===================================================================== CUDA-core statistics: one thread per (row, K-slice)
-    const int a = tid - 256;
+    const int a = (tid - 256) & 127;
+    const uint32_t set = (uint32_t)(tid - 256) >> 7;      // this set takes the chunks with ring.k % kTcAluSets == set
     TcRing ring;
 #ifdef MSAS_ABLATE
     long long alu_wait = 0;
 #endif
     int it = 0;
-    for (int t = tile_lo; t < tile_hi; ++t, ++it) {
+    for (int t = tile_lo; t < ((dbg & 256) ? tile_lo : tile_hi); ++t, ++it) {
       const TcTile tile = p.tiles[t];
       const TcGeom g = tc_geom(tile, nk, dbg);
       const int rp2 = 128 / g.kw;
@@ -433,6 +472,7 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
       uint64_t n2a = 0, n2b = 0, Da = 0, Db = 0;     // packed fp32 pairs, all zero bits = (0.f, 0.f)
       for (int ch = 0; ch < g.nch; ++ch) {
         const uint32_t off = ring.place(g.need);
+        if (ring.k % (uint32_t)kTcAluSets != set) { ++ring.k; continue; }
 #ifdef MSAS_ABLATE
         const long long c0 = clock64();
 #endif
@@ -446,7 +486,7 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
           uint4 x[8];
 #pragma unroll
           for (int u = 0; u < 8; ++u) x[u] = *reinterpret_cast<const uint4*>(sx + (((uint32_t)u ^ sw) << 4));
-          if (g.has_prev) {
+          if (g.has_prev && !(dbg & 2048)) {
             const unsigned char* su = sx + poff;
             uint4 v[8];
 #pragma unroll
@@ -475,8 +515,8 @@ k_score_tc(const __grid_constant__ CUtensorMap mx128, const __grid_constant__ CU
       const float D = sum_f32x2(Da) + sum_f32x2(Db);
       const int buf = it & 1;
       const uint32_t ph = (uint32_t)(it >> 1) & 1u;
-      mbar_wait(smem_u32(&ctrl->stat_empty[buf]), ph ^ 1u);
-      ctrl->rowstat[buf][0][a] = n2; ctrl->rowstat[buf][1][a] = D;      // slot a = j * rp2 + r
+      if (!(dbg & 128)) mbar_wait(smem_u32(&ctrl->stat_empty[buf]), ph ^ 1u);
+      ctrl->rowstat[buf][set][0][a] = n2; ctrl->rowstat[buf][set][1][a] = D;      // slot a = j * rp2 + r
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_full[buf]));
     }
@@ -663,21 +703,22 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
 // `pdl`: launch with programmatic stream serialization behind the query-prep kernel (the kernel waits for it itself).
 inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, const float* qinv, float* s, float* dnorm, float* rel,
                            int64_t N, int64_t nQ, int d, bool pdl, cudaStream_t st) {
-  CUtensorMap mx[4], mq[3];
-  for (int k = 0; k < 4; ++k)
-    if (!tc_make_map(&mx[k], X, N, d, 128 >> k)) return -1;
+  TcMaps maps;
+  for (int k = 0; k < 8; ++k)
+    if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
   for (int k = 0; k < 3; ++k)
-    if (!tc_make_map(&mq[k], Q, nQ, d, 64 >> k)) return -1;
+    if (!tc_make_map(&maps.q[k], Q, nQ, d, 64 >> k)) return -1;
   TcParams p;
   p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.s = s; p.dnorm = dnorm; p.rel = rel;
   p.d = d; p.n_kchunks = d / 64;
 #ifdef MSAS_ABLATE
   p.dbg = getenv("MSAS_ABLATE") ? atoi(getenv("MSAS_ABLATE")) : 0;
   static unsigned long long* dbuf = nullptr;
-  if (!dbuf) cudaMalloc(&dbuf, 1024 * 8 * 8);
+  if (!dbuf) cudaMalloc(&dbuf, 4096 * 8);
   p.dbg_t = dbuf;
+  p.dbg_rows = (int)N;
 #endif
-  if (launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl, mx[0], mx[1], mx[2], mx[3], mq[0], mq[1], mq[2], p) !=
+  if (launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl, maps, p) !=
       cudaSuccess)
     return -1;
 #ifdef MSAS_ABLATE
@@ -690,9 +731,12 @@ inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, c
     if (getenv("MSAS_TIMES")[0] == '2')
       for (int c = 0; c < sc.n_ctas; ++c) fprintf(stderr, "cta %d sm %d end %.1f\n", c, (int)h[c * 8 + 1], (double)(h[c * 8 + 3] - t0) * 1e-3);
     {
-      double pw = 0, aw = 0, tot = 0;
-      for (int c = 0; c < sc.n_ctas; ++c) { pw += (double)h[c * 8 + 4]; aw += (double)h[c * 8 + 6]; tot += (double)h[c * 8 + 7]; }
-      fprintf(stderr, "producer waits on empty %.1f%% of its time, ALU warp waits on full %.1f%%\n", 100 * pw / tot, 100 * aw / tot);
+
+    }
+    {
+      std::vector<unsigned long long> tt(128);
+      cudaMemcpy(tt.data(), dbuf + 2048, 128 * 8, cudaMemcpyDeviceToHost);
+      for (int b = 0; b < 2; ++b) { fprintf(stderr, "cta %d tile starts:", b ? 77 : 0); for (int i = 0; i < 12; ++i) fprintf(stderr, " %.1f", (double)(tt[b * 64 + i] - t0) * 1e-3); fprintf(stderr, "\n"); }
     }
     for (int k = 2; k < 4; ++k) {
       std::vector<double> v;
