@@ -38,9 +38,35 @@ constexpr int kSegThreads = 1024;
 struct SegSmem {
   double red[3][32];
   int ired[2][32];
-  unsigned int hist[256];
+  unsigned int hist[4][256];   // one histogram per radix pass (no reuse: no second cluster barrier per pass)
   int bcast[4];
+  double cx_d[4][3];           // cluster exchange: this CTA's block totals of reduction round 0..3
+  int cx_i[2];                 // cluster exchange: this CTA's (less, equal) counts
 };
+
+// ---- thread-block cluster helpers (a segment is shared by the CTAs of one cluster; cluster size 1 works too)
+__device__ __forceinline__ unsigned cluster_rank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ unsigned cluster_size() { unsigned r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ unsigned cluster_id_x() { unsigned r; asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+template <class T> __device__ __forceinline__ T dsmem_read(const T* local, unsigned rank);
+template <> __device__ __forceinline__ double dsmem_read<double>(const double* local, unsigned rank) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(local), ra; double v;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(a), "r"(rank));
+  asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(ra) : "memory");
+  return v;
+}
+template <> __device__ __forceinline__ int dsmem_read<int>(const int* local, unsigned rank) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(local), ra; int v;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(a), "r"(rank));
+  asm volatile("ld.shared::cluster.b32 %0, [%1];" : "=r"(v) : "r"(ra) : "memory");
+  return v;
+}
+template <> __device__ __forceinline__ unsigned dsmem_read<unsigned>(const unsigned* local, unsigned rank) {
+  return (unsigned)dsmem_read<int>(reinterpret_cast<const int*>(local), rank);
+}
 
 // fixed-order block sum of up to three doubles; result broadcast to every thread
 __device__ __forceinline__ void block_sum3(SegSmem& sm, double& a, double& b, double& c) {
@@ -75,22 +101,48 @@ __device__ __forceinline__ void block_scan2(SegSmem& sm, int fa, int fb, int& pa
   pb = eb + __popc(bb & lt);
 }
 
+// fixed-order sum of up to three doubles over all CTAs of the cluster; the result reaches every thread of every CTA.
+// `round` selects a private exchange slot (no slot is reused inside one launch, so one cluster barrier per round suffices).
+__device__ __forceinline__ void cluster_sum3(SegSmem& sm, int round, unsigned nc, double& a, double& b, double& c) {
+  block_sum3(sm, a, b, c);
+  if (nc == 1) return;
+  if (threadIdx.x == 0) { sm.cx_d[round][0] = a; sm.cx_d[round][1] = b; sm.cx_d[round][2] = c; }
+  cluster_sync_all();
+  // one lane per peer fetches its three totals (independent remote loads: one DSMEM latency, not 3 x nc of them)
+  if (threadIdx.x < nc) {
+    const double x = dsmem_read(&sm.cx_d[round][0], threadIdx.x), y = dsmem_read(&sm.cx_d[round][1], threadIdx.x),
+                 z = dsmem_read(&sm.cx_d[round][2], threadIdx.x);
+    sm.red[0][threadIdx.x] = x; sm.red[1][threadIdx.x] = y; sm.red[2][threadIdx.x] = z;
+  }
+  __syncthreads();
+  double x = 0, y = 0, z = 0;
+  for (unsigned r = 0; r < nc; ++r) { x += sm.red[0][r]; y += sm.red[1][r]; z += sm.red[2][r]; }   // rank order: same bits in every CTA
+  a = x; b = y; c = z;
+  __syncthreads();   // sm.red is reused by the next block_sum3
+}
+
+// One thread-block CLUSTER per segment (cluster size chosen by the host from the longest segment; 1 for images):
+// CTA `rank` owns the contiguous token slice [lo, hi) of the segment; sums, radix histograms and kept counts are
+// combined over distributed shared memory, so an 18 432-token video segment is a few microseconds of latency, not 70.
 template <bool FUSE, bool SELECT>
 __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
   __shared__ SegSmem sm;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int sidx = blockIdx.x;
+  const unsigned nc = cluster_size(), rank = cluster_rank();
+  const int sidx = (int)cluster_id_x();
   const DevSeg seg = a.segs[sidx];
   const int n = seg.n_rows;
   const int64_t base = seg.row0;
   const DevParams& p = a.prm;
+  const int per = (n + (int)nc - 1) / (int)nc;
+  const int lo = min(n, (int)rank * per), hi = min(n, lo + per);
   pdl_launch_dependents();
   pdl_wait();
 
   if (FUSE) {
     const bool temporal = seg.n_frames > 1;
     double ss = 0, sr = 0, sg = 0;
-    for (int i = tid; i < n; i += kSegThreads) {
+    for (int i = lo + tid; i < hi; i += kSegThreads) {
       const float si = a.s[base + i];
       ss += (double)si;
       sr += (double)a.rel[base + i];
@@ -104,21 +156,21 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         if (temporal && i >= seg.n_patches) sg += (double)g;
       } else if (temporal && i >= seg.n_patches) sg += (double)a.gamma[base + i];
     }
-    block_sum3(sm, ss, sr, sg);
+    cluster_sum3(sm, 0, nc, ss, sr, sg);
     const double mu_s = ss / n, mu_r = sr / n;
     const double gavg = temporal ? sg / ((double)(seg.n_frames - 1) * seg.n_patches) : 0.0;
     double vs = 0, vr = 0, dummy = 0;
-    for (int i = tid; i < n; i += kSegThreads) {
+    for (int i = lo + tid; i < hi; i += kSegThreads) {
       const double ds = (double)a.s[base + i] - mu_s, dr = (double)a.rel[base + i] - mu_r;
       vs += ds * ds; vr += dr * dr;
     }
-    block_sum3(sm, vs, vr, dummy);
+    cluster_sum3(sm, 1, nc, vs, vr, dummy);
     const double sd_s = sqrt(vs / n), sd_r = sqrt(vr / n);
     const double den_s = fmax(sd_s, 1e-6 * mu_s), den_r = fmax(sd_r, 1e-6);
     const float inv_s = den_s > 0.0 ? (float)(1.0 / den_s) : 0.f, inv_r = (float)(1.0 / den_r);
     const float at = temporal ? p.lambda_temp : 0.f;
     int below = 0;
-    for (int i = tid; i < n; i += kSegThreads) {
+    for (int i = lo + tid; i < hi; i += kSegThreads) {
       // differences in double (s, rel are fp32 values; the means are not representable in fp32)
       const float z = (float)(((double)a.s[base + i] - mu_s)) * inv_s;
       const float M = sigmoidf_acc(p.spatial_gain * z + p.spatial_bias);
@@ -131,8 +183,8 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
       below += M < p.tau_s ? 1 : 0;
     }
     double db = below, d1 = 0, d2 = 0;
-    block_sum3(sm, db, d1, d2);
-    if (tid == 0 && a.seg_out) {
+    cluster_sum3(sm, 2, nc, db, d1, d2);
+    if (rank == 0 && tid == 0 && a.seg_out) {
       mas_segment_out o;
       o.rho_spatial = (float)(db / n);
       o.gamma_avg = (float)gavg;
@@ -142,7 +194,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
       o.n_tokens = n; o.n_kept = 0;
       a.seg_out[sidx] = o;
     }
-    __syncthreads();   // mas_tok of this segment is re-read below by other threads
+    __syncthreads();   // mas_tok of this CTA's slice is re-read below by other threads of the same CTA
   }
 
   if (SELECT) {
@@ -151,20 +203,39 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
       int kk = seg.keep_k < n ? seg.keep_k : n;
       const int k_total = kk;
       unsigned prefix = 0, maskbits = 0;
+      if (tid < 256) { sm.hist[0][tid] = 0; sm.hist[1][tid] = 0; sm.hist[2][tid] = 0; sm.hist[3][tid] = 0; }
+      __syncthreads();
 #pragma unroll 1
       for (int pass = 0; pass < 4; ++pass) {
         const int shift = 24 - 8 * pass;
-        if (tid < 256) sm.hist[tid] = 0;
-        __syncthreads();
-        for (int i = tid; i < n; i += kSegThreads) {
-          const unsigned key = float_key(mas[i]);
-          if ((key & maskbits) == prefix) atomicAdd(&sm.hist[(key >> shift) & 255u], 1u);
+        for (int c0 = lo; c0 < hi; c0 += kSegThreads) {   // warp-uniform trip count: every lane takes part in the votes
+          const int i = c0 + tid;
+          const unsigned key = i < hi ? float_key(mas[i]) : 0u;
+          const bool act = i < hi && (key & maskbits) == prefix;
+          const unsigned bin = (key >> shift) & 255u;
+          // MAS scores share their leading bytes: aggregate equal bins inside the warp, one shared-memory atomic per bin
+          const unsigned am = __ballot_sync(0xffffffffu, act);
+          if (act) {
+            const unsigned peers = __match_any_sync(am, bin);
+            if (lane == __ffs(peers) - 1) atomicAdd(&sm.hist[pass][bin], (unsigned)__popc(peers));
+          }
         }
         __syncthreads();
-        if (warp == 0) {   // find the bin where the cumulative count reaches kk
+        if (nc > 1) {   // cluster-wide histogram: thread b sums bin b over the peers (independent remote loads), in place
+          cluster_sync_all();   // every CTA's histogram of this pass is complete and visible
+          unsigned v[8];
+          if (tid < 256) {
+#pragma unroll
+            for (unsigned r = 0; r < 8; ++r) v[r] = r < nc ? dsmem_read(&sm.hist[pass][tid], r) : 0u;
+          }
+          cluster_sync_all();   // every peer has read this CTA's bins before they are overwritten with the totals
+          if (tid < 256) sm.hist[pass][tid] = ((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]));
+          __syncthreads();
+        }
+        if (warp == 0) {   // find the bin where the cumulative count (over the whole cluster) reaches kk
           unsigned loc[8], tot = 0;
 #pragma unroll
-          for (int b = 0; b < 8; ++b) { loc[b] = sm.hist[lane * 8 + b]; tot += loc[b]; }
+          for (int b = 0; b < 8; ++b) { loc[b] = sm.hist[pass][lane * 8 + b]; tot += loc[b]; }
           unsigned inc = tot;
 #pragma unroll
           for (int o = 1; o < 32; o <<= 1) { unsigned u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
@@ -186,12 +257,24 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         __syncthreads();
       }
       // prefix = key of the k-th smallest; keep every key < prefix and the first kk keys == prefix (index order)
-      const int64_t off = seg.kept_off_static;
       int run_less = 0, run_eq = 0;
-      for (int c0 = 0; c0 < n; c0 += kSegThreads) {
+      if (nc > 1) {   // kept tokens of the lower-ranked CTAs come first: exchange the per-CTA (less, equal) counts
+        int cl = 0, ce = 0;
+        for (int i = lo + tid; i < hi; i += kSegThreads) { const unsigned key = float_key(mas[i]); cl += key < prefix; ce += key == prefix; }
+        double dl = cl, de = ce, d0 = 0;
+        block_sum3(sm, dl, de, d0);
+        if (tid == 0) { sm.cx_i[0] = (int)dl; sm.cx_i[1] = (int)de; }
+        cluster_sync_all();
+        int pl = 0, pe = 0;
+        if ((unsigned)lane < rank) { pl = dsmem_read(&sm.cx_i[0], (unsigned)lane); pe = dsmem_read(&sm.cx_i[1], (unsigned)lane); }
+        for (int o = 16; o > 0; o >>= 1) { pl += __shfl_xor_sync(0xffffffffu, pl, o); pe += __shfl_xor_sync(0xffffffffu, pe, o); }
+        run_less = pl; run_eq = pe;
+      }
+      const int64_t off = seg.kept_off_static;
+      for (int c0 = lo; c0 < hi; c0 += kSegThreads) {
         const int i = c0 + tid;
         unsigned key = 0xffffffffu;
-        bool valid = i < n;
+        bool valid = i < hi;
         if (valid) key = float_key(mas[i]);
         const int fl = valid && key < prefix, fe = valid && key == prefix;
         int pl, pe, tl, te;
@@ -207,30 +290,32 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         }
         run_less += tl; run_eq += te;
       }
-      if (tid == 0) {
+      if (rank == 0 && tid == 0) {
         a.seg_nkept[sidx] = k_total;
         if (a.seg_out) a.seg_out[sidx].n_kept = k_total;
       }
     } else {
       int cnt = 0;
-      for (int i = tid; i < n; i += kSegThreads) {
+      for (int i = lo + tid; i < hi; i += kSegThreads) {
         const bool keep = mas[i] <= p.cut;
         if (a.keep_mask) a.keep_mask[base + i] = keep ? 1 : 0;
         cnt += keep;
       }
       double dc = cnt, d1 = 0, d2 = 0;
-      block_sum3(sm, dc, d1, d2);
-      if (tid == 0) {
+      cluster_sum3(sm, 3, nc, dc, d1, d2);
+      if (rank == 0 && tid == 0) {
         a.seg_nkept[sidx] = (int)dc;
         if (a.seg_out) a.seg_out[sidx].n_kept = (int)dc;
       }
     }
   }
 
-  // ---- last block: per-request softmax + Eq. 7, and the kept_off table
+  // ---- last cluster: per-request softmax + Eq. 7, and the kept_off table (rank 0 only)
+  if (nc > 1) cluster_sync_all();   // no CTA leaves while a peer may still read its shared memory
+  if (rank != 0) return;
   __threadfence();
   __syncthreads();
-  if (tid == 0) sm.bcast[2] = (atomicAdd(a.done_counter, 1u) == gridDim.x - 1) ? 1 : 0;
+  if (tid == 0) sm.bcast[2] = (atomicAdd(a.done_counter, 1u) == (unsigned)a.n_segs - 1u) ? 1 : 0;
   __syncthreads();
   if (!sm.bcast[2]) return;
   __threadfence();
