@@ -35,34 +35,42 @@ def measured_peaks():
 
 
 class ClockSampler(threading.Thread):
-    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md 'clocks line')."""
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md 'clocks line'): one streaming
+    `nvidia-smi -lms` process, rows tagged with the host time so that only those inside the timed region count."""
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
     def __init__(self, index):
         super().__init__(daemon=True)
-        self.index, self.rows, self.stop_flag = index, [], False
+        self.index, self.rows, self.proc, self.t0, self.t1 = index, [], None, None, None
 
     def run(self):
-        while not self.stop_flag:
-            try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits"],
-                                     capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.rows.append([x.strip() for x in out.split(",")])
-            except Exception:
-                pass
-            time.sleep(0.05)
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                f = [x.strip() for x in line.split(",")]
+                if len(f) >= 6:
+                    self.rows.append((time.perf_counter(), f))
+        except Exception:
+            pass
+
+    def wait_ready(self, timeout=5.0):
+        t = time.perf_counter()
+        while not self.rows and time.perf_counter() - t < timeout:
+            time.sleep(0.01)
 
     def summary(self):
-        self.stop_flag = True
-        self.join(timeout=6)
-        if not self.rows:
+        if self.proc is not None:
+            self.proc.terminate()
+        self.join(timeout=3)
+        rows = [f for (t, f) in self.rows if self.t0 is not None and self.t0 <= t <= self.t1] or [f for (_, f) in self.rows[-3:]]
+        if not rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
-        sm = sorted(float(r[0]) for r in self.rows)
+        sm = sorted(float(r[0]) for r in rows)
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for i, n in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in self.rows)]
-        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons, "samples": len(self.rows)}
+        reasons = [n for i, n in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons, "samples": len(rows)}
 
 
 def algorithmic_bytes(w, kept_rows):
@@ -114,7 +122,7 @@ def run_reference(args, w):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="batched_images", choices=list(SEEDS))
     ap.add_argument("--impl", default="msas", choices=["msas", "reference"])
@@ -166,13 +174,16 @@ def main():
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
+        sampler.wait_ready()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    sampler.t0 = time.perf_counter()
     ev0.record(stream)
     for i in range(args.steps):
         plan.forward(Xs[i % 2], Qs[i % 2], out=out)
     ev1.record(stream)
     barrier()
+    sampler.t1 = time.perf_counter()
     ms = ev0.elapsed_time(ev1)
     # per-stage attribution: a second pass with CUDA events between the kernels on the same stream (these events
     # serialise the launches, so the stage times are measured apart from the timed region above, never inside it)
@@ -204,17 +215,10 @@ def main():
         d2h = w.n_tokens * (4 + 1) + plan.n_segs * 36 + (plan.n_segs + 1) * 8 + kept_rows * (4 + w.d * e)
         e2e = (e2e_ms, h2d, d2h, n_e2e)
 
-    if world > 1:
-        t = torch.tensor([ms, e2e[0] if e2e else 0.0], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_ms_max = float(t[0]), float(t[1])
-        if e2e:
-            e2e = (e2e_ms_max,) + e2e[1:]
-        tok = torch.tensor([w.n_tokens], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tok)
-        total_tokens = float(tok[0])
-    else:
-        total_tokens = float(w.n_tokens)
+    from paper_2604_02945_b200 import dist as D
+    ms, e2e_ms_max, total_tokens = D.reduce_timing(ms, w.n_tokens, device="cuda", extra_ms=e2e[0] if e2e else 0.0)
+    if e2e:
+        e2e = (e2e_ms_max,) + e2e[1:]
 
     if rank == 0:
         ms_step = ms / args.steps
@@ -245,15 +249,18 @@ def main():
                            "d2h_bytes_per_step": int(e2e[2]), "steps": e2e[3], "ms_per_step": e2e[0],
                            "api": "mas_forward_host (pinned host buffers in, MAS scores + mask + kept rows out)"}
         if world == 1 and not args.no_cpu_baseline:
-            n_req = {"single_image": 1, "batched_images": 40, "video": 1, "audio_vision": 3, "ragged": 12}[args.workload]
+            n_req = {"single_image": 1, "batched_images": 64, "video": 1, "audio_vision": 3, "ragged": 12}[args.workload]
             wb = w if args.workload != "video" else synth.video(seed=SEEDS["video"], R=1, T=8)
             fn, n_rows = oracle_sample(wb, min(n_req, wb.n_requests))
             t0 = time.perf_counter()
-            fn()
+            runs = 0
+            while runs == 0 or (time.perf_counter() - t0 < 10.0 and runs < 8):
+                fn()
+                runs += 1
             dt_o = time.perf_counter() - t0
-            line["cpu_baseline"] = {"value": n_rows / dt_o, "unit": "tokens/s", "cores": 1, "kind": "oracle",
+            line["cpu_baseline"] = {"value": runs * n_rows / dt_o, "unit": "tokens/s", "cores": 1, "kind": "oracle",
                                     "host_cores_available": os.cpu_count(),
-                                    "sample": "first %d request(s) = %d tokens, one run, %.1f s" % (n_req, n_rows, dt_o)}
+                                    "sample": "first %d request(s) = %d tokens, %d run(s), %.1f s" % (min(n_req, wb.n_requests), n_rows, runs, dt_o)}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
