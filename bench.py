@@ -73,6 +73,17 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons, "samples": len(rows)}
 
 
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the score kernel from the committed ncu capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    if os.path.exists(p):
+        for line in open(p).read().splitlines()[1:]:
+            k, v = line.split(",")
+            if k == workload:
+                return int(v)
+    return None
+
+
 def algorithmic_bytes(w, kept_rows):
     """X once + Q once + kept rows read and written + ~33 B of per-token scalars + 4 B per kept index."""
     e = 2 if w.dtype == "bf16" else 4
@@ -237,7 +248,7 @@ def main():
             "clocks": clocks,
             "gpu_launches": args.steps * plan.forward_launches,
             "roofline": {"bound": "hbm", "kernel": "score stage (a0-a3: norms, temporal difference, relevance contraction)",
-                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(args.workload),
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": score_bytes, "avg_launch_ms": score_ms,
                          "frac_of_8000_nominal": achieved / 8000.0},
             "stages_ms": {"score": score_ms, "segment_select": float(stage[:, 1].mean()), "gather": float(stage[:, 2].mean())},
