@@ -6,14 +6,16 @@
 //   query chunk Q[L, kc] into a multi-stage shared-memory ring.
 //   One elected thread issues tcgen05.mma (kind::f16, bf16 x bf16 -> fp32, M = 128, N = pad16(L), K = 16) accumulating
 //   S = X·Q^T in TMEM (two accumulators: the epilogue of tile i overlaps the MMAs of tile i+1).          (Eq. 6)
-//   Sixteen CUDA-core warps (four threads per token row) read the same shared-memory tiles — conflict-free thanks to
-//   the hardware swizzle — and accumulate sum x^2 and sum (x - x_prev)^2 with packed fp32x2 FMAs.    (Eq. 3, Eq. 5)
+//   Eight CUDA-core warps (two threads per token row and K-slice, half a 128-byte row each: the shorter the time a
+//   chunk spends being read, the more of the ring is in flight) read the same shared-memory tiles — conflict-free
+//   thanks to the hardware swizzle — and accumulate sum x^2 and sum (x - x_prev)^2 with packed fp32x2 FMAs. (Eq. 3, 5)
 //   Four epilogue warps read the accumulator rows with tcgen05.ld (one token row per thread, so the max over query
 //   tokens needs no shuffles), scale by 1/|q_j| and 1/|x_i| and write s, sqrt(D), rel: 12 B per token.
 //   The temporal ratio gamma = sqrt(D) / (|x_t| + |x_{t-1}|) is finished by the segment kernel, which has both norms
 //   from s; the previous row's norm is therefore never recomputed here.
 //
-// Persistent: one CTA per SM walks a host-built, cost-balanced (LPT) tile list.  Tiles never straddle a segment.
+// Persistent: one CTA per SM walks a host-built, cost-balanced tile list (round-robin bulk + gap filling).  Tiles never
+// straddle a segment.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -40,7 +42,8 @@ struct TcTile {            // 32 bytes
   int32_t pad_[2];
 };
 
-constexpr int kTcAluSets = 2;                        // ALU warp sets taking alternate chunks
+constexpr int kTcAluSets = 2;                        // ALU warp sets: each takes 8 / kTcAluSets of a row's eight 16-byte units
+constexpr int kTcAluUnits = 8 / kTcAluSets;
 constexpr int kTcAluWarps = 4 * kTcAluSets;          // per set: one (token row, K-slice) per thread
 constexpr int kTcThreads = 256 + 32 * kTcAluWarps;   // warps 0-7: TMA (X), MMA, TMEM, TMA (Q), 4 x epilogue; then the ALU warps
 constexpr int kTcSlots = 16;                         // mbarrier pairs of the chunk ring (slots are variable-sized)
@@ -291,7 +294,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 #endif
   pdl_launch_dependents();   // the segment kernel may be scheduled as SMs free up; it waits for this grid to complete
   if (warp == 1 && lane == 0) {
-    for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), (dbg & 32) ? 1 : 2); mbar_init(smem_u32(&ctrl->empty[i]), ((dbg & 512) ? 0 : 1) + ((dbg & 256) ? 0 : 4)); }
+    for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), (dbg & 32) ? 1 : 2); mbar_init(smem_u32(&ctrl->empty[i]), ((dbg & 512) ? 0 : 1) + ((dbg & 256) ? 0 : kTcAluWarps)); }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&ctrl->tmem_full[i]), 1); mbar_init(smem_u32(&ctrl->tmem_empty[i]), 4);
       mbar_init(smem_u32(&ctrl->stat_full[i]), kTcAluWarps); mbar_init(smem_u32(&ctrl->stat_empty[i]), 4);
@@ -453,7 +456,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   } else if (warp >= 8) {
     // ===================================================================== CUDA-core statistics: one thread per (row, K-slice)
     const int a = (tid - 256) & 127;
-    const uint32_t set = (uint32_t)(tid - 256) >> 7;      // this set takes the chunks with ring.k % kTcAluSets == set
+    const uint32_t set = (uint32_t)(tid - 256) >> 7;      // which share of the row's eight 16-byte units this thread reads
     TcRing ring;
 #ifdef MSAS_ABLATE
     long long alu_wait = 0;
@@ -472,7 +475,6 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       uint64_t n2a = 0, n2b = 0, Da = 0, Db = 0;     // packed fp32 pairs, all zero bits = (0.f, 0.f)
       for (int ch = 0; ch < g.nch; ++ch) {
         const uint32_t off = ring.place(g.need);
-        if (ring.k % (uint32_t)kTcAluSets != set) { ++ring.k; continue; }
 #ifdef MSAS_ABLATE
         const long long c0 = clock64();
 #endif
@@ -483,16 +485,17 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 #endif
         if (active) {
           const unsigned char* sx = ring0 + off + my_off;
-          uint4 x[8];
+          uint4 x[kTcAluUnits];
+          const uint32_t u0 = set * (uint32_t)kTcAluUnits;       // this set's share of the row's eight 16-byte units
 #pragma unroll
-          for (int u = 0; u < 8; ++u) x[u] = *reinterpret_cast<const uint4*>(sx + (((uint32_t)u ^ sw) << 4));
+          for (int u = 0; u < kTcAluUnits; ++u) x[u] = *reinterpret_cast<const uint4*>(sx + (((u0 + (uint32_t)u) ^ sw) << 4));
           if (g.has_prev && !(dbg & 2048)) {
             const unsigned char* su = sx + poff;
-            uint4 v[8];
+            uint4 v[kTcAluUnits];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) v[u] = *reinterpret_cast<const uint4*>(su + (((uint32_t)u ^ sw) << 4));
+            for (int u = 0; u < kTcAluUnits; ++u) v[u] = *reinterpret_cast<const uint4*>(su + (((u0 + (uint32_t)u) ^ sw) << 4));
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
+            for (int u = 0; u < kTcAluUnits; ++u) {
               const uint64_t x0 = bf16x2_to_f32x2(x[u].x), x1 = bf16x2_to_f32x2(x[u].y), x2 = bf16x2_to_f32x2(x[u].z), x3 = bf16x2_to_f32x2(x[u].w);
               const uint64_t e0 = sub_f32x2(x0, bf16x2_to_f32x2(v[u].x)), e1 = sub_f32x2(x1, bf16x2_to_f32x2(v[u].y));
               const uint64_t e2 = sub_f32x2(x2, bf16x2_to_f32x2(v[u].z)), e3 = sub_f32x2(x3, bf16x2_to_f32x2(v[u].w));
@@ -501,7 +504,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             }
           } else {
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
+            for (int u = 0; u < kTcAluUnits; ++u) {
               fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].x)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].y));
               fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].z)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].w));
             }
