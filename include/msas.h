@@ -169,6 +169,15 @@ int mas_forward(const mas_plan* plan, const void* X, const void* Q,
 int mas_forward_host(const mas_plan* plan, const void* h_X, const void* h_Q, void* d_X, void* d_Q,
                      const mas_outputs* d_out, const mas_outputs* h_out, mas_stream_t stream);
 
+/* ---- introspection (host only, no CUDA call): the tile schedule mas_plan_create would build for the tcgen05 score
+ * kernel on a device with `sm_count` SMs ("persistent CTAs over a host-built tile table; a tile
+ * never straddles a segment").  Writes up to `cap_tiles` records of 8 int32 each
+ * {cta, row_start, n_rows, q_row0, L, prev_delta, key_rows, 0} in per-CTA order and returns the number of tiles the
+ * schedule has (which may exceed cap_tiles), 0 if the shape does not take the fast path (fp32, d % 64 != 0), or a
+ * negative status (-MAS_ERR_*) for invalid descriptors.  Used by the CPU tests to check coverage and balance. */
+int32_t mas_score_schedule(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
+                           int32_t d, int32_t dtype, int32_t sm_count, int32_t* out_tiles, int32_t cap_tiles);
+
 #ifdef __cplusplus
 }
 #endif

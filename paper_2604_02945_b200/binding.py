@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host"]
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule"]
 
 
 class mas_segment(C.Structure):
@@ -83,6 +83,8 @@ def _load():
     lib.mas_select_compact.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
     lib.mas_forward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp]
     lib.mas_forward_host.argtypes = [vp, vp, vp, vp, vp, C.POINTER(mas_outputs), C.POINTER(mas_outputs), vp]
+    lib.mas_score_schedule.restype = i32
+    lib.mas_score_schedule.argtypes = [C.POINTER(mas_segment), i32, C.POINTER(i64), i32, i32, i32, i32, C.POINTER(i32), i32]
     for f in ("mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal",
               "mas_fuse", "mas_select_compact", "mas_forward", "mas_forward_host"):
         getattr(lib, f).restype = C.c_int
@@ -127,6 +129,20 @@ def make_segments(rows):
         arr[i] = mas_segment(req, mod, r0, T, P, k, 0)
         r0 += T * P
     return arr, r0
+
+
+def score_schedule(rows, q_off, d, dtype, sm_count=148):
+    """Host-only: the tile schedule of the tcgen05 score kernel as an int32 array [n_tiles, 8]
+    (cta, row_start, n_rows, q_row0, L, prev_delta, key_rows, 0); empty if the shape takes the generic path."""
+    segs, _ = make_segments(rows)
+    q = np.ascontiguousarray(q_off, np.int64)
+    qp = q.ctypes.data_as(C.POINTER(C.c_int64))
+    n = lib.mas_score_schedule(segs, len(list(rows)), qp, len(q) - 1, d, dtype, sm_count, None, 0)
+    if n < 0:
+        raise MasError(-n, "mas_score_schedule")
+    out = np.zeros((max(n, 1), 8), np.int32)
+    lib.mas_score_schedule(segs, len(list(rows)), qp, len(q) - 1, d, dtype, sm_count, out.ctypes.data_as(C.POINTER(C.c_int32)), n)
+    return out[:n]
 
 
 def workspace_bytes(segs, n_segs, q_off, d, dtype):

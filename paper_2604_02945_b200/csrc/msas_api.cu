@@ -267,6 +267,26 @@ extern "C" int64_t mas_plan_n_tokens(const mas_plan* p) { return p ? p->N : -1; 
 extern "C" int64_t mas_plan_n_queries(const mas_plan* p) { return p ? p->nQ : -1; }
 extern "C" int64_t mas_plan_kept_capacity(const mas_plan* p) { return p ? p->kept_cap : -1; }
 
+extern "C" int32_t mas_score_schedule(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
+                                      int32_t d, int32_t dtype, int32_t sm_count, int32_t* out_tiles, int32_t cap_tiles) {
+  int64_t N, nQ; int32_t nt, maxL;
+  const int st = validate(h_segs, n_segs, h_q_off, n_requests, d, dtype, nullptr, &N, &nQ, &nt, &maxL);
+  if (st != MAS_OK) return -st;
+  if (cap_tiles < 0 || (cap_tiles > 0 && !out_tiles)) return -MAS_ERR_INVALID_ARG;
+  std::vector<char> buf(tc_schedule_bytes(h_segs, n_segs));
+  TcSchedule sc;
+  tc_build_schedule(sc, h_segs, n_segs, h_q_off, d, dtype, sm_count, buf.data(), buf.data());
+  if (!sc.enabled) return 0;
+  const TcTile* t = reinterpret_cast<const TcTile*>(buf.data());
+  const int32_t* off = reinterpret_cast<const int32_t*>(buf.data() + (size_t)sc.n_tiles * sizeof(TcTile));
+  for (int c = 0; c < sc.n_ctas; ++c)
+    for (int i = off[c]; i < off[c + 1] && i < cap_tiles; ++i) {
+      int32_t* o = out_tiles + (size_t)i * 8;
+      o[0] = c; o[1] = t[i].row_start; o[2] = t[i].n_rows; o[3] = t[i].q_row0; o[4] = t[i].L; o[5] = t[i].prev_delta; o[6] = t[i].key_rows; o[7] = 0;
+    }
+  return sc.n_tiles;
+}
+
 // ------------------------------------------------------------------------------------------------ launches
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 

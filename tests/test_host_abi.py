@@ -83,3 +83,58 @@ def test_product_does_not_import_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle", src, flags=re.M), f
                 assert "mas_ref_" not in src and "mas_oracle" not in src, f
+
+
+def _segments_of(kind, rng):
+    """(rows, q_off) descriptor tables with the shapes of the five BASELINE.json configs (no token data needed)."""
+    rows, L = [], []
+    if kind == "images":
+        for r in range(64):
+            rows.append((r, 1, 1, 576, 144)); L.append(int(rng.integers(16, 65)))
+    elif kind == "video":
+        for r in range(8):
+            rows.append((r, 2, 32, 576, 2765)); L.append(48)
+    elif kind == "audio":
+        for r in range(16):
+            rows.append((r, 1, 1, 576, 144)); rows.append((r, 3, 1500, 1, 600)); L.append(64)
+    elif kind == "ragged":
+        for r in range(256):
+            n = int(rng.integers(144, 2881))
+            rows.append((r, 1, 1, n, 1) if rng.integers(2) else (r, 2, 5, n // 5, 1)); L.append(int(rng.integers(8, 129)))
+    elif kind == "tiny":
+        rows, L = [(0, 1, 1, 7, 1), (1, 2, 3, 5, 2)], [3, 128]
+    return rows, np.concatenate([[0], np.cumsum(L)]).astype(np.int64)
+
+
+@pytest.mark.parametrize("kind", ["images", "video", "audio", "ragged", "tiny"])
+def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
+    rng = np.random.default_rng(7)
+    rows, q_off = _segments_of(kind, rng)
+    t = B.score_schedule(rows, q_off, 4096, B.MAS_BF16, 148)
+    N = sum(r[2] * r[3] for r in rows)
+    assert len(t) > 0
+    cov = np.zeros(N, np.int32)
+    seg_of_row = np.concatenate([np.full(r[2] * r[3], k) for k, r in enumerate(rows)])
+    row0, P_of, q0_of = np.cumsum([0] + [r[2] * r[3] for r in rows]), [r[3] if r[2] > 1 else 0 for r in rows], [int(q_off[r[0]]) for r in rows]
+    for cta, rs, n, q0, L, pd, key, _ in t:
+        assert 1 <= n <= 128 and 0 <= cta < 148
+        cov[rs:rs + n] += 1
+        k = seg_of_row[rs]
+        assert seg_of_row[rs + n - 1] == k                       # a tile never straddles a segment
+        assert q0 == q0_of[k] and L == q_off[rows[k][0] + 1] - q_off[rows[k][0]] and pd == P_of[k]
+        assert key == (min(max(P_of[k] - (rs - row0[k]), 0), n) if pd else 0)   # rows of frame 0 have no previous frame
+    assert cov.min() == 1 and cov.max() == 1                     # every row exactly once
+    assert np.all(np.diff(t[:, 0]) >= 0)                         # grouped per CTA, CTAs in order
+    for c in np.unique(t[:, 0]):
+        assert np.all(np.diff(t[t[:, 0] == c, 1]) > 0)           # ascending rows inside a CTA
+    if N >= 148 * 128:
+        load = np.bincount(t[:, 0], weights=(t[:, 2] + 15) // 16 * 16, minlength=148)
+        assert load.max() <= 1.15 * load.mean()                  # rows per CTA within 15 % of the mean
+
+
+def test_score_schedule_rejects_bad_descriptors_and_generic_shapes(B):
+    rows, q_off = [(0, 1, 1, 576, 144)], np.array([0, 32], np.int64)
+    assert len(B.score_schedule(rows, q_off, 1024, B.MAS_F32)) == 0          # fp32 takes the generic path
+    assert len(B.score_schedule(rows, q_off, 1000, B.MAS_BF16)) == 0         # d % 64 != 0 too
+    with pytest.raises(B.MasError):
+        B.score_schedule(rows, np.array([0, 0], np.int64), 1024, B.MAS_BF16)  # L = 0
