@@ -36,11 +36,12 @@ struct SegArgs {
 constexpr int kSegThreads = 1024;
 
 struct SegSmem {
-  double red[3][32];
+  double red[6][32];
+  double tot[6];
   int ired[2][32];
   unsigned int hist[4][256];   // one histogram per radix pass (no reuse: no second cluster barrier per pass)
   int bcast[4];
-  double cx_d[4][3];           // cluster exchange: this CTA's block totals of reduction round 0..3
+  double cx_d[4][6];           // cluster exchange: this CTA's block totals of reduction round 0..3
   int cx_i[2];                 // cluster exchange: this CTA's (less, equal) counts
 };
 
@@ -68,15 +69,22 @@ template <> __device__ __forceinline__ unsigned dsmem_read<unsigned>(const unsig
   return (unsigned)dsmem_read<int>(reinterpret_cast<const int*>(local), rank);
 }
 
-// fixed-order block sum of up to three doubles; result broadcast to every thread
+// fixed-order block sum of up to three doubles (any block size that is a multiple of 32); result broadcast to every
+// thread.  The second round runs in warp 0 only: double shuffles are two SHFLs each and 32 warps doing them again
+// for the same 32 partials only queues up the shuffle pipe.
 __device__ __forceinline__ void block_sum3(SegSmem& sm, double& a, double& b, double& c) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
   __syncthreads();
   if (lane == 0) { sm.red[0][warp] = a; sm.red[1][warp] = b; sm.red[2][warp] = c; }
   __syncthreads();
-  double x = sm.red[0][lane], y = sm.red[1][lane], z = sm.red[2][lane];   // 32 warps
-  a = warp_sum(x); b = warp_sum(y); c = warp_sum(z);
+  if (warp == 0) {
+    double x = lane < nw ? sm.red[0][lane] : 0.0, y = lane < nw ? sm.red[1][lane] : 0.0, z = lane < nw ? sm.red[2][lane] : 0.0;
+    x = warp_sum(x); y = warp_sum(y); z = warp_sum(z);
+    if (lane == 0) { sm.tot[0] = x; sm.tot[1] = y; sm.tot[2] = z; }
+  }
+  __syncthreads();
+  a = sm.tot[0]; b = sm.tot[1]; c = sm.tot[2];
 }
 
 // exclusive prefix over the block of two small counts; also returns block totals
@@ -87,7 +95,8 @@ __device__ __forceinline__ void block_scan2(SegSmem& sm, int fa, int fb, int& pa
   __syncthreads();
   if (lane == 0) { sm.ired[0][warp] = __popc(ba); sm.ired[1][warp] = __popc(bb); }
   __syncthreads();
-  int wa = sm.ired[0][lane], wb = sm.ired[1][lane];
+  const int nw = blockDim.x >> 5;
+  int wa = lane < nw ? sm.ired[0][lane] : 0, wb = lane < nw ? sm.ired[1][lane] : 0;
   int ia = wa, ib = wb;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
@@ -121,12 +130,42 @@ __device__ __forceinline__ void cluster_sum3(SegSmem& sm, int round, unsigned nc
   __syncthreads();   // sm.red is reused by the next block_sum3
 }
 
+// six doubles at once (the one-pass segment statistics): same scheme, one block reduction and one cluster barrier
+__device__ __forceinline__ void cluster_sum6(SegSmem& sm, int round, unsigned nc, double (&v)[6]) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 6; ++k) v[k] = warp_sum(v[k]);
+  __syncthreads();
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < 6; ++k) sm.red[k][warp] = v[k];
+  }
+  __syncthreads();
+  if (warp == 0) {
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { const double x = warp_sum(lane < nw ? sm.red[k][lane] : 0.0); if (lane == 0) { sm.tot[k] = x; sm.cx_d[round][k] = x; } }
+  }
+  if (nc == 1) {
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 6; ++k) v[k] = sm.tot[k];
+    return;
+  }
+  cluster_sync_all();
+  if (threadIdx.x < 6 * nc) sm.red[threadIdx.x % 6][threadIdx.x / 6] = dsmem_read(&sm.cx_d[round][threadIdx.x % 6], threadIdx.x / 6);
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < 6; ++k) { double x = 0; for (unsigned r = 0; r < nc; ++r) x += sm.red[k][r]; v[k] = x; }   // rank order
+  __syncthreads();
+}
+
 // One thread-block CLUSTER per segment (cluster size chosen by the host from the longest segment; 1 for images):
 // CTA `rank` owns the contiguous token slice [lo, hi) of the segment; sums, radix histograms and kept counts are
 // combined over distributed shared memory, so an 18 432-token video segment is a few microseconds of latency, not 70.
 template <bool FUSE, bool SELECT>
 __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
   __shared__ SegSmem sm;
+  const int NT = blockDim.x;      // 256, 512 or 1024 (host: from the longest per-CTA slice)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned nc = cluster_size(), rank = cluster_rank();
   const int sidx = (int)cluster_id_x();
@@ -139,49 +178,69 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
   pdl_launch_dependents();
   pdl_wait();
 
+  constexpr int KPT = 4;          // tokens per thread whose scalars stay in registers between the passes
+  float c_s[KPT], c_r[KPT], c_g[KPT];
+  unsigned c_key[KPT];            // order-preserving keys of the cached tokens' MAS (selection passes)
+#pragma unroll
+  for (int it = 0; it < KPT; ++it) { c_s[it] = 0.f; c_r[it] = 0.f; c_g[it] = 0.f; c_key[it] = 0u; }
+
   if (FUSE) {
     const bool temporal = seg.n_frames > 1;
-    double ss = 0, sr = 0, sg = 0;
-    for (int i = lo + tid; i < hi; i += kSegThreads) {
-      const float si = a.s[base + i];
-      ss += (double)si;
-      sr += (double)a.rel[base + i];
-      if (a.gamma_raw) {   // finish Eq. 5's exact form: both norms are available here (same thread re-reads gamma below)
-        float g = 0.f;
-        if (temporal) {
-          if (i < seg.n_patches) g = 1.0f;
-          else { const float den = (si + a.s[base + i - seg.n_patches]) * a.sqrt_d; g = den > 0.f ? a.gamma[base + i] / den : 0.f; }
-        }
-        a.gamma[base + i] = g;
-        if (temporal && i >= seg.n_patches) sg += (double)g;
-      } else if (temporal && i >= seg.n_patches) sg += (double)a.gamma[base + i];
+    // pass A: one sweep gives sum and sum of squares (double: the cancellation in E[x^2] - mu^2 is ~1e-14 relative
+    // for these O(1) scalars); gamma is finished here (SPEC S2) because both norms are at hand
+    auto load_token = [&](int i, float& si, float& ri, float& gi) {
+      si = a.s[base + i];
+      ri = a.rel[base + i];
+      gi = 0.f;
+      if (temporal) {
+        if (a.gamma_raw) {
+          if (i < seg.n_patches) gi = 1.0f;
+          else { const float den = (si + a.s[base + i - seg.n_patches]) * a.sqrt_d; gi = den > 0.f ? a.gamma[base + i] / den : 0.f; }
+        } else gi = a.gamma[base + i];
+      }
+      if (a.gamma_raw) a.gamma[base + i] = gi;
+    };
+    double acc[6] = {0, 0, 0, 0, 0, 0};   // sum s, sum s^2, sum r, sum r^2, sum gamma (t >= 1), unused
+    auto accumulate = [&](int i, float si, float ri, float gi) {
+      acc[0] += (double)si; acc[1] += (double)si * (double)si; acc[2] += (double)ri; acc[3] += (double)ri * (double)ri;
+      if (temporal && i >= seg.n_patches) acc[4] += (double)gi;
+    };
+#pragma unroll
+    for (int it = 0; it < KPT; ++it) {
+      const int i = lo + tid + it * NT;
+      if (i < hi) { load_token(i, c_s[it], c_r[it], c_g[it]); accumulate(i, c_s[it], c_r[it], c_g[it]); }
     }
-    cluster_sum3(sm, 0, nc, ss, sr, sg);
-    const double mu_s = ss / n, mu_r = sr / n;
-    const double gavg = temporal ? sg / ((double)(seg.n_frames - 1) * seg.n_patches) : 0.0;
-    double vs = 0, vr = 0, dummy = 0;
-    for (int i = lo + tid; i < hi; i += kSegThreads) {
-      const double ds = (double)a.s[base + i] - mu_s, dr = (double)a.rel[base + i] - mu_r;
-      vs += ds * ds; vr += dr * dr;
-    }
-    cluster_sum3(sm, 1, nc, vs, vr, dummy);
-    const double sd_s = sqrt(vs / n), sd_r = sqrt(vr / n);
+    for (int i = lo + tid + KPT * NT; i < hi; i += NT) { float si, ri, gi; load_token(i, si, ri, gi); accumulate(i, si, ri, gi); }
+    cluster_sum6(sm, 0, nc, acc);
+    const double mu_s = acc[0] / n, mu_r = acc[2] / n;
+    const double gavg = temporal ? acc[4] / ((double)(seg.n_frames - 1) * seg.n_patches) : 0.0;
+    const double sd_s = sqrt(fmax(acc[1] / n - mu_s * mu_s, 0.0)), sd_r = sqrt(fmax(acc[3] / n - mu_r * mu_r, 0.0));
     const double den_s = fmax(sd_s, 1e-6 * mu_s), den_r = fmax(sd_r, 1e-6);
     const float inv_s = den_s > 0.0 ? (float)(1.0 / den_s) : 0.f, inv_r = (float)(1.0 / den_r);
     const float at = temporal ? p.lambda_temp : 0.f;
     int below = 0;
-    for (int i = lo + tid; i < hi; i += kSegThreads) {
-      // differences in double (s, rel are fp32 values; the means are not representable in fp32)
-      const float z = (float)(((double)a.s[base + i] - mu_s)) * inv_s;
+    // pass B: per-token M, g, MAS (differences in double: the means are not representable in fp32)
+    auto fuse_token = [&](int i, float si, float ri, float gi) {
+      const float z = (float)(((double)si - mu_s)) * inv_s;
       const float M = sigmoidf_acc(p.spatial_gain * z + p.spatial_bias);
-      const float zr = (float)(((double)a.rel[base + i] - mu_r)) * inv_r;
+      const float zr = (float)(((double)ri - mu_r)) * inv_r;
       const float g = sigmoidf_acc(p.rel_gain * zr + p.rel_bias);
-      const float gam = temporal ? a.gamma[base + i] : 0.f;
-      const float mas = 1.0f - g * (1.0f - p.lambda_spatial * (1.0f - M) - at * (1.0f - gam));
+      const float mas = 1.0f - g * (1.0f - p.lambda_spatial * (1.0f - M) - at * (1.0f - gi));
       if (a.m_spatial) a.m_spatial[base + i] = M;
       a.mas_tok[base + i] = mas;
       below += M < p.tau_s ? 1 : 0;
+      return mas;
+    };
+#pragma unroll
+    for (int it = 0; it < KPT; ++it) {
+      const int i = lo + tid + it * NT;
+      if (i < hi) c_key[it] = float_key(fuse_token(i, c_s[it], c_r[it], c_g[it]));
     }
+    for (int i = lo + tid + KPT * NT; i < hi; i += NT) {
+      float si = a.s[base + i], ri = a.rel[base + i], gi = temporal ? a.gamma[base + i] : 0.f;
+      fuse_token(i, si, ri, gi);
+    }
+    const double sd_s_out = sd_s;
     double db = below, d1 = 0, d2 = 0;
     cluster_sum3(sm, 2, nc, db, d1, d2);
     if (rank == 0 && tid == 0 && a.seg_out) {
@@ -190,7 +249,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
       o.gamma_avg = (float)gavg;
       o.alpha_mean = (float)mu_r;
       o.beta = 0.f; o.mas = 0.f;
-      o.mean_s = (float)mu_s; o.std_s = (float)sd_s;
+      o.mean_s = (float)mu_s; o.std_s = (float)sd_s_out;
       o.n_tokens = n; o.n_kept = 0;
       a.seg_out[sidx] = o;
     }
@@ -199,6 +258,18 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
 
   if (SELECT) {
     const float* mas = a.mas_tok + base;
+    if (!FUSE) {
+#pragma unroll
+      for (int it = 0; it < KPT; ++it) { const int i = lo + tid + it * NT; if (i < hi) c_key[it] = float_key(mas[i]); }
+    }
+    // visit this CTA's slice in index order, 1024 tokens at a time, with a block-uniform trip count (the callbacks
+    // vote and scan); the first KPT rounds take their keys from registers
+    auto for_each_round = [&](auto&& fn) {
+#pragma unroll
+      for (int it = 0; it < KPT; ++it)
+        if (lo + it * NT < hi) { const int i = lo + it * NT + tid; fn(i, i < hi, c_key[it]); }
+      for (int c0 = lo + KPT * NT; c0 < hi; c0 += NT) { const int i = c0 + tid; fn(i, i < hi, i < hi ? float_key(mas[i]) : 0u); }
+    };
     if (p.select_mode == MAS_SELECT_TOPK) {
       int kk = seg.keep_k < n ? seg.keep_k : n;
       const int k_total = kk;
@@ -208,10 +279,8 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
 #pragma unroll 1
       for (int pass = 0; pass < 4; ++pass) {
         const int shift = 24 - 8 * pass;
-        for (int c0 = lo; c0 < hi; c0 += kSegThreads) {   // warp-uniform trip count: every lane takes part in the votes
-          const int i = c0 + tid;
-          const unsigned key = i < hi ? float_key(mas[i]) : 0u;
-          const bool act = i < hi && (key & maskbits) == prefix;
+        for_each_round([&](int, bool valid, unsigned key) {
+          const bool act = valid && (key & maskbits) == prefix;
           const unsigned bin = (key >> shift) & 255u;
           // MAS scores share their leading bytes: aggregate equal bins inside the warp, one shared-memory atomic per bin
           const unsigned am = __ballot_sync(0xffffffffu, act);
@@ -219,7 +288,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
             const unsigned peers = __match_any_sync(am, bin);
             if (lane == __ffs(peers) - 1) atomicAdd(&sm.hist[pass][bin], (unsigned)__popc(peers));
           }
-        }
+        });
         __syncthreads();
         if (nc > 1) {   // cluster-wide histogram: thread b sums bin b over the peers (independent remote loads), in place
           cluster_sync_all();   // every CTA's histogram of this pass is complete and visible
@@ -260,7 +329,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
       int run_less = 0, run_eq = 0;
       if (nc > 1) {   // kept tokens of the lower-ranked CTAs come first: exchange the per-CTA (less, equal) counts
         int cl = 0, ce = 0;
-        for (int i = lo + tid; i < hi; i += kSegThreads) { const unsigned key = float_key(mas[i]); cl += key < prefix; ce += key == prefix; }
+        for_each_round([&](int, bool valid, unsigned key) { cl += valid && key < prefix; ce += valid && key == prefix; });
         double dl = cl, de = ce, d0 = 0;
         block_sum3(sm, dl, de, d0);
         if (tid == 0) { sm.cx_i[0] = (int)dl; sm.cx_i[1] = (int)de; }
@@ -271,11 +340,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         run_less = pl; run_eq = pe;
       }
       const int64_t off = seg.kept_off_static;
-      for (int c0 = lo; c0 < hi; c0 += kSegThreads) {
-        const int i = c0 + tid;
-        unsigned key = 0xffffffffu;
-        bool valid = i < hi;
-        if (valid) key = float_key(mas[i]);
+      for_each_round([&](int i, bool valid, unsigned key) {
         const int fl = valid && key < prefix, fe = valid && key == prefix;
         int pl, pe, tl, te;
         block_scan2(sm, fl, fe, pl, pe, tl, te);
@@ -289,18 +354,19 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
           }
         }
         run_less += tl; run_eq += te;
-      }
+      });
       if (rank == 0 && tid == 0) {
         a.seg_nkept[sidx] = k_total;
         if (a.seg_out) a.seg_out[sidx].n_kept = k_total;
       }
     } else {
       int cnt = 0;
-      for (int i = lo + tid; i < hi; i += kSegThreads) {
-        const bool keep = mas[i] <= p.cut;
-        if (a.keep_mask) a.keep_mask[base + i] = keep ? 1 : 0;
+      const unsigned cut_key = float_key(p.cut);
+      for_each_round([&](int i, bool valid, unsigned key) {
+        const bool keep = valid && key <= cut_key;     // the key order is the float order (and -0 == +0)
+        if (valid && a.keep_mask) a.keep_mask[base + i] = keep ? 1 : 0;
         cnt += keep;
-      }
+      });
       double dc = cnt, d1 = 0, d2 = 0;
       cluster_sum3(sm, 3, nc, dc, d1, d2);
       if (rank == 0 && tid == 0) {
@@ -321,7 +387,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
   __threadfence();
   if (FUSE && a.seg_out) {
     volatile mas_segment_out* so = a.seg_out;
-    for (int r = tid; r < a.n_requests; r += kSegThreads) {
+    for (int r = tid; r < a.n_requests; r += NT) {
       const int k0 = a.req_seg_off[r], k1 = a.req_seg_off[r + 1];
       float mx = -INFINITY;
       for (int k = k0; k < k1; ++k) mx = fmaxf(mx, p.kappa * so[k].alpha_mean);
@@ -337,12 +403,12 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
   }
   if (SELECT && a.kept_off) {
     if (p.select_mode == MAS_SELECT_TOPK) {
-      for (int k = tid; k < a.n_segs; k += kSegThreads) a.kept_off[k] = a.segs[k].kept_off_static;
+      for (int k = tid; k < a.n_segs; k += NT) a.kept_off[k] = a.segs[k].kept_off_static;
       if (tid == 0) a.kept_off[a.n_segs] = a.segs[a.n_segs - 1].kept_off_static + a.segs[a.n_segs - 1].keep_k;
     } else {
       volatile int32_t* nk = a.seg_nkept;
       long long run = 0;
-      for (int c0 = 0; c0 < a.n_segs; c0 += kSegThreads) {
+      for (int c0 = 0; c0 < a.n_segs; c0 += NT) {
         const int k = c0 + tid;
         const int v = k < a.n_segs ? nk[k] : 0;
         // inclusive scan of v over the block (values up to 2^31 in total fit a long long running sum)
@@ -352,7 +418,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         __syncthreads();
         if (lane == 31) sm.ired[0][warp] = inc;
         __syncthreads();
-        int wv = sm.ired[0][lane], winc = wv;
+        int wv = lane < (NT >> 5) ? sm.ired[0][lane] : 0, winc = wv;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += u; }
         const int wexc = __shfl_sync(0xffffffffu, winc - wv, warp);

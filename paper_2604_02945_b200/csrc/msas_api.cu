@@ -36,6 +36,7 @@ struct mas_plan {
   int32_t n_tiles = 0;
   int32_t max_L = 0;
   int32_t seg_cluster = 1;    // CTAs per segment in the segment kernel (from the longest segment)
+  int32_t seg_threads = 1024; // threads per CTA of the segment kernel
   DevParams prm{};
   Layout lay{};
   char* ws = nullptr;
@@ -225,6 +226,8 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     int c = 1;
     while (c < 8 && (int64_t)c * 2 * kSegThreads < longest) c *= 2;
     p->seg_cluster = c;
+    const int64_t slice = (longest + c - 1) / c;     // tokens per CTA: up to 4 stay in registers per thread
+    p->seg_threads = slice <= 1024 ? 256 : slice <= 2048 ? 512 : kSegThreads;
   }
   tc_build_schedule(p->tc, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched, p->ws + lay.tc_sched);
 
@@ -403,7 +406,7 @@ extern "C" int mas_fuse(const mas_plan* p, const float* s, const float* gamma, c
   cudaStream_t st = (cudaStream_t)stream;
   SegArgs a = seg_args(p, s, const_cast<float*>(gamma), rel, m_spatial, mas_tok, seg_out ? seg_out : p->at<mas_segment_out>(p->lay.segout),
                        nullptr, nullptr, nullptr, 0);
-  CK(launch_kc(k_segment<true, false>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3(kSegThreads), p->seg_cluster, st, false, a));
+  CK(launch_kc(k_segment<true, false>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3((unsigned)p->seg_threads), p->seg_cluster, st, false, a));
   return MAS_OK;
 }
 
@@ -417,7 +420,7 @@ extern "C" int mas_select_compact(const mas_plan* p, const void* X, const float*
   uint8_t* mask = keep_mask ? keep_mask : p->at<uint8_t>(p->lay.mask);
   int64_t* koff = kept_off ? kept_off : p->at<int64_t>(p->lay.keptoff);
   SegArgs a = seg_args(p, nullptr, nullptr, nullptr, nullptr, const_cast<float*>(mas_tok), seg_out, mask, kept_idx, koff, cap_rows);
-  CK(launch_kc(k_segment<false, true>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3(kSegThreads), p->seg_cluster, st, false, a));
+  CK(launch_kc(k_segment<false, true>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3((unsigned)p->seg_threads), p->seg_cluster, st, false, a));
   return launch_select_tail(p, X, mask, kept_idx, koff, Y, cap_rows, st);
 }
 
@@ -451,7 +454,7 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   }
   SegArgs a = seg_args(p, sb, gb, rb, m_spatial, mb, so, mask, kept_idx, koff, cap_rows, p->tc.enabled);
   if (pev) CK(cudaEventRecord(pev[1], st));
-  CK(launch_kc(k_segment<true, true>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3(kSegThreads), p->seg_cluster, st, pdl, a));
+  CK(launch_kc(k_segment<true, true>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3((unsigned)p->seg_threads), p->seg_cluster, st, pdl, a));
   if (p->prm.select_mode == MAS_SELECT_THRESHOLD && kept_idx) {
     CK(launch_k(k_compact_idx, dim3((unsigned)p->n_segs), dim3(kSegThreads), 0, st, pdl, (const DevSeg*)p->at<DevSeg>(p->lay.segs),
                 (const uint8_t*)mask, (const int64_t*)koff, kept_idx, cap_rows));
