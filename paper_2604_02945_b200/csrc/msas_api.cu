@@ -78,6 +78,14 @@ extern "C" int32_t mas_keep_count(int64_t n, double ratio) {
 }
 
 // ------------------------------------------------------------------------------------------------ validation + layout
+// Rows per tile of the generic (one CTA per tile) score kernels: 128, halved while the batch would not give every SM
+// of a B200 about two tiles (a single 576-token image becomes 36 tiles of 16 rows instead of 5 of 128).
+static int generic_tile_rows(int64_t n_total) {
+  int rows = kTileRows;
+  while (rows > 16 && n_total / rows < 296) rows >>= 1;
+  return rows;
+}
+
 static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_off, int32_t n_req, int32_t d, int32_t dtype,
                     const mas_params* prm, int64_t* N_out, int64_t* nQ_out, int32_t* n_tiles_out, int32_t* maxL_out) {
   if (!segs || !q_off || n_segs <= 0 || n_req <= 0) return MAS_ERR_INVALID_ARG;
@@ -105,7 +113,10 @@ static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_of
     if (prm && prm->select_mode == MAS_SELECT_TOPK && (s.keep_k < 1 || s.keep_k > n)) return MAS_ERR_INVALID_ARG;
     prev_req = s.request;
     row += n;
-    tiles += (n + kTileRows - 1) / kTileRows;
+  }
+  {
+    const int tr = generic_tile_rows(row);
+    for (int32_t k = 0; k < n_segs; ++k) { const int64_t n = (int64_t)segs[k].n_frames * segs[k].n_patches; tiles += (n + tr - 1) / tr; }
   }
   if (row > (int64_t)0x7fffffff - kTileRows) return MAS_ERR_UNSUPPORTED;   // kept_idx is int32
   if (prm) {
@@ -196,6 +207,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
   int64_t kept = 0;
   int32_t ti = 0;
   for (int32_t r = 0; r <= n_requests; ++r) hr[r] = n_segs;
+  const int tile_rows = generic_tile_rows(N);
   for (int32_t k = 0; k < n_segs; ++k) {
     const mas_segment& s = h_segs[k];
     DevSeg& ds = hs[k];
@@ -210,9 +222,9 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     ds.keep_k = params->select_mode == MAS_SELECT_TOPK ? s.keep_k : ds.n_rows;
     kept += params->select_mode == MAS_SELECT_TOPK ? s.keep_k : 0;
     if (hr[s.request] > k) hr[s.request] = k;
-    for (int32_t r0 = 0; r0 < ds.n_rows; r0 += kTileRows) {
+    for (int32_t r0 = 0; r0 < ds.n_rows; r0 += tile_rows) {
       ht[ti].row_start = (int32_t)(s.row0 + r0);
-      ht[ti].n_rows = ds.n_rows - r0 < kTileRows ? ds.n_rows - r0 : kTileRows;
+      ht[ti].n_rows = ds.n_rows - r0 < tile_rows ? ds.n_rows - r0 : tile_rows;
       ht[ti].seg = k;
       ++ti;
     }
