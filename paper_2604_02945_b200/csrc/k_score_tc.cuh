@@ -66,7 +66,11 @@ struct TcSchedule {
 struct TcParams {
   const TcTile* tiles;
   const int32_t* cta_off;
-  const float* qinv;
+  float* qinv;                       // [nQ] 1 / |q_j|, written by this kernel's own prologue (a0) and read by its epilogues
+  const void* Q;                     // query rows (bf16), for that prologue
+  long long nQ;
+  unsigned long long* q_ready;       // grid-wide arrival counter of the prologue (monotonic over launches)
+  unsigned long long q_target;       // value the counter reaches when every CTA of THIS launch has written its share
   float* s;
   float* dnorm;       // sqrt(sum (x - x_prev)^2) for rows that have a previous frame
   float* rel;
@@ -411,7 +415,28 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     const int q = warp - 4;                  // TMEM lane quarter this warp may access (warp % 4)
     const int r = q * 32 + lane;             // tile row
     const float inv_d = 1.0f / (float)p.d;
-    pdl_wait();                              // qinv comes from the query-prep kernel launched just before this one
+    // a0 inside the same launch: while the first tile streams in, these four warps compute 1 / |q_j| for this CTA's
+    // share of the query rows (row j belongs to CTA j % gridDim.x).  Every CTA of the grid is co-resident (cooperative
+    // launch), so the first epilogue may wait on the grid-wide counter for the other CTAs' shares.
+    {
+      const uint4* Qv = static_cast<const uint4*>(p.Q);
+      const int n16 = p.d >> 3;              // 16-byte pieces per bf16 row
+      for (long long j = (long long)blockIdx.x + (long long)q * gridDim.x; j < p.nQ; j += 4ll * gridDim.x) {
+        float acc = 0.f;
+        for (int i = lane; i < n16; i += 32) {
+          const uint4 v = ld_nc16(Qv + j * n16 + i);
+          const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+          for (int k = 0; k < 4; ++k) { const float a0 = bf_lo(w[k]), a1 = bf_hi(w[k]); acc = fmaf(a0, a0, acc); acc = fmaf(a1, a1, acc); }
+        }
+        acc = warp_sum(acc);
+        if (lane == 0) p.qinv[j] = acc > 0.f ? 1.0f / sqrtf(acc) : 0.f;
+      }
+      __threadfence();
+      asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
+      if (tid == 128) atomicAdd(p.q_ready, 1ull);
+    }
+    bool q_ok = false;
     int it = 0;
     for (int t = tile_lo; t < ((dbg & 128) ? tile_lo : tile_hi); ++t, ++it) {
       const TcTile tile = p.tiles[t];
@@ -422,6 +447,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const float* qinv = p.qinv + tile.q_row0;
       mbar_wait(smem_u32(&ctrl->tmem_full[acc]), ph);
       tc_fence_after();
+      if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
+        unsigned long long seen;
+        do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < p.q_target);
+        q_ok = true;
+      }
       float m = -INFINITY;
       for (int cb = 0; cb < nqb; ++cb) {
         uint32_t v[16];
@@ -430,7 +460,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
           const int col = cb * 16 + j;
-          if (col < tile.L) m = fmaxf(m, __uint_as_float(v[j]) * __ldg(qinv + col));
+          if (col < tile.L) m = fmaxf(m, __uint_as_float(v[j]) * qinv[col]);
         }
       }
       tc_fence_before();
@@ -703,16 +733,16 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
 }
 
 // returns 0 on success, -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error).
-// `pdl`: launch with programmatic stream serialization behind the query-prep kernel (the kernel waits for it itself).
-inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, const float* qinv, float* s, float* dnorm, float* rel,
-                           int64_t N, int64_t nQ, int d, bool pdl, cudaStream_t st) {
+// `q_ready` / `q_target`: the plan's monotonic arrival counter and the value it reaches at the end of this launch's prologue.
+inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, float* qinv, float* s, float* dnorm, float* rel,
+                           unsigned long long* q_ready, unsigned long long q_target, int64_t N, int64_t nQ, int d, cudaStream_t st) {
   TcMaps maps;
   for (int k = 0; k < 8; ++k)
     if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
   for (int k = 0; k < 3; ++k)
     if (!tc_make_map(&maps.q[k], Q, nQ, d, 64 >> k)) return -1;
   TcParams p;
-  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.s = s; p.dnorm = dnorm; p.rel = rel;
+  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.q_target = q_target; p.s = s; p.dnorm = dnorm; p.rel = rel;
   p.d = d; p.n_kchunks = d / 64;
 #ifdef MSAS_ABLATE
   p.dbg = getenv("MSAS_ABLATE") ? atoi(getenv("MSAS_ABLATE")) : 0;
@@ -721,9 +751,15 @@ inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, c
   p.dbg_t = dbuf;
   p.dbg_rows = (int)N;
 #endif
-  if (launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl, maps, p) !=
-      cudaSuccess)
-    return -1;
+  {   // cooperative launch: the query-norm prologue makes the CTAs wait on one another once, so all must be resident
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)sc.n_ctas); cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)sc.smem_bytes; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, k_score_tc, maps, p) != cudaSuccess) return -1;
+  }
 #ifdef MSAS_ABLATE
   if (getenv("MSAS_TIMES")) {
     cudaStreamSynchronize(st);

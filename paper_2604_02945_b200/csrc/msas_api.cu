@@ -35,6 +35,7 @@ struct mas_plan {
   int64_t N = 0, nQ = 0, kept_cap = 0;
   int32_t n_tiles = 0;
   int32_t max_L = 0;
+  mutable unsigned long long tc_epoch = 0;   // launches of the tcgen05 score kernel so far (its query-norm counter is monotonic)
   int32_t seg_cluster = 1;    // CTAs per segment in the segment kernel (from the longest segment)
   int32_t seg_threads = 1024; // threads per CTA of the segment kernel
   DevParams prm{};
@@ -378,8 +379,8 @@ static int launch_select_tail(const mas_plan* p, const void* X, const uint8_t* m
 
 extern "C" int32_t mas_plan_forward_launches(const mas_plan* p) {
   if (!p) return -1;
-  // [qprep +] score + segment (+ index compaction in threshold mode) + gather
-  return 4 + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
+  // [qprep, generic path only] + score + segment (+ index compaction in threshold mode) + gather
+  return (p->tc.enabled ? 3 : 4) + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
 }
 
 // ------------------------------------------------------------------------------------------------ staged entry points
@@ -456,12 +457,14 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   if (pev) CK(cudaEventRecord(pev[0], st));
   int rc;
   const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
-  if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
   if (p->tc.enabled) {
-    // a1-a3: TMA + tcgen05; gb receives sqrt(D), finished into gamma by the segment kernel
-    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->N, p->nQ, p->d, pdl, st);
+    // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
+    const unsigned long long target = ++p->tc_epoch * (unsigned long long)p->tc.n_ctas;
+    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, target, p->N,
+                         p->nQ, p->d, st);
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else {
+    if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
     if ((rc = launch_score_mma(p, X, Q, sb, gb, rb, nullptr, st)) != MAS_OK) return rc;
   }
   SegArgs a = seg_args(p, sb, gb, rb, m_spatial, mb, so, mask, kept_idx, koff, cap_rows, p->tc.enabled);
