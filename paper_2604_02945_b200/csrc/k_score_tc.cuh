@@ -34,7 +34,7 @@ namespace msas {
 
 struct TcTile {            // 32 bytes
   int32_t row_start;       // global row id of the first row
-  int32_t n_rows;          // valid rows, 1..128
+  int32_t n_rows;          // valid rows, 1..128, or up to 256 for a non-temporal "double" tile (two 128-row MMA halves sharing the query chunk)
   int32_t q_row0;          // first query row of the request
   int32_t L;               // query tokens of the request
   int32_t prev_delta;      // P if the segment is temporal (T > 1), else 0
@@ -52,7 +52,7 @@ constexpr int kTcCtrlBytes = 8192;
 constexpr int kTcRingBytes = (227 * 1024 - kTcCtrlBytes - 1024 - kTcBoxBytes) & ~1023;   // 1 KB alignment slack, 16 KB MMA over-read pad
 
 struct TcMaps {
-  CUtensorMap x[8];    // token rows: box = (16 * (i + 1)) rows x 64 columns
+  CUtensorMap x[16];   // token rows: box = (16 * (i + 1)) rows x 64 columns, up to the TMA limit of 256 rows
   CUtensorMap q[3];    // query rows: box = 64 / 32 / 16 rows x 64 columns
 };
 
@@ -106,7 +106,7 @@ struct TcRing {
 //   [kw x token slice (xbytes each)] [kw x previous-frame slice, temporal tiles only] [kw x query slice (qbytes each)]
 struct TcGeom {
   uint32_t xbytes, xall, qbytes, need;
-  int kw, nch, nqb;
+  int kw, nch, nqb, nh;   // nh = 128-row MMA halves of the tile (2 for a double tile)
   bool has_prev;
 };
 __device__ __forceinline__ TcGeom tc_geom(const TcTile& t, int nk, int dbg) {
@@ -118,6 +118,7 @@ __device__ __forceinline__ TcGeom tc_geom(const TcTile& t, int nk, int dbg) {
   int kw = rows16 <= 16 ? 8 : rows16 <= 32 ? 4 : rows16 <= 64 ? 2 : 1;
   while (kw > 1 && (kw * g.nqb > 16 || nk % kw != 0)) kw >>= 1;   // <= 32 KB of query rows per chunk; kw divides d / 64
   g.kw = kw;
+  g.nh = rows16 > 128 ? 2 : 1;
   g.nch = nk / kw;
   g.xall = g.xbytes * (g.has_prev ? 2u : 1u);
   g.qbytes = (uint32_t)g.nqb * 2048u;
@@ -305,8 +306,8 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 2) {   // TMEM: 2 accumulators x 128 fp32 columns
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctrl->tmem_base)), "r"(256) : "memory");
+  if (warp == 2) {   // TMEM: 2 tiles in flight x 2 halves x 128 fp32 columns (all 512 columns: one CTA per SM)
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctrl->tmem_base)), "r"(512) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   if (warp == 0 && lane == 0) {
@@ -388,7 +389,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
         if (!(dbg & 128)) mbar_wait(smem_u32(&ctrl->tmem_empty[acc]), acc_phase ^ 1u);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)acc * 128u;
+        const uint32_t d_tmem = tmem_base + (uint32_t)acc * 256u;
         for (int ch = 0; ch < g.nch; ++ch) {
           const uint32_t off = ring.place(g.need);
           mbar_wait(smem_u32(&ctrl->full[ring.slot()]), ring.parity());
@@ -396,12 +397,14 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           const uint32_t base = smem_u32(ring0 + off);
           if (!(dbg & 2)) {
             for (int j = 0; j < g.kw; ++j) {
-              // M = 128: rows past the tile read whatever follows in the ring (their accumulator rows are never used)
-              const uint64_t adesc = umma_desc_sw128(base + (uint32_t)j * g.xbytes);
               const uint64_t bdesc = umma_desc_sw128(base + (uint32_t)g.kw * g.xall + (uint32_t)j * g.qbytes);
+              for (int h = 0; h < g.nh; ++h) {
+                // M = 128: rows past the tile read whatever follows in the ring (their accumulator rows are never used)
+                const uint64_t adesc = umma_desc_sw128(base + (uint32_t)j * g.xbytes + (uint32_t)h * (uint32_t)kTcBoxBytes);
 #pragma unroll
-              for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
-                tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(ch | j | k));
+                for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
+                  tc_mma_bf16(d_tmem + (uint32_t)h * 128u, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(ch | j | k));
+              }
             }
           }
           tc_commit(smem_u32(&ctrl->empty[ring.slot()]));
@@ -452,35 +455,43 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < p.q_target);
         q_ok = true;
       }
-      float m = -INFINITY;
-      for (int cb = 0; cb < nqb; ++cb) {
-        uint32_t v[16];
-        tc_ld16(tmem_base + (uint32_t)acc * 128u + (uint32_t)cb * 16u + ((uint32_t)(q * 32) << 16), v);
-        tc_wait_ld();
+      float m[2] = {-INFINITY, -INFINITY};   // per 128-row half of the tile
+      for (int h = 0; h < g.nh; ++h)
+        for (int cb = 0; cb < nqb; ++cb) {
+          uint32_t v[16];
+          tc_ld16(tmem_base + (uint32_t)acc * 256u + (uint32_t)h * 128u + (uint32_t)cb * 16u + ((uint32_t)(q * 32) << 16), v);
+          tc_wait_ld();
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const int col = cb * 16 + j;
-          if (col < tile.L) m = fmaxf(m, __uint_as_float(v[j]) * qinv[col]);
+          for (int j = 0; j < 16; ++j) {
+            const int col = cb * 16 + j;
+            if (col < tile.L) m[h] = fmaxf(m[h], __uint_as_float(v[j]) * qinv[col]);
+          }
         }
-      }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->tmem_empty[acc]));
       mbar_wait(smem_u32(&ctrl->stat_full[acc]), ph);
-      float n2 = 0.f, D = 0.f;               // the ALU threads hold one partial per (row, K-slice of the chunk)
-      if (r < tile.n_rows) {
+      float n2[2] = {0.f, 0.f}, D[2] = {0.f, 0.f};
+      if (g.nh == 2) {                       // double tile: ALU thread `row` holds the whole row's sums, row = set * 128 + r
+#pragma unroll
+        for (int h = 0; h < 2; ++h) { n2[h] = ctrl->rowstat[acc][h][0][r]; D[h] = ctrl->rowstat[acc][h][1][r]; }
+      } else if (r < tile.n_rows) {          // one partial per (ALU set, K-slice of the chunk, row)
         const int rp2 = 128 / g.kw;
         for (int j = 0; j < g.kw; ++j)
 #pragma unroll
-          for (int st = 0; st < kTcAluSets; ++st) { n2 += ctrl->rowstat[acc][st][0][r + j * rp2]; D += ctrl->rowstat[acc][st][1][r + j * rp2]; }
+          for (int st = 0; st < kTcAluSets; ++st) { n2[0] += ctrl->rowstat[acc][st][0][r + j * rp2]; D[0] += ctrl->rowstat[acc][st][1][r + j * rp2]; }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_empty[acc]));
-      if (r < tile.n_rows) {
-        const int64_t row = (int64_t)tile.row_start + r;
-        p.s[row] = sqrtf(n2 * inv_d);
-        p.dnorm[row] = sqrtf(D);
-        p.rel[row] = n2 > 0.f ? m / sqrtf(n2) : 0.f;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int tr = h * 128 + r;
+        if (h < g.nh && tr < tile.n_rows) {
+          const int64_t row = (int64_t)tile.row_start + tr;
+          p.s[row] = sqrtf(n2[h] * inv_d);
+          p.dnorm[row] = sqrtf(D[h]);
+          p.rel[row] = n2[h] > 0.f ? m[h] / sqrtf(n2[h]) : 0.f;
+        }
       }
     }
   } else if (warp >= 8) {
@@ -496,7 +507,8 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const TcTile tile = p.tiles[t];
       const TcGeom g = tc_geom(tile, nk, dbg);
       const int rp2 = 128 / g.kw;
-      const int r = a & (rp2 - 1), j = a / rp2;
+      const bool dbl = g.nh == 2;                        // double tile: 256 threads = 256 rows, a whole row each, no previous frame
+      const int r = dbl ? (int)set * 128 + a : (a & (rp2 - 1)), j = dbl ? 0 : a / rp2;
       const bool active = r < tile.n_rows && !(dbg & 1);
       // hardware 128-byte swizzle: 16-byte unit u of row r sits at unit u ^ (r & 7)
       const uint32_t my_off = (uint32_t)j * g.xbytes + (uint32_t)r * 128u;
@@ -513,7 +525,17 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         alu_wait += clock64() - c0;
         if (tid == 256 && p.dbg_t && t == tile_lo && ch == 0) p.dbg_t[blockIdx.x * 8 + 2] = gtime();
 #endif
-        if (active) {
+        if (active && dbl) {
+          const unsigned char* sx = ring0 + off + my_off;
+          uint4 x[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) x[u] = *reinterpret_cast<const uint4*>(sx + (((uint32_t)u ^ sw) << 4));
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].x)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].y));
+            fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].z)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].w));
+          }
+        } else if (active) {
           const unsigned char* sx = ring0 + off + my_off;
           uint4 x[kTcAluUnits];
           const uint32_t u0 = set * (uint32_t)kTcAluUnits;       // this set's share of the row's eight 16-byte units
@@ -565,7 +587,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 #endif
   if (warp == 2) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(256) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
   }
 }
 
@@ -579,9 +601,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 // Short tiles keep the same bytes in flight (variable-size chunk ring) but re-stream the query chunks more often,
 // which is why only the fill phase uses them.
 struct TcCost {
-  double w_prev = 0.12, w_q = 0.20, c_tile = 2.0;
+  double w_prev = 0.25, w_q = 0.70, c_tile = 30.0;   // fitted to CTA finish times: ~27 us per MB of token rows, 12-19 us per MB of query rows, several us per tile
+  int hmax_plain = 256;
   TcCost() {
 #ifdef MSAS_ABLATE
+    if (getenv("MSAS_HMAX")) hmax_plain = atoi(getenv("MSAS_HMAX"));
     if (getenv("MSAS_WPREV")) w_prev = atof(getenv("MSAS_WPREV"));
     if (getenv("MSAS_WQ")) w_q = atof(getenv("MSAS_WQ"));
     if (getenv("MSAS_CTILE")) c_tile = atof(getenv("MSAS_CTILE"));
@@ -600,7 +624,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
   sc = TcSchedule();
   if (dtype != MAS_BF16 || d % 64 != 0 || sm_count < 1 || sm_count > 1000) return;
   const TcCost cw;
-  struct SegInfo { double w_row, c_fix; int L, P; };
+  struct SegInfo { double w_row, c_fix; int L, P, hmax; };   // hmax: tallest tile (256 = double tile, non-temporal only)
   std::vector<SegInfo> si(n_segs);
   double total = 0.0;
   int64_t n_full = 0;
@@ -610,9 +634,10 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     si[k].L = (int)(q_off[s.request + 1] - q_off[s.request]);
     si[k].P = s.n_frames > 1 ? s.n_patches : 0;
     si[k].w_row = 1.0 + (si[k].P > 0 ? cw.w_prev : 0.0);
+    si[k].hmax = si[k].P > 0 ? 128 : cw.hmax_plain;
     si[k].c_fix = cw.w_q * (((si[k].L + 15) / 16) * 16) + cw.c_tile;
-    total += (double)n * si[k].w_row + (double)((n + 127) / 128) * si[k].c_fix;
-    n_full += n / 128;
+    total += (double)n * si[k].w_row + (double)((n + si[k].hmax - 1) / si[k].hmax) * si[k].c_fix;
+    n_full += n / si[k].hmax;
   }
   const int n_ctas = (int)std::min<int64_t>(sm_count, std::max<int64_t>(1, (int64_t)(total / 64.0)));
 
@@ -631,7 +656,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     return (int)tiles.size() - 1;
   };
   double cost128_max = 0.0;
-  for (int32_t k = 0; k < n_segs; ++k) cost128_max = std::max(cost128_max, 128.0 * si[k].w_row + si[k].c_fix);
+  for (int32_t k = 0; k < n_segs; ++k) cost128_max = std::max(cost128_max, (double)si[k].hmax * si[k].w_row + si[k].c_fix);
   struct Piece { int32_t seg; int64_t r0, r1; };
   // one attempt at per-CTA target `target`; returns the heaviest CTA's load
   auto attempt = [&](double target) {
@@ -648,11 +673,11 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     for (int32_t k = 0; k < n_segs; ++k) {
       const int64_t n = (int64_t)segs[k].n_frames * segs[k].n_patches;
       int64_t r = 0;
-      while (n - r >= 128 && dealt < n_bulk) {
+      while (n - r >= si[k].hmax && dealt < n_bulk) {
         const int c = (int)(dealt % n_ctas);
-        per[c].push_back(make_tile(k, r, 128));
-        load[c] += 128.0 * si[k].w_row + si[k].c_fix;
-        r += 128; ++dealt;
+        per[c].push_back(make_tile(k, r, si[k].hmax));
+        load[c] += (double)si[k].hmax * si[k].w_row + si[k].c_fix;
+        r += si[k].hmax; ++dealt;
       }
       if (r < n) pieces.push_back(Piece{k, r, n});
     }
@@ -668,8 +693,8 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
         const int c = -top.second;
         const int64_t left = pc.r1 - r;
         int64_t h = (int64_t)((top.first - g.c_fix) / g.w_row) / 16 * 16;
-        h = std::max<int64_t>(32, std::min<int64_t>(128, h));
-        if (h >= left || left - h < 32) h = std::min<int64_t>(left, 128);
+        h = std::max<int64_t>(32, std::min<int64_t>(g.hmax, h));
+        if (h >= left || left - h < 32) h = std::min<int64_t>(left, g.hmax);
         per[c].push_back(make_tile(pc.seg, r, (int)h));
         load[c] += (double)((h + 15) / 16 * 16) * g.w_row + g.c_fix;
         heap.push(Gap(target - load[c], -c));
@@ -737,7 +762,7 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
 inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, float* qinv, float* s, float* dnorm, float* rel,
                            unsigned long long* q_ready, unsigned long long q_target, int64_t N, int64_t nQ, int d, cudaStream_t st) {
   TcMaps maps;
-  for (int k = 0; k < 8; ++k)
+  for (int k = 0; k < 16; ++k)
     if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
   for (int k = 0; k < 3; ++k)
     if (!tc_make_map(&maps.q[k], Q, nQ, d, 64 >> k)) return -1;
