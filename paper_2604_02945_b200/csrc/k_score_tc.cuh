@@ -13,6 +13,8 @@
 //   tokens needs no shuffles), scale by 1/|q_j| and 1/|x_i| and write s, sqrt(D), rel: 12 B per token.
 //   The temporal ratio gamma = sqrt(D) / (|x_t| + |x_{t-1}|) is finished by the segment kernel, which has both norms
 //   from s; the previous row's norm is therefore never recomputed here.
+//   The query norms (row a0) are computed by the epilogue warps while the first tile streams in; a non-temporal tile may
+//   be a 256-row "double" tile whose two 128-row MMA halves share one query chunk.
 //
 // Persistent: one CTA per SM walks a host-built, cost-balanced tile list (round-robin bulk + gap filling).  Tiles never
 // straddle a segment.
