@@ -269,3 +269,48 @@ FULL = [("batched_images", {}, [0, 31, 63]), ("video", {}, [5]), ("audio_vision"
 def test_forward_full_size_sampled(B, name, kw, sample):
     w = synth.make(name, **kw)
     _forward_and_compare(B, w, sample_requests=sample)
+
+
+# ---------------------------------------------------------------- segment sizes around every internal boundary
+def _random_workload(seed, seg_shapes, d, L_list, select_mode=0, cut=0.5, keep_ratio=0.3):
+    """seg_shapes: list of (request, modality, T, P); plain random rows (no planted structure needed here)."""
+    rng = np.random.default_rng(seed)
+    rows, n = [], 0
+    for (req, mod, T, P) in seg_shapes:
+        rows.append((req, mod, T, P, synth.keep_count(T * P, keep_ratio)))
+        n += T * P
+    X = rng.standard_normal((n, d)).astype(np.float32) * np.exp(0.5 * rng.standard_normal((n, 1))).astype(np.float32)
+    r0 = 0
+    for (req, mod, T, P) in seg_shapes:            # make temporal segments correlated, with some bit-identical rows
+        for t in range(1, T):
+            cur, prev = slice(r0 + t * P, r0 + (t + 1) * P), slice(r0 + (t - 1) * P, r0 + t * P)
+            X[cur] = 0.9 * X[prev] + 0.4 * X[cur]
+            same = np.nonzero(rng.random(P) < 0.3)[0]
+            X[r0 + t * P + same] = X[r0 + (t - 1) * P + same]      # copied in fp32: still bit-identical after rounding
+        r0 += T * P
+    q_off = np.concatenate([[0], np.cumsum(L_list)]).astype(np.int64)
+    Q = rng.standard_normal((int(q_off[-1]), d)).astype(np.float32)
+    Xb = synth.f32_to_bf16_bits(X)
+    return synth.Workload("sweep", d, "bf16", rows, q_off, Xb, synth.f32_to_bf16_bits(Q), select_mode=select_mode, cut=cut,
+                          salient=np.zeros(n, bool))
+
+
+SWEEPS = {
+    # double-tile boundaries of the score kernel (128 / 256 rows) and single-box heights, images and short videos
+    "tile_heights": ([(0, 1, 1, 1), (0, 1, 1, 15), (1, 1, 1, 129), (1, 2, 3, 90), (2, 1, 1, 200), (3, 1, 1, 256), (4, 1, 1, 257), (5, 1, 1, 600),
+                      (6, 2, 2, 130), (7, 3, 40, 1)], 128, [5, 33, 64, 1, 128, 17, 48, 9]),
+    # segment kernel: 2 CTAs per segment, 512 threads
+    "cluster2": ([(0, 1, 1, 2100), (0, 2, 3, 400), (1, 1, 1, 7)], 64, [12, 3]),
+    # 4 CTAs per segment
+    "cluster4": ([(0, 2, 5, 1000), (1, 1, 1, 300)], 64, [20, 6]),
+    # 8 CTAs per segment
+    "cluster8": ([(0, 1, 1, 9000), (1, 2, 2, 33)], 64, [7, 2]),
+}
+
+
+@pytest.mark.parametrize("name", list(SWEEPS), ids=list(SWEEPS))
+@pytest.mark.parametrize("mode", [0, 1], ids=["topk", "threshold"])
+def test_forward_segment_size_sweep(B, name, mode):
+    shapes, d, L = SWEEPS[name]
+    w = _random_workload(101 + mode, shapes, d, L, select_mode=mode, cut=0.45)
+    _forward_and_compare(B, w)
