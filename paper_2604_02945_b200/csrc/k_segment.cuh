@@ -39,7 +39,8 @@ struct SegSmem {
   double red[6][32];
   double tot[6];
   int ired[2][32];
-  unsigned int hist[4][256];   // one histogram per radix pass (no reuse: no second cluster barrier per pass)
+  unsigned int hist[4][256];   // one histogram per radix pass (never reused or overwritten: peers read them over DSMEM)
+  unsigned int htot[256];      // cluster-wide totals of the current pass
   int bcast[4];
   double cx_d[4][6];           // cluster exchange: this CTA's block totals of reduction round 0..3
   int cx_i[2];                 // cluster exchange: this CTA's (less, equal) counts
@@ -290,21 +291,22 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
           }
         });
         __syncthreads();
-        if (nc > 1) {   // cluster-wide histogram: thread b sums bin b over the peers (independent remote loads), in place
-          cluster_sync_all();   // every CTA's histogram of this pass is complete and visible
-          unsigned v[8];
+        const unsigned* hsrc = sm.hist[pass];
+        if (nc > 1) {   // cluster-wide histogram: thread b sums bin b over the peers (independent remote loads) into a
+          cluster_sync_all();   // private array, so the peers' bins are never overwritten: one cluster barrier per pass
           if (tid < 256) {
+            unsigned v[8];
 #pragma unroll
             for (unsigned r = 0; r < 8; ++r) v[r] = r < nc ? dsmem_read(&sm.hist[pass][tid], r) : 0u;
+            sm.htot[tid] = ((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]));
           }
-          cluster_sync_all();   // every peer has read this CTA's bins before they are overwritten with the totals
-          if (tid < 256) sm.hist[pass][tid] = ((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]));
           __syncthreads();
+          hsrc = sm.htot;
         }
         if (warp == 0) {   // find the bin where the cumulative count (over the whole cluster) reaches kk
           unsigned loc[8], tot = 0;
 #pragma unroll
-          for (int b = 0; b < 8; ++b) { loc[b] = sm.hist[pass][lane * 8 + b]; tot += loc[b]; }
+          for (int b = 0; b < 8; ++b) { loc[b] = hsrc[lane * 8 + b]; tot += loc[b]; }
           unsigned inc = tot;
 #pragma unroll
           for (int o = 1; o < 32; o <<= 1) { unsigned u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
