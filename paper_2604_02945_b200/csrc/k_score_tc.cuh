@@ -71,8 +71,8 @@ struct TcParams {
   float* qinv;                       // [nQ] 1 / |q_j|, written by this kernel's own prologue (a0) and read by its epilogues
   const void* Q;                     // query rows (bf16), for that prologue
   long long nQ;
-  unsigned long long* q_ready;       // grid-wide arrival counter of the prologue (monotonic over launches)
-  unsigned long long q_target;       // value the counter reaches when every CTA of THIS launch has written its share
+  unsigned long long* q_ready;       // [0] grid-wide arrival counter of the prologue, [1] CTAs that have left the kernel;
+                                     // both zero between launches (the last CTA to leave re-arms them: graph-replay safe)
   float* s;
   float* dnorm;       // sqrt(sum (x - x_prev)^2) for rows that have a previous frame
   float* rel;
@@ -454,7 +454,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       tc_fence_after();
       if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
         unsigned long long seen;
-        do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < p.q_target);
+        do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
         q_ok = true;
       }
       float m[2] = {-INFINITY, -INFINITY};   // per 128-row half of the tile
@@ -587,6 +587,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 #ifdef MSAS_ABLATE
   if (tid == 0 && p.dbg_t) p.dbg_t[blockIdx.x * 8 + 3] = gtime();
 #endif
+  if (tid == 0) {   // every CTA is past its wait on q_ready[0] by now; the last one out zeroes both counters
+    __threadfence();
+    if (atomicAdd(p.q_ready + 1, 1ull) == (unsigned long long)gridDim.x - 1ull) { p.q_ready[0] = 0ull; p.q_ready[1] = 0ull; __threadfence(); }
+  }
   if (warp == 2) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
@@ -760,16 +764,16 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
 }
 
 // returns 0 on success, -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error).
-// `q_ready` / `q_target`: the plan's monotonic arrival counter and the value it reaches at the end of this launch's prologue.
+// `q_ready`: two zero-initialised 64-bit words owned by the plan (the kernel leaves them zero).
 inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, float* qinv, float* s, float* dnorm, float* rel,
-                           unsigned long long* q_ready, unsigned long long q_target, int64_t N, int64_t nQ, int d, cudaStream_t st) {
+                           unsigned long long* q_ready, int64_t N, int64_t nQ, int d, cudaStream_t st) {
   TcMaps maps;
   for (int k = 0; k < 16; ++k)
     if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
   for (int k = 0; k < 3; ++k)
     if (!tc_make_map(&maps.q[k], Q, nQ, d, 64 >> k)) return -1;
   TcParams p;
-  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.q_target = q_target; p.s = s; p.dnorm = dnorm; p.rel = rel;
+  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.s = s; p.dnorm = dnorm; p.rel = rel;
   p.d = d; p.n_kchunks = d / 64;
 #ifdef MSAS_ABLATE
   p.dbg = getenv("MSAS_ABLATE") ? atoi(getenv("MSAS_ABLATE")) : 0;

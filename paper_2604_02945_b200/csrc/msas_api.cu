@@ -35,7 +35,6 @@ struct mas_plan {
   int64_t N = 0, nQ = 0, kept_cap = 0;
   int32_t n_tiles = 0;
   int32_t max_L = 0;
-  mutable unsigned long long tc_epoch = 0;   // launches of the tcgen05 score kernel so far (its query-norm counter is monotonic)
   int32_t seg_cluster = 1;    // CTAs per segment in the segment kernel (from the longest segment)
   int32_t seg_threads = 1024; // threads per CTA of the segment kernel
   DevParams prm{};
@@ -459,8 +458,7 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
   if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
-    const unsigned long long target = ++p->tc_epoch * (unsigned long long)p->tc.n_ctas;
-    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, target, p->N,
+    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
                          p->nQ, p->d, st);
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else {
