@@ -81,7 +81,6 @@ struct TcParams {
 #ifdef MSAS_ABLATE
   int dbg;            // development only: bit0 no ALU math, bit1 no MMA, bit2 no Q loads, bit3 no prev loads
   unsigned long long* dbg_t;
-  int dbg_rows;
 #endif
 };
 
@@ -248,60 +247,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   constexpr int dbg = 0;
 #endif
 
-#ifdef MSAS_ABLATE
-  if (dbg & 64) {   // probe mode: the bare streaming loop of _work/probe/tmabw.cu inside this kernel and harness
-    uint64_t* full = ctrl->full; uint64_t* empty = ctrl->empty;
-    if (tid == 0) { for (int i = 0; i < 12; ++i) { mbar_init(smem_u32(&full[i]), 1); mbar_init(smem_u32(&empty[i]), 1); } asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-    __syncthreads();
-    const int n_tiles = p.dbg_rows / 128;
-    if (tid == 0 && (dbg & 1024)) {   // the real tile list, one 128-row box per tile and K-slice
-      int stage = 0; uint32_t ph = 0;
-      for (int t = tile_lo; t < tile_hi; ++t) {
-        const int row = p.tiles[t].row_start;
-        for (int cg = 0; cg < nk; ++cg) {
-          mbar_wait(smem_u32(&empty[stage]), ph ^ 1u);
-          uint32_t bar = smem_u32(&full[stage]);
-          mbar_expect_tx(bar, 16384);
-          tma_load_2d(smem_u32(ring0 + stage * 16384), &mx128, bar, cg * 64, row);
-          if (++stage == 12) { stage = 0; ph ^= 1u; }
-        }
-      }
-    } else if (tid == 32 && (dbg & 1024)) {
-      int stage = 0; uint32_t ph = 0;
-      for (int t = tile_lo; t < tile_hi; ++t)
-        for (int cg = 0; cg < nk; ++cg) {
-          mbar_wait(smem_u32(&full[stage]), ph);
-          mbar_arrive(smem_u32(&empty[stage]));
-          if (++stage == 12) { stage = 0; ph ^= 1u; }
-        }
-    } else if (dbg & 1024) {
-    } else if (tid == 0) {
-      int stage = 0; uint32_t ph = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x)
-        for (int cg = 0; cg < nk; ++cg) {
-          mbar_wait(smem_u32(&empty[stage]), ph ^ 1u);
-          uint32_t bar = smem_u32(&full[stage]);
-          mbar_expect_tx(bar, 16384);
-          tma_load_2d(smem_u32(ring0 + stage * 16384), &mx128, bar, cg * 64, t * 128);
-          if (++stage == 12) { stage = 0; ph ^= 1u; }
-        }
-    } else if (tid == 32) {
-      int stage = 0; uint32_t ph = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x)
-        for (int cg = 0; cg < nk; ++cg) {
-          mbar_wait(smem_u32(&full[stage]), ph);
-          mbar_arrive(smem_u32(&empty[stage]));
-          if (++stage == 12) { stage = 0; ph ^= 1u; }
-        }
-    }
-    __syncthreads();
-    if (tid == 0 && p.dbg_t) p.dbg_t[blockIdx.x * 8 + 3] = gtime();
-    return;
-  }
-#endif
   pdl_launch_dependents();   // the segment kernel may be scheduled as SMs free up; it waits for this grid to complete
   if (warp == 1 && lane == 0) {
-    for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), (dbg & 32) ? 1 : 2); mbar_init(smem_u32(&ctrl->empty[i]), ((dbg & 512) ? 0 : 1) + ((dbg & 256) ? 0 : kTcAluWarps)); }
+    for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), 2); mbar_init(smem_u32(&ctrl->empty[i]), 1 + kTcAluWarps); }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&ctrl->tmem_full[i]), 1); mbar_init(smem_u32(&ctrl->tmem_empty[i]), 4);
       mbar_init(smem_u32(&ctrl->stat_full[i]), kTcAluWarps); mbar_init(smem_u32(&ctrl->stat_empty[i]), 4);
@@ -322,7 +270,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   tc_fence_after();
   const uint32_t tmem_base = ctrl->tmem_base;
 
-  if (warp == 0 || (warp == 3 && !(dbg & 32))) {
+  if (warp == 0 || warp == 3) {
     // ===================================================================== TMA producers (one thread each)
     // warp 0 streams the token rows (and the previous-frame rows), warp 3 the query rows.  A single thread issues about
     // one instruction every few cycles, so the per-chunk loop is kept to a few dozen instructions per producer.
@@ -355,7 +303,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           const uint32_t bar = smem_u32(&ctrl->full[ring.slot()]);
           const uint32_t base = smem_u32(ring0 + off);
           if (xprod) {
-            const bool ld_prev = g.has_prev && !(dbg & 4096);
+            const bool ld_prev = g.has_prev;
             mbar_expect_tx(bar, (uint32_t)g.kw * (ld_prev ? g.xall : g.xbytes));
             for (int j = 0; j < g.kw; ++j) {
               const int c0 = (ch * g.kw + j) * 64;
@@ -380,7 +328,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     }
   } else if (warp == 1) {
     // ===================================================================== MMA issuer (one thread)
-    if (lane == 0 && !(dbg & 512)) {
+    if (lane == 0) {
       TcRing ring;
       int it = 0;
       for (int t = tile_lo; t < tile_hi; ++t, ++it) {
@@ -389,7 +337,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         const uint32_t idesc = umma_idesc_bf16(((tile.L + 15) >> 4) << 4);
         const int acc = it & 1;
         const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
-        if (!(dbg & 128)) mbar_wait(smem_u32(&ctrl->tmem_empty[acc]), acc_phase ^ 1u);
+        mbar_wait(smem_u32(&ctrl->tmem_empty[acc]), acc_phase ^ 1u);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)acc * 256u;
         for (int ch = 0; ch < g.nch; ++ch) {
@@ -412,7 +360,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           tc_commit(smem_u32(&ctrl->empty[ring.slot()]));
           ++ring.k;
         }
-        if (!(dbg & 128)) tc_commit(smem_u32(&ctrl->tmem_full[acc]));
+        tc_commit(smem_u32(&ctrl->tmem_full[acc]));
       }
     }
   } else if (warp >= 4 && warp < 8) {
@@ -443,7 +391,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     }
     bool q_ok = false;
     int it = 0;
-    for (int t = tile_lo; t < ((dbg & 128) ? tile_lo : tile_hi); ++t, ++it) {
+    for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
       const TcGeom g = tc_geom(tile, nk, dbg);
       const int acc = it & 1;
@@ -501,11 +449,8 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     const int a = (tid - 256) & 127;
     const uint32_t set = (uint32_t)(tid - 256) >> 7;      // which share of the row's eight 16-byte units this thread reads
     TcRing ring;
-#ifdef MSAS_ABLATE
-    long long alu_wait = 0;
-#endif
     int it = 0;
-    for (int t = tile_lo; t < ((dbg & 256) ? tile_lo : tile_hi); ++t, ++it) {
+    for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
       const TcGeom g = tc_geom(tile, nk, dbg);
       const int rp2 = 128 / g.kw;
@@ -519,12 +464,8 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       uint64_t n2a = 0, n2b = 0, Da = 0, Db = 0;     // packed fp32 pairs, all zero bits = (0.f, 0.f)
       for (int ch = 0; ch < g.nch; ++ch) {
         const uint32_t off = ring.place(g.need);
-#ifdef MSAS_ABLATE
-        const long long c0 = clock64();
-#endif
         mbar_wait(smem_u32(&ctrl->full[ring.slot()]), ring.parity());
 #ifdef MSAS_ABLATE
-        alu_wait += clock64() - c0;
         if (tid == 256 && p.dbg_t && t == tile_lo && ch == 0) p.dbg_t[blockIdx.x * 8 + 2] = gtime();
 #endif
         if (active && dbl) {
@@ -543,7 +484,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           const uint32_t u0 = set * (uint32_t)kTcAluUnits;       // this set's share of the row's eight 16-byte units
 #pragma unroll
           for (int u = 0; u < kTcAluUnits; ++u) x[u] = *reinterpret_cast<const uint4*>(sx + (((u0 + (uint32_t)u) ^ sw) << 4));
-          if (g.has_prev && !(dbg & 2048)) {
+          if (g.has_prev) {
             const unsigned char* su = sx + poff;
             uint4 v[kTcAluUnits];
 #pragma unroll
@@ -572,14 +513,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const float D = sum_f32x2(Da) + sum_f32x2(Db);
       const int buf = it & 1;
       const uint32_t ph = (uint32_t)(it >> 1) & 1u;
-      if (!(dbg & 128)) mbar_wait(smem_u32(&ctrl->stat_empty[buf]), ph ^ 1u);
+      mbar_wait(smem_u32(&ctrl->stat_empty[buf]), ph ^ 1u);
       ctrl->rowstat[buf][set][0][a] = n2; ctrl->rowstat[buf][set][1][a] = D;      // slot a = j * rp2 + r
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_full[buf]));
     }
-#ifdef MSAS_ABLATE
-    if (tid == 256 && p.dbg_t) p.dbg_t[blockIdx.x * 8 + 6] = alu_wait;
-#endif
   }
 
   tc_fence_before();
@@ -780,7 +718,6 @@ inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, f
   static unsigned long long* dbuf = nullptr;
   if (!dbuf) cudaMalloc(&dbuf, 4096 * 8);
   p.dbg_t = dbuf;
-  p.dbg_rows = (int)N;
 #endif
   {   // cooperative launch: the query-norm prologue makes the CTAs wait on one another once, so all must be resident
     cudaLaunchConfig_t cfg = {};
