@@ -169,6 +169,12 @@ int mas_forward(const mas_plan* plan, const void* X, const void* Q,
 int mas_forward_host(const mas_plan* plan, const void* h_X, const void* h_Q, void* d_X, void* d_Q,
                      const mas_outputs* d_out, const mas_outputs* h_out, mas_stream_t stream);
 
+/* The fused bf16 fast path computes the query norms (row a0) in the prologue of its score kernel, which needs every
+ * CTA of that kernel resident at once (cooperative launch).  Where that is impossible (e.g. a partitioned GPU) the
+ * library falls back by itself to a separate query-norm launch; `on = 0` forces that fallback (tests, diagnosis),
+ * `on = 1` (default) restores the single-launch form.  Results are identical either way. */
+int mas_plan_set_inline_query_norms(mas_plan* plan, int32_t on);
+
 /* ---- introspection (host only, no CUDA call): the tile schedule mas_plan_create would build for the tcgen05 score
  * kernel on a device with `sm_count` SMs ("persistent CTAs over a host-built tile table; a tile
  * never straddles a segment").  Writes up to `cap_tiles` records of 8 int32 each

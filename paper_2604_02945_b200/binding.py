@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule"]
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms"]
 
 
 class mas_segment(C.Structure):
@@ -83,6 +83,8 @@ def _load():
     lib.mas_select_compact.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
     lib.mas_forward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp]
     lib.mas_forward_host.argtypes = [vp, vp, vp, vp, vp, C.POINTER(mas_outputs), C.POINTER(mas_outputs), vp]
+    lib.mas_plan_set_inline_query_norms.restype = C.c_int
+    lib.mas_plan_set_inline_query_norms.argtypes = [vp, i32]
     lib.mas_score_schedule.restype = i32
     lib.mas_score_schedule.argtypes = [C.POINTER(mas_segment), i32, C.POINTER(i64), i32, i32, i32, i32, C.POINTER(i32), i32]
     for f in ("mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal",
@@ -195,6 +197,10 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+    def set_inline_query_norms(self, on):
+        _check(lib.mas_plan_set_inline_query_norms(self._h, 1 if on else 0), "mas_plan_set_inline_query_norms")
+        self.forward_launches = int(lib.mas_plan_forward_launches(self._h))
 
     def enable_profiling(self, max_calls):
         _check(lib.mas_plan_enable_profiling(self._h, int(max_calls)), "mas_plan_enable_profiling")

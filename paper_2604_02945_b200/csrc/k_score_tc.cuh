@@ -69,7 +69,7 @@ struct TcParams {
   const TcTile* tiles;
   const int32_t* cta_off;
   float* qinv;                       // [nQ] 1 / |q_j|, written by this kernel's own prologue (a0) and read by its epilogues
-  const void* Q;                     // query rows (bf16), for that prologue
+  const void* Q;                     // query rows (bf16), for that prologue; NULL = qinv was computed by k_qprep before this launch
   long long nQ;
   unsigned long long* q_ready;       // [0] grid-wide arrival counter of the prologue, [1] CTAs that have left the kernel;
                                      // both zero between launches (the last CTA to leave re-arms them: graph-replay safe)
@@ -371,7 +371,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     // a0 inside the same launch: while the first tile streams in, these four warps compute 1 / |q_j| for this CTA's
     // share of the query rows (row j belongs to CTA j % gridDim.x).  Every CTA of the grid is co-resident (cooperative
     // launch), so the first epilogue may wait on the grid-wide counter for the other CTAs' shares.
-    {
+    if (p.Q != nullptr) {
       const uint4* Qv = static_cast<const uint4*>(p.Q);
       const int n16 = p.d >> 3;              // 16-byte pieces per bf16 row
       for (long long j = (long long)blockIdx.x + (long long)q * gridDim.x; j < p.nQ; j += 4ll * gridDim.x) {
@@ -389,7 +389,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
       if (tid == 128) atomicAdd(p.q_ready, 1ull);
     }
-    bool q_ok = false;
+    bool q_ok = p.Q == nullptr;
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
@@ -525,7 +525,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 #ifdef MSAS_ABLATE
   if (tid == 0 && p.dbg_t) p.dbg_t[blockIdx.x * 8 + 3] = gtime();
 #endif
-  if (tid == 0) {   // every CTA is past its wait on q_ready[0] by now; the last one out zeroes both counters
+  if (tid == 0 && p.Q != nullptr) {   // every CTA is past its wait on q_ready[0] by now; the last one out zeroes both counters
     __threadfence();
     if (atomicAdd(p.q_ready + 1, 1ull) == (unsigned long long)gridDim.x - 1ull) { p.q_ready[0] = 0ull; p.q_ready[1] = 0ull; __threadfence(); }
   }
@@ -701,10 +701,11 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// returns 0 on success, -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error).
+// returns 0 on success, 1 if the cooperative launch is not possible on this device / partition (nothing was enqueued),
+// -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error).
 // `q_ready`: two zero-initialised 64-bit words owned by the plan (the kernel leaves them zero).
 inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, float* qinv, float* s, float* dnorm, float* rel,
-                           unsigned long long* q_ready, int64_t N, int64_t nQ, int d, cudaStream_t st) {
+                           unsigned long long* q_ready, int64_t N, int64_t nQ, int d, bool inline_qprep, cudaStream_t st) {
   TcMaps maps;
   for (int k = 0; k < 16; ++k)
     if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
@@ -719,14 +720,19 @@ inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, f
   if (!dbuf) cudaMalloc(&dbuf, 4096 * 8);
   p.dbg_t = dbuf;
 #endif
-  {   // cooperative launch: the query-norm prologue makes the CTAs wait on one another once, so all must be resident
+  if (!inline_qprep) {   // qinv is already there: no CTA waits on another one, a plain launch will do
+    p.Q = nullptr;
+    if (launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, false, maps, p) != cudaSuccess) return -1;
+  } else {   // cooperative launch: the query-norm prologue makes the CTAs wait on one another once, so all must be resident
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)sc.n_ctas); cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)sc.smem_bytes; cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (cudaLaunchKernelEx(&cfg, k_score_tc, maps, p) != cudaSuccess) return -1;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, k_score_tc, maps, p);
+    if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) return 1;   // caller: run k_qprep, then launch with inline_qprep = false
+    if (e != cudaSuccess) return -1;
   }
 #ifdef MSAS_ABLATE
   if (getenv("MSAS_TIMES")) {

@@ -35,6 +35,7 @@ struct mas_plan {
   int64_t N = 0, nQ = 0, kept_cap = 0;
   int32_t n_tiles = 0;
   int32_t max_L = 0;
+  bool tc_inline_qnorm = true; // query norms in the score kernel's prologue (cooperative launch) vs a launch of their own
   int32_t seg_cluster = 1;    // CTAs per segment in the segment kernel (from the longest segment)
   int32_t seg_threads = 1024; // threads per CTA of the segment kernel
   DevParams prm{};
@@ -278,6 +279,11 @@ extern "C" int mas_plan_destroy(mas_plan* p) {
   delete p;
   return MAS_OK;
 }
+extern "C" int mas_plan_set_inline_query_norms(mas_plan* p, int32_t on) {
+  if (!p) return MAS_ERR_INVALID_ARG;
+  p->tc_inline_qnorm = on != 0;
+  return MAS_OK;
+}
 extern "C" int64_t mas_plan_n_tokens(const mas_plan* p) { return p ? p->N : -1; }
 extern "C" int64_t mas_plan_n_queries(const mas_plan* p) { return p ? p->nQ : -1; }
 extern "C" int64_t mas_plan_kept_capacity(const mas_plan* p) { return p ? p->kept_cap : -1; }
@@ -379,7 +385,7 @@ static int launch_select_tail(const mas_plan* p, const void* X, const uint8_t* m
 extern "C" int32_t mas_plan_forward_launches(const mas_plan* p) {
   if (!p) return -1;
   // [qprep, generic path only] + score + segment (+ index compaction in threshold mode) + gather
-  return (p->tc.enabled ? 3 : 4) + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
+  return (p->tc.enabled && p->tc_inline_qnorm ? 3 : 4) + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
 }
 
 // ------------------------------------------------------------------------------------------------ staged entry points
@@ -456,10 +462,21 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   if (pev) CK(cudaEventRecord(pev[0], st));
   int rc;
   const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
-  if (p->tc.enabled) {
+  if (p->tc.enabled && !p->tc_inline_qnorm) {
+    if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
+    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
+                         p->nQ, p->d, false, st);
+    if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
+  } else if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
     rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, st);
+                         p->nQ, p->d, true, st);
+    if (rc == 1) {   // not all CTAs can be co-resident here (e.g. an MPS partition): query norms in their own launch
+      (void)cudaGetLastError();
+      if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
+      rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
+                           p->nQ, p->d, false, st);
+    }
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else {
     if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;

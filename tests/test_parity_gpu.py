@@ -314,3 +314,20 @@ def test_forward_segment_size_sweep(B, name, mode):
     shapes, d, L = SWEEPS[name]
     w = _random_workload(101 + mode, shapes, d, L, select_mode=mode, cut=0.45)
     _forward_and_compare(B, w)
+
+
+def test_separate_query_norm_launch_gives_identical_results(B):
+    """The fallback for devices where the score kernel cannot be launched cooperatively: same bits."""
+    w = synth.video(seed=21, R=2, T=3, P=300, d=256, L=33)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    a = plan.forward(X, Q)
+    torch.cuda.synchronize()
+    n_inline = plan.forward_launches
+    plan.set_inline_query_norms(False)
+    assert plan.forward_launches == n_inline + 1
+    b = plan.forward(X, Q)
+    torch.cuda.synchronize()
+    for k in ("m_spatial", "gamma", "rel", "mas_tok", "keep_mask", "kept_idx", "kept_off", "Y"):
+        assert torch.equal(a[k], b[k]), k
+    plan.close()
