@@ -8,6 +8,9 @@
 // Eq. 3-7; constants PAPER.md:255), written out step by step, single thread, every sum a `double` accumulated in
 // index order, inputs converted exactly (bf16 -> double, fp32 -> double). No blocking, fusion or reordering.
 //
+// NEXT-1 (mas_ref_temporal_lsh): pinned by explicit signs of hand-expanded projections, identical / negated rows,
+// power-of-two scaling, and the collision law E[gamma] = theta / pi.
+//
 // Pins (tests/test_oracle_pins.py, `-m "not gpu"`): explicit hand-expanded dot products, closed forms
 // (sigma(+-1), 1/sqrt2, 1/3, sin(theta/2)), invariances (query permutation, power-of-two scaling, duplicate query),
 // softmax identities, Eq. 7 special cases, brute-force sort/count for selection, numpy float64 cross-checks,
@@ -134,6 +137,38 @@ int mas_ref_temporal(const mas_ref_segment* segs, int32_t n_segs, int64_t d, int
         gamma[i] = den > 0.0 ? std::sqrt(D) / den : 0.0;
       }
     }
+  }
+  return 0;
+}
+
+// NEXT-1: the LITERAL probe of Eq. 5: K = 64 sign-random-projection hashes
+// h_k(x) = [r_k . x >= 0] from a supplied matrix R[64, d]; sim = (1/K) sum_k 1[h_k(f_t) = h_k(f_{t-1})],
+// gamma = 1 - sim = popcount(sig_t xor sig_{t-1}) / 64.  Per patch (G5), keyframe gamma = 1 (G6), T = 1 -> 0.
+// sig[i] bit k = h_k(x_i).  proj_opt (may be NULL): the 64 projections of every row, row-major [N, 64].
+int mas_ref_temporal_lsh(const mas_ref_segment* segs, int32_t n_segs, int64_t d, int dtype, const void* X, const void* R,
+                         uint64_t* sig, double* proj_opt, double* gamma) {
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const int64_t T = segs[k].n_frames, P = segs[k].n_patches, r0 = segs[k].row0;
+    for (int64_t i = r0; i < r0 + T * P; ++i) {
+      uint64_t bits = 0;
+      for (int h = 0; h < 64; ++h) {
+        double acc = 0.0;
+        for (int64_t c = 0; c < d; ++c) acc += elem(R, dtype, (int64_t)h * d + c) * elem(X, dtype, i * d + c);
+        if (proj_opt) proj_opt[i * 64 + h] = acc;
+        if (acc >= 0.0) bits |= (uint64_t)1 << h;
+      }
+      sig[i] = bits;
+    }
+    for (int64_t t = 0; t < T; ++t)
+      for (int64_t p = 0; p < P; ++p) {
+        const int64_t i = r0 + t * P + p;
+        if (T == 1) { gamma[i] = 0.0; continue; }
+        if (t == 0) { gamma[i] = 1.0; continue; }
+        uint64_t x = sig[i] ^ sig[i - P];
+        int cnt = 0;
+        while (x) { cnt += (int)(x & 1); x >>= 1; }
+        gamma[i] = (double)cnt / 64.0;
+      }
   }
   return 0;
 }

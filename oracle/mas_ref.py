@@ -107,6 +107,18 @@ def temporal(segs, X):
     return g
 
 
+def temporal_lsh(segs, X, R, want_proj=False):
+    """NEXT-1: literal LSH probe of Eq. 5 with K = 64 hashes from R[64, d] (same dtype as X)."""
+    X = np.ascontiguousarray(X)
+    R = np.ascontiguousarray(R)
+    assert R.shape == (64, X.shape[1]) and R.dtype == X.dtype
+    sig = np.zeros(X.shape[0], np.uint64)
+    g = np.zeros(X.shape[0], np.float64)
+    proj = np.zeros((X.shape[0], 64), np.float64) if want_proj else None
+    _check(lib().mas_ref_temporal_lsh(segs, len(segs), C.c_int64(X.shape[1]), _dtype_code(X), _p(X), _p(R), _p(sig), _p(proj), _p(g)))
+    return (sig, g, proj) if want_proj else (sig, g)
+
+
 def crossmodal(segs, q_off, X, Q, want_S=False):
     X = np.ascontiguousarray(X)
     Q = np.ascontiguousarray(Q)

@@ -380,3 +380,54 @@ def test_planted_salient_tokens_are_preferentially_kept():
     kept = r["keep_mask"].astype(bool)
     recall = (kept & w.salient).sum() / max(1, min(w.salient.sum(), kept.sum()))
     assert recall > 0.6
+
+
+# ---------------------------------------------------------------- NEXT-1: literal LSH probe (Eq. 5)
+def test_lsh_hand_expanded_bits():
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")):
+        if line.startswith("lsh_"):
+            k, v = line.split("#")[0].split("=")
+            gold[k.strip()] = float(v)
+    R = np.zeros((64, 4), np.float32)
+    R[0], R[1], R[2], R[3] = (1, 1, 1, 1), (-1, 0, 0, 0), (2, 1, 5, 0), (0, 0, 0, -1)
+    X = np.array([[1, -2, 0, 3], [-1, 2, 0, -3]], np.float32)
+    segs = seg1(2, 1)
+    sig, g, proj = O.temporal_lsh(segs, X, R, want_proj=True)
+    low4 = (sig & np.uint64(15)).astype(int)
+    assert low4[0] == int(gold["lsh_bits_x"]) and low4[1] == int(gold["lsh_bits_negx"])
+    assert np.all((sig >> np.uint64(4)) == np.uint64((1 << 60) - 1))          # zero rows of R project to 0 -> bit set
+    assert list(proj[0, :4]) == [2, -1, 0, -3]
+    assert g[0] == 1.0 and g[1] == gold["lsh_gamma_x_vs_negx_4hashes"]         # keyframe; 3 of 64 bits differ
+
+
+def test_lsh_identical_negated_scaled_and_single_frame():
+    rng = np.random.default_rng(5)
+    d, P = 32, 6
+    R = rng.standard_normal((64, d)).astype(np.float32)
+    f0 = rng.standard_normal((P, d)).astype(np.float32)
+    X = np.concatenate([f0, f0, -f0, 4.0 * f0]).astype(np.float32)            # frames: x, x, -x, 4x
+    segs = seg1(4, P)
+    sig, g = O.temporal_lsh(segs, X, R)
+    assert np.all(g[:P] == 1.0)                                                # keyframe (G6)
+    assert np.all(g[P:2 * P] == 0.0)                                           # identical rows -> identical signatures
+    assert np.all(g[2 * P:3 * P] == 1.0)                                       # negation flips every (non-zero) projection
+    assert np.all(g[3 * P:] == 1.0) and np.array_equal(sig[3 * P:], sig[:P])   # 4x has x's signature; vs -x all differ
+    segs1 = seg1(1, 4 * P)
+    assert np.all(O.temporal_lsh(segs1, X, R)[1] == 0.0)                       # T = 1: term not applicable
+    assert np.all(np.abs(g * 64 - np.round(g * 64)) == 0)                      # multiples of 1 / K
+
+
+def test_lsh_collision_law_theta_over_pi():
+    """Sign random projections collide with probability 1 - theta / pi (Goemans-Williamson / Charikar): E[gamma] = theta / pi."""
+    rng = np.random.default_rng(9)
+    d, P = 24, 3000
+    R = rng.standard_normal((64, d)).astype(np.float32)
+    for theta in (0.3, 1.0, 2.2):
+        a = rng.standard_normal((P, d)); a /= np.linalg.norm(a, axis=1, keepdims=True)
+        b = rng.standard_normal((P, d)); b -= (b * a).sum(1, keepdims=True) * a; b /= np.linalg.norm(b, axis=1, keepdims=True)
+        X = np.concatenate([a, np.cos(theta) * a + np.sin(theta) * b]).astype(np.float32)
+        segs = seg1(2, P)
+        g = O.temporal_lsh(segs, X, R)[1][P:]
+        # the 64 hashes are shared by all pairs, so average over pairs AND hashes: tolerance from the spread over hashes
+        assert abs(g.mean() - theta / np.pi) < 0.03, (theta, g.mean())
