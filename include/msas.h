@@ -156,6 +156,16 @@ int mas_select_compact(const mas_plan* plan, const void* X, const float* mas_tok
                        uint8_t* keep_mask /*[N]*/, int32_t* kept_idx /*[cap_rows]*/, int64_t* kept_off /*[n_segs+1]*/,
                        void* Y /*[cap_rows, d] or NULL*/, int64_t cap_rows, mas_segment_out* seg_out, mas_stream_t stream);
 
+/* NEXT-1: the LITERAL temporal probe of Eq. 5: K = MAS_LSH_K sign-random-projection
+ * hashes h_k(x) = [r_k . x >= 0] from the caller's matrix Rm[MAS_LSH_K, d] (device, same dtype and row stride as X,
+ * 16-byte aligned; any seeded Gaussian matrix), sim = (1/K) sum_k 1[h_k(f_t) = h_k(f_{t-1})], gamma = 1 - sim.
+ * sig[N] (device, required): bit k of sig[i] = h_k(x_i) -- the paper's "temporal similarity cache", 8 B per token.
+ * gamma_lsh[N] (device, may be NULL): popcount(sig_t xor sig_{t-1}) / K per patch; keyframe 1; T = 1 segments 0.
+ * The exact form mas_temporal computes is what this estimates (E[gamma_lsh] = angle / pi). */
+#define MAS_LSH_K 64
+int mas_temporal_lsh(const mas_plan* plan, const void* X, const void* Rm, uint64_t* sig /*[N]*/, float* gamma_lsh /*[N] or NULL*/,
+                     mas_stream_t stream);
+
 /* ---- fused entry point: one streaming score pass over X (a1+a2+a3), one segment kernel (a4+a5), one gather (a6).
  * Same outputs as the staged calls; any output may be NULL except kept_idx/kept_off when Y is requested. */
 int mas_forward(const mas_plan* plan, const void* X, const void* Q,

@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms"]
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh"]
 
 
 class mas_segment(C.Structure):
@@ -79,6 +79,8 @@ def _load():
     lib.mas_spatial.argtypes = [vp, vp, vp, vp, vp]
     lib.mas_temporal.argtypes = [vp, vp, vp, vp]
     lib.mas_crossmodal.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.mas_temporal_lsh.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.mas_temporal_lsh.restype = C.c_int
     lib.mas_fuse.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.mas_select_compact.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
     lib.mas_forward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp]
@@ -234,6 +236,13 @@ class Plan:
         g = self._f32()
         _check(lib.mas_temporal(self._h, _ptr(X), _ptr(g), _stream_ptr(stream)), "mas_temporal")
         return g
+
+    def temporal_lsh(self, X, Rm, stream=None):
+        """NEXT-1: signatures (int64 view of the uint64 bits) and gamma of the literal LSH probe; Rm = [64, d] like X."""
+        sig = torch.zeros(self.N, dtype=torch.int64, device=self.device)
+        g = self._f32()
+        _check(lib.mas_temporal_lsh(self._h, _ptr(X), _ptr(Rm), _ptr(sig), _ptr(g), _stream_ptr(stream)), "mas_temporal_lsh")
+        return sig, g
 
     def crossmodal(self, X, Q, want_S=False, stream=None):
         rel = self._f32()

@@ -21,6 +21,7 @@ struct ScoreArgs {
   float* gamma;    // may be NULL
   float* rel;      // may be NULL
   float* S_opt;    // may be NULL, [N, kMaxL]
+  unsigned long long* sig;   // LSH mode (NEXT-1): Q is the hash matrix R[64, d] shared by all rows; bit k of sig[row] = [r_k . x >= 0]
   int d;
 };
 
@@ -126,7 +127,7 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
   constexpr int NPLANE = DT == 1 ? 1 : 2;          // fp32: hi and lo planes
   constexpr int PIECES = (LP * 8 + 255) / 256;     // 16-byte pieces per thread per chunk
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, c = lane & 3;
-  const int d = a.d, L = seg.L;
+  const int d = a.d, L = a.sig ? 64 : seg.L;
   const int esz = DT == 1 ? 2 : 4;
 
   const int rl = warp * 16 + g, rh = rl + 8;
@@ -141,7 +142,7 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
   const char* x_hi = Xb + row_hi * (int64_t)d * esz;
   const char* p_lo = x_lo - (int64_t)seg.n_patches * d * esz;
   const char* p_hi = x_hi - (int64_t)seg.n_patches * d * esz;
-  const char* Qb = static_cast<const char*>(a.Q) + (int64_t)seg.q0 * d * esz;
+  const char* Qb = static_cast<const char*>(a.Q) + (a.sig ? (int64_t)0 : (int64_t)seg.q0 * d * esz);
 
   float acc[NT][4];
 #pragma unroll
@@ -256,7 +257,7 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
           bh[k] = pack_bf16x2(xh[2 * k] - bf_lo(ah[k]), xh[2 * k + 1] - bf_hi(ah[k]));
         }
       }
-      if (a.rel != nullptr || a.S_opt != nullptr) {
+      if (a.rel != nullptr || a.S_opt != nullptr || a.sig != nullptr) {
 #pragma unroll
         for (int j = 0; j < NT; ++j) {
           const int qr = j * 8 + g;
@@ -281,6 +282,21 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
   n2l = quad_sum(n2l); n2h = quad_sum(n2h);
   npl = quad_sum(npl); nph = quad_sum(nph);
   Dl = quad_sum(Dl); Dh = quad_sum(Dh);
+  if (a.sig != nullptr) {   // NEXT-1: pack the 64 hash bits of each row (this thread holds columns 8j + 2c, 8j + 2c + 1)
+    unsigned long long bl = 0ull, bh = 0ull;
+#pragma unroll
+    for (int j = 0; j < NT; ++j) {
+      const int c0 = j * 8 + 2 * c;
+      if (c0 < 64) {
+        bl |= (unsigned long long)(acc[j][0] >= 0.f) << c0 | (unsigned long long)(acc[j][1] >= 0.f) << (c0 + 1);
+        bh |= (unsigned long long)(acc[j][2] >= 0.f) << c0 | (unsigned long long)(acc[j][3] >= 0.f) << (c0 + 1);
+      }
+    }
+    bl |= __shfl_xor_sync(0xffffffffu, bl, 1); bl |= __shfl_xor_sync(0xffffffffu, bl, 2);
+    bh |= __shfl_xor_sync(0xffffffffu, bh, 1); bh |= __shfl_xor_sync(0xffffffffu, bh, 2);
+    if (c == 0) { if (vlo) a.sig[row_lo] = bl; if (vhi) a.sig[row_hi] = bh; }
+    return;
+  }
   float ml = -INFINITY, mh = -INFINITY;
   const float* qinv = a.qinv + seg.q0;
 #pragma unroll
@@ -333,6 +349,27 @@ __global__ void __launch_bounds__(256) k_score_mma(ScoreArgs a) {
   else if (seg.L <= 32) score_tile_mma<DT, 4>(a, tile, seg, smem);
   else if (seg.L <= 64) score_tile_mma<DT, 8>(a, tile, seg, smem);
   else score_tile_mma<DT, 16>(a, tile, seg, smem);
+}
+
+// NEXT-1: signatures of the literal LSH probe (Eq. 5): the same one-pass tile kernel with the 64 hash
+// rows as its B operand.
+template <int DT>
+__global__ void __launch_bounds__(256) k_lsh_sig(ScoreArgs a) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const DevTile tile = a.tiles[blockIdx.x];
+  const DevSeg seg = a.segs[tile.seg];
+  score_tile_mma<DT, 8>(a, tile, seg, smem);
+}
+// gamma_lsh = popcount(sig_t xor sig_{t-1}) / 64 per patch; keyframe 1; single-frame segments 0
+__global__ void __launch_bounds__(128) k_lsh_gamma(const DevSeg* segs, const DevTile* tiles, const unsigned long long* sig, float* gamma) {
+  const DevTile tile = tiles[blockIdx.x];
+  const DevSeg seg = segs[tile.seg];
+  for (int r = threadIdx.x; r < tile.n_rows; r += blockDim.x) {
+    const int64_t row = (int64_t)tile.row_start + r;
+    float g = 0.f;
+    if (seg.n_frames > 1) g = (row - seg.row0) < seg.n_patches ? 1.0f : (float)__popcll(sig[row] ^ sig[row - seg.n_patches]) * (1.0f / 64.0f);
+    gamma[row] = g;
+  }
 }
 
 constexpr int score_mma_smem_bytes(int dt) { return 2 * (16 * 8 * 128) * (dt == 1 ? 1 : 2); }

@@ -166,6 +166,8 @@ static std::once_flag g_attr_once;
 static void set_kernel_attrs() {
   cudaFuncSetAttribute(k_score_mma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
   cudaFuncSetAttribute(k_score_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
+  cudaFuncSetAttribute(k_lsh_sig<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
+  cudaFuncSetAttribute(k_lsh_sig<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
   tc_set_kernel_attrs();
   (void)cudaGetLastError();
 }
@@ -323,7 +325,7 @@ static ScoreArgs score_args(const mas_plan* p, const void* X, const void* Q, flo
   ScoreArgs a;
   a.X = X; a.Q = Q; a.qinv = p->at<float>(p->lay.qinv);
   a.segs = p->at<DevSeg>(p->lay.segs); a.tiles = p->at<DevTile>(p->lay.tiles);
-  a.s = s; a.gamma = gamma; a.rel = rel; a.S_opt = S_opt; a.d = p->d;
+  a.s = s; a.gamma = gamma; a.rel = rel; a.S_opt = S_opt; a.sig = nullptr; a.d = p->d;
   return a;
 }
 
@@ -407,6 +409,22 @@ extern "C" int mas_temporal(const mas_plan* p, const void* X, float* gamma, mas_
   if (!p || !X || !gamma) return MAS_ERR_INVALID_ARG;
   if (!aligned16(X)) return MAS_ERR_UNSUPPORTED;
   return launch_rowstats(p, X, nullptr, gamma, (cudaStream_t)stream);
+}
+
+extern "C" int mas_temporal_lsh(const mas_plan* p, const void* X, const void* Rm, uint64_t* sig, float* gamma_lsh, mas_stream_t stream) {
+  if (!p || !X || !Rm || !sig) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(Rm)) return MAS_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  ScoreArgs a = score_args(p, X, Rm, nullptr, nullptr, nullptr, nullptr);
+  a.sig = reinterpret_cast<unsigned long long*>(sig);
+  if (p->dtype == MAS_BF16) k_lsh_sig<1><<<p->n_tiles, 256, score_mma_smem_bytes(1), st>>>(a);
+  else k_lsh_sig<0><<<p->n_tiles, 256, score_mma_smem_bytes(0), st>>>(a);
+  CK(cudaGetLastError());
+  if (gamma_lsh) {
+    k_lsh_gamma<<<p->n_tiles, 128, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->at<DevTile>(p->lay.tiles), a.sig, gamma_lsh);
+    CK(cudaGetLastError());
+  }
+  return MAS_OK;
 }
 
 extern "C" int mas_crossmodal(const mas_plan* p, const void* X, const void* Q, float* rel, float* S_opt, mas_stream_t stream) {

@@ -331,3 +331,65 @@ def test_separate_query_norm_launch_gives_identical_results(B):
     for k in ("m_spatial", "gamma", "rel", "mas_tok", "keep_mask", "kept_idx", "kept_off", "Y"):
         assert torch.equal(a[k], b[k]), k
     plan.close()
+
+
+# ---------------------------------------------------------------- NEXT-1: literal LSH temporal probe (Eq. 5)
+def _popcount64(a):
+    a = a.astype(np.uint64)
+    return np.array([bin(int(v)).count("1") for v in a], np.int64)
+
+
+@pytest.mark.parametrize("w", [synth.video(seed=31, R=2, T=4, P=300, d=256, L=8), synth.video(seed=32, R=1, T=3, P=70, d=200, L=4, dtype="f32"),
+                               synth.audio_vision(seed=33, R=2, d=128, L=5, P_img=130, T_aud=260)],
+                         ids=["video_bf16", "video_f32_d200", "audio_vision"])
+def test_temporal_lsh_matches_oracle(B, w):
+    rng = np.random.default_rng(1234)
+    Rf = rng.standard_normal((64, w.d)).astype(np.float32)
+    Rm = synth.f32_to_bf16_bits(Rf) if w.dtype == "bf16" else Rf
+    segs, n = O.make_segments(w.segments)
+    sig_r, g_r, proj = O.temporal_lsh(segs, w.X, Rm, want_proj=True)
+    plan = _plan(B, w)
+    sig_t, g_t = plan.temporal_lsh(B.to_device(w.X), B.to_device(Rm))
+    torch.cuda.synchronize()
+    sig_g = sig_t.cpu().numpy().view(np.uint64)
+    g_g = g_t.cpu().numpy()
+    # a hash bit is decided by the sign of a projection: both sides must agree wherever the oracle's projection is not
+    # within rounding distance of zero (fp32 accumulation of exact bf16 products: ~1e-5 |x||r|; fp32 inputs go through a
+    # hi/lo bf16 split: ~1e-4)
+    Xf = synth.bf16_bits_to_f32(w.X) if w.dtype == "bf16" else w.X
+    Rff = synth.bf16_bits_to_f32(Rm) if w.dtype == "bf16" else Rm
+    bound = 2e-4 * np.linalg.norm(Xf.astype(np.float64), axis=1)[:, None] * np.linalg.norm(Rff.astype(np.float64), axis=1)[None, :]
+    decided = np.abs(proj) > bound
+    bits_r = ((sig_r[:, None] >> np.arange(64, dtype=np.uint64)[None, :]) & np.uint64(1)).astype(bool)
+    bits_g = ((sig_g[:, None] >> np.arange(64, dtype=np.uint64)[None, :]) & np.uint64(1)).astype(bool)
+    assert decided.mean() > 0.99
+    assert np.array_equal(bits_r[decided], bits_g[decided])
+    # gamma: exact function of the GPU's own signatures ...
+    row = 0
+    for (req, mod, T, P, k) in w.segments:
+        sl = slice(row, row + T * P)
+        if T == 1:
+            assert np.all(g_g[sl] == 0.0)
+        else:
+            assert np.all(g_g[row:row + P] == 1.0)
+            want = _popcount64(sig_g[row + P:row + T * P] ^ sig_g[row:row + (T - 1) * P]) / 64.0
+            assert np.array_equal(g_g[row + P:row + T * P], want.astype(np.float32))
+        row += T * P
+    # ... and within the undecided bits of the two rows of the oracle's gamma
+    und = (~decided).sum(1)
+    row = 0
+    for (req, mod, T, P, k) in w.segments:
+        if T > 1:
+            i = np.arange(row + P, row + T * P)
+            assert np.all(np.abs(g_g[i] - g_r[i]) <= (und[i] + und[i - P]) / 64.0 + 1e-7)
+        row += T * P
+    # bit-identical rows (the static patches of the video recipe) collide on every hash
+    same = np.zeros(n, bool)
+    row = 0
+    for (req, mod, T, P, k) in w.segments:
+        if T > 1:
+            i = np.arange(row + P, row + T * P)
+            same[i] = np.all(w.X[i] == w.X[i - P], axis=1)
+        row += T * P
+    assert np.all(g_g[same] == 0.0)
+    plan.close()
