@@ -172,6 +172,13 @@ int mas_forward(const mas_plan* plan, const void* X, const void* Q,
                 float* m_spatial, float* gamma, float* rel, float* mas_tok, mas_segment_out* seg_out,
                 uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows, mas_stream_t stream);
 
+/* mas_forward plus the literal LSH probe of NEXT-1 in the same pass: on the bf16 fast path with every L_r <= 64 the hash
+ * rows Rm ride the score kernel's tensor-core contraction as 64 more B rows (no second sweep over X); otherwise the
+ * call is mas_forward followed by mas_temporal_lsh.  `out`: device pointers as for mas_forward (any may be NULL as
+ * there); sig[N] required, gamma_lsh[N] may be NULL. */
+int mas_forward_lsh(const mas_plan* plan, const void* X, const void* Q, const void* Rm, uint64_t* sig /*[N]*/,
+                    float* gamma_lsh /*[N] or NULL*/, const mas_outputs* out, mas_stream_t stream);
+
 /* ---- end-to-end convenience: HOST inputs -> HOST outputs.
  * Copies h_X -> d_X and h_Q -> d_Q (cudaMemcpyAsync; pinned host memory recommended), runs mas_forward into d_out,
  * copies every non-NULL member of h_out back (Y/kept_idx: only the rows actually kept) and SYNCHRONISES the stream

@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh"]
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh"]
 
 
 class mas_segment(C.Structure):
@@ -81,6 +81,8 @@ def _load():
     lib.mas_crossmodal.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.mas_temporal_lsh.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.mas_temporal_lsh.restype = C.c_int
+    lib.mas_forward_lsh.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(mas_outputs), vp]
+    lib.mas_forward_lsh.restype = C.c_int
     lib.mas_fuse.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.mas_select_compact.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
     lib.mas_forward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp]
@@ -269,6 +271,15 @@ class Plan:
                                _ptr(o.get("mas_tok")), _ptr(o.get("seg_out")), _ptr(o.get("keep_mask")), _ptr(o.get("kept_idx")),
                                _ptr(o.get("kept_off")), _ptr(o.get("Y")), o["cap_rows"], _stream_ptr(stream)), "mas_forward")
         return o
+
+    def forward_lsh(self, X, Q, Rm, out=None, stream=None):
+        """mas_forward + the literal LSH probe in one pass: returns (outputs, sig int64 view, gamma_lsh)."""
+        o = out if out is not None else self.alloc_outputs()
+        sig = torch.zeros(self.N, dtype=torch.int64, device=self.device)
+        g = self._f32()
+        _check(lib.mas_forward_lsh(self._h, _ptr(X), _ptr(Q), _ptr(Rm), _ptr(sig), _ptr(g), C.byref(self._bundle(o)), _stream_ptr(stream)),
+               "mas_forward_lsh")
+        return o, sig, g
 
     @staticmethod
     def _bundle(o):

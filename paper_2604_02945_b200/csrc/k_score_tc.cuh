@@ -56,6 +56,7 @@ constexpr int kTcRingBytes = (227 * 1024 - kTcCtrlBytes - 1024 - kTcBoxBytes) & 
 struct TcMaps {
   CUtensorMap x[16];   // token rows: box = (16 * (i + 1)) rows x 64 columns, up to the TMA limit of 256 rows
   CUtensorMap q[3];    // query rows: box = 64 / 32 / 16 rows x 64 columns
+  CUtensorMap r;       // NEXT-1: the 64 hash rows R[64, d] (box = 64 rows x 64 columns); valid only when TcParams::sig is set
 };
 
 struct TcSchedule {
@@ -73,6 +74,7 @@ struct TcParams {
   long long nQ;
   unsigned long long* q_ready;       // [0] grid-wide arrival counter of the prologue, [1] CTAs that have left the kernel;
                                      // both zero between launches (the last CTA to leave re-arms them: graph-replay safe)
+  unsigned long long* sig;           // NEXT-1 (literal LSH probe, Eq. 5): NULL = off; else the hash rows ride the MMA as 64 more B rows
   float* s;
   float* dnorm;       // sqrt(sum (x - x_prev)^2) for rows that have a previous frame
   float* rel;
@@ -107,15 +109,17 @@ struct TcRing {
 //   [kw x token slice (xbytes each)] [kw x previous-frame slice, temporal tiles only] [kw x query slice (qbytes each)]
 struct TcGeom {
   uint32_t xbytes, xall, qbytes, need;
-  int kw, nch, nqb, nh;   // nh = 128-row MMA halves of the tile (2 for a double tile)
+  int kw, nch, nqb, nqu, nh;   // nqb = 16-row boxes of B rows (queries + hash rows), nqu = those of the queries alone;
+                               // nh = 128-row MMA halves of the tile (2 for a double tile)
   bool has_prev;
 };
-__device__ __forceinline__ TcGeom tc_geom(const TcTile& t, int nk, int dbg) {
+__device__ __forceinline__ TcGeom tc_geom(const TcTile& t, int nk, int dbg, bool lsh = false) {
   TcGeom g;
   const int rows16 = (t.n_rows + 15) & ~15;
   g.xbytes = (uint32_t)rows16 * 128u;
   g.has_prev = t.prev_delta > 0 && t.key_rows < t.n_rows && !(dbg & 8);
-  g.nqb = (dbg & 4) ? 0 : (t.L + 15) >> 4;
+  g.nqu = (dbg & 4) ? 0 : (t.L + 15) >> 4;
+  g.nqb = g.nqu + (lsh ? 4 : 0);
   int kw = rows16 <= 16 ? 8 : rows16 <= 32 ? 4 : rows16 <= 64 ? 2 : 1;
   while (kw > 1 && (kw * g.nqb > 16 || nk % kw != 0)) kw >>= 1;   // <= 32 KB of query rows per chunk; kw divides d / 64
   g.kw = kw;
@@ -239,6 +243,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int tile_lo = p.cta_off[blockIdx.x], tile_hi = p.cta_off[blockIdx.x + 1];
   const int nk = p.n_kchunks;
+  const bool lsh = p.sig != nullptr;
 #ifdef MSAS_ABLATE
   const int dbg = p.dbg;
   auto gtime = [] { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; };
@@ -281,10 +286,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       // virtual start of the oldest chunk whose release has not been observed yet, tail.k its index.  Registers only.
       TcRing tail;
       int tail_t = tile_lo, tail_ch = 0;
-      TcGeom tg = tc_geom(p.tiles[tile_lo], nk, dbg);
+      TcGeom tg = tc_geom(p.tiles[tile_lo], nk, dbg, lsh);
       for (int t = tile_lo; t < tile_hi; ++t) {
         const TcTile tile = p.tiles[t];
-        const TcGeom g = tc_geom(tile, nk, dbg);
+        const TcGeom g = tc_geom(tile, nk, dbg, lsh);
         const CUtensorMap* mx = &maps.x[(g.xbytes >> 11) - 1];      // one box of rows16 rows per K-slice
         const int row = tile.row_start, prow = tile.row_start - tile.prev_delta;
         const uint32_t poff = (uint32_t)g.kw * g.xbytes;            // previous-frame slices follow the token slices
@@ -298,7 +303,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             mbar_wait(smem_u32(&ctrl->empty[tail.slot()]), tail.parity());
             tail.place(tg.need);
             ++tail.k;
-            if (++tail_ch == tg.nch && tail_t + 1 < tile_hi) { tail_ch = 0; tg = tc_geom(p.tiles[++tail_t], nk, dbg); }
+            if (++tail_ch == tg.nch && tail_t + 1 < tile_hi) { tail_ch = 0; tg = tc_geom(p.tiles[++tail_t], nk, dbg, lsh); }
           }
           const uint32_t bar = smem_u32(&ctrl->full[ring.slot()]);
           const uint32_t base = smem_u32(ring0 + off);
@@ -317,9 +322,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             for (int j = 0; j < g.kw; ++j) {
               const int c0 = (ch * g.kw + j) * 64;
               int qr = tile.q_row0;
-              for (int i = 0; i < (g.nqb >> 2); ++i) { tma_load_2d(sq, &mq64, bar, c0, qr); sq += 8192; qr += 64; }
-              if (g.nqb & 2) { tma_load_2d(sq, &mq32, bar, c0, qr); sq += 4096; qr += 32; }
-              if (g.nqb & 1) { tma_load_2d(sq, &mq16, bar, c0, qr); sq += 2048; }
+              for (int i = 0; i < (g.nqu >> 2); ++i) { tma_load_2d(sq, &mq64, bar, c0, qr); sq += 8192; qr += 64; }
+              if (g.nqu & 2) { tma_load_2d(sq, &mq32, bar, c0, qr); sq += 4096; qr += 32; }
+              if (g.nqu & 1) { tma_load_2d(sq, &mq16, bar, c0, qr); sq += 2048; }
+              if (lsh) { tma_load_2d(sq, &maps.r, bar, c0, 0); sq += 8192; }   // the hash rows follow the query rows: one B tile
             }
           }
           ++ring.k;
@@ -333,8 +339,8 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       int it = 0;
       for (int t = tile_lo; t < tile_hi; ++t, ++it) {
         const TcTile tile = p.tiles[t];
-        const TcGeom g = tc_geom(tile, nk, dbg);
-        const uint32_t idesc = umma_idesc_bf16(((tile.L + 15) >> 4) << 4);
+        const TcGeom g = tc_geom(tile, nk, dbg, lsh);
+        const uint32_t idesc = umma_idesc_bf16(g.nqb << 4);   // N = pad16(L) (+ 64 hash rows)
         const int acc = it & 1;
         const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
         mbar_wait(smem_u32(&ctrl->tmem_empty[acc]), acc_phase ^ 1u);
@@ -393,7 +399,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
-      const TcGeom g = tc_geom(tile, nk, dbg);
+      const TcGeom g = tc_geom(tile, nk, dbg, lsh);
       const int acc = it & 1;
       const uint32_t ph = (uint32_t)(it >> 1) & 1u;
       const int nqb = (tile.L + 15) >> 4;
@@ -417,6 +423,21 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             if (col < tile.L) m[h] = fmaxf(m[h], __uint_as_float(v[j]) * qinv[col]);
           }
         }
+      if (lsh) {   // NEXT-1: the 64 accumulator columns after the query columns are r_k . x: their signs are the hash bits
+        for (int h = 0; h < g.nh; ++h) {
+          unsigned long long bits = 0ull;
+#pragma unroll
+          for (int cb = 0; cb < 4; ++cb) {
+            uint32_t v[16];
+            tc_ld16(tmem_base + (uint32_t)acc * 256u + (uint32_t)h * 128u + (uint32_t)(g.nqu + cb) * 16u + ((uint32_t)(q * 32) << 16), v);
+            tc_wait_ld();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) bits |= (unsigned long long)(__uint_as_float(v[j]) >= 0.f) << (cb * 16 + j);
+          }
+          const int tr = h * 128 + r;
+          if (tr < tile.n_rows) p.sig[(int64_t)tile.row_start + tr] = bits;
+        }
+      }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->tmem_empty[acc]));
@@ -452,7 +473,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
-      const TcGeom g = tc_geom(tile, nk, dbg);
+      const TcGeom g = tc_geom(tile, nk, dbg, lsh);
       const int rp2 = 128 / g.kw;
       const bool dbl = g.nh == 2;                        // double tile: 256 threads = 256 rows, a whole row each, no previous frame
       const int r = dbl ? (int)set * 128 + a : (a & (rp2 - 1)), j = dbl ? 0 : a / rp2;
@@ -704,15 +725,18 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
 // returns 0 on success, 1 if the cooperative launch is not possible on this device / partition (nothing was enqueued),
 // -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error).
 // `q_ready`: two zero-initialised 64-bit words owned by the plan (the kernel leaves them zero).
+// `Rm` / `sig` (both NULL = off): NEXT-1, hash rows R[64, d] and the per-token signatures; requires every L <= 64.
 inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, float* qinv, float* s, float* dnorm, float* rel,
-                           unsigned long long* q_ready, int64_t N, int64_t nQ, int d, bool inline_qprep, cudaStream_t st) {
+                           unsigned long long* q_ready, int64_t N, int64_t nQ, int d, bool inline_qprep, const void* Rm, unsigned long long* sig,
+                           cudaStream_t st) {
   TcMaps maps;
   for (int k = 0; k < 16; ++k)
     if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
   for (int k = 0; k < 3; ++k)
     if (!tc_make_map(&maps.q[k], Q, nQ, d, 64 >> k)) return -1;
+  if (sig != nullptr) { if (!tc_make_map(&maps.r, Rm, 64, d, 64)) return -1; } else maps.r = maps.q[0];
   TcParams p;
-  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.s = s; p.dnorm = dnorm; p.rel = rel;
+  p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.sig = sig; p.s = s; p.dnorm = dnorm; p.rel = rel;
   p.d = d; p.n_kchunks = d / 64;
 #ifdef MSAS_ABLATE
   p.dbg = getenv("MSAS_ABLATE") ? atoi(getenv("MSAS_ABLATE")) : 0;

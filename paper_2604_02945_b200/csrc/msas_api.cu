@@ -461,9 +461,9 @@ extern "C" int mas_select_compact(const mas_plan* p, const void* X, const float*
 }
 
 // ------------------------------------------------------------------------------------------------ fused entry point
-extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, float* m_spatial, float* gamma, float* rel, float* mas_tok,
-                           mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows,
-                           mas_stream_t stream) {
+static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* m_spatial, float* gamma, float* rel, float* mas_tok,
+                        mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows,
+                        const void* Rm, unsigned long long* sig, mas_stream_t stream) {
   if (!p || !X || !Q || cap_rows < 0) return MAS_ERR_INVALID_ARG;
   if (Y && !kept_idx) return MAS_ERR_INVALID_ARG;
   if (!aligned16(X) || !aligned16(Q) || (Y && !aligned16(Y))) return MAS_ERR_UNSUPPORTED;
@@ -483,17 +483,17 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   if (p->tc.enabled && !p->tc_inline_qnorm) {
     if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
     rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, false, st);
+                         p->nQ, p->d, false, Rm, sig, st);
     if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
     rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, true, st);
+                         p->nQ, p->d, true, Rm, sig, st);
     if (rc == 1) {   // not all CTAs can be co-resident here (e.g. an MPS partition): query norms in their own launch
       (void)cudaGetLastError();
       if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
       rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                           p->nQ, p->d, false, st);
+                           p->nQ, p->d, false, Rm, sig, st);
     }
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else {
@@ -511,6 +511,30 @@ extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, floa
   rc = launch_gather(p, X, kept_idx, koff, Y, cap_rows, st, pdl);
   if (pev) CK(cudaEventRecord(pev[3], st));
   return rc;
+}
+
+extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, float* m_spatial, float* gamma, float* rel, float* mas_tok,
+                           mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows,
+                           mas_stream_t stream) {
+  return forward_impl(p, X, Q, m_spatial, gamma, rel, mas_tok, seg_out, keep_mask, kept_idx, kept_off, Y, cap_rows, nullptr, nullptr, stream);
+}
+
+extern "C" int mas_forward_lsh(const mas_plan* p, const void* X, const void* Q, const void* Rm, uint64_t* sig, float* gamma_lsh,
+                               const mas_outputs* o, mas_stream_t stream) {
+  if (!p || !Rm || !sig || !o) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(Rm)) return MAS_ERR_UNSUPPORTED;
+  // the hash rows ride the score kernel's MMA as 64 more B rows when the accumulator has room for them (L <= 64 everywhere)
+  const bool fused = p->tc.enabled && p->max_L <= 64;
+  int rc = forward_impl(p, X, Q, o->m_spatial, o->gamma, o->rel, o->mas_tok, o->seg_out, o->keep_mask, o->kept_idx, o->kept_off, o->Y,
+                        o->cap_rows, fused ? Rm : nullptr, fused ? reinterpret_cast<unsigned long long*>(sig) : nullptr, stream);
+  if (rc != MAS_OK) return rc;
+  if (!fused) return mas_temporal_lsh(p, X, Rm, sig, gamma_lsh, stream);
+  if (gamma_lsh) {
+    k_lsh_gamma<<<p->n_tiles, 128, 0, (cudaStream_t)stream>>>(p->at<DevSeg>(p->lay.segs), p->at<DevTile>(p->lay.tiles),
+                                                              reinterpret_cast<const unsigned long long*>(sig), gamma_lsh);
+    CK(cudaGetLastError());
+  }
+  return MAS_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ host-buffer convenience

@@ -393,3 +393,44 @@ def test_temporal_lsh_matches_oracle(B, w):
         row += T * P
     assert np.all(g_g[same] == 0.0)
     plan.close()
+
+
+@pytest.mark.parametrize("w", [synth.video(seed=41, R=2, T=4, P=300, d=256, L=48), synth.batched_images(seed=42, R=3, d=512, L_lo=5, L_hi=64, P=600),
+                               synth.ragged(seed=43, R=6, d=128, n_lo=50, n_hi=500, L_lo=60, L_hi=128)],
+                         ids=["video_fused", "images_fused_double_tiles", "ragged_L128_staged_fallback"])
+def test_forward_lsh_one_pass(B, w):
+    """mas_forward_lsh = mas_forward (same outputs up to the summation grouping of the row statistics, which follows the
+    chunk geometry) + signatures that match the oracle on every decided bit."""
+    rng = np.random.default_rng(4321)
+    Rm = synth.f32_to_bf16_bits(rng.standard_normal((64, w.d)).astype(np.float32))
+    segs, n = O.make_segments(w.segments)
+    sig_r, g_r, proj = O.temporal_lsh(segs, w.X, Rm, want_proj=True)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    base = plan.forward(X, Q)
+    o, sig_t, g_t = plan.forward_lsh(X, Q, B.to_device(Rm))
+    torch.cuda.synchronize()
+    for k in ("m_spatial", "gamma", "rel", "mas_tok"):
+        assert torch.allclose(base[k], o[k], rtol=2e-5, atol=1e-6), k
+    assert torch.equal(base["kept_off"], o["kept_off"])
+    assert (base["keep_mask"] != o["keep_mask"]).float().mean().item() < 1e-3          # only exact near-ties may flip
+    tot = int(o["kept_off"][-1].item())
+    assert torch.equal(o["Y"][:tot].view(torch.uint8), X[o["kept_idx"][:tot].long()].view(torch.uint8))
+    sig_g = sig_t.cpu().numpy().view(np.uint64)
+    Xf, Rf = synth.bf16_bits_to_f32(w.X).astype(np.float64), synth.bf16_bits_to_f32(Rm).astype(np.float64)
+    decided = np.abs(proj) > 2e-4 * np.linalg.norm(Xf, axis=1)[:, None] * np.linalg.norm(Rf, axis=1)[None, :]
+    sh = np.arange(64, dtype=np.uint64)[None, :]
+    bits_r = ((sig_r[:, None] >> sh) & np.uint64(1)).astype(bool)
+    bits_g = ((sig_g[:, None] >> sh) & np.uint64(1)).astype(bool)
+    assert decided.mean() > 0.99 and np.array_equal(bits_r[decided], bits_g[decided])
+    g_g = g_t.cpu().numpy()
+    row = 0
+    for (req, mod, T, P, k) in w.segments:
+        if T == 1:
+            assert np.all(g_g[row:row + P] == 0.0)
+        else:
+            assert np.all(g_g[row:row + P] == 1.0)
+            want = _popcount64(sig_g[row + P:row + T * P] ^ sig_g[row:row + (T - 1) * P]) / 64.0
+            assert np.array_equal(g_g[row + P:row + T * P], want.astype(np.float32))
+        row += T * P
+    plan.close()
