@@ -15,6 +15,8 @@
 //   from s; the previous row's norm is therefore never recomputed here.
 //   The query norms (row a0) are computed by the epilogue warps while the first tile streams in; a non-temporal tile may
 //   be a 256-row "double" tile whose two 128-row MMA halves share one query chunk.
+//   NEXT-1 (literal LSH probe of Eq. 5): when TcParams::sig is set, 64 hash rows follow the query rows in the B tile and
+//   the epilogue packs the signs of their 64 accumulator columns into a per-token signature.
 //
 // Persistent: one CTA per SM walks a host-built, cost-balanced tile list (round-robin bulk + gap filling).  Tiles never
 // straddle a segment.
