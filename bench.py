@@ -139,6 +139,7 @@ def main():
     ap.add_argument("--impl", default="msas", choices=["msas", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--lsh", action="store_true", help="NEXT-1: time mas_forward_lsh (forward + literal LSH probe in the same pass)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "msas" else args.warmup
 
@@ -171,6 +172,18 @@ def main():
     Qs = [B.to_device(w.Q), B.to_device(w.Q)]
     out = plan.alloc_outputs()
     stream = torch.cuda.current_stream()
+    if args.lsh:   # the step becomes mas_forward_lsh: same outputs plus 8 B/token signatures and gamma_lsh
+        import ctypes as C
+        Rm = B.to_device(synth.f32_to_bf16_bits(np.random.default_rng(99).standard_normal((64, w.d)).astype(np.float32)))
+        sig = torch.zeros(plan.N, dtype=torch.int64, device="cuda")
+        glsh = torch.zeros(plan.N, dtype=torch.float32, device="cuda")
+        bundle = plan._bundle(out)
+
+        def forward(X, Q, out=None):
+            B._check(B.lib.mas_forward_lsh(plan._h, B._ptr(X), B._ptr(Q), B._ptr(Rm), B._ptr(sig), B._ptr(glsh), C.byref(bundle),
+                                           B._stream_ptr(None)), "mas_forward_lsh")
+        plan.forward = forward
+        args.no_e2e = True
 
     def barrier():
         if world > 1:
@@ -243,7 +256,7 @@ def main():
             "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": args.workload, "requests": w.n_requests, "segments": len(w.segments), "tokens": w.n_tokens,
                        "d": w.d, "query_tokens": int(w.q_off[-1]), "kept_rows": kept_rows,
-                       "select": "threshold" if w.select_mode else "topk", "parallelism": "dp%d (independent requests)" % world,
+                       "select": "threshold" if w.select_mode else "topk", "entry": "mas_forward_lsh" if args.lsh else "mas_forward", "parallelism": "dp%d (independent requests)" % world,
                        "l2": "X = %.0f MB per copy, two rotating input copies (> %.0f MB L2 on configs 2-5)" % (w.X.nbytes / 1e6, L2_BYTES / 1e6)},
             "clocks": clocks,
             "gpu_launches": args.steps * plan.forward_launches,
