@@ -8,6 +8,8 @@
 // Eq. 3-7; constants PAPER.md:255), written out step by step, single thread, every sum a `double` accumulated in
 // index order, inputs converted exactly (bf16 -> double, fp32 -> double). No blocking, fusion or reordering.
 //
+// NEXT-4 (mas_ref_draft_entropy): pinned by uniform -> log V, one-hot -> 0, the two-level closed form, shift invariance and
+// scipy.stats.entropy of a float64 softmax.
 // NEXT-1 (mas_ref_temporal_lsh): pinned by explicit signs of hand-expanded projections, identical / negated rows,
 // power-of-two scaling, and the collision law E[gamma] = theta / pi.
 //
@@ -169,6 +171,28 @@ int mas_ref_temporal_lsh(const mas_ref_segment* segs, int32_t n_segs, int64_t d,
         while (x) { cnt += (int)(x & 1); x >>= 1; }
         gamma[i] = (double)cnt / 64.0;
       }
+  }
+  return 0;
+}
+
+// NEXT-4: draft-confidence entropy, Eq. 9-10: for each decode step (row) with
+// logits l_v over the vocabulary, p = softmax(l), H = - sum_v p_v log p_v (natural log), Speculate = [H <= theta_conf].
+// Written as the definition: two passes per row in double (max, then the sums), no online rescaling.
+int mas_ref_draft_entropy(const void* logits, int64_t n_rows, int64_t V, int64_t row_stride, int dtype, double theta_conf,
+                          double* H, uint8_t* speculate) {
+  for (int64_t r = 0; r < n_rows; ++r) {
+    double m = -INFINITY;
+    for (int64_t v = 0; v < V; ++v) m = std::max(m, elem(logits, dtype, r * row_stride + v));
+    double Z = 0.0;
+    for (int64_t v = 0; v < V; ++v) Z += std::exp(elem(logits, dtype, r * row_stride + v) - m);
+    double h = 0.0;
+    for (int64_t v = 0; v < V; ++v) {
+      const double lp = elem(logits, dtype, r * row_stride + v) - m - std::log(Z);   // log p_v
+      const double pv = std::exp(lp);
+      if (pv > 0.0) h -= pv * lp;                                                    // 0 log 0 = 0
+    }
+    H[r] = h;
+    if (speculate) speculate[r] = h <= theta_conf ? 1 : 0;
   }
   return 0;
 }

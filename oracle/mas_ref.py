@@ -107,6 +107,16 @@ def temporal(segs, X):
     return g
 
 
+def draft_entropy(logits, theta_conf):
+    """NEXT-4: Eq. 9-10 per row of logits[n_rows, V] (float32 or bf16 bits): (H float64, speculate uint8)."""
+    L = np.ascontiguousarray(logits)
+    H = np.zeros(L.shape[0], np.float64)
+    flag = np.zeros(L.shape[0], np.uint8)
+    _check(lib().mas_ref_draft_entropy(_p(L), C.c_int64(L.shape[0]), C.c_int64(L.shape[1]), C.c_int64(L.shape[1]), _dtype_code(L),
+                                       C.c_double(theta_conf), _p(H), _p(flag)))
+    return H, flag
+
+
 def temporal_lsh(segs, X, R, want_proj=False):
     """NEXT-1: literal LSH probe of Eq. 5 with K = 64 hashes from R[64, d] (same dtype as X)."""
     X = np.ascontiguousarray(X)

@@ -431,3 +431,36 @@ def test_lsh_collision_law_theta_over_pi():
         g = O.temporal_lsh(segs, X, R)[1][P:]
         # the 64 hashes are shared by all pairs, so average over pairs AND hashes: tolerance from the spread over hashes
         assert abs(g.mean() - theta / np.pi) < 0.03, (theta, g.mean())
+
+
+# ---------------------------------------------------------------- NEXT-4: draft-confidence entropy (Eq. 9-10)
+def test_entropy_closed_forms():
+    V = 1000
+    uni = np.full((1, V), 3.25, np.float32)
+    onehot = np.full((1, V), -1e4, np.float32); onehot[0, 17] = 0.0
+    k, a, b = 10, 2.0, -1.0                                    # k logits at a, V - k at b: closed form below
+    two = np.full((1, V), b, np.float32); two[0, :k] = a
+    L = np.concatenate([uni, onehot, two])
+    H, flag = O.draft_entropy(L, theta_conf=1.0)
+    assert abs(H[0] - np.log(V)) < 1e-12                       # uniform: log V
+    assert abs(H[1]) < 1e-12                                   # one-hot: 0
+    Z = k * np.exp(a) + (V - k) * np.exp(b)
+    pa, pb = np.exp(a) / Z, np.exp(b) / Z
+    assert abs(H[2] - (-(k * pa * np.log(pa) + (V - k) * pb * np.log(pb)))) < 1e-12
+    assert list(flag) == [0, 1, int(H[2] <= 1.0)]              # Eq. 10: speculate iff H <= theta
+
+
+def test_entropy_matches_scipy_and_is_shift_invariant():
+    from scipy.special import softmax
+    from scipy.stats import entropy
+    rng = np.random.default_rng(3)
+    L = (rng.standard_normal((6, 4097)) * np.array([[0.1], [1], [3], [6], [10], [0.5]])).astype(np.float32)
+    H, _ = O.draft_entropy(L, 2.0)
+    want = np.array([entropy(softmax(row.astype(np.float64))) for row in L])
+    assert np.allclose(H, want, rtol=1e-12, atol=1e-12)
+    H2, _ = O.draft_entropy((L + 8.0).astype(np.float32), 2.0)       # + 8 is exact for these magnitudes? compare loosely
+    assert np.allclose(H, H2, rtol=1e-5)
+    Lb = synth.f32_to_bf16_bits(L)
+    Hb, _ = O.draft_entropy(Lb, 2.0)
+    wantb = np.array([entropy(softmax(row.astype(np.float64))) for row in synth.bf16_bits_to_f32(Lb)])
+    assert np.allclose(Hb, wantb, rtol=1e-12, atol=1e-12)            # bf16 decoding
