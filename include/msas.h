@@ -179,6 +179,15 @@ int mas_forward(const mas_plan* plan, const void* X, const void* Q,
 int mas_forward_lsh(const mas_plan* plan, const void* X, const void* Q, const void* Rm, uint64_t* sig /*[N]*/,
                     float* gamma_lsh /*[N] or NULL*/, const mas_outputs* out, mas_stream_t stream);
 
+/* NEXT-4: the draft-confidence entropy of Eq. 9 and the speculate rule of Eq. 10, the
+ * consumer-side step next to the MAS pass.  logits[n_rows, V] (device, fp32 or bf16, row stride `row_stride` elements,
+ * base and stride 16-byte aligned, n_rows <= 65535): per row p = softmax(l), H = -sum_v p_v ln p_v,
+ * speculate = [H <= theta_conf].  H[n_rows] fp32 and speculate[n_rows] u8 (device; either may be NULL).  Needs
+ * mas_draft_entropy_workspace_bytes of device workspace; no plan.  Every logit is read once. */
+int mas_draft_entropy_workspace_bytes(int64_t n_rows, int64_t V, size_t* out_bytes);
+int mas_draft_entropy(const void* logits, int64_t n_rows, int64_t V, int64_t row_stride, int32_t dtype, float theta_conf,
+                      float* H, uint8_t* speculate, void* d_workspace, size_t workspace_bytes, mas_stream_t stream);
+
 /* ---- end-to-end convenience: HOST inputs -> HOST outputs.
  * Copies h_X -> d_X and h_Q -> d_Q (cudaMemcpyAsync; pinned host memory recommended), runs mas_forward into d_out,
  * copies every non-NULL member of h_out back (Y/kept_idx: only the rows actually kept) and SYNCHRONISES the stream

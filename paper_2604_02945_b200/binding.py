@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh"]
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy"]
 
 
 class mas_segment(C.Structure):
@@ -89,6 +89,10 @@ def _load():
     lib.mas_forward_host.argtypes = [vp, vp, vp, vp, vp, C.POINTER(mas_outputs), C.POINTER(mas_outputs), vp]
     lib.mas_plan_set_inline_query_norms.restype = C.c_int
     lib.mas_plan_set_inline_query_norms.argtypes = [vp, i32]
+    lib.mas_draft_entropy_workspace_bytes.argtypes = [i64, i64, C.POINTER(C.c_size_t)]
+    lib.mas_draft_entropy_workspace_bytes.restype = C.c_int
+    lib.mas_draft_entropy.argtypes = [vp, i64, i64, i64, i32, C.c_float, vp, vp, vp, C.c_size_t, vp]
+    lib.mas_draft_entropy.restype = C.c_int
     lib.mas_score_schedule.restype = i32
     lib.mas_score_schedule.argtypes = [C.POINTER(mas_segment), i32, C.POINTER(i64), i32, i32, i32, i32, C.POINTER(i32), i32]
     for f in ("mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal",
@@ -295,6 +299,20 @@ class Plan:
         _check(lib.mas_forward_host(self._h, _ptr(h_X), _ptr(h_Q), _ptr(d_X), _ptr(d_Q), C.byref(self._bundle(d_out)),
                                     C.byref(self._bundle(h_out)) if h_out is not None else None, _stream_ptr(stream)),
                "mas_forward_host")
+
+
+def draft_entropy(logits, theta_conf, workspace=None, H=None, speculate=None, stream=None):
+    """NEXT-4: Eq. 9-10 per row of a device tensor logits[n_rows, V] (float32 or bfloat16): (H float32, speculate uint8)."""
+    n, V = logits.shape
+    dt = MAS_BF16 if logits.dtype == torch.bfloat16 else MAS_F32
+    nb = C.c_size_t(0)
+    _check(lib.mas_draft_entropy_workspace_bytes(n, V, C.byref(nb)), "mas_draft_entropy_workspace_bytes")
+    ws = workspace if workspace is not None else torch.empty(nb.value, dtype=torch.uint8, device=logits.device)
+    H = H if H is not None else torch.empty(n, dtype=torch.float32, device=logits.device)
+    sp = speculate if speculate is not None else torch.empty(n, dtype=torch.uint8, device=logits.device)
+    _check(lib.mas_draft_entropy(_ptr(logits), n, V, logits.stride(0), dt, float(theta_conf), _ptr(H), _ptr(sp), _ptr(ws), ws.numel(),
+                                 _stream_ptr(stream)), "mas_draft_entropy")
+    return H, sp
 
 
 def seg_out_numpy(t):

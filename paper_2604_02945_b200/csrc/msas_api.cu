@@ -12,6 +12,7 @@
 #include "../../include/msas.h"
 #include "k_score_simple.cuh"
 #include "k_score_tc.cuh"
+#include "k_entropy.cuh"
 #include "k_segment.cuh"
 
 using namespace msas;
@@ -534,6 +535,41 @@ extern "C" int mas_forward_lsh(const mas_plan* p, const void* X, const void* Q, 
                                                               reinterpret_cast<const unsigned long long*>(sig), gamma_lsh);
     CK(cudaGetLastError());
   }
+  return MAS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ NEXT-4: draft-confidence entropy
+static int entropy_geometry(int64_t n_rows, int64_t V, int* splits, int64_t* chunk) {
+  int dev = 0, sm = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess) (void)cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
+  (void)cudaGetLastError();
+  *splits = entropy_splits(n_rows, V, sm);
+  *chunk = ((V + *splits - 1) / *splits + 7) / 8 * 8;
+  *splits = (int)((V + *chunk - 1) / *chunk);
+  return MAS_OK;
+}
+extern "C" int mas_draft_entropy_workspace_bytes(int64_t n_rows, int64_t V, size_t* out_bytes) {
+  if (!out_bytes || n_rows < 1 || V < 1) return MAS_ERR_INVALID_ARG;
+  *out_bytes = (size_t)n_rows * 256 * sizeof(EntTriple);   // upper bound: 256 splits per row
+  return MAS_OK;
+}
+extern "C" int mas_draft_entropy(const void* logits, int64_t n_rows, int64_t V, int64_t row_stride, int32_t dtype, float theta_conf,
+                                 float* H, uint8_t* speculate, void* d_workspace, size_t workspace_bytes, mas_stream_t stream) {
+  if (!logits || n_rows < 1 || V < 1 || row_stride < V || (!H && !speculate) || !d_workspace) return MAS_ERR_INVALID_ARG;
+  if (dtype != MAS_F32 && dtype != MAS_BF16) return MAS_ERR_INVALID_ARG;
+  const int esz = dtype == MAS_BF16 ? 2 : 4;
+  if (!aligned16(logits) || (row_stride * esz) % 16 != 0 || n_rows > 65535) return MAS_ERR_UNSUPPORTED;
+  int splits; int64_t chunk;
+  entropy_geometry(n_rows, V, &splits, &chunk);
+  if (workspace_bytes < (size_t)n_rows * splits * sizeof(EntTriple)) return MAS_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  EntTriple* part = static_cast<EntTriple*>(d_workspace);
+  const dim3 grid((unsigned)splits, (unsigned)n_rows);
+  if (dtype == MAS_BF16) k_entropy_partial<1><<<grid, 256, 0, st>>>(logits, V, row_stride, chunk, part);
+  else k_entropy_partial<0><<<grid, 256, 0, st>>>(logits, V, row_stride, chunk, part);
+  CK(cudaGetLastError());
+  k_entropy_finish<<<(unsigned)((n_rows + 3) / 4), 128, 0, st>>>(part, splits, n_rows, theta_conf, H, speculate);
+  CK(cudaGetLastError());
   return MAS_OK;
 }
 

@@ -268,6 +268,19 @@ CONFIGS = {
 }
 
 
+def draft_logits(seed=7, n_rows=256, V=151936, dtype="bf16"):
+    """NEXT-4 input: draft-model logits for `n_rows` decode steps over a Qwen-sized vocabulary (PAPER.md:141-149 reads
+    them from Qwen2-VL-2B, which is not available): Gaussian logits whose per-row scale is log-uniform in [0.3, 8]
+    (flat to peaked distributions) plus a handful of boosted tokens.  Returns [n_rows, V] float32 or bf16 bits."""
+    rng = _rng(seed, 0)
+    scale = np.exp(rng.uniform(np.log(0.3), np.log(8.0), n_rows)).astype(np.float32)
+    L = rng.standard_normal((n_rows, V), dtype=np.float32) * scale[:, None]
+    for r in range(n_rows):
+        hot = rng.integers(0, V, size=int(rng.integers(1, 6)))
+        L[r, hot] += rng.uniform(2.0, 12.0, size=hot.size).astype(np.float32)
+    return _store(L, dtype)
+
+
 def make(name, **kw):
     return CONFIGS[name](**kw)
 

@@ -434,3 +434,23 @@ def test_forward_lsh_one_pass(B, w):
             assert np.array_equal(g_g[row + P:row + T * P], want.astype(np.float32))
         row += T * P
     plan.close()
+
+
+# ---------------------------------------------------------------- NEXT-4: draft-confidence entropy (Eq. 9-10)
+@pytest.mark.parametrize("n,V,dtype", [(5, 1000, "f32"), (7, 4100, "bf16"), (64, 151936, "bf16"), (3, 151936, "f32"), (300, 8, "bf16")],
+                         ids=["small_f32", "ragged_bf16", "qwen_vocab_bf16", "qwen_vocab_f32_few_rows", "tiny_vocab_many_rows"])
+def test_draft_entropy_matches_oracle(B, n, V, dtype):
+    L = synth.draft_logits(seed=11, n_rows=n, V=V, dtype=dtype)
+    theta = 2.5
+    H_r, f_r = O.draft_entropy(L, theta)
+    Vp = (V + 7) // 8 * 8 + 8                                        # padded row stride (16-byte multiple), not V
+    dev = torch.zeros((n, Vp), dtype=torch.bfloat16 if dtype == "bf16" else torch.float32, device="cuda")
+    dev[:, :V] = B.to_device(L)
+    dev[:, V:] = 50.0                                                # poison the padding: it must not be read
+    H, sp = B.draft_entropy(dev[:, :V], theta)
+    torch.cuda.synchronize()
+    H = H.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(H - H_r) <= 2e-4 * np.abs(H_r) + 2e-4), np.abs(H - H_r).max()
+    decided = np.abs(H_r - theta) > 1e-3
+    assert np.array_equal(sp.cpu().numpy()[decided], f_r[decided])
+    assert H.min() >= -1e-4 and H.max() <= np.log(V) + 1e-3
