@@ -568,8 +568,8 @@ extern "C" int mas_draft_entropy(const void* logits, int64_t n_rows, int64_t V, 
   if (dtype == MAS_BF16) k_entropy_partial<1><<<grid, 256, 0, st>>>(logits, V, row_stride, chunk, part);
   else k_entropy_partial<0><<<grid, 256, 0, st>>>(logits, V, row_stride, chunk, part);
   CK(cudaGetLastError());
-  k_entropy_finish<<<(unsigned)((n_rows + 3) / 4), 128, 0, st>>>(part, splits, n_rows, theta_conf, H, speculate);
-  CK(cudaGetLastError());
+  CK(launch_k(k_entropy_finish, dim3((unsigned)((n_rows + 3) / 4)), dim3(128), 0, st, true, (const EntTriple*)part, splits, n_rows, theta_conf,
+              H, speculate));
   return MAS_OK;
 }
 
