@@ -213,11 +213,14 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
     }
     for (int i = lo + tid + KPT * NT; i < hi; i += NT) { float si, ri, gi; load_token(i, si, ri, gi); accumulate(i, si, ri, gi); }
     cluster_sum6(sm, 0, nc, acc);
-    const double mu_s = acc[0] / n, mu_r = acc[2] / n;
-    const double gavg = temporal ? acc[4] / ((double)(seg.n_frames - 1) * seg.n_patches) : 0.0;
-    const double sd_s = sqrt(fmax(acc[1] / n - mu_s * mu_s, 0.0)), sd_r = sqrt(fmax(acc[3] / n - mu_r * mu_r, 0.0));
-    const double den_s = fmax(sd_s, 1e-6 * mu_s), den_r = fmax(sd_r, 1e-6);
-    const float inv_s = den_s > 0.0 ? (float)(1.0 / den_s) : 0.f, inv_r = (float)(1.0 / den_r);
+    // one double division per thread (1 / n); the variances stay in double (E[x^2] - mu^2 cancels), everything after the
+    // square root is needed to fp32 accuracy only (double division and sqrt are long software routines)
+    const double inv_n = 1.0 / (double)n;
+    const double mu_s = acc[0] * inv_n, mu_r = acc[2] * inv_n;
+    const float gavg = temporal ? (float)acc[4] / ((float)(seg.n_frames - 1) * (float)seg.n_patches) : 0.f;
+    const float sd_s = sqrtf((float)fmax(acc[1] * inv_n - mu_s * mu_s, 0.0)), sd_r = sqrtf((float)fmax(acc[3] * inv_n - mu_r * mu_r, 0.0));
+    const float den_s = fmaxf(sd_s, 1e-6f * (float)mu_s), den_r = fmaxf(sd_r, 1e-6f);
+    const float inv_s = den_s > 0.f ? 1.0f / den_s : 0.f, inv_r = 1.0f / den_r;
     const float at = temporal ? p.lambda_temp : 0.f;
     int below = 0;
     // pass B: per-token M, g, MAS (differences in double: the means are not representable in fp32)
@@ -241,16 +244,16 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
       float si = a.s[base + i], ri = a.rel[base + i], gi = temporal ? a.gamma[base + i] : 0.f;
       fuse_token(i, si, ri, gi);
     }
-    const double sd_s_out = sd_s;
+    const float sd_s_out = sd_s;
     double db = below, d1 = 0, d2 = 0;
     cluster_sum3(sm, 2, nc, db, d1, d2);
     if (rank == 0 && tid == 0 && a.seg_out) {
       mas_segment_out o;
       o.rho_spatial = (float)(db / n);
-      o.gamma_avg = (float)gavg;
+      o.gamma_avg = gavg;
       o.alpha_mean = (float)mu_r;
       o.beta = 0.f; o.mas = 0.f;
-      o.mean_s = (float)mu_s; o.std_s = (float)sd_s_out;
+      o.mean_s = (float)mu_s; o.std_s = sd_s_out;
       o.n_tokens = n; o.n_kept = 0;
       a.seg_out[sidx] = o;
     }
@@ -283,12 +286,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         for_each_round([&](int, bool valid, unsigned key) {
           const bool act = valid && (key & maskbits) == prefix;
           const unsigned bin = (key >> shift) & 255u;
-          // MAS scores share their leading bytes: aggregate equal bins inside the warp, one shared-memory atomic per bin
-          const unsigned am = __ballot_sync(0xffffffffu, act);
-          if (act) {
-            const unsigned peers = __match_any_sync(am, bin);
-            if (lane == __ffs(peers) - 1) atomicAdd(&sm.hist[pass][bin], (unsigned)__popc(peers));
-          }
+          if (act) atomicAdd(&sm.hist[pass][bin], 1u);
         });
         __syncthreads();
         const unsigned* hsrc = sm.hist[pass];
