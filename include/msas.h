@@ -40,7 +40,9 @@ enum { MAS_OK = 0, MAS_ERR_INVALID_ARG = 1, MAS_ERR_UNSUPPORTED = 2, MAS_ERR_WOR
 
 typedef enum { MAS_F32 = 0, MAS_BF16 = 1 } mas_dtype;
 typedef enum { MAS_MOD_IMAGE = 1, MAS_MOD_VIDEO = 2, MAS_MOD_AUDIO = 3 } mas_modality;   /* text is the query, never a segment */
-typedef enum { MAS_SELECT_TOPK = 0, MAS_SELECT_THRESHOLD = 1 } mas_select_mode;
+/* MAS_SELECT_ADAPTIVE (NEXT-3, "beta_m >= 1 - MAS_m"): top-k with keep_k = clamp(ceil((1 - MAS_s) N_s - 1e-9), 1, N_s)
+ * taken on the device from the segment score of the fuse step (double arithmetic on the fp32 MAS_s); keep_k in the table is ignored. */
+typedef enum { MAS_SELECT_TOPK = 0, MAS_SELECT_THRESHOLD = 1, MAS_SELECT_ADAPTIVE = 2 } mas_select_mode;
 
 typedef void* mas_stream_t;          /* a cudaStream_t (0 = the legacy default stream) */
 
@@ -122,7 +124,7 @@ int mas_plan_destroy(mas_plan* plan);                    /* frees the host objec
 /* plan queries (host) */
 int64_t mas_plan_n_tokens(const mas_plan* plan);         /* N */
 int64_t mas_plan_n_queries(const mas_plan* plan);        /* sum L_r */
-int64_t mas_plan_kept_capacity(const mas_plan* plan);    /* top-k: sum keep_k ; threshold: N (worst case) */
+int64_t mas_plan_kept_capacity(const mas_plan* plan);    /* top-k: sum keep_k ; threshold, adaptive: N (worst case) */
 int32_t mas_plan_forward_launches(const mas_plan* plan); /* number of kernels one mas_forward enqueues */
 
 /* Profiling aid (bench.py's roofline leg).  After mas_plan_enable_profiling(plan, max_calls > 0) every mas_forward
@@ -150,8 +152,9 @@ int mas_fuse(const mas_plan* plan, const float* s, const float* gamma, const flo
              float* m_spatial /*[N] or NULL*/, float* mas_tok /*[N]*/, mas_segment_out* seg_out /*[n_segs]*/, mas_stream_t stream);
 
 /* S5: selection on mas_tok, index compaction, row gather. Y may be NULL (indices only). cap_rows >= sum keep_k
- * (top-k) or any value >= 0 (threshold): nothing is written past cap_rows and kept_off[n_segs] still holds the
- * true total so the caller detects overflow. seg_out (may be NULL): only n_kept is written. */
+ * (top-k) or any value >= 0 (threshold, adaptive): nothing is written past cap_rows and kept_off[n_segs] still holds the
+ * true total so the caller detects overflow. seg_out (may be NULL): only n_kept is written. Adaptive mode READS
+ * seg_out[k].mas (as mas_fuse left it) to size each segment's keep count: seg_out NULL is INVALID_ARG there. */
 int mas_select_compact(const mas_plan* plan, const void* X, const float* mas_tok,
                        uint8_t* keep_mask /*[N]*/, int32_t* kept_idx /*[cap_rows]*/, int64_t* kept_off /*[n_segs+1]*/,
                        void* Y /*[cap_rows, d] or NULL*/, int64_t cap_rows, mas_segment_out* seg_out, mas_stream_t stream);

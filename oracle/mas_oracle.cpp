@@ -309,12 +309,19 @@ int mas_ref_select_compact(const mas_ref_segment* segs, int32_t n_segs, int64_t 
   for (int32_t k = 0; k < n_segs; ++k) {
     const int64_t r0 = segs[k].row0, n = static_cast<int64_t>(segs[k].n_frames) * segs[k].n_patches;
     for (int64_t i = r0; i < r0 + n; ++i) keep_mask[i] = 0;
-    if (prm->select_mode == 0) {
+    if (prm->select_mode == 0 || prm->select_mode == 2) {
       // the keep_k smallest under the strict total order (MAS_i, i): stable sort by value keeps lower index first
       std::vector<int64_t> order(static_cast<size_t>(n));
       for (int64_t i = 0; i < n; ++i) order[static_cast<size_t>(i)] = r0 + i;
       std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return mas_tok[a] < mas_tok[b]; });
       int64_t kk = segs[k].keep_k;
+      if (prm->select_mode == 2) {
+        // NEXT-3 (adaptive retention): the scheduler's constraint beta_m >= 1 - MAS_m (Eq. 11) read as the
+        // smallest admissible retention: keep_k = ceil((1 - MAS_s) N_s), clamped to [1, N_s]; MAS_s from the fuse step
+        if (!out) return 1;
+        kk = static_cast<int64_t>(std::ceil((1.0 - static_cast<double>(out[k].mas)) * static_cast<double>(n) - 1e-9));
+        kk = std::min<int64_t>(n, std::max<int64_t>(1, kk));
+      }
       if (kk < 0 || kk > n) return 1;
       for (int64_t j = 0; j < kk; ++j) keep_mask[order[static_cast<size_t>(j)]] = 1;
     } else {

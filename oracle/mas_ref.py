@@ -156,7 +156,8 @@ def fuse(segs, params, s, gamma, rel):
     return m, mas, out
 
 
-def select_compact(segs, params, X, mas_tok, cap_rows=None, want_Y=True):
+def select_compact(segs, params, X, mas_tok, cap_rows=None, want_Y=True, seg_mas=None):
+    """seg_mas: per-segment MAS_s, needed by the adaptive mode (select_mode = 2) only."""
     X = np.ascontiguousarray(X)
     mas_tok = np.ascontiguousarray(mas_tok, np.float64)
     n, d = X.shape
@@ -167,6 +168,9 @@ def select_compact(segs, params, X, mas_tok, cap_rows=None, want_Y=True):
     off = np.zeros(len(segs) + 1, np.int64)
     Y = np.zeros((max(cap_rows, 1), d), X.dtype) if want_Y else None
     out = (SegmentOut * len(segs))()
+    if seg_mas is not None:
+        for k, v in enumerate(seg_mas):
+            out[k].mas = float(v)
     _check(lib().mas_ref_select_compact(segs, len(segs), C.c_int64(d), _dtype_code(X), C.byref(params), _p(X), _p(mas_tok),
                                         _p(mask), _p(idx), _p(off), _p(Y), C.c_int64(cap_rows), out))
     return mask, idx, off, Y, out

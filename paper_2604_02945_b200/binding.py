@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libmsas.so")
 MAS_OK, MAS_ERR_INVALID_ARG, MAS_ERR_UNSUPPORTED, MAS_ERR_WORKSPACE, MAS_ERR_CUDA = 0, 1, 2, 3, 4
 MAS_F32, MAS_BF16 = 0, 1
 MAS_MOD_IMAGE, MAS_MOD_VIDEO, MAS_MOD_AUDIO = 1, 2, 3
-MAS_SELECT_TOPK, MAS_SELECT_THRESHOLD = 0, 1
+MAS_SELECT_TOPK, MAS_SELECT_THRESHOLD, MAS_SELECT_ADAPTIVE = 0, 1, 2
 MAS_MAX_QUERY_TOKENS = 128
 
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
@@ -262,8 +262,11 @@ class Plan:
         _check(lib.mas_fuse(self._h, _ptr(s), _ptr(gamma), _ptr(rel), _ptr(m), _ptr(mas), _ptr(so), _stream_ptr(stream)), "mas_fuse")
         return m, mas, so
 
-    def select_compact(self, X, mas_tok, cap_rows=None, want_Y=True, stream=None):
+    def select_compact(self, X, mas_tok, cap_rows=None, want_Y=True, stream=None, seg_out=None):
+        """seg_out: the fuse step's segment records (adaptive mode reads their MAS_s); a fresh zeroed table otherwise."""
         o = self.alloc_outputs(cap_rows, want_Y)
+        if seg_out is not None:
+            o["seg_out"] = seg_out
         _check(lib.mas_select_compact(self._h, _ptr(X), _ptr(mas_tok), _ptr(o["keep_mask"]), _ptr(o["kept_idx"]), _ptr(o["kept_off"]),
                                       _ptr(o["Y"]), o["cap_rows"], _ptr(o["seg_out"]), _stream_ptr(stream)), "mas_select_compact")
         return o

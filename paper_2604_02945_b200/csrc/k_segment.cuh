@@ -274,9 +274,16 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         if (lo + it * NT < hi) { const int i = lo + it * NT + tid; fn(i, i < hi, c_key[it]); }
       for (int c0 = lo + KPT * NT; c0 < hi; c0 += NT) { const int i = c0 + tid; fn(i, i < hi, i < hi ? float_key(mas[i]) : 0u); }
     };
-    if (p.select_mode == MAS_SELECT_TOPK) {
+    if (p.select_mode != MAS_SELECT_THRESHOLD) {
       int kk = seg.keep_k < n ? seg.keep_k : n;
+      if (p.select_mode == MAS_SELECT_ADAPTIVE) {
+        // NEXT-3 (beta_m >= 1 - MAS_m): the smallest retention the constraint admits, from the segment score the
+        // fuse launch left in seg_out; the decision is taken in double on the fp32 MAS_s
+        const double want = ceil((1.0 - (double)a.seg_out[sidx].mas) * (double)n - 1e-9);
+        kk = want < 1.0 ? 1 : (want > (double)n ? n : (int)want);
+      }
       const int k_total = kk;
+      const bool static_off = p.select_mode == MAS_SELECT_TOPK;   // else positions are data dependent: k_compact_idx writes kept_idx
       unsigned prefix = 0, maskbits = 0;
       if (tid < 256) { sm.hist[0][tid] = 0; sm.hist[1][tid] = 0; sm.hist[2][tid] = 0; sm.hist[3][tid] = 0; }
       __syncthreads();
@@ -348,7 +355,7 @@ __global__ void __launch_bounds__(kSegThreads) k_segment(SegArgs a) {
         const bool keep = fl || (fe && eq_before < kk);
         if (valid) {
           if (a.keep_mask) a.keep_mask[base + i] = keep ? 1 : 0;
-          if (keep && a.kept_idx) {
+          if (keep && a.kept_idx && static_off) {
             const int64_t pos = off + run_less + pl + (eq_before < kk ? eq_before : kk);
             if (pos < a.cap_rows) a.kept_idx[pos] = (int32_t)(base + i);
           }

@@ -122,7 +122,7 @@ static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_of
   }
   if (row > (int64_t)0x7fffffff - kTileRows) return MAS_ERR_UNSUPPORTED;   // kept_idx is int32
   if (prm) {
-    if (prm->select_mode != MAS_SELECT_TOPK && prm->select_mode != MAS_SELECT_THRESHOLD) return MAS_ERR_INVALID_ARG;
+    if (prm->select_mode != MAS_SELECT_TOPK && prm->select_mode != MAS_SELECT_THRESHOLD && prm->select_mode != MAS_SELECT_ADAPTIVE) return MAS_ERR_INVALID_ARG;
     if (!(prm->lambda_spatial >= 0.f) || !(prm->lambda_temp >= 0.f) || !(prm->lambda_spatial + prm->lambda_temp <= 1.0f + 1e-6f))
       return MAS_ERR_INVALID_ARG;
   }
@@ -378,7 +378,7 @@ static int launch_gather(const mas_plan* p, const void* X, const int32_t* kept_i
 
 static int launch_select_tail(const mas_plan* p, const void* X, const uint8_t* mask, int32_t* kept_idx, const int64_t* kept_off,
                               void* Y, int64_t cap_rows, cudaStream_t st) {
-  if (p->prm.select_mode == MAS_SELECT_THRESHOLD && kept_idx) {
+  if (p->prm.select_mode != MAS_SELECT_TOPK && kept_idx) {
     k_compact_idx<<<p->n_segs, kSegThreads, 0, st>>>(p->at<DevSeg>(p->lay.segs), mask, kept_off, kept_idx, cap_rows);
     CK(cudaGetLastError());
   }
@@ -388,7 +388,9 @@ static int launch_select_tail(const mas_plan* p, const void* X, const uint8_t* m
 extern "C" int32_t mas_plan_forward_launches(const mas_plan* p) {
   if (!p) return -1;
   // [qprep, generic path only] + score + segment (+ index compaction in threshold mode) + gather
-  return (p->tc.enabled && p->tc_inline_qnorm ? 3 : 4) + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0);
+  // adaptive mode: fuse and select are two launches (MAS_s needs every segment of the request before any keep count exists)
+  return (p->tc.enabled && p->tc_inline_qnorm ? 3 : 4) + (p->prm.select_mode == MAS_SELECT_THRESHOLD ? 1 : 0) +
+         (p->prm.select_mode == MAS_SELECT_ADAPTIVE ? 2 : 0);
 }
 
 // ------------------------------------------------------------------------------------------------ staged entry points
@@ -450,6 +452,7 @@ extern "C" int mas_fuse(const mas_plan* p, const float* s, const float* gamma, c
 extern "C" int mas_select_compact(const mas_plan* p, const void* X, const float* mas_tok, uint8_t* keep_mask, int32_t* kept_idx,
                                   int64_t* kept_off, void* Y, int64_t cap_rows, mas_segment_out* seg_out, mas_stream_t stream) {
   if (!p || !mas_tok || cap_rows < 0) return MAS_ERR_INVALID_ARG;
+  if (p->prm.select_mode == MAS_SELECT_ADAPTIVE && !seg_out) return MAS_ERR_INVALID_ARG;
   if (Y && (!X || !kept_idx)) return MAS_ERR_INVALID_ARG;
   if (Y && !aligned16(X)) return MAS_ERR_UNSUPPORTED;
   if (Y && !aligned16(Y)) return MAS_ERR_UNSUPPORTED;
@@ -503,8 +506,15 @@ static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* 
   }
   SegArgs a = seg_args(p, sb, gb, rb, m_spatial, mb, so, mask, kept_idx, koff, cap_rows, p->tc.enabled);
   if (pev) CK(cudaEventRecord(pev[1], st));
-  CK(launch_kc(k_segment<true, true>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3((unsigned)p->seg_threads), p->seg_cluster, st, pdl, a));
-  if (p->prm.select_mode == MAS_SELECT_THRESHOLD && kept_idx) {
+  const dim3 sgrid((unsigned)(p->n_segs * p->seg_cluster)), sblock((unsigned)p->seg_threads);
+  if (p->prm.select_mode == MAS_SELECT_ADAPTIVE) {   // keep counts come from MAS_s, which the LAST cluster of the fuse launch writes
+    CK(launch_kc(k_segment<true, false>, sgrid, sblock, p->seg_cluster, st, pdl, a));
+    a.gamma_raw = 0;
+    CK(launch_kc(k_segment<false, true>, sgrid, sblock, p->seg_cluster, st, pdl, a));
+  } else {
+    CK(launch_kc(k_segment<true, true>, sgrid, sblock, p->seg_cluster, st, pdl, a));
+  }
+  if (p->prm.select_mode != MAS_SELECT_TOPK && kept_idx) {
     CK(launch_k(k_compact_idx, dim3((unsigned)p->n_segs), dim3(kSegThreads), 0, st, pdl, (const DevSeg*)p->at<DevSeg>(p->lay.segs),
                 (const uint8_t*)mask, (const int64_t*)koff, kept_idx, cap_rows));
   }
@@ -602,7 +612,7 @@ extern "C" int mas_forward_host(const mas_plan* p, const void* h_X, const void* 
     if (h_out->kept_idx || h_out->Y) {
       int64_t* total_h = reinterpret_cast<int64_t*>(static_cast<char*>(p->pinned) + p->lay.tables_end);
       int64_t total = p->kept_cap;
-      if (p->prm.select_mode == MAS_SELECT_THRESHOLD) {   // the kept count is data dependent: read it before sizing the copies
+      if (p->prm.select_mode != MAS_SELECT_TOPK) {   // the kept count is data dependent: read it before sizing the copies
         CK(cudaMemcpyAsync(total_h, koff + p->n_segs, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         total = *total_h;

@@ -12,7 +12,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 MOD_IMAGE, MOD_VIDEO, MOD_AUDIO = 1, 2, 3
-SELECT_TOPK, SELECT_THRESHOLD = 0, 1
+SELECT_TOPK, SELECT_THRESHOLD, SELECT_ADAPTIVE = 0, 1, 2
 GRID = 24  # 24 x 24 = 576 patch tokens per image / frame
 
 
@@ -56,7 +56,7 @@ class Workload:
         return len(self.q_off) - 1
 
     def kept_capacity(self):
-        if self.select_mode == SELECT_THRESHOLD:
+        if self.select_mode != SELECT_TOPK:
             return self.n_tokens
         return int(sum(s[4] for s in self.segments))
 

@@ -17,15 +17,29 @@ def assert_close(gpu, ref, name):
         name, bad.size, ref.size, bad[np.argmax(err[bad] - tol[bad])], gpu[bad[0]], ref[bad[0]])
 
 
-def check_selection(rows, select_mode, cut, ref_mas, gpu_mask, gpu_idx, gpu_off, row_base=0):
+def adaptive_keep(seg_mas, n):
+    """NEXT-3 rule restated: the smallest retention Eq. 11's constraint beta >= 1 - MAS_s admits."""
+    return int(min(n, max(1, np.ceil((1.0 - float(seg_mas)) * n - 1e-9))))
+
+
+def check_selection(rows, select_mode, cut, ref_mas, gpu_mask, gpu_idx, gpu_off, row_base=0, gpu_seg_mas=None, ref_so=None, ref_m=None):
     """rows: (request, modality, T, P, keep_k) of the compared segments; arrays cover exactly these segments
-    (gpu_idx holds global ids: subtract row_base).  SPEC.md parity rules for selection."""
+    (gpu_idx holds global ids: subtract row_base).  SPEC.md parity rules for selection.
+    Adaptive mode (2): the keep count is an integer decided by a float, so it is checked (a) exactly against the rule
+    applied to the GPU's own fp32 MAS_s and (b) against the oracle's count within what the MAS_s tolerance can move it;
+    the selection itself is then the top-k comparison at the GPU's count."""
     gpu_mask = np.asarray(gpu_mask).astype(bool)
     r0 = 0
     for k, (_, _, T, P, kk) in enumerate(rows):
         n = T * P
         mas = np.asarray(ref_mas[r0:r0 + n], np.float64)
-        if select_mode == 0:
+        if select_mode == 2:
+            kk = int(gpu_off[k + 1] - gpu_off[k])
+            assert kk == adaptive_keep(np.float32(gpu_seg_mas[k]), n), (k, kk, float(gpu_seg_mas[k]), n)
+            near = np.count_nonzero(np.abs(np.asarray(ref_m[r0:r0 + n]) - 0.3) <= 1e-3 * 0.3) if ref_m is not None else 0
+            tol = RTOL * abs(ref_so[k].mas) + ATOL + 0.6 * near / n
+            assert abs(kk - ref_so[k].n_kept) <= 1 + int(np.ceil(tol * n)), (k, kk, ref_so[k].n_kept, tol * n)
+        if select_mode in (0, 2):
             order = np.sort(mas)
             c = order[kk - 1] if kk >= n else 0.5 * (order[kk - 1] + order[kk])
             ref_keep = np.zeros(n, bool)

@@ -464,3 +464,19 @@ def test_entropy_matches_scipy_and_is_shift_invariant():
     Hb, _ = O.draft_entropy(Lb, 2.0)
     wantb = np.array([entropy(softmax(row.astype(np.float64))) for row in synth.bf16_bits_to_f32(Lb)])
     assert np.allclose(Hb, wantb, rtol=1e-12, atol=1e-12)            # bf16 decoding
+
+
+# ---------------------------------------------------------------- NEXT-3: adaptive retention from Eq. 11's constraint
+def test_adaptive_retention_rule():
+    """keep_k = ceil((1 - MAS_s) N_s) clamped to [1, N_s] (beta_m >= 1 - MAS_m), ties and order as in top-k."""
+    n = 10
+    X = np.arange(n * 4, dtype=np.float32).reshape(n, 4)
+    mas_tok = np.array([0.5, 0.1, 0.9, 0.1, 0.3, 0.7, 0.2, 0.8, 0.4, 0.6])
+    prm = O.default_params(select_mode=2)
+    for seg_mas, want_k in ((0.3, 7), (1.0, 1), (0.0, 10), (0.25, 8), (0.95, 1), (0.9, 1), (0.89, 2)):
+        mask, idx, off, Y, out = O.select_compact(seg1(1, n), prm, X, mas_tok, seg_mas=[seg_mas])
+        assert int(off[1]) == want_k == int(mask.sum()) == out[0].n_kept
+        assert want_k >= (1.0 - seg_mas) * n - 1e-9 and want_k - 1 < max((1.0 - seg_mas) * n, 1)      # smallest admissible retention
+        order = sorted(range(n), key=lambda i: (mas_tok[i], i))[:want_k]                               # same order as top-k
+        assert list(idx[:want_k]) == sorted(order)
+        assert np.array_equal(Y[:want_k], X[sorted(order)])

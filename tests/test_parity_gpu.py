@@ -138,7 +138,8 @@ def _forward_and_compare(B, w, sample_requests=None, **prm):
         assert np.array_equal(host["gamma"][lo:hi] == 0.0, ref["gamma"] == 0.0)
         P.check_seg_out(rows, so[ks[0]:ks[-1] + 1], ref["seg_out"], ref["m_spatial"])
         off = host["kept_off"][ks[0]:ks[-1] + 2]
-        P.check_selection(rows, w.select_mode, w.cut, ref["mas_tok"], host["keep_mask"][lo:hi], host["kept_idx"], off, row_base=lo)
+        P.check_selection(rows, w.select_mode, w.cut, ref["mas_tok"], host["keep_mask"][lo:hi], host["kept_idx"], off, row_base=lo,
+                          gpu_seg_mas=so["mas"][ks[0]:ks[-1] + 1], ref_so=ref["seg_out"], ref_m=ref["m_spatial"])
     # whole-batch structural properties (hold at any size)
     total = int(host["kept_off"][-1])
     assert host["keep_mask"].sum() == total
@@ -314,6 +315,57 @@ def test_forward_segment_size_sweep(B, name, mode):
     shapes, d, L = SWEEPS[name]
     w = _random_workload(101 + mode, shapes, d, L, select_mode=mode, cut=0.45)
     _forward_and_compare(B, w)
+
+
+# ---------------------------------------------------------------- NEXT-3: adaptive retention (beta >= 1 - MAS_s)
+@pytest.mark.parametrize("name", ["images", "video", "audio_vision", "cluster8", "tile_heights"])
+def test_forward_adaptive_retention(B, name):
+    if name in SWEEPS:
+        shapes, d, L = SWEEPS[name]
+        w = _random_workload(300, shapes, d, L, select_mode=2, cut=0.45)
+    else:
+        w = {"images": synth.batched_images(seed=41, R=5, d=512, L_lo=3, L_hi=70, P=333),
+             "video": synth.video(seed=42, R=2, T=4, P=576, d=256, L=48),
+             "audio_vision": synth.audio_vision(seed=43, R=2, d=256, L=64, P_img=576, T_aud=300)}[name]
+        w.select_mode = 2
+    plan = _plan(B, w)
+    assert plan.kept_capacity == w.n_tokens
+    host, so = _forward_and_compare(B, w)
+    nk = np.array([int(v) for v in so["n_kept"]])
+    nt = np.array([s[2] * s[3] for s in w.segments])
+    assert np.all(nk >= 1) and np.all(nk <= nt)
+    assert np.all(nk >= (1.0 - so["mas"].astype(np.float64)) * nt - 1e-6)         # the constraint itself
+    plan.close()
+
+
+def test_staged_adaptive_select_on_shared_scalars(B):
+    """mas_select_compact in adaptive mode reads MAS_s from the fuse step's records: bit-exact against the oracle given the
+    same fp32 MAS_s and token scores; NULL records are refused."""
+    rng = np.random.default_rng(47)
+    rows = [(0, 1, 1, 576, 1), (0, 3, 1500, 1, 1), (1, 2, 5, 300, 1), (2, 1, 1, 1, 1), (3, 2, 33, 555, 1), (3, 1, 1, 130, 1)]
+    segs, n = O.make_segments(rows)
+    X = rng.standard_normal((n, 64)).astype(np.float32)
+    plan = B.Plan(rows, [0, 4, 8, 12, 16], 64, B.MAS_F32, B.default_params(select_mode=2))
+    prm = O.default_params(select_mode=2)
+    vals = (rng.integers(0, 64, n) / 64.0).astype(np.float32)
+    seg_mas = np.array([0.3, 0.999, 0.0, 0.5, 0.123456, 1.0], np.float32)
+    so_in = torch.zeros(len(rows) * 36, dtype=torch.uint8, device="cuda")
+    so_np = B.seg_out_numpy(so_in.cpu()).copy()
+    so_np["mas"] = seg_mas
+    so_in.copy_(torch.from_numpy(so_np.view(np.uint8).reshape(-1)))
+    o = plan.select_compact(torch.from_numpy(X).cuda(), torch.from_numpy(vals).cuda(), seg_out=so_in)
+    mask_r, idx_r, off_r, Y_r, so_r = O.select_compact(segs, prm, X, vals, seg_mas=seg_mas)
+    off = o["kept_off"].cpu().numpy()
+    assert np.array_equal(off, off_r)
+    assert list(np.diff(off)) == [P.adaptive_keep(m, r[2] * r[3]) for m, r in zip(seg_mas, rows)]
+    assert np.array_equal(o["keep_mask"].cpu().numpy(), mask_r)
+    tot = int(off[-1])
+    assert np.array_equal(o["kept_idx"].cpu().numpy()[:tot], idx_r[:tot])
+    assert np.array_equal(o["Y"].cpu().numpy()[:tot], Y_r[:tot])
+    from paper_2604_02945_b200.binding import lib, _ptr
+    rc = lib.mas_select_compact(plan._h, None, _ptr(torch.from_numpy(vals).cuda()), None, None, None, None, 0, None, None)
+    assert rc == B.MAS_ERR_INVALID_ARG
+    plan.close()
 
 
 def test_separate_query_norm_launch_gives_identical_results(B):
