@@ -10,6 +10,10 @@
 //
 // NEXT-4 (mas_ref_draft_entropy): pinned by uniform -> log V, one-hot -> 0, the two-level closed form, shift invariance and
 // scipy.stats.entropy of a float64 softmax.
+// NEXT-2 (mas_ref_learned_heads): pinned by a hand-worked two-segment example (tests/golden/closed_forms.txt, heads_*), the
+// ReLU clip it contains, w_sp = 0 -> M = sigmoid(b_sp), a dead hidden layer -> uniform beta, token-order invariance and
+// numpy float64 matrix products.
+// NEXT-3 (select_mode 2 of mas_ref_select_compact): pinned by worked counts (MAS_s 0.3, N 10 -> 7; 1 -> 1; 0 -> N) and minimality.
 // NEXT-1 (mas_ref_temporal_lsh): pinned by explicit signs of hand-expanded projections, identical / negated rows,
 // power-of-two scaling, and the collision law E[gamma] = theta / pi.
 //
@@ -361,6 +365,79 @@ int mas_ref_forward(const mas_ref_segment* segs, int32_t n_segs, const int64_t* 
   if ((rc = mas_ref_fuse(segs, n_segs, prm, s, gamma, rel, m_spatial, mas_tok, out))) return rc;
   if (keep_mask && kept_off)
     if ((rc = mas_ref_select_compact(segs, n_segs, d, dtype, prm, X, mas_tok, keep_mask, kept_idx, kept_off, Y, cap_rows, out))) return rc;
+  return 0;
+}
+
+// NEXT-2: the paper's LEARNED heads, with weights supplied by the caller (the trained ones are unpublished).
+//   Eq. 3: M_i = sigmoid(w_sp . x_i + b_sp)  -- a 1x1 convolution C -> 1 on each patch's channel vector;
+//   Eq. 4:    rho = |{i : M_i < tau_s}| / N_s;
+//   Eq. 6: alpha_s = MLP([p ; z_s]) with p = mean of the request's query rows, z_s = mean of the segment's
+//     token rows, MLP = one hidden ReLU layer of `hidden` units: alpha = w2 . relu(W1z z + W1p p + b1) + b2 (reading N2);
+//   beta = softmax of alpha over the request's segments, as printed (no temperature); Eq. 7 with reading G8.
+// W[64, d]: row 0 = w_sp, rows 1..hidden = W1z.  Wp[64, d]: rows 1..hidden = W1p.  b1, w2: entries 1..hidden.  Other rows
+// and entries are ignored.  gamma[N] is the temporal probe's output (S2); it is read for segments with T > 1 only.
+int mas_ref_learned_heads(const mas_ref_segment* segs, int32_t n_segs, const int64_t* q_off, int64_t d, int dtype,
+                          const mas_ref_params* prm, const void* X, const void* Q, const double* gamma, const void* W,
+                          const void* Wp, const double* b1, const double* w2, double b_sp, double b2, int32_t hidden,
+                          double* m_spatial, mas_ref_segment_out* out) {
+  if (hidden < 1 || hidden > 63) return 1;
+  std::vector<double> z(static_cast<size_t>(d)), pm(static_cast<size_t>(d));
+  for (int32_t k = 0; k < n_segs; ++k) {
+    const int64_t T = segs[k].n_frames, P = segs[k].n_patches, r0 = segs[k].row0, n = T * P;
+    const int64_t qa = q_off[segs[k].request], qb = q_off[segs[k].request + 1];
+    if (qb <= qa) return 1;
+    int64_t below = 0;
+    for (int64_t i = r0; i < r0 + n; ++i) {
+      double u = 0.0;
+      for (int64_t c = 0; c < d; ++c) u += elem(W, dtype, c) * elem(X, dtype, i * d + c);
+      const double M = sigmoid(u + b_sp);                       // Eq. 3
+      if (M < prm->tau_s) ++below;                              // Eq. 4, strict <
+      if (m_spatial) m_spatial[i] = M;
+    }
+    for (int64_t c = 0; c < d; ++c) {                           // z_s, p: plain column means
+      double a = 0.0;
+      for (int64_t i = r0; i < r0 + n; ++i) a += elem(X, dtype, i * d + c);
+      z[static_cast<size_t>(c)] = a / static_cast<double>(n);
+      double b = 0.0;
+      for (int64_t j = qa; j < qb; ++j) b += elem(Q, dtype, j * d + c);
+      pm[static_cast<size_t>(c)] = b / static_cast<double>(qb - qa);
+    }
+    double alpha = b2;
+    for (int32_t h = 1; h <= hidden; ++h) {
+      double pre = b1[h];
+      for (int64_t c = 0; c < d; ++c) pre += elem(W, dtype, h * d + c) * z[static_cast<size_t>(c)] + elem(Wp, dtype, h * d + c) * pm[static_cast<size_t>(c)];
+      alpha += w2[h] * std::max(pre, 0.0);
+    }
+    double gavg = 0.0;
+    if (T > 1) {
+      for (int64_t t = 1; t < T; ++t) {
+        double gt = 0.0;
+        for (int64_t q = 0; q < P; ++q) gt += gamma[r0 + t * P + q];
+        gavg += gt / static_cast<double>(P);
+      }
+      gavg /= static_cast<double>(T - 1);
+    }
+    out[k].rho_spatial = static_cast<double>(below) / static_cast<double>(n);
+    out[k].gamma_avg = gavg;
+    out[k].alpha_mean = alpha;
+    out[k].mean_s = 0.0; out[k].std_s = 0.0; out[k].mean_r = 0.0; out[k].std_r = 0.0;
+    out[k].n_tokens = n; out[k].n_kept = 0; out[k].beta = 0.0; out[k].mas = 0.0;
+  }
+  int32_t k0 = 0;
+  while (k0 < n_segs) {
+    int32_t k1 = k0;
+    while (k1 < n_segs && segs[k1].request == segs[k0].request) ++k1;
+    double mx = out[k0].alpha_mean;
+    for (int32_t k = k0; k < k1; ++k) mx = std::max(mx, out[k].alpha_mean);
+    double zs = 0.0;
+    for (int32_t k = k0; k < k1; ++k) zs += std::exp(out[k].alpha_mean - mx);
+    for (int32_t k = k0; k < k1; ++k) {
+      const double a = segs[k].n_frames > 1 ? 1.0 : 0.0;
+      out[k].beta = std::exp(out[k].alpha_mean - mx) / zs;
+      out[k].mas = 1.0 - out[k].beta * (1.0 - prm->lambda_spatial * out[k].rho_spatial - a * prm->lambda_temp * (1.0 - out[k].gamma_avg));  // Eq. 7, G8
+    }
+    k0 = k1;
+  }
   return 0;
 }
 

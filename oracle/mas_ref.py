@@ -117,6 +117,26 @@ def draft_entropy(logits, theta_conf):
     return H, flag
 
 
+def learned_heads(segs, q_off, params, X, Q, gamma, W, Wp, b1, w2, b_sp, b2, hidden):
+    """NEXT-2: Eq. 3 / Eq. 6 with supplied weights.  W, Wp: [64, d] in X's dtype; b1, w2: [64].  -> (m_spatial, seg_out)."""
+    X = np.ascontiguousarray(X)
+    Q = np.ascontiguousarray(Q)
+    W = np.ascontiguousarray(W)
+    Wp = np.ascontiguousarray(Wp)
+    assert W.shape == (64, X.shape[1]) == Wp.shape and W.dtype == X.dtype == Wp.dtype == Q.dtype
+    q_off = np.ascontiguousarray(q_off, np.int64)
+    g = np.ascontiguousarray(gamma, np.float64)
+    b1 = np.ascontiguousarray(b1, np.float64)
+    w2 = np.ascontiguousarray(w2, np.float64)
+    assert b1.shape == (64,) == w2.shape and g.shape == (X.shape[0],)
+    m = np.zeros(X.shape[0], np.float64)
+    out = (SegmentOut * len(segs))()
+    _check(lib().mas_ref_learned_heads(segs, len(segs), _p(q_off), C.c_int64(X.shape[1]), _dtype_code(X), C.byref(params), _p(X), _p(Q),
+                                       _p(g), _p(W), _p(Wp), _p(b1), _p(w2), C.c_double(b_sp), C.c_double(b2), C.c_int32(hidden),
+                                       _p(m), out))
+    return m, out
+
+
 def temporal_lsh(segs, X, R, want_proj=False):
     """NEXT-1: literal LSH probe of Eq. 5 with K = 64 hashes from R[64, d] (same dtype as X)."""
     X = np.ascontiguousarray(X)

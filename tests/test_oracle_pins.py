@@ -480,3 +480,88 @@ def test_adaptive_retention_rule():
         order = sorted(range(n), key=lambda i: (mas_tok[i], i))[:want_k]                               # same order as top-k
         assert list(idx[:want_k]) == sorted(order)
         assert np.array_equal(Y[:want_k], X[sorted(order)])
+
+
+# ---------------------------------------------------------------- NEXT-2: learned heads (Eq. 3, Eq. 6 with supplied weights)
+def _heads_weights(d, hidden, w_sp, W1z, W1p, b1, w2):
+    W = np.zeros((64, d), np.float32)
+    Wp = np.zeros((64, d), np.float32)
+    B1 = np.zeros(64)
+    W2 = np.zeros(64)
+    W[0] = w_sp
+    W[1:1 + hidden] = W1z
+    Wp[1:1 + hidden] = W1p
+    B1[1:1 + hidden] = b1
+    W2[1:1 + hidden] = w2
+    W[1 + hidden:] = 7.0          # rows past `hidden` are ignored
+    Wp[0] = -3.0                  # so is row 0 of Wp
+    B1[0] = 5.0
+    W2[0] = 5.0
+    return W, Wp, B1, W2
+
+
+def test_learned_heads_worked_example():
+    segs, n = O.make_segments([(0, 1, 1, 2, 1), (0, 2, 2, 1, 1)])
+    X = f32([[1, 0], [0, 2], [2, 2], [-2, 0]])
+    Q = f32([[1, 1], [3, -1]])
+    W, Wp, b1, w2 = _heads_weights(2, 2, [1, -1], [[1, 0], [0, 1]], [[0.5, 0], [0, 1]], [-1.25, 0.25], [2, 3])
+    m, out = O.learned_heads(segs, [0, 2], O.default_params(), X, Q, [0, 0, 1, 0.25], W, Wp, b1, w2, 0.0, -0.5, 2)
+    assert np.allclose(m, [GOLD["heads_M_u1"], GOLD["heads_M_um2"], 0.5, GOLD["heads_M_um2"]], rtol=0, atol=1e-15)
+    assert out[0].rho_spatial == 0.5 == out[1].rho_spatial
+    assert out[0].alpha_mean == GOLD["heads_alpha_A"] and out[1].alpha_mean == GOLD["heads_alpha_B"]
+    assert abs(out[0].beta - GOLD["heads_beta_A"]) < 1e-15 and abs(out[0].beta + out[1].beta - 1.0) < 1e-15
+    assert out[0].gamma_avg == 0.0 and out[1].gamma_avg == 0.25
+    assert abs(out[0].mas - GOLD["heads_mas_A"]) < 1e-14 and abs(out[1].mas - GOLD["heads_mas_B"]) < 1e-14
+
+
+def test_learned_heads_special_cases_and_numpy():
+    rng = np.random.default_rng(5)
+    d, hidden = 24, 5
+    rows = [(0, 1, 1, 30, 1), (0, 2, 3, 7, 1), (1, 1, 1, 11, 1)]
+    segs, n = O.make_segments(rows)
+    X = rng.standard_normal((n, d)).astype(np.float32)
+    Q = rng.standard_normal((9, d)).astype(np.float32)
+    q_off = [0, 4, 9]
+    gamma = rng.random(n)
+    w_sp = rng.standard_normal(d).astype(np.float32) * 0.3
+    W1z, W1p = rng.standard_normal((hidden, d)).astype(np.float32), rng.standard_normal((hidden, d)).astype(np.float32)
+    b1, w2 = rng.standard_normal(hidden), rng.standard_normal(hidden)
+    W, Wp, B1, W2 = _heads_weights(d, hidden, w_sp, W1z, W1p, b1, w2)
+    prm = O.default_params()
+    m, out = O.learned_heads(segs, q_off, prm, X, Q, gamma, W, Wp, B1, W2, 0.1, -0.2, hidden)
+    # library routines in float64: matrix products and column means
+    X64, Q64 = X.astype(np.float64), Q.astype(np.float64)
+    assert np.allclose(m, 1.0 / (1.0 + np.exp(-(X64 @ w_sp.astype(np.float64) + 0.1))), rtol=1e-13, atol=0)
+    r0 = 0
+    alphas = []
+    for k, (req, _, T, P, _) in enumerate(rows):
+        nk = T * P
+        z = X64[r0:r0 + nk].mean(axis=0)
+        p = Q64[q_off[req]:q_off[req + 1]].mean(axis=0)
+        pre = W1z.astype(np.float64) @ z + W1p.astype(np.float64) @ p + b1
+        alphas.append(float(w2 @ np.maximum(pre, 0.0) - 0.2))
+        assert abs(out[k].alpha_mean - alphas[-1]) < 1e-12
+        assert out[k].rho_spatial == np.count_nonzero(m[r0:r0 + nk] < 0.3) / nk
+        r0 += nk
+    e = np.exp(np.array(alphas[:2]) - max(alphas[:2]))
+    assert abs(out[0].beta - e[0] / e.sum()) < 1e-14 and out[2].beta == 1.0          # request 1 has one segment
+    assert abs(out[1].gamma_avg - gamma[30 + 7:30 + 21].reshape(2, 7).mean(axis=1).mean()) < 1e-15
+    # token order inside a single-frame segment does not matter (means), the map is permuted with it
+    perm = rng.permutation(30)
+    X2 = X.copy()
+    X2[:30] = X[:30][perm]
+    m2, out2 = O.learned_heads(segs, q_off, prm, X2, Q, gamma, W, Wp, B1, W2, 0.1, -0.2, hidden)
+    assert np.array_equal(m2[:30], m[:30][perm]) and abs(out2[0].alpha_mean - out[0].alpha_mean) < 1e-12
+    # w_sp = 0: M = sigmoid(b_sp) everywhere, rho is 0 or 1 by the strict compare
+    W0 = W.copy()
+    W0[0] = 0
+    for b, rho in ((math.log(0.3 / 0.7) - 1e-9, 1.0), (math.log(0.3 / 0.7) + 1e-9, 0.0)):
+        m0, out0 = O.learned_heads(segs, q_off, prm, X, Q, gamma, W0, Wp, B1, W2, b, -0.2, hidden)
+        assert np.allclose(m0, 1.0 / (1.0 + math.exp(-b)), rtol=1e-15) and all(o.rho_spatial == rho for o in out0)
+    # a dead hidden layer (every unit clipped): alpha = b2 for every segment -> uniform beta
+    Bd = B1.copy()
+    Bd[1:1 + hidden] = -1e6
+    _, outd = O.learned_heads(segs, q_off, prm, X, Q, gamma, W, Wp, Bd, W2, 0.1, -0.2, hidden)
+    assert all(o.alpha_mean == -0.2 for o in outd) and outd[0].beta == 0.5 == outd[1].beta
+    # Eq. 7 single image, beta = 1: MAS = lambda_sp * rho
+    assert abs(out[2].mas - 0.6 * out[2].rho_spatial) < 1e-15
