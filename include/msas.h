@@ -182,6 +182,41 @@ int mas_forward(const mas_plan* plan, const void* X, const void* Q,
 int mas_forward_lsh(const mas_plan* plan, const void* X, const void* Q, const void* Rm, uint64_t* sig /*[N]*/,
                     float* gamma_lsh /*[N] or NULL*/, const mas_outputs* out, mas_stream_t stream);
 
+/* NEXT-2: the paper's LEARNED heads with caller-supplied weights (the trained ones are unpublished), giving the
+ * per-modality descriptors of PAPER.md:118-124 as printed:
+ *   Eq. 3   m_spatial_i = sigmoid(w_sp . x_i + b_spatial)            (1x1 convolution C -> 1 per patch)
+ *   Eq. 4      rho_s = |{i : m_spatial_i < tau_s}| / N_s
+ *   Eq. 6 alpha_s = w2 . relu(W1z z_s + W1p p_r + b1) + b2,  z_s = mean of the segment's rows of X,
+ *                            p_r = mean of the request's rows of Q (one hidden ReLU layer of `hidden` units: reading N2)
+ *   PAPER.md:116             beta_s = softmax of alpha over the request's segments (no temperature)
+ *   Eq. 7 (reading G8)       MAS_s = 1 - beta_s (1 - lambda_sp rho_s - [T > 1] lambda_t (1 - gamma_avg_s))
+ * W[MAS_HEADS_ROWS, d]: row 0 = w_sp, rows 1..hidden = W1z; Wp[MAS_HEADS_ROWS, d]: rows 1..hidden = W1p; b1, w2[MAS_HEADS_ROWS]:
+ * entries 1..hidden.  Other rows / entries are ignored but must be readable and finite.  W and Wp: device, dtype and row
+ * stride of X, 16-byte aligned; b1, w2: device fp32.  The struct itself is host memory, read during the call.
+ * gamma[N]: the temporal probe's output (mas_temporal / mas_forward); NULL allowed iff no segment has T > 1.
+ * Outputs: m_spatial[N] and seg_out[n_segs] (rho_spatial, gamma_avg, alpha_mean = alpha_s, beta, mas, n_tokens; mean_s, std_s,
+ * n_kept = 0).  X is read once (one tile kernel with W as the B operand of its MMA); three launches.
+ * Errors: INVALID_ARG (NULL, hidden outside 1..63, gamma NULL with a temporal segment), UNSUPPORTED (alignment). */
+#define MAS_HEADS_ROWS 64
+typedef struct {
+  const void* W;
+  const void* Wp;
+  const float* b1;
+  const float* w2;
+  float b_spatial;
+  float b2;
+  int32_t hidden;
+  int32_t reserved_;
+} mas_heads;
+int mas_learned_heads(const mas_plan* plan, const void* X, const void* Q, const float* gamma /*[N] or NULL*/, const mas_heads* heads,
+                      float* m_spatial /*[N]*/, mas_segment_out* seg_out /*[n_segs]*/, mas_stream_t stream);
+/* mas_forward plus the learned heads in the same pass: on the bf16 fast path with every L_r <= 64 the weight rows W ride the
+ * score kernel's tensor-core contraction as 64 more B rows (no second sweep over X); otherwise the call is mas_forward followed
+ * by mas_learned_heads.  `out` as for mas_forward_lsh; the learned descriptors go to heads_m_spatial[N] / heads_seg_out[n_segs]
+ * (their gamma_avg is the one of this pass); the training-free outputs in `out` are unchanged by the presence of the heads. */
+int mas_forward_heads(const mas_plan* plan, const void* X, const void* Q, const mas_heads* heads, float* heads_m_spatial /*[N]*/,
+                      mas_segment_out* heads_seg_out /*[n_segs]*/, const mas_outputs* out, mas_stream_t stream);
+
 /* NEXT-4: the draft-confidence entropy of Eq. 9 and the speculate rule of Eq. 10, the
  * consumer-side step next to the MAS pass.  logits[n_rows, V] (device, fp32 or bf16, row stride `row_stride` elements,
  * base and stride 16-byte aligned, n_rows <= 65535): per row p = softmax(l), H = -sum_v p_v ln p_v,

@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy"]
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads"]
 
 
 class mas_segment(C.Structure):
@@ -49,6 +49,11 @@ class mas_outputs(C.Structure):
     _fields_ = [("m_spatial", C.c_void_p), ("gamma", C.c_void_p), ("rel", C.c_void_p), ("mas_tok", C.c_void_p),
                 ("seg_out", C.c_void_p), ("keep_mask", C.c_void_p), ("kept_idx", C.c_void_p), ("kept_off", C.c_void_p),
                 ("Y", C.c_void_p), ("cap_rows", C.c_int64)]
+
+
+class mas_heads(C.Structure):
+    _fields_ = [("W", C.c_void_p), ("Wp", C.c_void_p), ("b1", C.c_void_p), ("w2", C.c_void_p), ("b_spatial", C.c_float),
+                ("b2", C.c_float), ("hidden", C.c_int32), ("reserved_", C.c_int32)]
 
 
 def _load():
@@ -93,6 +98,10 @@ def _load():
     lib.mas_draft_entropy_workspace_bytes.restype = C.c_int
     lib.mas_draft_entropy.argtypes = [vp, i64, i64, i64, i32, C.c_float, vp, vp, vp, C.c_size_t, vp]
     lib.mas_draft_entropy.restype = C.c_int
+    lib.mas_learned_heads.argtypes = [vp, vp, vp, vp, C.POINTER(mas_heads), vp, vp, vp]
+    lib.mas_learned_heads.restype = C.c_int
+    lib.mas_forward_heads.argtypes = [vp, vp, vp, C.POINTER(mas_heads), vp, vp, C.POINTER(mas_outputs), vp]
+    lib.mas_forward_heads.restype = C.c_int
     lib.mas_score_schedule.restype = i32
     lib.mas_score_schedule.argtypes = [C.POINTER(mas_segment), i32, C.POINTER(i64), i32, i32, i32, i32, C.POINTER(i32), i32]
     for f in ("mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal",
@@ -249,6 +258,25 @@ class Plan:
         g = self._f32()
         _check(lib.mas_temporal_lsh(self._h, _ptr(X), _ptr(Rm), _ptr(sig), _ptr(g), _stream_ptr(stream)), "mas_temporal_lsh")
         return sig, g
+
+    def learned_heads(self, X, Q, gamma, W, Wp, b1, w2, b_spatial, b2, hidden, stream=None):
+        """NEXT-2: Eq. 3 / Eq. 6 with supplied weights (W, Wp: [64, d] like X; b1, w2: fp32 [64]) -> (m_spatial, seg_out)."""
+        hd = mas_heads(_ptr(W), _ptr(Wp), _ptr(b1), _ptr(w2), float(b_spatial), float(b2), int(hidden), 0)
+        m = self._f32()
+        so = torch.zeros(self.n_segs * 36, dtype=torch.uint8, device=self.device)
+        _check(lib.mas_learned_heads(self._h, _ptr(X), _ptr(Q), _ptr(gamma), C.byref(hd), _ptr(m), _ptr(so), _stream_ptr(stream)),
+               "mas_learned_heads")
+        return m, so
+
+    def forward_heads(self, X, Q, W, Wp, b1, w2, b_spatial, b2, hidden, out=None, stream=None):
+        """mas_forward + the learned heads in one pass: returns (outputs, learned m_spatial, learned seg_out)."""
+        o = out if out is not None else self.alloc_outputs()
+        hd = mas_heads(_ptr(W), _ptr(Wp), _ptr(b1), _ptr(w2), float(b_spatial), float(b2), int(hidden), 0)
+        m = self._f32()
+        so = torch.zeros(self.n_segs * 36, dtype=torch.uint8, device=self.device)
+        _check(lib.mas_forward_heads(self._h, _ptr(X), _ptr(Q), C.byref(hd), _ptr(m), _ptr(so), C.byref(self._bundle(o)), _stream_ptr(stream)),
+               "mas_forward_heads")
+        return o, m, so
 
     def crossmodal(self, X, Q, want_S=False, stream=None):
         rel = self._f32()

@@ -22,6 +22,12 @@ struct ScoreArgs {
   float* rel;      // may be NULL
   float* S_opt;    // may be NULL, [N, kMaxL]
   unsigned long long* sig;   // LSH mode (NEXT-1): Q is the hash matrix R[64, d] shared by all rows; bit k of sig[row] = [r_k . x >= 0]
+  // learned-heads mode (NEXT-2): Q is the weight matrix W[64, d] shared by all rows (row 0 = Eq. 3's 1x1 conv, rows 1.. = the
+  // z-half of Eq. 6's first layer).  Per row: m_spatial = sigmoid(w_0 . x + heads_bias); per tile: heads_part[tile][0] = number of
+  // rows with m_spatial < heads_tau, heads_part[tile][c] = sum over the tile's rows of w_c . x (c = 1..63)
+  float* heads_part;
+  float* heads_m;
+  float heads_bias, heads_tau;
   int d;
 };
 
@@ -127,7 +133,8 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
   constexpr int NPLANE = DT == 1 ? 1 : 2;          // fp32: hi and lo planes
   constexpr int PIECES = (LP * 8 + 255) / 256;     // 16-byte pieces per thread per chunk
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, c = lane & 3;
-  const int d = a.d, L = a.sig ? 64 : seg.L;
+  const bool shared_b = a.sig != nullptr || a.heads_part != nullptr;   // one 64-row B operand for every tile
+  const int d = a.d, L = shared_b ? 64 : seg.L;
   const int esz = DT == 1 ? 2 : 4;
 
   const int rl = warp * 16 + g, rh = rl + 8;
@@ -142,7 +149,7 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
   const char* x_hi = Xb + row_hi * (int64_t)d * esz;
   const char* p_lo = x_lo - (int64_t)seg.n_patches * d * esz;
   const char* p_hi = x_hi - (int64_t)seg.n_patches * d * esz;
-  const char* Qb = static_cast<const char*>(a.Q) + (a.sig ? (int64_t)0 : (int64_t)seg.q0 * d * esz);
+  const char* Qb = static_cast<const char*>(a.Q) + (shared_b ? (int64_t)0 : (int64_t)seg.q0 * d * esz);
 
   float acc[NT][4];
 #pragma unroll
@@ -257,7 +264,7 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
           bh[k] = pack_bf16x2(xh[2 * k] - bf_lo(ah[k]), xh[2 * k + 1] - bf_hi(ah[k]));
         }
       }
-      if (a.rel != nullptr || a.S_opt != nullptr || a.sig != nullptr) {
+      if (a.rel != nullptr || a.S_opt != nullptr || shared_b) {
 #pragma unroll
         for (int j = 0; j < NT; ++j) {
           const int qr = j * 8 + g;
@@ -295,6 +302,37 @@ __device__ __forceinline__ void score_tile_mma(const ScoreArgs& a, const DevTile
     bl |= __shfl_xor_sync(0xffffffffu, bl, 1); bl |= __shfl_xor_sync(0xffffffffu, bl, 2);
     bh |= __shfl_xor_sync(0xffffffffu, bh, 1); bh |= __shfl_xor_sync(0xffffffffu, bh, 2);
     if (c == 0) { if (vlo) a.sig[row_lo] = bl; if (vhi) a.sig[row_hi] = bh; }
+    return;
+  }
+  if (a.heads_part != nullptr) {   // NEXT-2: column 0 -> the spatial map, columns 1..63 -> per-tile column sums (fixed order: no atomics)
+    float cs[NT][2];
+#pragma unroll
+    for (int j = 0; j < NT; ++j) {
+      cs[j][0] = (vlo ? acc[j][0] : 0.f) + (vhi ? acc[j][2] : 0.f);
+      cs[j][1] = (vlo ? acc[j][1] : 0.f) + (vhi ? acc[j][3] : 0.f);
+    }
+    if (c == 0) {   // this thread holds column 0 of its two rows
+      int below = 0;
+      if (vlo) { const float M = sigmoidf_acc(acc[0][0] + a.heads_bias); a.heads_m[row_lo] = M; below += M < a.heads_tau; }
+      if (vhi) { const float M = sigmoidf_acc(acc[0][2] + a.heads_bias); a.heads_m[row_hi] = M; below += M < a.heads_tau; }
+      cs[0][0] = (float)below;
+    }
+    float* red = reinterpret_cast<float*>(smem);   // the B-operand buffers are free after the last barrier of the K loop
+#pragma unroll
+    for (int j = 0; j < NT; ++j)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        float v = cs[j][e];
+        v += __shfl_xor_sync(0xffffffffu, v, 4); v += __shfl_xor_sync(0xffffffffu, v, 8); v += __shfl_xor_sync(0xffffffffu, v, 16);
+        if (g == 0 && j * 8 + 2 * c + e < 64) red[warp * 64 + j * 8 + 2 * c + e] = v;
+      }
+    __syncthreads();
+    if (tid < 64) {
+      float t = 0.f;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) t += red[w * 64 + tid];
+      a.heads_part[(int64_t)blockIdx.x * 64 + tid] = t;
+    }
     return;
   }
   float ml = -INFINITY, mh = -INFINITY;
@@ -355,6 +393,14 @@ __global__ void __launch_bounds__(256) k_score_mma(ScoreArgs a) {
 // rows as its B operand.
 template <int DT>
 __global__ void __launch_bounds__(256) k_lsh_sig(ScoreArgs a) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const DevTile tile = a.tiles[blockIdx.x];
+  const DevSeg seg = a.segs[tile.seg];
+  score_tile_mma<DT, 8>(a, tile, seg, smem);
+}
+// NEXT-2: projections of every row on the 64 head weight rows (Eq. 3's conv + the z-half of Eq. 6's first layer)
+template <int DT>
+__global__ void __launch_bounds__(256) k_heads_proj(ScoreArgs a) {
   extern __shared__ __align__(16) unsigned char smem[];
   const DevTile tile = a.tiles[blockIdx.x];
   const DevSeg seg = a.segs[tile.seg];

@@ -43,7 +43,8 @@ struct TcTile {            // 32 bytes
   int32_t L;               // query tokens of the request
   int32_t prev_delta;      // P if the segment is temporal (T > 1), else 0
   int32_t key_rows;        // leading rows of the tile that belong to frame 0 (no previous frame)
-  int32_t pad_[2];
+  int32_t rank;            // position of the tile when all tiles are sorted by row_start (slot of its learned-head partials)
+  int32_t pad_;
 };
 
 constexpr int kTcAluSets = 2;                        // ALU warp sets: each takes 8 / kTcAluSets of a row's eight 16-byte units
@@ -77,6 +78,12 @@ struct TcParams {
   unsigned long long* q_ready;       // [0] grid-wide arrival counter of the prologue, [1] CTAs that have left the kernel;
                                      // both zero between launches (the last CTA to leave re-arms them: graph-replay safe)
   unsigned long long* sig;           // NEXT-1 (literal LSH probe, Eq. 5): NULL = off; else the hash rows ride the MMA as 64 more B rows
+  // NEXT-2 (learned heads, Eq. 3 / Eq. 6): NULL = off; else the 64 weight rows W ride the MMA like the hash rows (never both):
+  // heads_m[row] = sigmoid(w_0 . x + heads_bias); heads_part[(2 * rank + half) * 64 + c] = per 128-row half of the tile, the
+  // number of rows with heads_m < heads_tau (c = 0) and the column sums of w_c . x (c = 1..63); rank = TcTile::rank
+  float* heads_part;
+  float* heads_m;
+  float heads_bias, heads_tau;
   float* s;
   float* dnorm;       // sqrt(sum (x - x_prev)^2) for rows that have a previous frame
   float* rel;
@@ -229,6 +236,7 @@ struct TcCtrl {                      // lives at the (1024-aligned) start of dyn
   uint32_t tmem_base;
   uint32_t pad_[31];
   float rowstat[2][kTcAluSets][2][128];   // partial sum x^2, sum (x - x_prev)^2 per (ALU set, K-slice, tile row), double buffered
+  float hred[2][4][64];              // NEXT-2: per-warp column sums of the 64 head columns, double buffered
 };
 static_assert(sizeof(TcCtrl) <= kTcCtrlBytes, "control block too large");
 
@@ -245,7 +253,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int tile_lo = p.cta_off[blockIdx.x], tile_hi = p.cta_off[blockIdx.x + 1];
   const int nk = p.n_kchunks;
-  const bool lsh = p.sig != nullptr;
+  const bool lsh = p.sig != nullptr || p.heads_part != nullptr;   // 64 more B rows after the query rows (hash rows or head weights)
 #ifdef MSAS_ABLATE
   const int dbg = p.dbg;
   auto gtime = [] { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; };
@@ -425,7 +433,54 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             if (col < tile.L) m[h] = fmaxf(m[h], __uint_as_float(v[j]) * qinv[col]);
           }
         }
-      if (lsh) {   // NEXT-1: the 64 accumulator columns after the query columns are r_k . x: their signs are the hash bits
+      if (p.heads_part != nullptr) {   // NEXT-2: column 0 -> the learned spatial map, all 64 -> per-half column sums (fixed order)
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+          float tot[2] = {0.f, 0.f};
+          if (h < g.nh) {
+            const int tr = h * 128 + r;
+            const bool valid = tr < tile.n_rows;
+#pragma unroll
+            for (int grp = 0; grp < 2; ++grp) {
+              float x[32];
+#pragma unroll
+              for (int cb = 0; cb < 2; ++cb) {
+                uint32_t v[16];
+                tc_ld16(tmem_base + (uint32_t)acc * 256u + (uint32_t)h * 128u + (uint32_t)(g.nqu + grp * 2 + cb) * 16u + ((uint32_t)(q * 32) << 16), v);
+                tc_wait_ld();
+#pragma unroll
+                for (int j = 0; j < 16; ++j) x[cb * 16 + j] = valid ? __uint_as_float(v[j]) : 0.f;
+              }
+              if (grp == 0) {
+                float below = 0.f;
+                if (valid) {
+                  const float M = sigmoidf_acc(x[0] + p.heads_bias);
+                  p.heads_m[(int64_t)tile.row_start + tr] = M;
+                  below = M < p.heads_tau ? 1.f : 0.f;
+                }
+                x[0] = below;
+              }
+              // transpose-reduce over the warp: 31 shuffles leave the total of column `lane` in lane `lane`
+#pragma unroll
+              for (int w = 16; w >= 1; w >>= 1) {
+                const bool up = (lane & w) != 0;
+#pragma unroll
+                for (int i = 0; i < w; ++i) {
+                  const float send = up ? x[i] : x[i + w], keep = up ? x[i + w] : x[i];
+                  x[i] = keep + __shfl_xor_sync(0xffffffffu, send, w);
+                }
+              }
+              tot[grp] = x[0];
+            }
+          }
+          const int hb = (it * 2 + h) & 1;
+          ctrl->hred[hb][q][lane] = tot[0];
+          ctrl->hred[hb][q][32 + lane] = tot[1];
+          asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
+          if (r < 64)
+            p.heads_part[((int64_t)tile.rank * 2 + h) * 64 + r] = (ctrl->hred[hb][0][r] + ctrl->hred[hb][1][r]) + (ctrl->hred[hb][2][r] + ctrl->hred[hb][3][r]);
+        }
+      } else if (lsh) {   // NEXT-1: the 64 accumulator columns after the query columns are r_k . x: their signs are the hash bits
         for (int h = 0; h < g.nh; ++h) {
           unsigned long long bits = 0ull;
 #pragma unroll
@@ -579,10 +634,13 @@ struct TcCost {
 #endif
   }
 };
-inline size_t tc_schedule_bytes(const mas_segment* segs, int32_t n_segs) {
+inline size_t tc_max_tiles(const mas_segment* segs, int32_t n_segs) {
   size_t tiles = 0;   // upper bound: every segment in 32-row tiles plus one remainder each
   for (int32_t k = 0; k < n_segs; ++k) tiles += (size_t)(((int64_t)segs[k].n_frames * segs[k].n_patches + 31) / 32) + 1;
-  return tiles * sizeof(TcTile) + 1024 * sizeof(int32_t) + 256;
+  return tiles;
+}
+inline size_t tc_schedule_bytes(const mas_segment* segs, int32_t n_segs) {
+  return tc_max_tiles(segs, n_segs) * sizeof(TcTile) + 1024 * sizeof(int32_t) + 256;
 }
 
 // Builds the tile list (grouped per CTA) and the per-CTA offsets into `h_dst`; `d_dst` is where the image will live.
@@ -688,6 +746,12 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     for (int i : per[c]) ht[w++] = tiles[i];
   }
   hoff[n_ctas] = w;
+  {   // rank of every tile in row order: tiles never straddle segments, so a segment's tiles are one contiguous rank range
+    std::vector<int> order(n_tiles);
+    for (int i = 0; i < n_tiles; ++i) order[i] = i;
+    std::sort(order.begin(), order.end(), [&](int a, int b) { return ht[a].row_start < ht[b].row_start; });
+    for (int i = 0; i < n_tiles; ++i) ht[order[i]].rank = i;
+  }
   sc.smem_bytes = kTcCtrlBytes + 1024 + kTcRingBytes + kTcBoxBytes;
   sc.n_ctas = n_ctas;
   sc.n_tiles = n_tiles;
@@ -724,22 +788,27 @@ inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, i
              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+struct TcHeads { float* part; float* m; float bias, tau; };   // NEXT-2 riding the score kernel (Rm = the weight rows W[64, d])
+
 // returns 0 on success, 1 if the cooperative launch is not possible on this device / partition (nothing was enqueued),
 // -1 on a CUDA / driver error (cudaGetLastError holds the code when it is a launch error).
 // `q_ready`: two zero-initialised 64-bit words owned by the plan (the kernel leaves them zero).
 // `Rm` / `sig` (both NULL = off): NEXT-1, hash rows R[64, d] and the per-token signatures; requires every L <= 64.
+// `hf` (NULL = off): NEXT-2, Rm = the head weight rows; same requirement; sig is ignored then.
 inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, float* qinv, float* s, float* dnorm, float* rel,
                            unsigned long long* q_ready, int64_t N, int64_t nQ, int d, bool inline_qprep, const void* Rm, unsigned long long* sig,
-                           cudaStream_t st) {
+                           const TcHeads* hf, cudaStream_t st) {
   TcMaps maps;
   for (int k = 0; k < 16; ++k)
     if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
   for (int k = 0; k < 3; ++k)
     if (!tc_make_map(&maps.q[k], Q, nQ, d, 64 >> k)) return -1;
-  if (sig != nullptr) { if (!tc_make_map(&maps.r, Rm, 64, d, 64)) return -1; } else maps.r = maps.q[0];
+  if (sig != nullptr || hf != nullptr) { if (!tc_make_map(&maps.r, Rm, 64, d, 64)) return -1; } else maps.r = maps.q[0];
   TcParams p;
   p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.sig = sig; p.s = s; p.dnorm = dnorm; p.rel = rel;
   p.d = d; p.n_kchunks = d / 64;
+  p.heads_part = hf ? hf->part : nullptr; p.heads_m = hf ? hf->m : nullptr; p.heads_bias = hf ? hf->bias : 0.f; p.heads_tau = hf ? hf->tau : 0.f;
+  if (hf) p.sig = nullptr;
 #ifdef MSAS_ABLATE
   p.dbg = getenv("MSAS_ABLATE") ? atoi(getenv("MSAS_ABLATE")) : 0;
   static unsigned long long* dbuf = nullptr;

@@ -14,6 +14,7 @@
 #include "k_score_tc.cuh"
 #include "k_entropy.cuh"
 #include "k_segment.cuh"
+#include "k_heads.cuh"
 
 using namespace msas;
 
@@ -27,8 +28,8 @@ static thread_local int g_last_cuda = 0;
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-  size_t segs, tiles, req, tc_sched, tables_end;   // uploaded tables (contiguous from 0)
-  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, total;
+  size_t segs, tiles, req, tc_sched, tc_segrank, tables_end;   // uploaded tables (contiguous from 0)
+  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, heads_part, heads_cq, total;
 };
 
 struct mas_plan {
@@ -130,7 +131,7 @@ static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_of
   return MAS_OK;
 }
 
-static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes) {
+static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes, size_t tc_tiles_max) {
   Layout l{};
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
@@ -138,6 +139,7 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.tiles = take(sizeof(DevTile) * n_tiles);
   l.req = take(sizeof(int32_t) * (n_req + 1));
   l.tc_sched = take(tc_bytes);
+  l.tc_segrank = take(sizeof(int32_t) * (n_segs + 1));   // first tile rank of every segment (TcTile::rank), NEXT-2
   l.tables_end = o;
   l.qinv = take(sizeof(float) * nQ);
   l.s = take(sizeof(float) * N);
@@ -149,6 +151,8 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.nkept = take(sizeof(int32_t) * n_segs);
   l.keptoff = take(sizeof(int64_t) * (n_segs + 1));
   l.counter = take(256);
+  l.heads_part = take(sizeof(float) * kHeadRows * std::max((size_t)n_tiles, 2 * tc_tiles_max));   // NEXT-2 scratch: per-tile column sums, per-request p-half
+  l.heads_cq = take(sizeof(float) * kHeadRows * kHeadSlabs * (size_t)n_req);
   l.total = o;
   return l;
 }
@@ -159,7 +163,7 @@ extern "C" int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_seg
   int64_t N, nQ; int32_t nt, maxL;
   int st = validate(h_segs, n_segs, h_q_off, n_requests, d, dtype, nullptr, &N, &nQ, &nt, &maxL);
   if (st != MAS_OK) return st;
-  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs)).total;
+  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs), tc_max_tiles(h_segs, n_segs)).total;
   return MAS_OK;
 }
 
@@ -169,6 +173,8 @@ static void set_kernel_attrs() {
   cudaFuncSetAttribute(k_score_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
   cudaFuncSetAttribute(k_lsh_sig<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
   cudaFuncSetAttribute(k_lsh_sig<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
+  cudaFuncSetAttribute(k_heads_proj<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
+  cudaFuncSetAttribute(k_heads_proj<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
   tc_set_kernel_attrs();
   (void)cudaGetLastError();
 }
@@ -184,7 +190,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
   if (st != MAS_OK) return st;
   if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0) return MAS_ERR_UNSUPPORTED;
   const size_t tc_bytes = tc_schedule_bytes(h_segs, n_segs);
-  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes);
+  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes, tc_max_tiles(h_segs, n_segs));
   if (workspace_bytes < lay.total) return MAS_ERR_WORKSPACE;
 
   mas_plan* p = new (std::nothrow) mas_plan();
@@ -224,6 +230,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     ds.q0 = (int32_t)h_q_off[s.request];
     ds.L = (int32_t)(h_q_off[s.request + 1] - h_q_off[s.request]);
     ds.keep_k = params->select_mode == MAS_SELECT_TOPK ? s.keep_k : ds.n_rows;
+    ds.tile0 = ti;
     kept += params->select_mode == MAS_SELECT_TOPK ? s.keep_k : 0;
     if (hr[s.request] > k) hr[s.request] = k;
     for (int32_t r0 = 0; r0 < ds.n_rows; r0 += tile_rows) {
@@ -246,6 +253,18 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     p->seg_threads = slice <= 1024 ? 256 : slice <= 2048 ? 512 : kSegThreads;
   }
   tc_build_schedule(p->tc, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched, p->ws + lay.tc_sched);
+  if (p->tc.enabled) {   // per-segment range of tile ranks (slots of the learned-head partials)
+    const TcTile* tt = reinterpret_cast<const TcTile*>(h + lay.tc_sched);
+    int32_t* sr = reinterpret_cast<int32_t*>(h + lay.tc_segrank);
+    std::vector<int32_t> cnt(n_segs + 1, 0);
+    for (int i = 0; i < p->tc.n_tiles; ++i) {
+      int32_t lo = 0, hi = n_segs - 1;   // segment holding row_start (segments tile [0, N) in order)
+      while (lo < hi) { const int32_t mid = (lo + hi + 1) / 2; if (h_segs[mid].row0 <= tt[i].row_start) lo = mid; else hi = mid - 1; }
+      ++cnt[lo + 1];
+    }
+    sr[0] = 0;
+    for (int32_t k = 0; k < n_segs; ++k) sr[k + 1] = sr[k] + cnt[k + 1];
+  }
 
   e = cudaMemcpyAsync(p->ws, p->pinned, lay.tables_end, cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(p->ws + lay.counter, 0, 256, stream);
@@ -327,6 +346,7 @@ static ScoreArgs score_args(const mas_plan* p, const void* X, const void* Q, flo
   a.X = X; a.Q = Q; a.qinv = p->at<float>(p->lay.qinv);
   a.segs = p->at<DevSeg>(p->lay.segs); a.tiles = p->at<DevTile>(p->lay.tiles);
   a.s = s; a.gamma = gamma; a.rel = rel; a.S_opt = S_opt; a.sig = nullptr; a.d = p->d;
+  a.heads_part = nullptr; a.heads_m = nullptr; a.heads_bias = 0.f; a.heads_tau = 0.f;
   return a;
 }
 
@@ -464,10 +484,56 @@ extern "C" int mas_select_compact(const mas_plan* p, const void* X, const float*
   return launch_select_tail(p, X, mask, kept_idx, koff, Y, cap_rows, st);
 }
 
+// NEXT-2: learned heads (k_heads.cuh)
+static int heads_check(const mas_plan* p, const void* X, const void* Q, const float* gamma, bool gamma_follows, const mas_heads* hd) {
+  if (!p || !X || !Q || !hd) return MAS_ERR_INVALID_ARG;
+  if (!hd->W || !hd->Wp || !hd->b1 || !hd->w2 || hd->hidden < 1 || hd->hidden >= kHeadRows) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(Q) || !aligned16(hd->W) || !aligned16(hd->Wp) || p->d > 65536) return MAS_ERR_UNSUPPORTED;
+  if (!gamma && !gamma_follows) {
+    const DevSeg* hs = reinterpret_cast<const DevSeg*>(static_cast<const char*>(p->pinned) + p->lay.segs);
+    for (int32_t k = 0; k < p->n_segs; ++k)
+      if (hs[k].n_frames > 1) return MAS_ERR_INVALID_ARG;
+  }
+  return MAS_OK;
+}
+// p-half of the first layer, then per segment: partial sums -> hidden layer -> alpha; last CTA: softmax, Eq. 7
+static int heads_tail(const mas_plan* p, const void* Q, const float* gamma, const mas_heads* hd, bool tc_slots, mas_segment_out* seg_out,
+                      cudaStream_t st) {
+  float* cq = p->at<float>(p->lay.heads_cq);
+  const size_t qs = (size_t)((p->d + kHeadSlabs - 1) / kHeadSlabs) * sizeof(float);
+  const dim3 qgrid((unsigned)p->n_requests, kHeadSlabs);
+  if (p->dtype == MAS_BF16) k_heads_q<1><<<qgrid, 256, qs, st>>>(Q, hd->Wp, p->at<int32_t>(p->lay.req), p->at<DevSeg>(p->lay.segs), cq, p->d);
+  else k_heads_q<0><<<qgrid, 256, qs, st>>>(Q, hd->Wp, p->at<int32_t>(p->lay.req), p->at<DevSeg>(p->lay.segs), cq, p->d);
+  CK(cudaGetLastError());
+  HeadsArgs h;
+  h.segs = p->at<DevSeg>(p->lay.segs); h.req_seg_off = p->at<int32_t>(p->lay.req);
+  h.n_segs = p->n_segs; h.n_requests = p->n_requests; h.tile_rows = generic_tile_rows(p->N); h.hidden = hd->hidden;
+  h.prm = p->prm; h.part = p->at<float>(p->lay.heads_part); h.slot_rank = tc_slots ? p->at<int32_t>(p->lay.tc_segrank) : nullptr;
+  h.cq = cq; h.gamma = gamma; h.b1 = hd->b1; h.w2 = hd->w2; h.b2 = hd->b2;
+  h.seg_out = seg_out; h.done_counter = p->at<unsigned int>(p->lay.counter);
+  k_heads_finish<<<p->n_segs, 256, 0, st>>>(h);
+  CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+extern "C" int mas_learned_heads(const mas_plan* p, const void* X, const void* Q, const float* gamma, const mas_heads* hd, float* m_spatial,
+                                 mas_segment_out* seg_out, mas_stream_t stream) {
+  if (!m_spatial || !seg_out) return MAS_ERR_INVALID_ARG;
+  int rc = heads_check(p, X, Q, gamma, false, hd);
+  if (rc != MAS_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  ScoreArgs a = score_args(p, X, hd->W, nullptr, nullptr, nullptr, nullptr);
+  a.heads_part = p->at<float>(p->lay.heads_part); a.heads_m = m_spatial; a.heads_bias = hd->b_spatial; a.heads_tau = p->prm.tau_s;
+  if (p->dtype == MAS_BF16) k_heads_proj<1><<<p->n_tiles, 256, score_mma_smem_bytes(1), st>>>(a);
+  else k_heads_proj<0><<<p->n_tiles, 256, score_mma_smem_bytes(0), st>>>(a);
+  CK(cudaGetLastError());
+  return heads_tail(p, Q, gamma, hd, false, seg_out, st);
+}
+
 // ------------------------------------------------------------------------------------------------ fused entry point
 static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* m_spatial, float* gamma, float* rel, float* mas_tok,
                         mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows,
-                        const void* Rm, unsigned long long* sig, mas_stream_t stream) {
+                        const void* Rm, unsigned long long* sig, const TcHeads* hf, mas_stream_t stream) {
   if (!p || !X || !Q || cap_rows < 0) return MAS_ERR_INVALID_ARG;
   if (Y && !kept_idx) return MAS_ERR_INVALID_ARG;
   if (!aligned16(X) || !aligned16(Q) || (Y && !aligned16(Y))) return MAS_ERR_UNSUPPORTED;
@@ -487,17 +553,17 @@ static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* 
   if (p->tc.enabled && !p->tc_inline_qnorm) {
     if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
     rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, false, Rm, sig, st);
+                         p->nQ, p->d, false, Rm, sig, hf, st);
     if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
     rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, true, Rm, sig, st);
+                         p->nQ, p->d, true, Rm, sig, hf, st);
     if (rc == 1) {   // not all CTAs can be co-resident here (e.g. an MPS partition): query norms in their own launch
       (void)cudaGetLastError();
       if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
       rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                           p->nQ, p->d, false, Rm, sig, st);
+                           p->nQ, p->d, false, Rm, sig, hf, st);
     }
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else {
@@ -527,7 +593,27 @@ static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* 
 extern "C" int mas_forward(const mas_plan* p, const void* X, const void* Q, float* m_spatial, float* gamma, float* rel, float* mas_tok,
                            mas_segment_out* seg_out, uint8_t* keep_mask, int32_t* kept_idx, int64_t* kept_off, void* Y, int64_t cap_rows,
                            mas_stream_t stream) {
-  return forward_impl(p, X, Q, m_spatial, gamma, rel, mas_tok, seg_out, keep_mask, kept_idx, kept_off, Y, cap_rows, nullptr, nullptr, stream);
+  return forward_impl(p, X, Q, m_spatial, gamma, rel, mas_tok, seg_out, keep_mask, kept_idx, kept_off, Y, cap_rows, nullptr, nullptr, nullptr, stream);
+}
+
+extern "C" int mas_forward_heads(const mas_plan* p, const void* X, const void* Q, const mas_heads* hd, float* heads_m_spatial,
+                                 mas_segment_out* heads_seg_out, const mas_outputs* o, mas_stream_t stream) {
+  if (!heads_m_spatial || !heads_seg_out || !o) return MAS_ERR_INVALID_ARG;
+  int rc = heads_check(p, X, Q, nullptr, true, hd);
+  if (rc != MAS_OK) return rc;
+  const float* gam = o->gamma ? o->gamma : p->at<float>(p->lay.gamma);   // finished by the segment kernel of this same call
+  // the weight rows ride the score kernel's MMA as 64 more B rows when the accumulator has room for them (L <= 64 everywhere)
+  if (p->tc.enabled && p->max_L <= 64) {
+    TcHeads hf{p->at<float>(p->lay.heads_part), heads_m_spatial, hd->b_spatial, p->prm.tau_s};
+    rc = forward_impl(p, X, Q, o->m_spatial, o->gamma, o->rel, o->mas_tok, o->seg_out, o->keep_mask, o->kept_idx, o->kept_off, o->Y,
+                      o->cap_rows, hd->W, nullptr, &hf, stream);
+    if (rc != MAS_OK) return rc;
+    return heads_tail(p, Q, gam, hd, true, heads_seg_out, (cudaStream_t)stream);
+  }
+  rc = forward_impl(p, X, Q, o->m_spatial, o->gamma, o->rel, o->mas_tok, o->seg_out, o->keep_mask, o->kept_idx, o->kept_off, o->Y,
+                    o->cap_rows, nullptr, nullptr, nullptr, stream);
+  if (rc != MAS_OK) return rc;
+  return mas_learned_heads(p, X, Q, gam, hd, heads_m_spatial, heads_seg_out, stream);
 }
 
 extern "C" int mas_forward_lsh(const mas_plan* p, const void* X, const void* Q, const void* Rm, uint64_t* sig, float* gamma_lsh,
@@ -537,7 +623,7 @@ extern "C" int mas_forward_lsh(const mas_plan* p, const void* X, const void* Q, 
   // the hash rows ride the score kernel's MMA as 64 more B rows when the accumulator has room for them (L <= 64 everywhere)
   const bool fused = p->tc.enabled && p->max_L <= 64;
   int rc = forward_impl(p, X, Q, o->m_spatial, o->gamma, o->rel, o->mas_tok, o->seg_out, o->keep_mask, o->kept_idx, o->kept_off, o->Y,
-                        o->cap_rows, fused ? Rm : nullptr, fused ? reinterpret_cast<unsigned long long*>(sig) : nullptr, stream);
+                        o->cap_rows, fused ? Rm : nullptr, fused ? reinterpret_cast<unsigned long long*>(sig) : nullptr, nullptr, stream);
   if (rc != MAS_OK) return rc;
   if (!fused) return mas_temporal_lsh(p, X, Rm, sig, gamma_lsh, stream);
   if (gamma_lsh) {

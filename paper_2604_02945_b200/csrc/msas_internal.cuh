@@ -21,7 +21,7 @@ struct DevSeg {
   int32_t q0;                // first query row of the request
   int32_t L;                 // query tokens of the request
   int32_t keep_k;
-  int32_t pad_;
+  int32_t tile0;             // index of the segment's first generic tile (DevTile table)
 };
 
 // One score tile: up to kTileRows consecutive rows of one segment.

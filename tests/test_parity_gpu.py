@@ -506,3 +506,126 @@ def test_draft_entropy_matches_oracle(B, n, V, dtype):
     decided = np.abs(H_r - theta) > 1e-3
     assert np.array_equal(sp.cpu().numpy()[decided], f_r[decided])
     assert H.min() >= -1e-4 and H.max() <= np.log(V) + 1e-3
+
+
+# ---------------------------------------------------------------- NEXT-2: learned heads (Eq. 3, Eq. 6 with supplied weights)
+def _head_weights(rng, d, hidden, dtype):
+    W = np.zeros((64, d), np.float32)
+    Wp = np.zeros((64, d), np.float32)
+    W[0] = rng.standard_normal(d) * (1.5 / np.sqrt(d))               # logits of O(1): M spreads around tau_s
+    W[1:1 + hidden] = rng.standard_normal((hidden, d)) / np.sqrt(d)
+    Wp[1:1 + hidden] = rng.standard_normal((hidden, d)) / np.sqrt(d)
+    W[1 + hidden:] = 3.0                                             # ignored rows
+    b1 = np.zeros(64, np.float32)
+    w2 = np.zeros(64, np.float32)
+    b1[1:1 + hidden] = 0.3 * rng.standard_normal(hidden)
+    w2[1:1 + hidden] = rng.standard_normal(hidden)
+    b1[0] = w2[0] = 9.0                                              # ignored entries
+    if dtype == "bf16":
+        return synth.f32_to_bf16_bits(W), synth.f32_to_bf16_bits(Wp), b1, w2
+    return W, Wp, b1, w2
+
+
+@pytest.mark.parametrize("w", [synth.batched_images(seed=51, R=5, d=512, L_lo=3, L_hi=70, P=333), synth.video(seed=52, R=2, T=4, P=576, d=256, L=48),
+                               synth.video(seed=53, R=2, T=5, P=50, d=200, L=9, dtype="f32"), synth.audio_vision(seed=54, R=3, d=256, L=64, P_img=576, T_aud=300),
+                               synth.single_image(seed=55, d=1024, dtype="f32")],
+                         ids=["images", "video", "video_f32_d200", "audio_vision", "single_image_f32"])
+@pytest.mark.parametrize("hidden", [1, 16, 63])
+def test_learned_heads(B, w, hidden):
+    rng = np.random.default_rng(500 + hidden)
+    W, Wp, b1, w2 = _head_weights(rng, w.d, hidden, w.dtype)
+    b_sp, b2 = -0.8, 0.15
+    segs, n = O.make_segments(w.segments)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    gam = plan.temporal(X)
+    m, so = plan.learned_heads(X, Q, gam, B.to_device(W), B.to_device(Wp), torch.from_numpy(b1).cuda(), torch.from_numpy(w2).cuda(), b_sp, b2, hidden)
+    torch.cuda.synchronize()
+    g = B.seg_out_numpy(so)
+    ref_m, ref = O.learned_heads(segs, w.q_off, _oracle_params(w), w.X, w.Q, gam.cpu().numpy().astype(np.float64), W, Wp, b1, w2, b_sp, b2, hidden)
+    P.assert_close(m.cpu().numpy(), ref_m, "m_spatial (learned)")
+    r0 = 0
+    for k, (_, _, T, Pn, _) in enumerate(w.segments):
+        nk = T * Pn
+        near = np.count_nonzero(np.abs(ref_m[r0:r0 + nk] - 0.3) <= 1e-3 * 0.3)
+        assert abs(float(g["rho_spatial"][k]) - ref[k].rho_spatial) <= near / nk + 1e-6
+        # alpha: fp32 accumulation of O(1) pre-activations over `hidden` units
+        assert abs(float(g["alpha_mean"][k]) - ref[k].alpha_mean) <= 1e-3 * abs(ref[k].alpha_mean) + 2e-4 * np.sum(np.abs(w2)), (k, float(g["alpha_mean"][k]), ref[k].alpha_mean)
+        assert abs(float(g["gamma_avg"][k]) - ref[k].gamma_avg) <= 1e-5
+        assert abs(float(g["beta"][k]) - ref[k].beta) <= 2e-3
+        assert abs(float(g["mas"][k]) - ref[k].mas) <= 2e-3 + 0.6 * near / nk
+        assert int(g["n_tokens"][k]) == nk
+        r0 += nk
+    # softmax identity per request on the GPU's own numbers
+    req = np.array([s[0] for s in w.segments])
+    for r in range(w.n_requests):
+        assert abs(float(g["beta"][req == r].sum()) - 1.0) < 1e-5
+    plan.close()
+
+
+def _check_learned(B, w, m, so, gamma_np, W, Wp, b1, w2, b_sp, b2, hidden):
+    segs, n = O.make_segments(w.segments)
+    g = B.seg_out_numpy(so)
+    ref_m, ref = O.learned_heads(segs, w.q_off, _oracle_params(w), w.X, w.Q, gamma_np.astype(np.float64), W, Wp, b1, w2, b_sp, b2, hidden)
+    P.assert_close(m.cpu().numpy(), ref_m, "m_spatial (learned)")
+    r0 = 0
+    for k, (_, _, T, Pn, _) in enumerate(w.segments):
+        nk = T * Pn
+        near = np.count_nonzero(np.abs(ref_m[r0:r0 + nk] - 0.3) <= 1e-3 * 0.3)
+        assert abs(float(g["rho_spatial"][k]) - ref[k].rho_spatial) <= near / nk + 1e-6
+        assert abs(float(g["alpha_mean"][k]) - ref[k].alpha_mean) <= 1e-3 * abs(ref[k].alpha_mean) + 2e-4 * np.sum(np.abs(w2)), (k, float(g["alpha_mean"][k]), ref[k].alpha_mean)
+        assert abs(float(g["gamma_avg"][k]) - ref[k].gamma_avg) <= 1e-5
+        assert abs(float(g["beta"][k]) - ref[k].beta) <= 2e-3
+        assert abs(float(g["mas"][k]) - ref[k].mas) <= 2e-3 + 0.6 * near / nk
+        assert int(g["n_tokens"][k]) == nk
+        r0 += nk
+
+
+@pytest.mark.parametrize("name", ["images", "video", "audio_vision_L64", "tile_heights", "cluster8", "images_L70_fallback", "video_f32_fallback"])
+def test_forward_heads_one_pass(B, name):
+    """mas_forward_heads = mas_forward (same outputs up to the summation grouping of the row statistics) + the learned
+    descriptors, with the weight rows riding the score kernel's MMA where the fast path applies (else the staged fallback)."""
+    if name in SWEEPS:
+        shapes, d, L = SWEEPS[name]
+        w = _random_workload(400, shapes, d, [min(l, 64) for l in L])
+    else:
+        w = {"images": lambda: synth.batched_images(seed=61, R=6, d=512, L_lo=3, L_hi=64, P=333),
+             "video": lambda: synth.video(seed=62, R=2, T=4, P=576, d=256, L=48),
+             "audio_vision_L64": lambda: synth.audio_vision(seed=63, R=2, d=256, L=64, P_img=576, T_aud=300),
+             "images_L70_fallback": lambda: synth.batched_images(seed=64, R=4, d=512, L_lo=60, L_hi=70, P=200),
+             "video_f32_fallback": lambda: synth.video(seed=65, R=1, T=3, P=70, d=200, L=4, dtype="f32")}[name]()
+    hidden = 24
+    rng = np.random.default_rng(77)
+    W, Wp, b1, w2 = _head_weights(rng, w.d, hidden, w.dtype)
+    b_sp, b2 = -0.8, 0.15
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    base = plan.forward(X, Q)
+    o, m, so = plan.forward_heads(X, Q, B.to_device(W), B.to_device(Wp), torch.from_numpy(b1).cuda(), torch.from_numpy(w2).cuda(), b_sp, b2, hidden)
+    torch.cuda.synchronize()
+    for k in ("m_spatial", "gamma", "rel", "mas_tok"):
+        assert torch.allclose(base[k], o[k], rtol=2e-5, atol=1e-6), k
+    assert torch.equal(base["kept_off"], o["kept_off"])
+    assert (base["keep_mask"] != o["keep_mask"]).float().mean().item() < 1e-3          # only exact near-ties may flip
+    tot = int(o["kept_off"][-1].item())
+    assert torch.equal(o["Y"][:tot].view(torch.uint8), X[o["kept_idx"][:tot].long()].view(torch.uint8))
+    _check_learned(B, w, m, so, o["gamma"].cpu().numpy(), W, Wp, b1, w2, b_sp, b2, hidden)
+    # twice in a row on the same plan: the scratch partials and counters are re-armed
+    o2, m2, so2 = plan.forward_heads(X, Q, B.to_device(W), B.to_device(Wp), torch.from_numpy(b1).cuda(), torch.from_numpy(w2).cuda(), b_sp, b2, hidden)
+    torch.cuda.synchronize()
+    assert torch.equal(m, m2) and torch.equal(so, so2)
+    plan.close()
+
+
+def test_learned_heads_argument_checks(B):
+    w = synth.video(seed=56, R=1, T=3, P=40, d=64, L=4)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    W, Wp, b1, w2 = _head_weights(np.random.default_rng(1), w.d, 4, "bf16")
+    args = (B.to_device(W), B.to_device(Wp), torch.from_numpy(b1).cuda(), torch.from_numpy(w2).cuda(), 0.0, 0.0)
+    for hidden in (0, 64):
+        with pytest.raises(Exception):
+            plan.learned_heads(X, Q, plan.temporal(X), *args, hidden)
+    with pytest.raises(Exception):
+        plan.learned_heads(X, Q, None, *args, 4)             # temporal segment without gamma
+    plan.close()
