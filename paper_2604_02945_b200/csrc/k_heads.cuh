@@ -16,38 +16,97 @@ constexpr int kHeadRows = MAS_HEADS_ROWS;   // 64
 constexpr int kHeadSlabs = 8;               // column slabs of the p-half (grid.y of k_heads_q)
 
 // cq[r][y][h] = (1 / L_r) sum over the columns of slab y of Wp[h][c] * sum_j Q[q0_r + j][c]  (the p-half of the first layer, in
-// kHeadSlabs partial sums that k_heads_finish adds in slab order): one CTA per (request, slab), the slab's column sums of the
-// request's query rows in shared memory, then one warp per weight row.
+// kHeadSlabs partial sums that k_heads_finish adds in slab order).  One CTA per (request, slab); the slab is walked in chunks of
+// 64 16-byte vectors: the chunk's column sums of the request's query rows go to shared memory (4 row groups x 64 vectors,
+// four loads in flight per thread), then warp w takes weight rows 8w..8w+7, two vectors per lane and row (16 loads in flight).
 template <int DT>
 __global__ void __launch_bounds__(256) k_heads_q(const void* __restrict__ Q, const void* __restrict__ Wp, const int32_t* __restrict__ req_seg_off,
                                                  const DevSeg* __restrict__ segs, float* __restrict__ cq, int d) {
-  extern __shared__ float qsum[];
-  const int r = blockIdx.x, y = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int VE = DT == 1 ? 8 : 4;          // elements per 16-byte vector
+  constexpr int CH = 64 * VE;                  // columns per chunk
+  __shared__ float qs[4][CH];
+  __shared__ float qsum[CH];
+  const int r = blockIdx.x, y = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int k0 = req_seg_off[r];
   if (k0 >= req_seg_off[r + 1]) return;   // a request without segments is never read
   const DevSeg seg = segs[k0];
   const int L = seg.L;
-  const int cw = (d + kHeadSlabs - 1) / kHeadSlabs, c0 = y * cw, c1 = min(d, c0 + cw);
-  auto ld = [&](const void* base, int64_t at) {
-    return DT == 1 ? __bfloat162float(static_cast<const __nv_bfloat16*>(base)[at]) : static_cast<const float*>(base)[at];
-  };
-  for (int col = c0 + threadIdx.x; col < c1; col += 256) {
-    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-    const int64_t at = (int64_t)seg.q0 * d + col;
-    int j = 0;
-    for (; j + 3 < L; j += 4) {
-      a0 += ld(Q, at + (int64_t)j * d); a1 += ld(Q, at + (int64_t)(j + 1) * d);
-      a2 += ld(Q, at + (int64_t)(j + 2) * d); a3 += ld(Q, at + (int64_t)(j + 3) * d);
+  const int cw = (((d + kHeadSlabs - 1) / kHeadSlabs) + VE - 1) / VE * VE;   // slab width, a whole number of vectors (d % VE == 0)
+  const int c0 = min(d, y * cw), c1 = min(d, c0 + cw);
+  auto unpack = [](const uint4& u, float (&f)[VE]) {
+    if (DT == 1) {
+      const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { f[(2 * k) % VE] = bf_lo(w[k]); f[(2 * k + 1) % VE] = bf_hi(w[k]); }
+    } else {
+      f[0] = __uint_as_float(u.x); f[1] = __uint_as_float(u.y); f[2 % VE] = __uint_as_float(u.z); f[3 % VE] = __uint_as_float(u.w);
     }
-    for (; j < L; ++j) a0 += ld(Q, at + (int64_t)j * d);
-    qsum[col - c0] = (a0 + a1) + (a2 + a3);
+  };
+  const int esz = DT == 1 ? 2 : 4;
+  const char* Qb = static_cast<const char*>(Q);
+  const char* Wb = static_cast<const char*>(Wp);
+  float racc[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) racc[i] = 0.f;
+  for (int cb = c0; cb < c1; cb += CH) {
+    {   // column sums of the query rows: vector v of the chunk, rows j = rg, rg + 4, ...
+      const int v = tid & 63, rg = tid >> 6;
+      const int col = cb + v * VE;
+      float a[VE];
+#pragma unroll
+      for (int e = 0; e < VE; ++e) a[e] = 0.f;
+      if (col < c1) {
+        int jq = rg;
+        for (; jq + 12 < L; jq += 16) {
+          uint4 u[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) u[k] = ld_nc16(Qb + ((int64_t)(seg.q0 + jq + 4 * k) * d + col) * esz);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            float f[VE];
+            unpack(u[k], f);
+#pragma unroll
+            for (int e = 0; e < VE; ++e) a[e] += f[e];
+          }
+        }
+        for (; jq < L; jq += 4) {
+          float f[VE];
+          unpack(ld_nc16(Qb + ((int64_t)(seg.q0 + jq) * d + col) * esz), f);
+#pragma unroll
+          for (int e = 0; e < VE; ++e) a[e] += f[e];
+        }
+      }
+#pragma unroll
+      for (int e = 0; e < VE; ++e) qs[rg][v * VE + e] = a[e];
+    }
+    __syncthreads();
+    for (int e = tid; e < CH; e += 256) qsum[e] = (qs[0][e] + qs[1][e]) + (qs[2][e] + qs[3][e]);
+    __syncthreads();
+    {   // weight rows 8 * warp .. 8 * warp + 7, vectors lane and lane + 32 of the chunk
+      uint4 u[8][2];
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const int col = cb + (lane + 32 * k) * VE;
+          u[i][k] = col < c1 ? ld_nc16(Wb + ((int64_t)(warp * 8 + i) * d + col) * esz) : make_uint4(0, 0, 0, 0);
+        }
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          float f[VE];
+          unpack(u[i][k], f);
+#pragma unroll
+          for (int e = 0; e < VE; ++e) racc[i] = fmaf(f[e], qsum[(lane + 32 * k) * VE + e], racc[i]);
+        }
+    }
+    __syncthreads();   // qs / qsum are rewritten by the next chunk
   }
-  __syncthreads();
-  for (int h = warp; h < kHeadRows; h += 8) {
-    float a = 0.f;
-    for (int col = c0 + lane; col < c1; col += 32) a = fmaf(ld(Wp, (int64_t)h * d + col), qsum[col - c0], a);
-    a = warp_sum(a);
-    if (lane == 0) cq[((int64_t)r * kHeadSlabs + y) * kHeadRows + h] = a / (float)L;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const float t = warp_sum(racc[i]);
+    if (lane == 0) cq[((int64_t)r * kHeadSlabs + y) * kHeadRows + warp * 8 + i] = t / (float)L;
   }
 }
 
@@ -69,24 +128,39 @@ struct HeadsArgs {
 
 // One CTA per segment: per-tile partials summed in tile order (double), gamma_avg, the hidden layer, alpha; the last CTA
 // does the per-request softmax and Eq. 7.
-__global__ void __launch_bounds__(256) k_heads_finish(HeadsArgs a) {
+__global__ void __launch_bounds__(1024) k_heads_finish(HeadsArgs a) {
   __shared__ SegSmem sm;
   __shared__ double colsum[kHeadRows];
-  const int tid = threadIdx.x;
+  __shared__ double colpart[16][kHeadRows];
+  const int tid = threadIdx.x, NT = blockDim.x, NG = NT >> 6;   // 256 or 1024 threads (host: from the longest segment)
+  pdl_wait();
   const int sidx = blockIdx.x;
   const DevSeg seg = a.segs[sidx];
   const int n = seg.n_rows;
   const int slot_lo = a.slot_rank ? 2 * a.slot_rank[sidx] : seg.tile0;
   const int slot_hi = a.slot_rank ? 2 * a.slot_rank[sidx + 1] : seg.tile0 + (n + a.tile_rows - 1) / a.tile_rows;
+  {   // column c = tid % 64; the four thread groups take every fourth slot, four loads in flight each: a fixed summation tree
+    const int c = tid & 63, grp = tid >> 6;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int t = slot_lo + grp;
+    for (; t + 3 * NG < slot_hi; t += 4 * NG) {
+      const float v0 = a.part[(int64_t)t * kHeadRows + c], v1 = a.part[(int64_t)(t + NG) * kHeadRows + c];
+      const float v2 = a.part[(int64_t)(t + 2 * NG) * kHeadRows + c], v3 = a.part[(int64_t)(t + 3 * NG) * kHeadRows + c];
+      s0 += (double)v0; s1 += (double)v1; s2 += (double)v2; s3 += (double)v3;
+    }
+    for (; t < slot_hi; t += NG) s0 += (double)a.part[(int64_t)t * kHeadRows + c];
+    colpart[grp][c] = (s0 + s1) + (s2 + s3);
+  }
+  __syncthreads();
   if (tid < kHeadRows) {
     double s = 0.0;
-    for (int t = slot_lo; t < slot_hi; ++t) s += (double)a.part[(int64_t)t * kHeadRows + tid];
+    for (int gq = 0; gq < NG; ++gq) s += colpart[gq][tid];
     colsum[tid] = s;
   }
   double gs = 0.0, d1 = 0.0, d2 = 0.0;
   const bool temporal = seg.n_frames > 1;
   if (temporal)
-    for (int i = seg.n_patches + tid; i < n; i += 256) gs += (double)a.gamma[seg.row0 + i];
+    for (int i = seg.n_patches + tid; i < n; i += NT) gs += (double)a.gamma[seg.row0 + i];
   block_sum3(sm, gs, d1, d2);   // its barriers also publish colsum
   double contrib = 0.0;
   if (tid >= 1 && tid <= a.hidden) {
@@ -115,7 +189,7 @@ __global__ void __launch_bounds__(256) k_heads_finish(HeadsArgs a) {
   __threadfence();
   volatile mas_segment_out* so = a.seg_out;
   const DevParams& p = a.prm;
-  for (int r = tid; r < a.n_requests; r += 256) {
+  for (int r = tid; r < a.n_requests; r += NT) {
     const int k0 = a.req_seg_off[r], k1 = a.req_seg_off[r + 1];
     float mx = -INFINITY;
     for (int k = k0; k < k1; ++k) mx = fmaxf(mx, so[k].alpha_mean);

@@ -465,6 +465,7 @@ __global__ void __launch_bounds__(kSegThreads) k_compact_idx(const DevSeg* segs,
 __global__ void __launch_bounds__(256) k_gather(const char* __restrict__ X, char* __restrict__ Y, const int32_t* __restrict__ kept_idx,
                                                 const int64_t* __restrict__ total_ptr, int64_t cap_rows, int row_bytes) {
   const int lane = threadIdx.x & 31;
+  pdl_launch_dependents();   // a kernel chained behind the gather (the learned-heads finish) may be scheduled as SMs free up
   pdl_wait();
   const int64_t total = *total_ptr < cap_rows ? *total_ptr : cap_rows;
   const int64_t n_warps = (int64_t)gridDim.x * 8;

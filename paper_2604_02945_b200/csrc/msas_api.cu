@@ -497,22 +497,25 @@ static int heads_check(const mas_plan* p, const void* X, const void* Q, const fl
   return MAS_OK;
 }
 // p-half of the first layer, then per segment: partial sums -> hidden layer -> alpha; last CTA: softmax, Eq. 7
-static int heads_tail(const mas_plan* p, const void* Q, const float* gamma, const mas_heads* hd, bool tc_slots, mas_segment_out* seg_out,
-                      cudaStream_t st) {
+static int heads_q(const mas_plan* p, const void* Q, const mas_heads* hd, cudaStream_t st) {
   float* cq = p->at<float>(p->lay.heads_cq);
-  const size_t qs = (size_t)((p->d + kHeadSlabs - 1) / kHeadSlabs) * sizeof(float);
+  const size_t qs = 0;
   const dim3 qgrid((unsigned)p->n_requests, kHeadSlabs);
   if (p->dtype == MAS_BF16) k_heads_q<1><<<qgrid, 256, qs, st>>>(Q, hd->Wp, p->at<int32_t>(p->lay.req), p->at<DevSeg>(p->lay.segs), cq, p->d);
   else k_heads_q<0><<<qgrid, 256, qs, st>>>(Q, hd->Wp, p->at<int32_t>(p->lay.req), p->at<DevSeg>(p->lay.segs), cq, p->d);
   CK(cudaGetLastError());
+  return MAS_OK;
+}
+static int heads_finish(const mas_plan* p, const float* gamma, const mas_heads* hd, bool tc_slots, mas_segment_out* seg_out, cudaStream_t st,
+                        bool pdl = false) {
+  float* cq = p->at<float>(p->lay.heads_cq);
   HeadsArgs h;
   h.segs = p->at<DevSeg>(p->lay.segs); h.req_seg_off = p->at<int32_t>(p->lay.req);
   h.n_segs = p->n_segs; h.n_requests = p->n_requests; h.tile_rows = generic_tile_rows(p->N); h.hidden = hd->hidden;
   h.prm = p->prm; h.part = p->at<float>(p->lay.heads_part); h.slot_rank = tc_slots ? p->at<int32_t>(p->lay.tc_segrank) : nullptr;
   h.cq = cq; h.gamma = gamma; h.b1 = hd->b1; h.w2 = hd->w2; h.b2 = hd->b2;
   h.seg_out = seg_out; h.done_counter = p->at<unsigned int>(p->lay.counter);
-  k_heads_finish<<<p->n_segs, 256, 0, st>>>(h);
-  CK(cudaGetLastError());
+  CK(launch_k(k_heads_finish, dim3((unsigned)p->n_segs), dim3(p->seg_cluster * p->seg_threads > 1024 ? 1024u : 256u), 0, st, pdl, h));
   return MAS_OK;
 }
 
@@ -527,7 +530,8 @@ extern "C" int mas_learned_heads(const mas_plan* p, const void* X, const void* Q
   if (p->dtype == MAS_BF16) k_heads_proj<1><<<p->n_tiles, 256, score_mma_smem_bytes(1), st>>>(a);
   else k_heads_proj<0><<<p->n_tiles, 256, score_mma_smem_bytes(0), st>>>(a);
   CK(cudaGetLastError());
-  return heads_tail(p, Q, gamma, hd, false, seg_out, st);
+  if ((rc = heads_q(p, Q, hd, st)) != MAS_OK) return rc;
+  return heads_finish(p, gamma, hd, false, seg_out, st);
 }
 
 // ------------------------------------------------------------------------------------------------ fused entry point
@@ -605,10 +609,11 @@ extern "C" int mas_forward_heads(const mas_plan* p, const void* X, const void* Q
   // the weight rows ride the score kernel's MMA as 64 more B rows when the accumulator has room for them (L <= 64 everywhere)
   if (p->tc.enabled && p->max_L <= 64) {
     TcHeads hf{p->at<float>(p->lay.heads_part), heads_m_spatial, hd->b_spatial, p->prm.tau_s};
+    if ((rc = heads_q(p, Q, hd, (cudaStream_t)stream)) != MAS_OK) return rc;   // independent of X: ahead of the PDL-chained kernels
     rc = forward_impl(p, X, Q, o->m_spatial, o->gamma, o->rel, o->mas_tok, o->seg_out, o->keep_mask, o->kept_idx, o->kept_off, o->Y,
                       o->cap_rows, hd->W, nullptr, &hf, stream);
     if (rc != MAS_OK) return rc;
-    return heads_tail(p, Q, gam, hd, true, heads_seg_out, (cudaStream_t)stream);
+    return heads_finish(p, gam, hd, true, heads_seg_out, (cudaStream_t)stream, p->prof_slots == 0);
   }
   rc = forward_impl(p, X, Q, o->m_spatial, o->gamma, o->rel, o->mas_tok, o->seg_out, o->keep_mask, o->kept_idx, o->kept_off, o->Y,
                     o->cap_rows, nullptr, nullptr, nullptr, stream);
