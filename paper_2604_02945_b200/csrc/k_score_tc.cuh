@@ -38,7 +38,8 @@ namespace msas {
 
 struct TcTile {            // 32 bytes
   int32_t row_start;       // global row id of the first row
-  int32_t n_rows;          // valid rows, 1..128, or up to 256 for a non-temporal "double" tile (two 128-row MMA halves sharing the query chunk)
+  int32_t n_rows;          // valid rows, 1..128; up to 256 for a non-temporal "double" tile (two 128-row MMA halves sharing the query
+                           // chunk), up to 384 for a "tall" one (three halves; requires pad16(L) <= 64)
   int32_t q_row0;          // first query row of the request
   int32_t L;               // query tokens of the request
   int32_t prev_delta;      // P if the segment is temporal (T > 1), else 0
@@ -118,7 +119,7 @@ struct TcRing {
 //   [kw x token slice (xbytes each)] [kw x previous-frame slice, temporal tiles only] [kw x query slice (qbytes each)]
 struct TcGeom {
   uint32_t xbytes, xall, qbytes, need;
-  int kw, nch, nqb, nqu, nh;   // nqb = 16-row boxes of B rows (queries + hash rows), nqu = those of the queries alone;
+  int kw, nch, nqb, nqu, nh, hstride;   // nqb = 16-row boxes of B rows (queries + hash rows), nqu = those of the queries alone;
                                // nh = 128-row MMA halves of the tile (2 for a double tile)
   bool has_prev;
 };
@@ -132,7 +133,8 @@ __device__ __forceinline__ TcGeom tc_geom(const TcTile& t, int nk, int dbg, bool
   int kw = rows16 <= 16 ? 8 : rows16 <= 32 ? 4 : rows16 <= 64 ? 2 : 1;
   while (kw > 1 && (kw * g.nqb > 16 || nk % kw != 0)) kw >>= 1;   // <= 32 KB of query rows per chunk; kw divides d / 64
   g.kw = kw;
-  g.nh = rows16 > 128 ? 2 : 1;
+  g.nh = (rows16 + 127) >> 7;            // 3 = a TALL tile (257..384 rows): only where pad16(L) <= 64, accumulator halves 64 columns apart
+  g.hstride = g.nh > 2 ? 64 : 128;
   g.nch = nk / kw;
   g.xall = g.xbytes * (g.has_prev ? 2u : 1u);
   g.qbytes = (uint32_t)g.nqb * 2048u;
@@ -236,7 +238,10 @@ struct TcCtrl {                      // lives at the (1024-aligned) start of dyn
   uint32_t tmem_base;
   uint32_t pad_[31];
   float rowstat[2][kTcAluSets][2][128];   // partial sum x^2, sum (x - x_prev)^2 per (ALU set, K-slice, tile row), double buffered
-  float hred[2][4][64];              // NEXT-2: per-warp column sums of the 64 head columns, double buffered
+  union {
+    float hred[2][4][64];            // NEXT-2: per-warp column sums of the 64 head columns, double buffered (never on tall tiles)
+    float rowstat3[2][kTcAluSets][128];   // tall tiles: partial sum x^2 of the third half's rows (half a row per ALU set), double buffered
+  };
 };
 static_assert(sizeof(TcCtrl) <= kTcCtrlBytes, "control block too large");
 
@@ -300,7 +305,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       for (int t = tile_lo; t < tile_hi; ++t) {
         const TcTile tile = p.tiles[t];
         const TcGeom g = tc_geom(tile, nk, dbg, lsh);
-        const CUtensorMap* mx = &maps.x[(g.xbytes >> 11) - 1];      // one box of rows16 rows per K-slice
+        const bool tall = g.nh > 2;                                 // 257..384 rows: a 256-row box and a second one for the rest
+        const CUtensorMap* mx = &maps.x[((tall ? 32768u : g.xbytes) >> 11) - 1];      // one box of rows16 rows per K-slice
+        const CUtensorMap* mx2 = &maps.x[tall ? ((g.xbytes - 32768u) >> 11) - 1 : 0];
         const int row = tile.row_start, prow = tile.row_start - tile.prev_delta;
         const uint32_t poff = (uint32_t)g.kw * g.xbytes;            // previous-frame slices follow the token slices
 #ifdef MSAS_ABLATE
@@ -324,6 +331,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
               const int c0 = (ch * g.kw + j) * 64;
               const uint32_t dst = base + (uint32_t)j * g.xbytes;
               tma_load_2d(dst, mx, bar, c0, row);      // rows past the end of X are zero-filled by the TMA unit
+              if (tall) tma_load_2d(dst + 32768u, mx2, bar, c0, row + 256);
               if (ld_prev) tma_load_2d(dst + poff, mx, bar, c0, prow);
             }
           } else {
@@ -369,7 +377,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
                 const uint64_t adesc = umma_desc_sw128(base + (uint32_t)j * g.xbytes + (uint32_t)h * (uint32_t)kTcBoxBytes);
 #pragma unroll
                 for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
-                  tc_mma_bf16(d_tmem + (uint32_t)h * 128u, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(ch | j | k));
+                  tc_mma_bf16(d_tmem + (uint32_t)(h * g.hstride), adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(ch | j | k));
               }
             }
           }
@@ -421,11 +429,12 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
         q_ok = true;
       }
-      float m[2] = {-INFINITY, -INFINITY};   // per 128-row half of the tile
-      for (int h = 0; h < g.nh; ++h)
-        for (int cb = 0; cb < nqb; ++cb) {
+      float m[3] = {-INFINITY, -INFINITY, -INFINITY};   // per 128-row half of the tile
+#pragma unroll
+      for (int h = 0; h < 3; ++h)
+        for (int cb = 0; cb < (h < g.nh ? nqb : 0); ++cb) {
           uint32_t v[16];
-          tc_ld16(tmem_base + (uint32_t)acc * 256u + (uint32_t)h * 128u + (uint32_t)cb * 16u + ((uint32_t)(q * 32) << 16), v);
+          tc_ld16(tmem_base + (uint32_t)acc * 256u + (uint32_t)(h * g.hstride) + (uint32_t)cb * 16u + ((uint32_t)(q * 32) << 16), v);
           tc_wait_ld();
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
@@ -499,10 +508,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->tmem_empty[acc]));
       mbar_wait(smem_u32(&ctrl->stat_full[acc]), ph);
-      float n2[2] = {0.f, 0.f}, D[2] = {0.f, 0.f};
-      if (g.nh == 2) {                       // double tile: ALU thread `row` holds the whole row's sums, row = set * 128 + r
+      float n2[3] = {0.f, 0.f, 0.f}, D[3] = {0.f, 0.f, 0.f};
+      if (g.nh >= 2) {                       // double tile: ALU thread `row` holds the whole row's sums, row = set * 128 + r
 #pragma unroll
         for (int h = 0; h < 2; ++h) { n2[h] = ctrl->rowstat[acc][h][0][r]; D[h] = ctrl->rowstat[acc][h][1][r]; }
+        if (g.nh > 2) n2[2] = ctrl->rowstat3[acc][0][r] + ctrl->rowstat3[acc][1][r];   // third half: half a row per ALU set
       } else if (r < tile.n_rows) {          // one partial per (ALU set, K-slice of the chunk, row)
         const int rp2 = 128 / g.kw;
         for (int j = 0; j < g.kw; ++j)
@@ -512,7 +522,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_empty[acc]));
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
+      for (int h = 0; h < 3; ++h) {
         const int tr = h * 128 + r;
         if (h < g.nh && tr < tile.n_rows) {
           const int64_t row = (int64_t)tile.row_start + tr;
@@ -532,7 +542,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const TcTile tile = p.tiles[t];
       const TcGeom g = tc_geom(tile, nk, dbg, lsh);
       const int rp2 = 128 / g.kw;
-      const bool dbl = g.nh == 2;                        // double tile: 256 threads = 256 rows, a whole row each, no previous frame
+      const bool dbl = g.nh >= 2;                        // double tile: 256 threads = 256 rows, a whole row each, no previous frame
+      const bool act3 = g.nh > 2 && 256 + a < tile.n_rows && !(dbg & 1);   // tall tile: row 256 + a, half of it per ALU set
+      uint64_t n3a = 0, n3b = 0;
       const int r = dbl ? (int)set * 128 + a : (a & (rp2 - 1)), j = dbl ? 0 : a / rp2;
       const bool active = r < tile.n_rows && !(dbg & 1);
       // hardware 128-byte swizzle: 16-byte unit u of row r sits at unit u ^ (r & 7)
@@ -555,6 +567,18 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           for (int u = 0; u < 8; ++u) {
             fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].x)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].y));
             fma_sq_f32x2(n2a, bf16x2_to_f32x2(x[u].z)); fma_sq_f32x2(n2b, bf16x2_to_f32x2(x[u].w));
+          }
+          if (act3) {
+            const unsigned char* s3 = ring0 + off + (uint32_t)(256 + a) * 128u;
+            const uint32_t u3 = set * (uint32_t)kTcAluUnits, sw3 = (uint32_t)(a & 7);
+            uint4 y[kTcAluUnits];
+#pragma unroll
+            for (int u = 0; u < kTcAluUnits; ++u) y[u] = *reinterpret_cast<const uint4*>(s3 + (((u3 + (uint32_t)u) ^ sw3) << 4));
+#pragma unroll
+            for (int u = 0; u < kTcAluUnits; ++u) {
+              fma_sq_f32x2(n3a, bf16x2_to_f32x2(y[u].x)); fma_sq_f32x2(n3b, bf16x2_to_f32x2(y[u].y));
+              fma_sq_f32x2(n3a, bf16x2_to_f32x2(y[u].z)); fma_sq_f32x2(n3b, bf16x2_to_f32x2(y[u].w));
+            }
           }
         } else if (active) {
           const unsigned char* sx = ring0 + off + my_off;
@@ -593,6 +617,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const uint32_t ph = (uint32_t)(it >> 1) & 1u;
       mbar_wait(smem_u32(&ctrl->stat_empty[buf]), ph ^ 1u);
       ctrl->rowstat[buf][set][0][a] = n2; ctrl->rowstat[buf][set][1][a] = D;      // slot a = j * rp2 + r
+      if (g.nh > 2) ctrl->rowstat3[buf][set][a] = sum_f32x2(n3a) + sum_f32x2(n3b);
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->stat_full[buf]));
     }
@@ -623,10 +648,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 // Short tiles keep the same bytes in flight (variable-size chunk ring) but re-stream the query chunks more often,
 // which is why only the fill phase uses them.
 struct TcCost {
-  double w_prev = 0.25, w_q = 0.70, c_tile = 30.0;   // fitted to CTA finish times: ~27 us per MB of token rows, 12-19 us per MB of query rows, several us per tile
-  int hmax_plain = 256;
+  double w_prev = 0.25, w_q = 0.70, c_tile = 50.0;   // fitted to CTA finish times: ~27 us per MB of token rows, 12-19 us per MB of query rows, several us per tile
+  int hmax_plain = 256, hmax_tall = 384;   // tallest non-temporal tile; tall = three MMA halves, where pad16(L) <= 64
   TcCost() {
 #ifdef MSAS_ABLATE
+    if (getenv("MSAS_HTALL")) hmax_tall = atoi(getenv("MSAS_HTALL"));
     if (getenv("MSAS_HMAX")) hmax_plain = atoi(getenv("MSAS_HMAX"));
     if (getenv("MSAS_WPREV")) w_prev = atof(getenv("MSAS_WPREV"));
     if (getenv("MSAS_WQ")) w_q = atof(getenv("MSAS_WQ"));
@@ -645,7 +671,7 @@ inline size_t tc_schedule_bytes(const mas_segment* segs, int32_t n_segs) {
 
 // Builds the tile list (grouped per CTA) and the per-CTA offsets into `h_dst`; `d_dst` is where the image will live.
 inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n_segs, const int64_t* q_off, int32_t d, int32_t dtype,
-                              int sm_count, char* h_dst, char* d_dst) {
+                              int sm_count, char* h_dst, char* d_dst, bool tall_tiles = true) {
   sc = TcSchedule();
   if (dtype != MAS_BF16 || d % 64 != 0 || sm_count < 1 || sm_count > 1000) return;
   const TcCost cw;
@@ -659,7 +685,9 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     si[k].L = (int)(q_off[s.request + 1] - q_off[s.request]);
     si[k].P = s.n_frames > 1 ? s.n_patches : 0;
     si[k].w_row = 1.0 + (si[k].P > 0 ? cw.w_prev : 0.0);
-    si[k].hmax = si[k].P > 0 ? 128 : cw.hmax_plain;
+    // tall tiles (three MMA halves, 48 KB chunks) pay where they save a tile of a SHORT segment (a 576-token image: 2 tiles
+    // instead of 3); on long segments the double tile keeps more chunks in flight (measured: ragged mix +2 % with tall tiles)
+    si[k].hmax = si[k].P > 0 ? 128 : (tall_tiles && si[k].L <= 64 && n <= 2 * cw.hmax_tall ? std::max(cw.hmax_plain, cw.hmax_tall) : cw.hmax_plain);
     si[k].c_fix = cw.w_q * (((si[k].L + 15) / 16) * 16) + cw.c_tile;
     total += (double)n * si[k].w_row + (double)((n + si[k].hmax - 1) / si[k].hmax) * si[k].c_fix;
     n_full += n / si[k].hmax;

@@ -28,7 +28,7 @@ static thread_local int g_last_cuda = 0;
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-  size_t segs, tiles, req, tc_sched, tc_segrank, tables_end;   // uploaded tables (contiguous from 0)
+  size_t segs, tiles, req, tc_sched, tc_sched_x, tc_segrank, tables_end;   // uploaded tables (contiguous from 0)
   size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, heads_part, heads_cq, total;
 };
 
@@ -47,6 +47,7 @@ struct mas_plan {
   size_t pinned_bytes = 0;
   int sm_count = 148;
   TcSchedule tc{};            // tcgen05 fast-path schedule (tc.enabled == false -> generic kernels)
+  TcSchedule tcx{};           // the same without tall tiles (their accumulator halves are 64 columns apart), for mas_forward_lsh / mas_forward_heads
   mutable std::vector<cudaEvent_t> prof_ev;   // profiling ring: 4 events per slot
   mutable int64_t prof_calls = 0;
   int32_t prof_slots = 0;
@@ -139,6 +140,7 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.tiles = take(sizeof(DevTile) * n_tiles);
   l.req = take(sizeof(int32_t) * (n_req + 1));
   l.tc_sched = take(tc_bytes);
+  l.tc_sched_x = take(tc_bytes);   // without tall tiles: the schedule of the calls that add 64 B rows (NEXT-1, NEXT-2)
   l.tc_segrank = take(sizeof(int32_t) * (n_segs + 1));   // first tile rank of every segment (TcTile::rank), NEXT-2
   l.tables_end = o;
   l.qinv = take(sizeof(float) * nQ);
@@ -253,11 +255,12 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     p->seg_threads = slice <= 1024 ? 256 : slice <= 2048 ? 512 : kSegThreads;
   }
   tc_build_schedule(p->tc, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched, p->ws + lay.tc_sched);
-  if (p->tc.enabled) {   // per-segment range of tile ranks (slots of the learned-head partials)
-    const TcTile* tt = reinterpret_cast<const TcTile*>(h + lay.tc_sched);
+  tc_build_schedule(p->tcx, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched_x, p->ws + lay.tc_sched_x, false);
+  if (p->tcx.enabled) {   // per-segment range of tile ranks (slots of the learned-head partials)
+    const TcTile* tt = reinterpret_cast<const TcTile*>(h + lay.tc_sched_x);
     int32_t* sr = reinterpret_cast<int32_t*>(h + lay.tc_segrank);
     std::vector<int32_t> cnt(n_segs + 1, 0);
-    for (int i = 0; i < p->tc.n_tiles; ++i) {
+    for (int i = 0; i < p->tcx.n_tiles; ++i) {
       int32_t lo = 0, hi = n_segs - 1;   // segment holding row_start (segments tile [0, N) in order)
       while (lo < hi) { const int32_t mid = (lo + hi + 1) / 2; if (h_segs[mid].row0 <= tt[i].row_start) lo = mid; else hi = mid - 1; }
       ++cnt[lo + 1];
@@ -554,19 +557,20 @@ static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* 
   if (pev) CK(cudaEventRecord(pev[0], st));
   int rc;
   const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
+  const TcSchedule& sc = (Rm != nullptr || hf != nullptr) ? p->tcx : p->tc;
   if (p->tc.enabled && !p->tc_inline_qnorm) {
     if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
-    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
+    rc = tc_launch_score(sc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
                          p->nQ, p->d, false, Rm, sig, hf, st);
     if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
-    rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
+    rc = tc_launch_score(sc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
                          p->nQ, p->d, true, Rm, sig, hf, st);
     if (rc == 1) {   // not all CTAs can be co-resident here (e.g. an MPS partition): query norms in their own launch
       (void)cudaGetLastError();
       if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
-      rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
+      rc = tc_launch_score(sc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
                            p->nQ, p->d, false, Rm, sig, hf, st);
     }
     if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }

@@ -117,9 +117,12 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
     seg_of_row = np.concatenate([np.full(r[2] * r[3], k) for k, r in enumerate(rows)])
     row0, P_of, q0_of = np.cumsum([0] + [r[2] * r[3] for r in rows]), [r[3] if r[2] > 1 else 0 for r in rows], [int(q_off[r[0]]) for r in rows]
     for cta, rs, n, q0, L, pd, key, _ in t:
-        assert 1 <= n <= (128 if pd else 256) and 0 <= cta < 148     # 256 = a double tile (non-temporal segments only)
-        cov[rs:rs + n] += 1
         k = seg_of_row[rs]
+        # 256 = a double tile (non-temporal segments only); 384 = a tall one (three accumulator halves 64 TMEM columns apart:
+        # needs L <= 64; cut only from short segments)
+        tall_ok = not pd and L <= 64 and rows[k][2] * rows[k][3] <= 768
+        assert 1 <= n <= (128 if pd else 384 if tall_ok else 256) and 0 <= cta < 148
+        cov[rs:rs + n] += 1
         pd_expected = P_of[k]
         assert seg_of_row[rs + n - 1] == k                       # a tile never straddles a segment
         assert q0 == q0_of[k] and L == q_off[rows[k][0] + 1] - q_off[rows[k][0]] and pd == P_of[k]
@@ -133,10 +136,11 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
         # along), 0.7 per padded query row, a per-tile constant (csrc/k_score_tc.cuh TcCost)
         rows16 = (t[:, 2] + 15) // 16 * 16
         has_prev = (t[:, 5] > 0) & (t[:, 6] < t[:, 2])
-        cost = rows16 * (1.0 + 0.25 * has_prev) + 0.7 * ((t[:, 4] + 15) // 16 * 16) + 30.0
+        cost = rows16 * (1.0 + 0.25 * has_prev) + 0.7 * ((t[:, 4] + 15) // 16 * 16) + 50.0
         load = np.bincount(t[:, 0], weights=cost, minlength=148)
         assert load.max() <= 1.2 * load.mean()     # a batch of 64 images is only ~1.4 tiles per CTA
-        assert np.bincount(t[:, 0], weights=rows16, minlength=148).max() <= 1.3 * rows16.sum() / 148
+        if len(t) >= 4 * 148:   # rows follow the cost only where a CTA holds several tiles (else one tall tile vs several short ones)
+            assert np.bincount(t[:, 0], weights=rows16, minlength=148).max() <= 1.3 * rows16.sum() / 148
 
 
 def test_score_schedule_rejects_bad_descriptors_and_generic_shapes(B):
