@@ -14,6 +14,9 @@
 // ReLU clip it contains, w_sp = 0 -> M = sigmoid(b_sp), a dead hidden layer -> uniform beta, token-order invariance and
 // numpy float64 matrix products.
 // NEXT-3 (select_mode 2 of mas_ref_select_compact): pinned by worked counts (MAS_s 0.3, N 10 -> 7; 1 -> 1; 0 -> N) and minimality.
+// NEXT-3 (mas_ref_spatial_pool, mas_ref_merge_dropped, mas_ref_gather_residual): pinned by scipy.ndimage.uniform_filter (sum / count),
+// k = 1 identity, hand-counted corner / edge / centre windows; numpy masked means, the identity n_dropped * mean + kept sum = frame
+// sum; static video -> zero residuals, key frames -> copies, residual + previous = original exactly on small integers.
 // NEXT-1 (mas_ref_temporal_lsh): pinned by explicit signs of hand-expanded projections, identical / negated rows,
 // power-of-two scaling, and the collision law E[gamma] = theta / pi.
 //
@@ -437,6 +440,81 @@ int mas_ref_learned_heads(const mas_ref_segment* segs, int32_t n_segs, const int
       out[k].mas = 1.0 - out[k].beta * (1.0 - prm->lambda_spatial * out[k].rho_spatial - a * prm->lambda_temp * (1.0 - out[k].gamma_avg));  // Eq. 7, G8
     }
     k0 = k1;
+  }
+  return 0;
+}
+
+// NEXT-3, the rest of PAPER.md:98 / 105 ("coarsely compressed", "represented using only the residual difference").
+//
+// (a) Spatial pooling of the per-token scalar map (Eq. 3's AvgPool, reading G1: a k x k window on the H x W patch grid of every
+//     frame, H = P / W; the mean runs over the window cells that lie inside the grid).  Window of cell (i, j): rows
+//     i - (k-1)/2 .. i + k/2, columns j - (k-1)/2 .. j + k/2.
+int mas_ref_spatial_pool(const mas_ref_segment* segs, int32_t n_segs, const int32_t* grid_w, int32_t k, const double* s, double* out) {
+  if (k < 1) return 1;
+  for (int32_t q = 0; q < n_segs; ++q) {
+    const int64_t T = segs[q].n_frames, P = segs[q].n_patches, r0 = segs[q].row0, W = grid_w[q];
+    if (W < 1 || P % W != 0) return 1;
+    const int64_t H = P / W, lo = (k - 1) / 2, hi = k / 2;
+    for (int64_t t = 0; t < T; ++t)
+      for (int64_t i = 0; i < H; ++i)
+        for (int64_t j = 0; j < W; ++j) {
+          double acc = 0.0;
+          int64_t cnt = 0;
+          for (int64_t a = i - lo; a <= i + hi; ++a)
+            for (int64_t b = j - lo; b <= j + hi; ++b)
+              if (a >= 0 && a < H && b >= 0 && b < W) { acc += s[r0 + t * P + a * W + b]; ++cnt; }
+          out[r0 + t * P + i * W + j] = acc / static_cast<double>(cnt);
+        }
+  }
+  return 0;
+}
+
+// (b) Coarse compression: the dropped tokens (keep_mask = 0) of every frame merged into ONE mean token.  Frames are numbered
+//     segment by segment; Ymerge[f] = mean of the frame's dropped rows (zeros when none is dropped), n_dropped[f] their number.
+int mas_ref_merge_dropped(const mas_ref_segment* segs, int32_t n_segs, int64_t d, int dtype, const void* X, const uint8_t* keep_mask,
+                          double* Ymerge, int64_t* n_dropped) {
+  int64_t f = 0;
+  for (int32_t q = 0; q < n_segs; ++q)
+    for (int64_t t = 0; t < segs[q].n_frames; ++t, ++f) {
+      const int64_t P = segs[q].n_patches, r0 = segs[q].row0 + t * P;
+      int64_t cnt = 0;
+      for (int64_t i = 0; i < P; ++i) cnt += keep_mask[r0 + i] ? 0 : 1;
+      n_dropped[f] = cnt;
+      for (int64_t c = 0; c < d; ++c) {
+        double acc = 0.0;
+        for (int64_t i = 0; i < P; ++i)
+          if (!keep_mask[r0 + i]) acc += elem(X, dtype, (r0 + i) * d + c);
+        Ymerge[f * d + c] = cnt ? acc / static_cast<double>(cnt) : 0.0;
+      }
+    }
+  return 0;
+}
+
+// (c) Residual coding of the kept rows: a kept token of frame t >= 1 of a temporal segment is emitted as x_t - x_{t-1} (same
+//     patch, previous frame), everything else as a copy.  The difference of two bf16 values is exact in fp32, so the emitted
+//     bf16 is its round-to-nearest-even; fp32 inputs: one fp32 subtraction.  Y has the dtype of X.
+int mas_ref_gather_residual(const mas_ref_segment* segs, int32_t n_segs, int64_t d, int dtype, const void* X, const int32_t* kept_idx,
+                            int64_t n_kept, void* Y) {
+  for (int64_t j = 0; j < n_kept; ++j) {
+    const int64_t row = kept_idx[j];
+    int32_t q = 0;
+    while (q + 1 < n_segs && segs[q + 1].row0 <= row) ++q;
+    const int64_t P = segs[q].n_patches;
+    const bool res = segs[q].n_frames > 1 && row - segs[q].row0 >= P;
+    for (int64_t c = 0; c < d; ++c) {
+      if (dtype == REF_BF16) {
+        float v = static_cast<float>(elem(X, dtype, row * d + c));
+        if (res) v -= static_cast<float>(elem(X, dtype, (row - P) * d + c));   // exact
+        uint32_t u;
+        std::memcpy(&u, &v, 4);
+        const uint32_t rnd = ((u >> 16) & 1u) + 0x7FFFu;                         // round to nearest even (finite inputs)
+        static_cast<uint16_t*>(Y)[j * d + c] = static_cast<uint16_t>((u + rnd) >> 16);
+      } else {
+        float v = static_cast<const float*>(X)[row * d + c];
+        if (res) v = v - static_cast<const float*>(X)[(row - P) * d + c];
+        static_cast<float*>(Y)[j * d + c] = v;
+      }
+    }
   }
   return 0;
 }

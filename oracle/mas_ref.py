@@ -137,6 +137,35 @@ def learned_heads(segs, q_off, params, X, Q, gamma, W, Wp, b1, w2, b_sp, b2, hid
     return m, out
 
 
+def spatial_pool(segs, grid_w, k, s):
+    """NEXT-3a: k x k count-valid window mean of the per-token scalar map on each frame's H x W grid (W per segment)."""
+    s = np.ascontiguousarray(s, np.float64)
+    gw = np.ascontiguousarray(grid_w, np.int32)
+    out = np.zeros_like(s)
+    _check(lib().mas_ref_spatial_pool(segs, len(segs), _p(gw), C.c_int32(k), _p(s), _p(out)))
+    return out
+
+
+def merge_dropped(segs, X, keep_mask):
+    """NEXT-3b: one mean token per frame from the dropped rows -> (Ymerge float64 [F, d], n_dropped int64 [F])."""
+    X = np.ascontiguousarray(X)
+    m = np.ascontiguousarray(keep_mask, np.uint8)
+    F = int(sum(sg.n_frames for sg in segs))
+    Y = np.zeros((F, X.shape[1]), np.float64)
+    nd = np.zeros(F, np.int64)
+    _check(lib().mas_ref_merge_dropped(segs, len(segs), C.c_int64(X.shape[1]), _dtype_code(X), _p(X), _p(m), _p(Y), _p(nd)))
+    return Y, nd
+
+
+def gather_residual(segs, X, kept_idx):
+    """NEXT-3c: kept rows, frames t >= 1 of temporal segments as x_t - x_{t-1}; Y has X's dtype."""
+    X = np.ascontiguousarray(X)
+    idx = np.ascontiguousarray(kept_idx, np.int32)
+    Y = np.zeros((len(idx), X.shape[1]), X.dtype)
+    _check(lib().mas_ref_gather_residual(segs, len(segs), C.c_int64(X.shape[1]), _dtype_code(X), _p(X), _p(idx), C.c_int64(len(idx)), _p(Y)))
+    return Y
+
+
 def temporal_lsh(segs, X, R, want_proj=False):
     """NEXT-1: literal LSH probe of Eq. 5 with K = 64 hashes from R[64, d] (same dtype as X)."""
     X = np.ascontiguousarray(X)

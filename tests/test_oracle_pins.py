@@ -565,3 +565,77 @@ def test_learned_heads_special_cases_and_numpy():
     assert all(o.alpha_mean == -0.2 for o in outd) and outd[0].beta == 0.5 == outd[1].beta
     # Eq. 7 single image, beta = 1: MAS = lambda_sp * rho
     assert abs(out[2].mas - 0.6 * out[2].rho_spatial) < 1e-15
+
+
+# ---------------------------------------------------------------- NEXT-3: pooling, merged token, residual coding
+def test_spatial_pool_against_uniform_filter_and_hand_counts():
+    from scipy.ndimage import uniform_filter
+    rng = np.random.default_rng(3)
+    rows = [(0, 1, 1, 24 * 24, 1), (0, 2, 3, 6 * 5, 1), (1, 3, 7, 1, 1)]      # image 24 x 24, video 3 frames of 6 x 5, audio P = 1
+    segs, n = O.make_segments(rows)
+    gw = [24, 5, 1]
+    s = rng.random(n)
+    assert np.array_equal(O.spatial_pool(segs, gw, 1, s), s)                  # k = 1 is the identity
+    for k in (2, 3, 5):
+        out = O.spatial_pool(segs, gw, k, s)
+        r0 = 0
+        for (_, _, T, P, _), W in zip(rows, gw):
+            H = P // W
+            for t in range(T):
+                g = s[r0:r0 + P].reshape(H, W)
+                # library routine: zero-padded window sums of the map and of ones; origin shifts the even window like the oracle's
+                org = 0 if k % 2 else -1
+                num = uniform_filter(g, size=k, mode="constant", origin=org) * k * k
+                den = uniform_filter(np.ones_like(g), size=k, mode="constant", origin=org) * k * k
+                assert np.allclose(out[r0:r0 + P].reshape(H, W), num / den, rtol=1e-12, atol=1e-14), (k, W)
+                r0 += P
+    # hand counts on a 3 x 3 grid holding 1..9, k = 3: centre = 5, corner (0,0) = (1+2+4+5)/4 = 3, edge (0,1) = (1+2+3+4+5+6)/6 = 3.5
+    seg9, _ = O.make_segments([(0, 1, 1, 9, 1)])
+    out = O.spatial_pool(seg9, [3], 3, np.arange(1.0, 10.0))
+    assert out[4] == 5.0 and out[0] == 3.0 and out[1] == 3.5 and out[8] == 7.0
+    assert np.all(O.spatial_pool(seg9, [3], 3, np.full(9, 0.25)) == 0.25)     # a constant map stays constant
+
+
+def test_merge_dropped_means():
+    rng = np.random.default_rng(8)
+    rows = [(0, 1, 1, 7, 1), (0, 2, 3, 5, 1)]
+    segs, n = O.make_segments(rows)
+    X = rng.integers(-8, 9, (n, 6)).astype(np.float32)
+    mask = (rng.random(n) < 0.4).astype(np.uint8)
+    mask[7:12] = 1                                   # frame 0 of the video: nothing dropped
+    mask[12:17] = 0                                  # frame 1: everything dropped
+    Y, nd = O.merge_dropped(segs, X, mask)
+    assert Y.shape == (4, 6) and list(nd) == [int((mask[:7] == 0).sum()), 0, 5, int((mask[17:22] == 0).sum())]
+    assert np.all(Y[1] == 0.0)
+    assert np.array_equal(Y[2], X[12:17].astype(np.float64).mean(axis=0))
+    for f, (a, b) in enumerate([(0, 7), (7, 12), (12, 17), (17, 22)]):
+        kept_sum = X[a:b][mask[a:b] == 1].astype(np.float64).sum(axis=0)
+        assert np.allclose(nd[f] * Y[f] + kept_sum, X[a:b].astype(np.float64).sum(axis=0), rtol=0, atol=1e-12)
+    # bf16 storage decodes exactly
+    Yb, _ = O.merge_dropped(segs, synth.f32_to_bf16_bits(X), mask)
+    assert np.array_equal(Yb, Y)
+
+
+def test_gather_residual_rules():
+    rng = np.random.default_rng(9)
+    rows = [(0, 1, 1, 4, 1), (0, 2, 3, 5, 1)]        # image rows 0..3, video rows 4..18 (3 frames of 5 patches)
+    segs, n = O.make_segments(rows)
+    X = rng.integers(-20, 21, (n, 8)).astype(np.float32)
+    X[14:19] = X[9:14]                               # frame 2 identical to frame 1
+    idx = np.array([1, 3, 4, 8, 9, 12, 14, 18], np.int32)
+    for store in (lambda a: a, synth.f32_to_bf16_bits):
+        Xs = store(X)
+        Y = O.gather_residual(segs, Xs, idx)
+        Yf = Y if Y.dtype == np.float32 else (Y.astype(np.uint32) << 16).view(np.float32)
+        assert np.array_equal(Yf[:4], X[[1, 3, 4, 8]])               # image rows and key-frame rows are copies
+        assert np.array_equal(Yf[4], X[9] - X[4]) and np.array_equal(Yf[5], X[12] - X[7])
+        assert np.all(Yf[6:] == 0.0)                                 # static frame: zero residual
+        assert np.array_equal(Yf[4] + X[4], X[9])                    # residual + previous = original (small integers: exact)
+    # bf16 rounding of an inexact difference: nearest even
+    Xb = np.zeros((2, 8), np.float32)
+    Xb[1, 0], Xb[0, 0] = 1.0, 2.0 ** -9                              # 1 - 2^-9 needs 9 bits: ties to even -> 1.0
+    Xb[1, 1], Xb[0, 1] = 1.0, 3 * 2.0 ** -10                         # 1 - 3*2^-10: nearest bf16 is 1 - 2^-8... = 0.99609375
+    seg2, _ = O.make_segments([(0, 2, 2, 1, 1)])
+    Yb = O.gather_residual(seg2, synth.f32_to_bf16_bits(Xb), np.array([1], np.int32))
+    got = (Yb.astype(np.uint32) << 16).view(np.float32)[0]
+    assert got[0] == 1.0 and got[1] == 0.99609375
