@@ -217,6 +217,29 @@ int mas_learned_heads(const mas_plan* plan, const void* X, const void* Q, const 
 int mas_forward_heads(const mas_plan* plan, const void* X, const void* Q, const mas_heads* heads, float* heads_m_spatial /*[N]*/,
                       mas_segment_out* heads_seg_out /*[n_segs]*/, const mas_outputs* out, mas_stream_t stream);
 
+/* NEXT-3, the rest of PAPER.md:98 / 105 ("coarsely compressed", "represented using only the residual difference").
+ * All pointers device unless said otherwise.
+ *
+ * mas_spatial_pool: Eq. 3's AvgPool as a k x k window mean (1 <= k <= 31) of the per-token scalar map s[N] (mas_spatial's output)
+ * on the H x W patch grid of every frame, W = h_grid_w[segment] (HOST array [n_segs], read during the call), H = P / W; the window
+ * of cell (i, j) spans rows i-(k-1)/2 .. i+k/2 and the same columns, and the mean runs over the cells inside the grid.  The
+ * pooled map goes to s_pooled[N] (must not alias s) and can be fed to mas_fuse in place of s.  INVALID_ARG if W < 1 or P % W != 0.
+ *
+ * mas_merge_dropped: one mean token per frame from the rows the selection dropped (keep_mask = 0).  Frames are numbered segment
+ * by segment (mas_plan_n_frames of them): Ymerge[f, :] fp32 = mean of frame f's dropped rows (zeros if none), n_dropped[f] their
+ * number.  Reads every dropped row once.
+ *
+ * mas_gather_residual: like the gather step of mas_select_compact (kept_idx / kept_off as produced there), but a kept token of
+ * frame t >= 1 of a temporal segment is written as x_t - x_{t-1} (same patch, previous frame; bf16: the exact difference rounded
+ * to nearest even), everything else as a copy.  Y[cap_rows, d] has the dtype of X; nothing is written past cap_rows. */
+int64_t mas_plan_n_frames(const mas_plan* plan);         /* sum of n_frames over the segments */
+int mas_spatial_pool(const mas_plan* plan, const int32_t* h_grid_w /*host [n_segs]*/, int32_t k, const float* s /*[N]*/,
+                     float* s_pooled /*[N]*/, mas_stream_t stream);
+int mas_merge_dropped(const mas_plan* plan, const void* X, const uint8_t* keep_mask /*[N]*/, float* Ymerge /*[n_frames, d]*/,
+                      int32_t* n_dropped /*[n_frames]*/, mas_stream_t stream);
+int mas_gather_residual(const mas_plan* plan, const void* X, const int32_t* kept_idx, const int64_t* kept_off /*[n_segs+1]*/,
+                        void* Y /*[cap_rows, d]*/, int64_t cap_rows, mas_stream_t stream);
+
 /* NEXT-4: the draft-confidence entropy of Eq. 9 and the speculate rule of Eq. 10, the
  * consumer-side step next to the MAS pass.  logits[n_rows, V] (device, fp32 or bf16, row stride `row_stride` elements,
  * base and stride 16-byte aligned, n_rows <= 65535): per row p = softmax(l), H = -sum_v p_v ln p_v,

@@ -21,7 +21,8 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads"]
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads", "mas_plan_n_frames", "mas_spatial_pool", "mas_merge_dropped",
+           "mas_gather_residual"]
 
 
 class mas_segment(C.Structure):
@@ -102,6 +103,14 @@ def _load():
     lib.mas_learned_heads.restype = C.c_int
     lib.mas_forward_heads.argtypes = [vp, vp, vp, C.POINTER(mas_heads), vp, vp, C.POINTER(mas_outputs), vp]
     lib.mas_forward_heads.restype = C.c_int
+    lib.mas_plan_n_frames.argtypes = [vp]
+    lib.mas_plan_n_frames.restype = C.c_int64
+    lib.mas_spatial_pool.argtypes = [vp, C.POINTER(C.c_int32), i32, vp, vp, vp]
+    lib.mas_spatial_pool.restype = C.c_int
+    lib.mas_merge_dropped.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.mas_merge_dropped.restype = C.c_int
+    lib.mas_gather_residual.argtypes = [vp, vp, vp, vp, vp, i64, vp]
+    lib.mas_gather_residual.restype = C.c_int
     lib.mas_score_schedule.restype = i32
     lib.mas_score_schedule.argtypes = [C.POINTER(mas_segment), i32, C.POINTER(i64), i32, i32, i32, i32, C.POINTER(i32), i32]
     for f in ("mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal",
@@ -277,6 +286,26 @@ class Plan:
         _check(lib.mas_forward_heads(self._h, _ptr(X), _ptr(Q), C.byref(hd), _ptr(m), _ptr(so), C.byref(self._bundle(o)), _stream_ptr(stream)),
                "mas_forward_heads")
         return o, m, so
+
+    # ---- NEXT-3: pooling, merged token, residual coding
+    def spatial_pool(self, s, grid_w, k, stream=None):
+        gw = (C.c_int32 * self.n_segs)(*[int(v) for v in grid_w])
+        out = self._f32()
+        _check(lib.mas_spatial_pool(self._h, gw, int(k), _ptr(s), _ptr(out), _stream_ptr(stream)), "mas_spatial_pool")
+        return out
+
+    def merge_dropped(self, X, keep_mask, stream=None):
+        F = int(lib.mas_plan_n_frames(self._h))
+        Y = torch.zeros((F, self.d), dtype=torch.float32, device=self.device)
+        nd = torch.zeros(F, dtype=torch.int32, device=self.device)
+        _check(lib.mas_merge_dropped(self._h, _ptr(X), _ptr(keep_mask), _ptr(Y), _ptr(nd), _stream_ptr(stream)), "mas_merge_dropped")
+        return Y, nd
+
+    def gather_residual(self, X, kept_idx, kept_off, cap_rows=None, stream=None):
+        cap = self.kept_capacity if cap_rows is None else int(cap_rows)
+        Y = torch.zeros((max(cap, 1), self.d), dtype=X.dtype, device=self.device)
+        _check(lib.mas_gather_residual(self._h, _ptr(X), _ptr(kept_idx), _ptr(kept_off), _ptr(Y), cap, _stream_ptr(stream)), "mas_gather_residual")
+        return Y
 
     def crossmodal(self, X, Q, want_S=False, stream=None):
         rel = self._f32()

@@ -1,0 +1,141 @@
+// k_compress.cuh — NEXT-3, the rest of PAPER.md:98 / 105: spatial pooling of the scalar map (Eq. 3's AvgPool),
+// one merged mean token per frame from the dropped rows ("coarsely compressed"), residual coding of kept video rows
+// ("represented using only the residual difference").  All three are plain HBM / L2 streaming kernels.
+#pragma once
+#include "msas_internal.cuh"
+
+namespace msas {
+
+// One frame of the batch: its first row and its patch count (frames are numbered segment by segment).
+struct DevFrame {
+  int64_t row0;
+  int32_t n_patches;
+  int32_t seg;
+};
+
+// (a) k x k count-valid window mean of s on each frame's H x W grid; one thread per token (the map is 4 B per token: L2 resident).
+__global__ void __launch_bounds__(256) k_spatial_pool(const DevSeg* __restrict__ segs, const DevTile* __restrict__ tiles,
+                                                      const int32_t* __restrict__ grid_w, int k, const float* __restrict__ s,
+                                                      float* __restrict__ out) {
+  const DevTile tile = tiles[blockIdx.x];
+  const DevSeg seg = segs[tile.seg];
+  const int W = grid_w[tile.seg], H = seg.n_patches / W, lo = (k - 1) / 2, hi = k / 2;
+  for (int r = threadIdx.x; r < tile.n_rows; r += blockDim.x) {
+    const int64_t row = (int64_t)tile.row_start + r;
+    const int64_t in_seg = row - seg.row0;
+    const int t = (int)(in_seg / seg.n_patches), c = (int)(in_seg - (int64_t)t * seg.n_patches), i = c / W, j = c - i * W;
+    const float* g = s + seg.row0 + (int64_t)t * seg.n_patches;
+    float acc = 0.f;
+    int cnt = 0;
+    for (int a = max(i - lo, 0); a <= min(i + hi, H - 1); ++a)
+      for (int b = max(j - lo, 0); b <= min(j + hi, W - 1); ++b) { acc += g[a * W + b]; ++cnt; }
+    out[row] = acc / (float)cnt;
+  }
+}
+
+// (b) mean of a frame's dropped rows: one CTA per (frame, slab of 256 16-byte column vectors); each warp takes every 8th row of
+// the frame (skipping kept rows: the mask byte is warp-uniform), lanes cover the slab's vectors; fp32 sums, fixed order.
+template <int DT>
+__global__ void __launch_bounds__(256) k_merge_dropped(const DevFrame* __restrict__ frames, const void* __restrict__ X,
+                                                       const uint8_t* __restrict__ keep_mask, float* __restrict__ Ymerge,
+                                                       int32_t* __restrict__ n_dropped, int d) {
+  constexpr int VE = DT == 1 ? 8 : 4;            // elements per 16-byte vector
+  constexpr int VPL = 8;                         // vectors per lane: the slab is 32 lanes x 8 vectors
+  __shared__ float part[8][32 * VPL * VE / 8];   // [warp][slab columns / 8]: reduced in 8 rounds of 1/8 slab each
+  __shared__ int cnt_s[8];
+  const DevFrame fr = frames[blockIdx.x];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int c0 = blockIdx.y * (32 * VPL * VE);   // first column of the slab
+  const int esz = DT == 1 ? 2 : 4;
+  float acc[VPL][VE];
+#pragma unroll
+  for (int v = 0; v < VPL; ++v)
+#pragma unroll
+    for (int e = 0; e < VE; ++e) acc[v][e] = 0.f;
+  int cnt = 0;
+  for (int p = warp; p < fr.n_patches; p += 8) {
+    const int64_t row = fr.row0 + p;
+    if (keep_mask[row]) continue;
+    ++cnt;
+    const char* src = static_cast<const char*>(X) + row * (int64_t)d * esz;
+    uint4 u[VPL];
+#pragma unroll
+    for (int v = 0; v < VPL; ++v) {
+      const int col = c0 + (v * 32 + lane) * VE;
+      u[v] = col < d ? ld_nc16(src + (int64_t)col * esz) : make_uint4(0, 0, 0, 0);
+    }
+#pragma unroll
+    for (int v = 0; v < VPL; ++v) {
+      if (DT == 1) {
+        const uint32_t w[4] = {u[v].x, u[v].y, u[v].z, u[v].w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { acc[v][(2 * q) % VE] += bf_lo(w[q]); acc[v][(2 * q + 1) % VE] += bf_hi(w[q]); }
+      } else {
+        acc[v][0] += __uint_as_float(u[v].x); acc[v][1] += __uint_as_float(u[v].y);
+        acc[v][2 % VE] += __uint_as_float(u[v].z); acc[v][3 % VE] += __uint_as_float(u[v].w);
+      }
+    }
+  }
+  if (lane == 0) cnt_s[warp] = cnt;
+  __syncthreads();
+  int total = 0;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) total += cnt_s[w];
+  const float inv = total > 0 ? 1.0f / (float)total : 0.f;
+  if (blockIdx.y == 0 && threadIdx.x == 0) n_dropped[blockIdx.x] = total;
+  // cross-warp reduction, one vector index v at a time (1/8 of the slab per round keeps shared memory at 8 KB)
+#pragma unroll
+  for (int v = 0; v < VPL; ++v) {
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < VE; ++e) part[warp][lane * VE + e] = acc[v][e];
+    __syncthreads();
+    for (int i = threadIdx.x; i < 32 * VE; i += 256) {
+      float t = 0.f;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) t += part[w][i];
+      const int col = c0 + v * 32 * VE + i;   // i = lane * VE + e
+      if (col < d) Ymerge[(int64_t)blockIdx.x * d + col] = t * inv;
+    }
+  }
+}
+
+// (c) gather with residual coding: kept row j of a temporal segment's frame t >= 1 is written as x_t - x_{t-1}; one warp per row.
+template <int DT>
+__global__ void __launch_bounds__(256) k_gather_residual(const DevSeg* __restrict__ segs, int n_segs, const char* __restrict__ X,
+                                                         char* __restrict__ Y, const int32_t* __restrict__ kept_idx,
+                                                         const int64_t* __restrict__ total_ptr, int64_t cap_rows, int d) {
+  const int lane = threadIdx.x & 31;
+  const int64_t total = *total_ptr < cap_rows ? *total_ptr : cap_rows;
+  const int64_t n_warps = (int64_t)gridDim.x * 8;
+  const int esz = DT == 1 ? 2 : 4;
+  const int n16 = (d * esz) >> 4;
+  for (int64_t j = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5); j < total; j += n_warps) {
+    const int64_t row = kept_idx[j];
+    int lo = 0, hi = n_segs - 1;               // the segment holding `row` (segments tile [0, N) in order)
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (segs[mid].row0 <= row) lo = mid; else hi = mid - 1; }
+    const DevSeg sg = segs[lo];
+    const bool res = sg.n_frames > 1 && row - sg.row0 >= sg.n_patches;
+    const uint4* src = reinterpret_cast<const uint4*>(X + row * (int64_t)d * esz);
+    const uint4* prv = reinterpret_cast<const uint4*>(X + (row - sg.n_patches) * (int64_t)d * esz);
+    uint4* dst = reinterpret_cast<uint4*>(Y + j * (int64_t)d * esz);
+    for (int i = lane; i < n16; i += 32) {
+      uint4 v = ld_nc16(src + i);
+      if (res) {
+        const uint4 q = ld_nc16(prv + i);
+        if (DT == 1) {   // the difference of two bf16 values is exact in fp32; cvt.rn rounds it to nearest even
+          v.x = pack_bf16x2(bf_lo(v.x) - bf_lo(q.x), bf_hi(v.x) - bf_hi(q.x));
+          v.y = pack_bf16x2(bf_lo(v.y) - bf_lo(q.y), bf_hi(v.y) - bf_hi(q.y));
+          v.z = pack_bf16x2(bf_lo(v.z) - bf_lo(q.z), bf_hi(v.z) - bf_hi(q.z));
+          v.w = pack_bf16x2(bf_lo(v.w) - bf_lo(q.w), bf_hi(v.w) - bf_hi(q.w));
+        } else {
+          v.x = __float_as_uint(__uint_as_float(v.x) - __uint_as_float(q.x)); v.y = __float_as_uint(__uint_as_float(v.y) - __uint_as_float(q.y));
+          v.z = __float_as_uint(__uint_as_float(v.z) - __uint_as_float(q.z)); v.w = __float_as_uint(__uint_as_float(v.w) - __uint_as_float(q.w));
+        }
+      }
+      st_na16(dst + i, v);
+    }
+  }
+}
+
+}  // namespace msas

@@ -15,6 +15,7 @@
 #include "k_entropy.cuh"
 #include "k_segment.cuh"
 #include "k_heads.cuh"
+#include "k_compress.cuh"
 
 using namespace msas;
 
@@ -28,8 +29,8 @@ static thread_local int g_last_cuda = 0;
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-  size_t segs, tiles, req, tc_sched, tc_sched_x, tc_segrank, tables_end;   // uploaded tables (contiguous from 0)
-  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, heads_part, heads_cq, total;
+  size_t segs, tiles, req, tc_sched, tc_sched_x, tc_segrank, frames, tables_end;   // uploaded tables (contiguous from 0)
+  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, heads_part, gridw, heads_cq, total;
 };
 
 struct mas_plan {
@@ -37,6 +38,7 @@ struct mas_plan {
   int64_t N = 0, nQ = 0, kept_cap = 0;
   int32_t n_tiles = 0;
   int32_t max_L = 0;
+  int64_t n_frames = 0;       // sum of T over the segments
   bool tc_inline_qnorm = true; // query norms in the score kernel's prologue (cooperative launch) vs a launch of their own
   int32_t seg_cluster = 1;    // CTAs per segment in the segment kernel (from the longest segment)
   int32_t seg_threads = 1024; // threads per CTA of the segment kernel
@@ -132,7 +134,8 @@ static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_of
   return MAS_OK;
 }
 
-static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes, size_t tc_tiles_max) {
+static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes, size_t tc_tiles_max,
+                          int64_t n_frames) {
   Layout l{};
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
@@ -142,6 +145,7 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.tc_sched = take(tc_bytes);
   l.tc_sched_x = take(tc_bytes);   // without tall tiles: the schedule of the calls that add 64 B rows (NEXT-1, NEXT-2)
   l.tc_segrank = take(sizeof(int32_t) * (n_segs + 1));   // first tile rank of every segment (TcTile::rank), NEXT-2
+  l.frames = take(sizeof(DevFrame) * (size_t)n_frames);   // NEXT-3: first row and patch count of every frame
   l.tables_end = o;
   l.qinv = take(sizeof(float) * nQ);
   l.s = take(sizeof(float) * N);
@@ -154,9 +158,16 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.keptoff = take(sizeof(int64_t) * (n_segs + 1));
   l.counter = take(256);
   l.heads_part = take(sizeof(float) * kHeadRows * std::max((size_t)n_tiles, 2 * tc_tiles_max));   // NEXT-2 scratch: per-tile column sums, per-request p-half
+  l.gridw = take(sizeof(int32_t) * n_segs);   // NEXT-3 scratch: the caller's grid widths
   l.heads_cq = take(sizeof(float) * kHeadRows * kHeadSlabs * (size_t)n_req);
   l.total = o;
   return l;
+}
+
+static int64_t count_frames(const mas_segment* segs, int32_t n_segs) {
+  int64_t f = 0;
+  for (int32_t k = 0; k < n_segs; ++k) f += segs[k].n_frames;
+  return f;
 }
 
 extern "C" int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
@@ -165,7 +176,7 @@ extern "C" int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_seg
   int64_t N, nQ; int32_t nt, maxL;
   int st = validate(h_segs, n_segs, h_q_off, n_requests, d, dtype, nullptr, &N, &nQ, &nt, &maxL);
   if (st != MAS_OK) return st;
-  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs), tc_max_tiles(h_segs, n_segs)).total;
+  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs), tc_max_tiles(h_segs, n_segs), count_frames(h_segs, n_segs)).total;
   return MAS_OK;
 }
 
@@ -192,7 +203,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
   if (st != MAS_OK) return st;
   if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0) return MAS_ERR_UNSUPPORTED;
   const size_t tc_bytes = tc_schedule_bytes(h_segs, n_segs);
-  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes, tc_max_tiles(h_segs, n_segs));
+  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes, tc_max_tiles(h_segs, n_segs), count_frames(h_segs, n_segs));
   if (workspace_bytes < lay.total) return MAS_ERR_WORKSPACE;
 
   mas_plan* p = new (std::nothrow) mas_plan();
@@ -241,6 +252,17 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
       ht[ti].seg = k;
       ++ti;
     }
+  }
+  {
+    DevFrame* hf = reinterpret_cast<DevFrame*>(h + lay.frames);
+    int64_t f = 0;
+    for (int32_t k = 0; k < n_segs; ++k)
+      for (int32_t t = 0; t < h_segs[k].n_frames; ++t, ++f) {
+        hf[f].row0 = h_segs[k].row0 + (int64_t)t * h_segs[k].n_patches;
+        hf[f].n_patches = h_segs[k].n_patches;
+        hf[f].seg = k;
+      }
+    p->n_frames = f;
   }
   for (int32_t r = n_requests - 1; r >= 0; --r)   // requests without segments get an empty range
     if (hr[r] > hr[r + 1]) hr[r] = hr[r + 1];
@@ -311,6 +333,7 @@ extern "C" int mas_plan_set_inline_query_norms(mas_plan* p, int32_t on) {
 }
 extern "C" int64_t mas_plan_n_tokens(const mas_plan* p) { return p ? p->N : -1; }
 extern "C" int64_t mas_plan_n_queries(const mas_plan* p) { return p ? p->nQ : -1; }
+extern "C" int64_t mas_plan_n_frames(const mas_plan* p) { return p ? p->n_frames : -1; }
 extern "C" int64_t mas_plan_kept_capacity(const mas_plan* p) { return p ? p->kept_cap : -1; }
 
 extern "C" int32_t mas_score_schedule(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
@@ -485,6 +508,52 @@ extern "C" int mas_select_compact(const mas_plan* p, const void* X, const float*
   SegArgs a = seg_args(p, nullptr, nullptr, nullptr, nullptr, const_cast<float*>(mas_tok), seg_out, mask, kept_idx, koff, cap_rows);
   CK(launch_kc(k_segment<false, true>, dim3((unsigned)(p->n_segs * p->seg_cluster)), dim3((unsigned)p->seg_threads), p->seg_cluster, st, false, a));
   return launch_select_tail(p, X, mask, kept_idx, koff, Y, cap_rows, st);
+}
+
+// NEXT-3: pooling, merged token, residual coding (k_compress.cuh)
+extern "C" int mas_spatial_pool(const mas_plan* p, const int32_t* h_grid_w, int32_t k, const float* s, float* s_pooled, mas_stream_t stream) {
+  if (!p || !h_grid_w || !s || !s_pooled || s == s_pooled || k < 1 || k > 31) return MAS_ERR_INVALID_ARG;
+  const DevSeg* hs = reinterpret_cast<const DevSeg*>(static_cast<const char*>(p->pinned) + p->lay.segs);
+  for (int32_t q = 0; q < p->n_segs; ++q)
+    if (h_grid_w[q] < 1 || hs[q].n_patches % h_grid_w[q] != 0) return MAS_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  CK(cudaMemcpyAsync(p->at<int32_t>(p->lay.gridw), h_grid_w, sizeof(int32_t) * p->n_segs, cudaMemcpyHostToDevice, st));
+  k_spatial_pool<<<p->n_tiles, 256, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->at<DevTile>(p->lay.tiles), p->at<int32_t>(p->lay.gridw), k, s, s_pooled);
+  CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+extern "C" int mas_merge_dropped(const mas_plan* p, const void* X, const uint8_t* keep_mask, float* Ymerge, int32_t* n_dropped,
+                                 mas_stream_t stream) {
+  if (!p || !X || !keep_mask || !Ymerge || !n_dropped) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X)) return MAS_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int slab = p->dtype == MAS_BF16 ? 2048 : 1024;
+  const dim3 grid((unsigned)p->n_frames, (unsigned)((p->d + slab - 1) / slab));
+  if (p->dtype == MAS_BF16) k_merge_dropped<1><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, p->d);
+  else k_merge_dropped<0><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, p->d);
+  CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+extern "C" int mas_gather_residual(const mas_plan* p, const void* X, const int32_t* kept_idx, const int64_t* kept_off, void* Y,
+                                   int64_t cap_rows, mas_stream_t stream) {
+  if (!p || !X || !kept_idx || !kept_off || !Y || cap_rows < 0) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(Y)) return MAS_ERR_UNSUPPORTED;
+  if (cap_rows == 0) return MAS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t rows = cap_rows < p->kept_cap ? cap_rows : p->kept_cap;
+  int64_t grid = (rows + 7) / 8;
+  const int64_t gmax = (int64_t)p->sm_count * 16;
+  grid = grid > gmax ? gmax : grid < 1 ? 1 : grid;
+  if (p->dtype == MAS_BF16)
+    k_gather_residual<1><<<(unsigned)grid, 256, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->n_segs, static_cast<const char*>(X),
+                                                         static_cast<char*>(Y), kept_idx, kept_off + p->n_segs, cap_rows, p->d);
+  else
+    k_gather_residual<0><<<(unsigned)grid, 256, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->n_segs, static_cast<const char*>(X),
+                                                         static_cast<char*>(Y), kept_idx, kept_off + p->n_segs, cap_rows, p->d);
+  CK(cudaGetLastError());
+  return MAS_OK;
 }
 
 // NEXT-2: learned heads (k_heads.cuh)

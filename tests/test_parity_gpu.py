@@ -629,3 +629,76 @@ def test_learned_heads_argument_checks(B):
     with pytest.raises(Exception):
         plan.learned_heads(X, Q, None, *args, 4)             # temporal segment without gamma
     plan.close()
+
+
+# ---------------------------------------------------------------- NEXT-3: pooling, merged token, residual coding
+def _grid_w(w):
+    """A grid width per segment: the largest divisor of P not above sqrt(P) (24 for 576; 1 for audio frames)."""
+    out = []
+    for (_, _, T, P, _) in w.segments:
+        W = max(v for v in range(1, int(P ** 0.5) + 1) if P % v == 0)
+        out.append(P // W if P // W <= 64 else W)
+    return out
+
+
+@pytest.mark.parametrize("w", [synth.batched_images(seed=71, R=4, d=128, L_lo=3, L_hi=9, P=576), synth.video(seed=72, R=2, T=4, P=300, d=128, L=8),
+                               synth.audio_vision(seed=73, R=2, d=64, L=5, P_img=130, T_aud=260)], ids=["images", "video", "audio_vision"])
+@pytest.mark.parametrize("k", [1, 2, 3, 5])
+def test_spatial_pool(B, w, k):
+    segs, n = O.make_segments(w.segments)
+    gw = _grid_w(w)
+    plan = _plan(B, w)
+    s, _ = plan.spatial(B.to_device(w.X))
+    out = plan.spatial_pool(s, gw, k)
+    torch.cuda.synchronize()
+    ref = O.spatial_pool(segs, gw, k, s.cpu().numpy().astype(np.float64))        # both sides pool the same fp32 map
+    assert np.allclose(out.cpu().numpy(), ref, rtol=2e-6, atol=0)
+    if k == 1:
+        assert torch.equal(out, s)
+    with pytest.raises(Exception):
+        plan.spatial_pool(s, [7] * len(gw), k)                                   # 7 divides none of these P
+    plan.close()
+
+
+@pytest.mark.parametrize("w", [synth.batched_images(seed=74, R=5, d=512, L_lo=3, L_hi=9, P=333), synth.video(seed=75, R=2, T=4, P=300, d=2304, L=8),
+                               synth.video(seed=76, R=1, T=3, P=70, d=200, L=4, dtype="f32"), synth.audio_vision(seed=77, R=2, d=256, L=5, P_img=130, T_aud=260)],
+                         ids=["images", "video_d2304", "video_f32_d200", "audio_vision"])
+def test_merge_dropped_and_residual_gather(B, w):
+    segs, n = O.make_segments(w.segments)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    o = plan.forward(X, Q)
+    torch.cuda.synchronize()
+    mask = o["keep_mask"].cpu().numpy()
+    # merged token: fp32 sums of up to P rows against the oracle's double mean
+    Y, nd = plan.merge_dropped(X, o["keep_mask"])
+    torch.cuda.synchronize()
+    Yr, ndr = O.merge_dropped(segs, w.X, mask)
+    assert np.array_equal(nd.cpu().numpy(), ndr)
+    Xf = (synth.bf16_bits_to_f32(w.X) if w.dtype == "bf16" else w.X).astype(np.float64)
+    scale = np.sqrt((Xf ** 2).mean())
+    assert np.allclose(Y.cpu().numpy(), Yr, rtol=1e-4, atol=1e-5 * scale)
+    # residual gather: bit-exact against the oracle on the GPU's own kept list
+    tot = int(o["kept_off"][-1].item())
+    idx = o["kept_idx"][:tot].cpu().numpy()
+    Yres = plan.gather_residual(X, o["kept_idx"], o["kept_off"])
+    torch.cuda.synchronize()
+    ref = O.gather_residual(segs, w.X, idx)
+    got = Yres[:tot].cpu()
+    got = got.view(torch.int16).numpy().view(np.uint16) if w.dtype == "bf16" else got.numpy()
+    assert np.array_equal(got, ref)
+    # key-frame and image rows are plain copies: identical to the plain gather there
+    seg_of = np.concatenate([np.full(s[2] * s[3], k) for k, s in enumerate(w.segments)])
+    row0 = np.concatenate([[0], np.cumsum([s[2] * s[3] for s in w.segments])])
+    is_res = np.array([w.segments[seg_of[r]][2] > 1 and r - row0[seg_of[r]] >= w.segments[seg_of[r]][3] for r in idx])
+    plain = o["Y"][:tot].cpu()
+    plain = plain.view(torch.int16).numpy().view(np.uint16) if w.dtype == "bf16" else plain.numpy()
+    assert np.array_equal(got[~is_res], plain[~is_res])
+    # capacity: nothing past cap_rows
+    cap = max(1, tot // 3)
+    Yc = plan.gather_residual(X, o["kept_idx"], o["kept_off"], cap_rows=cap)
+    torch.cuda.synchronize()
+    gc = Yc[:cap].cpu()
+    gc = gc.view(torch.int16).numpy().view(np.uint16) if w.dtype == "bf16" else gc.numpy()
+    assert np.array_equal(gc, ref[:cap])
+    plan.close()
