@@ -33,19 +33,27 @@ __global__ void __launch_bounds__(256) k_spatial_pool(const DevSeg* __restrict__
   }
 }
 
-// (b) mean of a frame's dropped rows: one CTA per (frame, slab of 256 16-byte column vectors); each warp takes every 8th row of
-// the frame (skipping kept rows: the mask byte is warp-uniform), lanes cover the slab's vectors; fp32 sums, fixed order.
+// (b) mean of a frame's dropped rows.  One CTA per (frame, slab of 128 16-byte column vectors, row split): each warp takes
+// every 8th row of its row range, four rows at a time (mask bytes first, then 16 predicated vector loads per lane), lanes cover
+// the slab's vectors; fp32 sums in a fixed order.  With one row split the CTA writes the mean; with several (few frames: a
+// batch of images) it writes partial sums and k_merge_finish adds them in split order.
+constexpr int kMergeCtas = 1184;                 // CTAs aimed at when a batch has few frames (8 per SM); also the scratch slabs
+constexpr int kMergeVPL = 4;                     // vectors per lane: a slab is 32 lanes x 4 vectors
 template <int DT>
 __global__ void __launch_bounds__(256) k_merge_dropped(const DevFrame* __restrict__ frames, const void* __restrict__ X,
                                                        const uint8_t* __restrict__ keep_mask, float* __restrict__ Ymerge,
-                                                       int32_t* __restrict__ n_dropped, int d) {
+                                                       int32_t* __restrict__ n_dropped, float* __restrict__ part,
+                                                       int32_t* __restrict__ cnt_part, int d) {
   constexpr int VE = DT == 1 ? 8 : 4;            // elements per 16-byte vector
-  constexpr int VPL = 8;                         // vectors per lane: the slab is 32 lanes x 8 vectors
-  __shared__ float part[8][32 * VPL * VE / 8];   // [warp][slab columns / 8]: reduced in 8 rounds of 1/8 slab each
+  constexpr int VPL = kMergeVPL;
+  constexpr int SLAB = 32 * VPL * VE;            // columns per slab
+  __shared__ float red[8][32 * VE];              // [warp][one vector index of the slab]
   __shared__ int cnt_s[8];
   const DevFrame fr = frames[blockIdx.x];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int c0 = blockIdx.y * (32 * VPL * VE);   // first column of the slab
+  const int RS = gridDim.z, rs = blockIdx.z;
+  const int per = (fr.n_patches + RS - 1) / RS, p_lo = min(fr.n_patches, rs * per), p_hi = min(fr.n_patches, p_lo + per);
+  const int c0 = blockIdx.y * SLAB;
   const int esz = DT == 1 ? 2 : 4;
   float acc[VPL][VE];
 #pragma unroll
@@ -53,26 +61,33 @@ __global__ void __launch_bounds__(256) k_merge_dropped(const DevFrame* __restric
 #pragma unroll
     for (int e = 0; e < VE; ++e) acc[v][e] = 0.f;
   int cnt = 0;
-  for (int p = warp; p < fr.n_patches; p += 8) {
-    const int64_t row = fr.row0 + p;
-    if (keep_mask[row]) continue;
-    ++cnt;
-    const char* src = static_cast<const char*>(X) + row * (int64_t)d * esz;
-    uint4 u[VPL];
+  for (int p0 = p_lo + warp; p0 < p_hi; p0 += 32) {   // rows p0, p0 + 8, p0 + 16, p0 + 24
+    bool drop[4];
 #pragma unroll
-    for (int v = 0; v < VPL; ++v) {
-      const int col = c0 + (v * 32 + lane) * VE;
-      u[v] = col < d ? ld_nc16(src + (int64_t)col * esz) : make_uint4(0, 0, 0, 0);
+    for (int q = 0; q < 4; ++q) { const int pr = p0 + 8 * q; drop[q] = pr < p_hi && keep_mask[fr.row0 + pr] == 0; }
+    uint4 u[4][VPL];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const char* src = static_cast<const char*>(X) + (fr.row0 + p0 + 8 * q) * (int64_t)d * esz;
+#pragma unroll
+      for (int v = 0; v < VPL; ++v) {
+        const int col = c0 + (v * 32 + lane) * VE;
+        u[q][v] = (drop[q] && col < d) ? ld_nc16(src + (int64_t)col * esz) : make_uint4(0, 0, 0, 0);
+      }
     }
 #pragma unroll
-    for (int v = 0; v < VPL; ++v) {
-      if (DT == 1) {
-        const uint32_t w[4] = {u[v].x, u[v].y, u[v].z, u[v].w};
+    for (int q = 0; q < 4; ++q) {
+      cnt += drop[q] ? 1 : 0;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) { acc[v][(2 * q) % VE] += bf_lo(w[q]); acc[v][(2 * q + 1) % VE] += bf_hi(w[q]); }
-      } else {
-        acc[v][0] += __uint_as_float(u[v].x); acc[v][1] += __uint_as_float(u[v].y);
-        acc[v][2 % VE] += __uint_as_float(u[v].z); acc[v][3 % VE] += __uint_as_float(u[v].w);
+      for (int v = 0; v < VPL; ++v) {
+        if (DT == 1) {
+          const uint32_t w[4] = {u[q][v].x, u[q][v].y, u[q][v].z, u[q][v].w};
+#pragma unroll
+          for (int k = 0; k < 4; ++k) { acc[v][(2 * k) % VE] += bf_lo(w[k]); acc[v][(2 * k + 1) % VE] += bf_hi(w[k]); }
+        } else {
+          acc[v][0] += __uint_as_float(u[q][v].x); acc[v][1] += __uint_as_float(u[q][v].y);
+          acc[v][2 % VE] += __uint_as_float(u[q][v].z); acc[v][3 % VE] += __uint_as_float(u[q][v].w);
+        }
       }
     }
   }
@@ -81,22 +96,41 @@ __global__ void __launch_bounds__(256) k_merge_dropped(const DevFrame* __restric
   int total = 0;
 #pragma unroll
   for (int w = 0; w < 8; ++w) total += cnt_s[w];
-  const float inv = total > 0 ? 1.0f / (float)total : 0.f;
-  if (blockIdx.y == 0 && threadIdx.x == 0) n_dropped[blockIdx.x] = total;
-  // cross-warp reduction, one vector index v at a time (1/8 of the slab per round keeps shared memory at 8 KB)
+  const bool final_ = RS == 1;
+  const float scale = final_ ? (total > 0 ? 1.0f / (float)total : 0.f) : 1.0f;
+  if (blockIdx.y == 0 && threadIdx.x == 0) {
+    if (final_) n_dropped[blockIdx.x] = total; else cnt_part[blockIdx.x * RS + rs] = total;
+  }
+  float* dst = final_ ? Ymerge + (int64_t)blockIdx.x * d : part + ((int64_t)(blockIdx.x * RS + rs) * gridDim.y + blockIdx.y) * SLAB - c0;
 #pragma unroll
   for (int v = 0; v < VPL; ++v) {
     __syncthreads();
 #pragma unroll
-    for (int e = 0; e < VE; ++e) part[warp][lane * VE + e] = acc[v][e];
+    for (int e = 0; e < VE; ++e) red[warp][lane * VE + e] = acc[v][e];
     __syncthreads();
     for (int i = threadIdx.x; i < 32 * VE; i += 256) {
       float t = 0.f;
 #pragma unroll
-      for (int w = 0; w < 8; ++w) t += part[w][i];
+      for (int w = 0; w < 8; ++w) t += red[w][i];
       const int col = c0 + v * 32 * VE + i;   // i = lane * VE + e
-      if (col < d) Ymerge[(int64_t)blockIdx.x * d + col] = t * inv;
+      if (col < d) dst[col] = t * scale;
     }
+  }
+}
+// adds the row splits' partial sums in split order: one CTA per (frame, slab)
+__global__ void __launch_bounds__(256) k_merge_finish(const float* __restrict__ part, const int32_t* __restrict__ cnt_part,
+                                                      float* __restrict__ Ymerge, int32_t* __restrict__ n_dropped, int RS, int slab, int d) {
+  const int f = blockIdx.x, y = blockIdx.y;
+  int total = 0;
+  for (int r = 0; r < RS; ++r) total += cnt_part[f * RS + r];
+  if (y == 0 && threadIdx.x == 0) n_dropped[f] = total;
+  const float inv = total > 0 ? 1.0f / (float)total : 0.f;
+  for (int i = threadIdx.x; i < slab; i += 256) {
+    const int col = y * slab + i;
+    if (col >= d) break;
+    float t = 0.f;
+    for (int r = 0; r < RS; ++r) t += part[((int64_t)(f * RS + r) * gridDim.y + y) * slab + i];
+    Ymerge[(int64_t)f * d + col] = t * inv;
   }
 }
 

@@ -30,7 +30,7 @@ static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; 
 
 struct Layout {
   size_t segs, tiles, req, tc_sched, tc_sched_x, tc_segrank, frames, tables_end;   // uploaded tables (contiguous from 0)
-  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, heads_part, gridw, heads_cq, total;
+  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, heads_part, gridw, heads_cq, merge_part, merge_cnt, total;
 };
 
 struct mas_plan {
@@ -39,6 +39,7 @@ struct mas_plan {
   int32_t n_tiles = 0;
   int32_t max_L = 0;
   int64_t n_frames = 0;       // sum of T over the segments
+  int32_t max_patches = 0;    // largest P
   bool tc_inline_qnorm = true; // query norms in the score kernel's prologue (cooperative launch) vs a launch of their own
   int32_t seg_cluster = 1;    // CTAs per segment in the segment kernel (from the longest segment)
   int32_t seg_threads = 1024; // threads per CTA of the segment kernel
@@ -158,6 +159,8 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.keptoff = take(sizeof(int64_t) * (n_segs + 1));
   l.counter = take(256);
   l.heads_part = take(sizeof(float) * kHeadRows * std::max((size_t)n_tiles, 2 * tc_tiles_max));   // NEXT-2 scratch: per-tile column sums, per-request p-half
+  l.merge_part = take(sizeof(float) * 1024 * (size_t)kMergeCtas);   // NEXT-3 scratch: row-split partial sums of the merged tokens
+  l.merge_cnt = take(sizeof(int32_t) * (size_t)kMergeCtas);
   l.gridw = take(sizeof(int32_t) * n_segs);   // NEXT-3 scratch: the caller's grid widths
   l.heads_cq = take(sizeof(float) * kHeadRows * kHeadSlabs * (size_t)n_req);
   l.total = o;
@@ -263,6 +266,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
         hf[f].seg = k;
       }
     p->n_frames = f;
+    for (int32_t k = 0; k < n_segs; ++k) p->max_patches = std::max(p->max_patches, h_segs[k].n_patches);
   }
   for (int32_t r = n_requests - 1; r >= 0; --r)   // requests without segments get an empty range
     if (hr[r] > hr[r + 1]) hr[r] = hr[r + 1];
@@ -528,11 +532,24 @@ extern "C" int mas_merge_dropped(const mas_plan* p, const void* X, const uint8_t
   if (!p || !X || !keep_mask || !Ymerge || !n_dropped) return MAS_ERR_INVALID_ARG;
   if (!aligned16(X)) return MAS_ERR_UNSUPPORTED;
   cudaStream_t st = (cudaStream_t)stream;
-  const int slab = p->dtype == MAS_BF16 ? 2048 : 1024;
-  const dim3 grid((unsigned)p->n_frames, (unsigned)((p->d + slab - 1) / slab));
-  if (p->dtype == MAS_BF16) k_merge_dropped<1><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, p->d);
-  else k_merge_dropped<0><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, p->d);
+  const int slab = 32 * kMergeVPL * (p->dtype == MAS_BF16 ? 8 : 4);
+  const int64_t slabs = (p->d + slab - 1) / slab;
+  if (slabs > 65535) return MAS_ERR_UNSUPPORTED;
+  // few frames (a batch of images): split each frame's rows over several CTAs, partial sums added in split order afterwards;
+  // the scratch holds kMergeCtas slabs at most
+  int64_t rs = (kMergeCtas + p->n_frames * slabs - 1) / (p->n_frames * slabs);
+  rs = std::max<int64_t>(1, std::min<int64_t>(rs, std::min<int64_t>(16, (p->max_patches + 63) / 64)));
+  while (rs > 1 && p->n_frames * slabs * rs > kMergeCtas) --rs;
+  const dim3 grid((unsigned)p->n_frames, (unsigned)slabs, (unsigned)rs);
+  float* part = p->at<float>(p->lay.merge_part);
+  int32_t* cnt = p->at<int32_t>(p->lay.merge_cnt);
+  if (p->dtype == MAS_BF16) k_merge_dropped<1><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, part, cnt, p->d);
+  else k_merge_dropped<0><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, part, cnt, p->d);
   CK(cudaGetLastError());
+  if (rs > 1) {
+    k_merge_finish<<<dim3((unsigned)p->n_frames, (unsigned)slabs), 256, 0, st>>>(part, cnt, Ymerge, n_dropped, (int)rs, slab, p->d);
+    CK(cudaGetLastError());
+  }
   return MAS_OK;
 }
 
