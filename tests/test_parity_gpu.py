@@ -702,3 +702,41 @@ def test_merge_dropped_and_residual_gather(B, w):
     gc = gc.view(torch.int16).numpy().view(np.uint16) if w.dtype == "bf16" else gc.numpy()
     assert np.array_equal(gc, ref[:cap])
     plan.close()
+
+
+# ---------------------------------------------------------------- CUDA graph capture and replay of mas_forward
+@pytest.mark.parametrize("w", [synth.batched_images(seed=81, R=6, d=512, L_lo=3, L_hi=64, P=333), synth.video(seed=82, R=2, T=4, P=300, d=256, L=33)],
+                         ids=["images", "video"])
+def test_forward_in_a_cuda_graph(B, w):
+    """The launch-bound inner loop of a server is one graph launch: cooperative score kernel + PDL-chained segment and
+    gather kernels are captured once and replayed on new inputs; the grid-wide counters re-arm themselves."""
+    plan = _plan(B, w)
+    Xs, Qs = B.to_device(w.X).clone(), B.to_device(w.Q).clone()           # static buffers of the graph
+    out = plan.alloc_outputs()
+    eager = plan.forward(Xs, Qs)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        plan.forward(Xs, Qs, out=out)                                    # warm-up on the capture stream
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        plan.forward(Xs, Qs, out=out)
+    for rep in range(3):
+        g.replay()
+    torch.cuda.synchronize()
+    for k in ("m_spatial", "gamma", "rel", "mas_tok", "keep_mask", "kept_idx", "kept_off", "Y"):
+        assert torch.equal(eager[k], out[k]), k
+    # new inputs through the same graph: rows reversed inside the static buffer
+    w2 = synth.batched_images(seed=83, R=6, d=512, L_lo=3, L_hi=64, P=333) if w.name.startswith("batched") else synth.video(seed=84, R=2, T=4, P=300, d=256, L=33)
+    if w2.X.shape == w.X.shape and w2.Q.shape == w.Q.shape and np.array_equal(w2.q_off, w.q_off):
+        Xs.copy_(B.to_device(w2.X)); Qs.copy_(B.to_device(w2.Q))
+        g.replay()
+        torch.cuda.synchronize()
+        fresh = plan.forward(B.to_device(w2.X), B.to_device(w2.Q))
+        torch.cuda.synchronize()
+        for k in ("mas_tok", "keep_mask", "kept_idx", "Y"):
+            assert torch.equal(fresh[k], out[k]), k
+    plan.close()
