@@ -51,7 +51,7 @@ struct TcTile {            // 32 bytes
 constexpr int kTcAluSets = 2;                        // ALU warp sets: each takes 8 / kTcAluSets of a row's eight 16-byte units
 constexpr int kTcAluUnits = 8 / kTcAluSets;
 constexpr int kTcAluWarps = 4 * kTcAluSets;          // per set: one (token row, K-slice) per thread
-constexpr int kTcThreads = 256 + 32 * kTcAluWarps;   // warps 0-7: TMA (X), MMA, TMEM, TMA (Q), 4 x epilogue; then the ALU warps
+constexpr int kTcThreads = 256 + 32 * kTcAluWarps;   // 16 warps: 3 single-thread roles, 1 TMEM allocator, 4 epilogue, 8 statistics (roles by scheduler partition: see the kernel)
 constexpr int kTcSlots = 16;                         // mbarrier pairs of the chunk ring (slots are variable-sized)
 constexpr int kTcBoxBytes = 128 * 128;               // 128 rows x 64 bf16 columns
 constexpr int kTcCtrlBytes = 8192;
@@ -65,6 +65,7 @@ struct TcMaps {
 
 struct TcSchedule {
   bool enabled = false;
+  bool roles_split = false;      // long temporal sweep: keep the statistics warps off the producers' scheduler partition
   int n_ctas = 0, n_tiles = 0, smem_bytes = 0;
   const TcTile* d_tiles = nullptr;
   const int32_t* d_cta_off = nullptr;
@@ -90,6 +91,7 @@ struct TcParams {
   float* rel;
   int d;
   int n_kchunks;
+  int roles_split;    // warp-role layout (see the kernel): 1 = the single-thread roles alone on scheduler partition 0
 #ifdef MSAS_ABLATE
   int dbg;            // development only: bit0 no ALU math, bit1 no MMA, bit2 no Q loads, bit3 no prev loads
   unsigned long long* dbg_t;
@@ -256,6 +258,17 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   TcCtrl* ctrl = reinterpret_cast<TcCtrl*>(smem);
   unsigned char* ring0 = smem + kTcCtrlBytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  // Warp roles by scheduler partition (SMSP = warp % 4).  The three single-thread roles that keep the pipeline fed share SMSP 0
+  // with one (mostly waiting) epilogue warp, so the arithmetic warps never compete with them for issue slots:
+  //   SMSP 0: warp 0 TMA token rows, warp 4 TMA query rows, warp 8 MMA issuer, warp 12 epilogue (TMEM lanes 0-31)
+  //   SMSP 1-3: warps 1, 2, 3 epilogue (lane quarter = warp % 4); warps 5-7, 9-11, 13, 14 statistics; warp 15 TMEM allocation
+  // That helps long temporal sweeps (config 3: -5 %), where the statistics warps are busiest; elsewhere two statistics warps
+  // per partition (roles_split = 0: warps 0 TMA X, 1 MMA, 2 TMEM, 3 TMA Q, 4-7 epilogue, 8-15 statistics) measure 2 % faster.
+  const bool split = p.roles_split != 0;
+  const bool is_xprod = warp == 0, is_qprod = warp == (split ? 4 : 3), is_mma = warp == (split ? 8 : 1), is_tmem = warp == (split ? 15 : 2);
+  const bool is_epi = split ? (warp == 12 || (warp >= 1 && warp <= 3)) : (warp >= 4 && warp < 8);
+  const bool is_alu = !is_xprod && !is_qprod && !is_mma && !is_tmem && !is_epi;
+  const int alu_idx = !split ? warp - 8 : warp < 8 ? warp - 5 : warp < 12 ? warp - 6 : warp - 7;   // split: 5,6,7 -> 0..2; 9,10,11 -> 3..5; 13,14 -> 6,7
   const int tile_lo = p.cta_off[blockIdx.x], tile_hi = p.cta_off[blockIdx.x + 1];
   const int nk = p.n_kchunks;
   const bool lsh = p.sig != nullptr || p.heads_part != nullptr;   // 64 more B rows after the query rows (hash rows or head weights)
@@ -268,7 +281,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 #endif
 
   pdl_launch_dependents();   // the segment kernel may be scheduled as SMs free up; it waits for this grid to complete
-  if (warp == 1 && lane == 0) {
+  if (is_mma && lane == 0) {
     for (int i = 0; i < kTcSlots; ++i) { mbar_init(smem_u32(&ctrl->full[i]), 2); mbar_init(smem_u32(&ctrl->empty[i]), 1 + kTcAluWarps); }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&ctrl->tmem_full[i]), 1); mbar_init(smem_u32(&ctrl->tmem_empty[i]), 4);
@@ -276,11 +289,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 2) {   // TMEM: 2 tiles in flight x 2 halves x 128 fp32 columns (all 512 columns: one CTA per SM)
+  if (is_tmem) {   // TMEM: 2 tiles in flight x 2 halves x 128 fp32 columns (all 512 columns: one CTA per SM)
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctrl->tmem_base)), "r"(512) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  if (warp == 0 && lane == 0) {
+  if (is_xprod && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&mx128) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&mq64) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&mq16) : "memory");
@@ -290,12 +303,12 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   tc_fence_after();
   const uint32_t tmem_base = ctrl->tmem_base;
 
-  if (warp == 0 || warp == 3) {
+  if (is_xprod || is_qprod) {
     // ===================================================================== TMA producers (one thread each)
     // warp 0 streams the token rows (and the previous-frame rows), warp 3 the query rows.  A single thread issues about
     // one instruction every few cycles, so the per-chunk loop is kept to a few dozen instructions per producer.
     if (lane == 0) {
-      const bool xprod = warp == 0;
+      const bool xprod = is_xprod;
       TcRing ring;
       // `tail` replays the same placement sequence one released chunk at a time: tail.vhead is (a lower bound of) the
       // virtual start of the oldest chunk whose release has not been observed yet, tail.k its index.  Registers only.
@@ -350,7 +363,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         }
       }
     }
-  } else if (warp == 1) {
+  } else if (is_mma) {
     // ===================================================================== MMA issuer (one thread)
     if (lane == 0) {
       TcRing ring;
@@ -387,9 +400,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         tc_commit(smem_u32(&ctrl->tmem_full[acc]));
       }
     }
-  } else if (warp >= 4 && warp < 8) {
+  } else if (is_epi) {
     // ===================================================================== epilogue: one accumulator row per thread
-    const int q = warp - 4;                  // TMEM lane quarter this warp may access (warp % 4)
+    const int q = warp & 3;                  // TMEM lane quarter this warp may access (warp % 4)
     const int r = q * 32 + lane;             // tile row
     const float inv_d = 1.0f / (float)p.d;
     // a0 inside the same launch: while the first tile streams in, these four warps compute 1 / |q_j| for this CTA's
@@ -411,7 +424,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       }
       __threadfence();
       asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
-      if (tid == 128) atomicAdd(p.q_ready, 1ull);
+      if (q == 0 && lane == 0) atomicAdd(p.q_ready, 1ull);
     }
     bool q_ok = p.Q == nullptr;
     int it = 0;
@@ -532,10 +545,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         }
       }
     }
-  } else if (warp >= 8) {
+  } else if (is_alu) {
     // ===================================================================== CUDA-core statistics: one thread per (row, K-slice)
-    const int a = (tid - 256) & 127;
-    const uint32_t set = (uint32_t)(tid - 256) >> 7;      // which share of the row's eight 16-byte units this thread reads
+    const int a = (alu_idx & 3) * 32 + lane;
+    const uint32_t set = (uint32_t)alu_idx >> 2;          // which share of the row's eight 16-byte units this thread reads
     TcRing ring;
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
@@ -556,7 +569,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         const uint32_t off = ring.place(g.need);
         mbar_wait(smem_u32(&ctrl->full[ring.slot()]), ring.parity());
 #ifdef MSAS_ABLATE
-        if (tid == 256 && p.dbg_t && t == tile_lo && ch == 0) p.dbg_t[blockIdx.x * 8 + 2] = gtime();
+        if (alu_idx == 0 && lane == 0 && p.dbg_t && t == tile_lo && ch == 0) p.dbg_t[blockIdx.x * 8 + 2] = gtime();
 #endif
         if (active && dbl) {
           const unsigned char* sx = ring0 + off + my_off;
@@ -586,11 +599,15 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           const uint32_t u0 = set * (uint32_t)kTcAluUnits;       // this set's share of the row's eight 16-byte units
 #pragma unroll
           for (int u = 0; u < kTcAluUnits; ++u) x[u] = *reinterpret_cast<const uint4*>(sx + (((u0 + (uint32_t)u) ^ sw) << 4));
-          if (g.has_prev) {
+          if (g.has_prev && !(dbg & 16)) {
             const unsigned char* su = sx + poff;
             uint4 v[kTcAluUnits];
 #pragma unroll
             for (int u = 0; u < kTcAluUnits; ++u) v[u] = *reinterpret_cast<const uint4*>(su + (((u0 + (uint32_t)u) ^ sw) << 4));
+            if (dbg & 32) {   // development only: the loads without the arithmetic
+#pragma unroll
+              for (int u = 0; u < kTcAluUnits; ++u) n2a ^= (uint64_t)(x[u].x ^ x[u].y ^ x[u].z ^ x[u].w ^ v[u].x ^ v[u].y ^ v[u].z ^ v[u].w);
+            } else
 #pragma unroll
             for (int u = 0; u < kTcAluUnits; ++u) {
               const uint64_t x0 = bf16x2_to_f32x2(x[u].x), x1 = bf16x2_to_f32x2(x[u].y), x2 = bf16x2_to_f32x2(x[u].z), x3 = bf16x2_to_f32x2(x[u].w);
@@ -632,7 +649,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     __threadfence();
     if (atomicAdd(p.q_ready + 1, 1ull) == (unsigned long long)gridDim.x - 1ull) { p.q_ready[0] = 0ull; p.q_ready[1] = 0ull; __threadfence(); }
   }
-  if (warp == 2) {
+  if (is_tmem) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
   }
@@ -649,10 +666,12 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 // which is why only the fill phase uses them.
 struct TcCost {
   double w_prev = 0.25, w_q = 0.70, c_tile = 50.0;   // fitted to CTA finish times: ~27 us per MB of token rows, 12-19 us per MB of query rows, several us per tile
+  int roles = -1;              // development override of the warp-role layout (-1 = by the schedule)
   int hmax_plain = 256, hmax_tall = 384;   // tallest non-temporal tile; tall = three MMA halves, where pad16(L) <= 64
   TcCost() {
 #ifdef MSAS_ABLATE
     if (getenv("MSAS_HTALL")) hmax_tall = atoi(getenv("MSAS_HTALL"));
+    if (getenv("MSAS_ROLES")) roles = atoi(getenv("MSAS_ROLES"));
     if (getenv("MSAS_HMAX")) hmax_plain = atoi(getenv("MSAS_HMAX"));
     if (getenv("MSAS_WPREV")) w_prev = atof(getenv("MSAS_WPREV"));
     if (getenv("MSAS_WQ")) w_q = atof(getenv("MSAS_WQ"));
@@ -785,6 +804,11 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
   sc.n_tiles = n_tiles;
   sc.d_tiles = reinterpret_cast<const TcTile*>(d_dst);
   sc.d_cta_off = reinterpret_cast<const int32_t*>(d_dst + (size_t)n_tiles * sizeof(TcTile));
+  {   // warp-role layout: see the kernel
+    int64_t rows = 0, rows_prev = 0;
+    for (int i = 0; i < n_tiles; ++i) { rows += ht[i].n_rows; if (ht[i].prev_delta > 0 && ht[i].key_rows < ht[i].n_rows) rows_prev += ht[i].n_rows; }
+    sc.roles_split = cw.roles >= 0 ? cw.roles != 0 : (rows_prev * 10 >= rows * 4 && n_tiles >= 4 * n_ctas);
+  }
   sc.enabled = true;
 }
 
@@ -834,7 +858,7 @@ inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, f
   if (sig != nullptr || hf != nullptr) { if (!tc_make_map(&maps.r, Rm, 64, d, 64)) return -1; } else maps.r = maps.q[0];
   TcParams p;
   p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.sig = sig; p.s = s; p.dnorm = dnorm; p.rel = rel;
-  p.d = d; p.n_kchunks = d / 64;
+  p.d = d; p.n_kchunks = d / 64; p.roles_split = sc.roles_split ? 1 : 0;
   p.heads_part = hf ? hf->part : nullptr; p.heads_m = hf ? hf->m : nullptr; p.heads_bias = hf ? hf->bias : 0.f; p.heads_tau = hf ? hf->tau : 0.f;
   if (hf) p.sig = nullptr;
 #ifdef MSAS_ABLATE
