@@ -859,6 +859,9 @@ inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, f
   TcParams p;
   p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.sig = sig; p.s = s; p.dnorm = dnorm; p.rel = rel;
   p.d = d; p.n_kchunks = d / 64; p.roles_split = sc.roles_split ? 1 : 0;
+#ifdef MSAS_ABLATE
+  if (getenv("MSAS_ROLES")) p.roles_split = atoi(getenv("MSAS_ROLES"));
+#endif
   p.heads_part = hf ? hf->part : nullptr; p.heads_m = hf ? hf->m : nullptr; p.heads_bias = hf ? hf->bias : 0.f; p.heads_tau = hf ? hf->tau : 0.f;
   if (hf) p.sig = nullptr;
 #ifdef MSAS_ABLATE
