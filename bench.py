@@ -166,7 +166,9 @@ def main():
     w = synth.make(args.workload, seed=SEEDS[args.workload] + 1000 * rank)
     dt = B.MAS_BF16 if w.dtype == "bf16" else B.MAS_F32
     e = 2 if w.dtype == "bf16" else 4
-    plan = B.Plan(w.segments, w.q_off, w.d, dt, B.default_params(select_mode=w.select_mode, cut=w.cut))
+    def make_plan():
+        return B.Plan(w.segments, w.q_off, w.d, dt, B.default_params(select_mode=w.select_mode, cut=w.cut))
+    plan = make_plan()
     # two rotating input copies so that no step finds its rows in L2 (X alone is already > L2 on configs 2-5)
     Xs = [B.to_device(w.X), B.to_device(w.X)]
     Qs = [B.to_device(w.Q), B.to_device(w.Q)]
@@ -227,14 +229,24 @@ def main():
         hQ = torch.from_numpy(w.Q).view(hX.dtype).pin_memory()
         h_out = {k: (torch.empty_like(v, device="cpu").pin_memory() if isinstance(v, torch.Tensor) else v) for k, v in out.items()}
         h_out["gamma"] = h_out["rel"] = h_out["m_spatial"] = None          # the user-facing result: MAS scores, mask, kept rows
-        n_e2e = max(3, min(args.steps, 10))
-        plan.forward_host(hX, hQ, Xs[0], Qs[0], out, h_out)
+        n_e2e = max(4, min(args.steps, 10))
+        # two plans on two streams, called alternately: the device-to-host copies of one step overlap the host-to-device
+        # copies of the next (PCIe is full duplex); every step still copies its inputs in and its results out
+        plan2 = make_plan()
+        outs, h_outs = [out, plan2.alloc_outputs()], [h_out, {k: (v.clone().pin_memory() if isinstance(v, torch.Tensor) else v) for k, v in h_out.items()}]
+        plans, streams = [plan, plan2], [torch.cuda.Stream(), torch.cuda.Stream()]
+        torch.cuda.synchronize()
+        for i in range(2):
+            plans[i].forward_host_async(hX, hQ, Xs[i], Qs[i], outs[i], h_outs[i], stream=streams[i])
+        torch.cuda.synchronize()
         barrier()
         t0 = time.perf_counter()
         for i in range(n_e2e):
-            plan.forward_host(hX, hQ, Xs[i % 2], Qs[i % 2], out, h_out)
+            plans[i % 2].forward_host_async(hX, hQ, Xs[i % 2], Qs[i % 2], outs[i % 2], h_outs[i % 2], stream=streams[i % 2])
         torch.cuda.synchronize()
         e2e_ms = 1e3 * (time.perf_counter() - t0) / n_e2e
+        assert torch.equal(h_outs[0]["keep_mask"], h_outs[1]["keep_mask"]) and int(h_outs[1]["kept_off"][-1]) == kept_rows
+        plan2.close()
         h2d = w.X.nbytes + w.Q.nbytes
         d2h = w.n_tokens * (4 + 1) + plan.n_segs * 36 + (plan.n_segs + 1) * 8 + kept_rows * (4 + w.d * e)
         e2e = (e2e_ms, h2d, d2h, n_e2e)
@@ -271,7 +283,7 @@ def main():
         if e2e:
             line["e2e"] = {"value": total_tokens / (e2e[0] * 1e-3), "unit": "tokens/s", "h2d_bytes_per_step": int(e2e[1]),
                            "d2h_bytes_per_step": int(e2e[2]), "steps": e2e[3], "ms_per_step": e2e[0],
-                           "api": "mas_forward_host (pinned host buffers in, MAS scores + mask + kept rows out)"}
+                           "api": "mas_forward_host_async, two plans on two streams called alternately (pinned host buffers in, MAS scores + mask + kept rows out, every step)"}
         if world == 1 and not args.no_cpu_baseline:
             n_req = {"single_image": 1, "batched_images": 64, "video": 1, "audio_vision": 3, "ragged": 12}[args.workload]
             wb = w if args.workload != "video" else synth.video(seed=SEEDS["video"], R=1, T=8)

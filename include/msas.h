@@ -255,6 +255,13 @@ int mas_draft_entropy(const void* logits, int64_t n_rows, int64_t V, int64_t row
  * before returning. d_out members needed by the requested h_out members must be non-NULL. */
 int mas_forward_host(const mas_plan* plan, const void* h_X, const void* h_Q, void* d_X, void* d_Q,
                      const mas_outputs* d_out, const mas_outputs* h_out, mas_stream_t stream);
+/* The same without the final synchronisation: everything is enqueued on `stream` and the host outputs are valid once the caller
+ * has synchronised it (in threshold / adaptive mode the call still waits once, for the kept count, before it sizes the last two
+ * copies).  Two plans on two streams, called alternately, overlap one step's device-to-host copies with the next step's
+ * host-to-device copies (PCIe is full duplex): bench.py's `e2e` leg does exactly that.  Host buffers must be pinned for the
+ * copies to be asynchronous and must stay untouched until the stream has been synchronised. */
+int mas_forward_host_async(const mas_plan* plan, const void* h_X, const void* h_Q, void* d_X, void* d_Q,
+                     const mas_outputs* d_out, const mas_outputs* h_out, mas_stream_t stream);
 
 /* The fused bf16 fast path computes the query norms (row a0) in the prologue of its score kernel, which needs every
  * CTA of that kernel resident at once (cooperative launch).  Where that is impossible (e.g. a partitioned GPU) the

@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads", "mas_plan_n_frames", "mas_spatial_pool", "mas_merge_dropped",
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_forward_host_async", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads", "mas_plan_n_frames", "mas_spatial_pool", "mas_merge_dropped",
            "mas_gather_residual"]
 
 
@@ -93,6 +93,8 @@ def _load():
     lib.mas_select_compact.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
     lib.mas_forward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp]
     lib.mas_forward_host.argtypes = [vp, vp, vp, vp, vp, C.POINTER(mas_outputs), C.POINTER(mas_outputs), vp]
+    lib.mas_forward_host_async.argtypes = [vp, vp, vp, vp, vp, C.POINTER(mas_outputs), C.POINTER(mas_outputs), vp]
+    lib.mas_forward_host_async.restype = C.c_int
     lib.mas_plan_set_inline_query_norms.restype = C.c_int
     lib.mas_plan_set_inline_query_norms.argtypes = [vp, i32]
     lib.mas_draft_entropy_workspace_bytes.argtypes = [i64, i64, C.POINTER(C.c_size_t)]
@@ -359,6 +361,13 @@ class Plan:
         _check(lib.mas_forward_host(self._h, _ptr(h_X), _ptr(h_Q), _ptr(d_X), _ptr(d_Q), C.byref(self._bundle(d_out)),
                                     C.byref(self._bundle(h_out)) if h_out is not None else None, _stream_ptr(stream)),
                "mas_forward_host")
+
+
+    def forward_host_async(self, h_X, h_Q, d_X, d_Q, d_out, h_out, stream=None):
+        """As forward_host, without the final synchronisation (results valid once the stream is synchronised)."""
+        _check(lib.mas_forward_host_async(self._h, _ptr(h_X), _ptr(h_Q), _ptr(d_X), _ptr(d_Q), C.byref(self._bundle(d_out)),
+                                          C.byref(self._bundle(h_out)) if h_out is not None else None, _stream_ptr(stream)),
+               "mas_forward_host_async")
 
 
 def draft_entropy(logits, theta_conf, workspace=None, H=None, speculate=None, stream=None):

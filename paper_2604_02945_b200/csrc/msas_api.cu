@@ -765,8 +765,8 @@ extern "C" int mas_draft_entropy(const void* logits, int64_t n_rows, int64_t V, 
 }
 
 // ------------------------------------------------------------------------------------------------ host-buffer convenience
-extern "C" int mas_forward_host(const mas_plan* p, const void* h_X, const void* h_Q, void* d_X, void* d_Q, const mas_outputs* d_out,
-                                const mas_outputs* h_out, mas_stream_t stream) {
+static int forward_host_impl(const mas_plan* p, const void* h_X, const void* h_Q, void* d_X, void* d_Q, const mas_outputs* d_out,
+                             const mas_outputs* h_out, mas_stream_t stream, bool final_sync) {
   if (!p || !h_X || !h_Q || !d_X || !d_Q || !d_out) return MAS_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t esz = p->dtype == MAS_BF16 ? 2 : 4;
@@ -806,6 +806,14 @@ extern "C" int mas_forward_host(const mas_plan* p, const void* h_X, const void* 
       }
     }
   }
-  CK(cudaStreamSynchronize(st));
+  if (final_sync) CK(cudaStreamSynchronize(st));
   return MAS_OK;
+}
+extern "C" int mas_forward_host(const mas_plan* p, const void* h_X, const void* h_Q, void* d_X, void* d_Q, const mas_outputs* d_out,
+                                const mas_outputs* h_out, mas_stream_t stream) {
+  return forward_host_impl(p, h_X, h_Q, d_X, d_Q, d_out, h_out, stream, true);
+}
+extern "C" int mas_forward_host_async(const mas_plan* p, const void* h_X, const void* h_Q, void* d_X, void* d_Q, const mas_outputs* d_out,
+                                      const mas_outputs* h_out, mas_stream_t stream) {
+  return forward_host_impl(p, h_X, h_Q, d_X, d_Q, d_out, h_out, stream, false);
 }

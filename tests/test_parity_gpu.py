@@ -247,6 +247,39 @@ def test_forward_host_matches_device_path(B):
     plan.close()
 
 
+@pytest.mark.parametrize("mode", [0, 1], ids=["topk", "threshold"])
+def test_forward_host_async_two_plans_two_streams(B, mode):
+    """The pipelined end-to-end pattern of bench.py: two plans on two streams called alternately, results valid after the
+    streams are synchronised, identical to the blocking call."""
+    ws = [synth.video(seed=91 + i, R=2, T=3, P=200, d=256, L=12) for i in range(2)]
+    for w in ws:
+        w.select_mode, w.cut = mode, 0.45
+    plans = [_plan(B, w) for w in ws]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    hXs = [torch.from_numpy(w.X).view(torch.bfloat16).pin_memory() for w in ws]
+    hQs = [torch.from_numpy(w.Q).view(torch.bfloat16).pin_memory() for w in ws]
+    dXs = [torch.empty(w.X.shape, dtype=torch.bfloat16, device="cuda") for w in ws]
+    dQs = [torch.empty(w.Q.shape, dtype=torch.bfloat16, device="cuda") for w in ws]
+    d_outs = [p.alloc_outputs() for p in plans]
+    h_outs = [{k: (torch.zeros_like(v, device="cpu").pin_memory() if isinstance(v, torch.Tensor) else v) for k, v in d.items()} for d in d_outs]
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for i in range(2):
+            plans[i].forward_host_async(hXs[i], hQs[i], dXs[i], dQs[i], d_outs[i], h_outs[i], stream=streams[i])
+    for st in streams:
+        st.synchronize()
+    for i in range(2):
+        ref = plans[i].forward(B.to_device(ws[i].X), B.to_device(ws[i].Q))
+        torch.cuda.synchronize()
+        tot = int(ref["kept_off"][-1].item())
+        for k in ("mas_tok", "keep_mask", "kept_off", "seg_out"):
+            assert torch.equal(h_outs[i][k].view(torch.uint8), ref[k].cpu().view(torch.uint8)), k
+        assert torch.equal(h_outs[i]["kept_idx"][:tot], ref["kept_idx"][:tot].cpu())
+        assert torch.equal(h_outs[i]["Y"][:tot].view(torch.uint8), ref["Y"][:tot].cpu().view(torch.uint8))
+    for p in plans:
+        p.close()
+
+
 def test_unsupported_inputs_fail_loudly(B):
     w = synth.batched_images(seed=34, R=1, d=64, L_lo=4, L_hi=4, P=32)
     plan = _plan(B, w)
