@@ -143,6 +143,13 @@ int mas_spatial(const mas_plan* plan, const void* X, float* s /*[N]*/, float* m_
 /* S2 (Eq. 5 exact form): gamma[N]; 0 for T = 1 segments, 1 on keyframe rows. */
 int mas_temporal(const mas_plan* plan, const void* X, float* gamma /*[N]*/, mas_stream_t stream);
 
+/* a0-a3 in ONE pass over X (the score stage of mas_forward on its own): s[N] (S1's RMS), gamma[N] (S2; may be NULL: skipped) and
+ * rel[N] (S3).  On the bf16 / d % 64 == 0 fast path this is the TMA + tcgen05 score kernel (plus one elementwise launch that
+ * finishes gamma when it is asked for); otherwise the generic tile kernels.  Outputs as mas_spatial / mas_temporal /
+ * mas_crossmodal give them (within summation order). */
+int mas_score(const mas_plan* plan, const void* X, const void* Q, float* s /*[N]*/, float* gamma /*[N] or NULL*/, float* rel /*[N]*/,
+              mas_stream_t stream);
+
 /* S3 (Eq. 6 training-free): rel[N] = max_j cos(x_i, q_j). S_opt (may be NULL) receives the raw dot products
  * S_ij, row-major [N, MAS_MAX_QUERY_TOKENS] with columns >= L_r left untouched (tests only). */
 int mas_crossmodal(const mas_plan* plan, const void* X, const void* Q, float* rel /*[N]*/, float* S_opt, mas_stream_t stream);

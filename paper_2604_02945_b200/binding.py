@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_forward_host_async", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads", "mas_plan_n_frames", "mas_spatial_pool", "mas_merge_dropped",
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_forward_host_async", "mas_score", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads", "mas_plan_n_frames", "mas_spatial_pool", "mas_merge_dropped",
            "mas_gather_residual"]
 
 
@@ -95,6 +95,8 @@ def _load():
     lib.mas_forward_host.argtypes = [vp, vp, vp, vp, vp, C.POINTER(mas_outputs), C.POINTER(mas_outputs), vp]
     lib.mas_forward_host_async.argtypes = [vp, vp, vp, vp, vp, C.POINTER(mas_outputs), C.POINTER(mas_outputs), vp]
     lib.mas_forward_host_async.restype = C.c_int
+    lib.mas_score.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.mas_score.restype = C.c_int
     lib.mas_plan_set_inline_query_norms.restype = C.c_int
     lib.mas_plan_set_inline_query_norms.argtypes = [vp, i32]
     lib.mas_draft_entropy_workspace_bytes.argtypes = [i64, i64, C.POINTER(C.c_size_t)]
@@ -308,6 +310,12 @@ class Plan:
         Y = torch.zeros((max(cap, 1), self.d), dtype=X.dtype, device=self.device)
         _check(lib.mas_gather_residual(self._h, _ptr(X), _ptr(kept_idx), _ptr(kept_off), _ptr(Y), cap, _stream_ptr(stream)), "mas_gather_residual")
         return Y
+
+    def score(self, X, Q, want_gamma=True, out=None, stream=None):
+        """a0-a3 in one pass: (s, gamma or None, rel).  `out` = (s, gamma, rel) buffers to reuse."""
+        s, g, r = out if out is not None else (self._f32(), self._f32() if want_gamma else None, self._f32())
+        _check(lib.mas_score(self._h, _ptr(X), _ptr(Q), _ptr(s), _ptr(g) if want_gamma else None, _ptr(r), _stream_ptr(stream)), "mas_score")
+        return s, (g if want_gamma else None), r
 
     def crossmodal(self, X, Q, want_S=False, stream=None):
         rel = self._f32()

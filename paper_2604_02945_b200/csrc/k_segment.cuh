@@ -482,6 +482,23 @@ __global__ void __launch_bounds__(256) k_gather(const char* __restrict__ X, char
   }
 }
 
+// mas_score on the tcgen05 path: gamma = sqrt(D) / (|x_t| + |x_{t-1}|) from the score kernel's sqrt(D) and s (the same
+// arithmetic as k_segment's in-place finish); key-frame rows 1, single-frame segments 0
+__global__ void __launch_bounds__(256) k_gamma_finish(const DevSeg* __restrict__ segs, const DevTile* __restrict__ tiles,
+                                                      const float* __restrict__ s, float* __restrict__ gamma, float sqrt_d) {
+  const DevTile tile = tiles[blockIdx.x];
+  const DevSeg seg = segs[tile.seg];
+  for (int r = threadIdx.x; r < tile.n_rows; r += blockDim.x) {
+    const int64_t row = (int64_t)tile.row_start + r;
+    float gi = 0.f;
+    if (seg.n_frames > 1) {
+      if (row - seg.row0 < seg.n_patches) gi = 1.0f;
+      else { const float den = (s[row] + s[row - seg.n_patches]) * sqrt_d; gi = den > 0.f ? gamma[row] / den : 0.f; }
+    }
+    gamma[row] = gi;
+  }
+}
+
 // staged mas_spatial second phase: m_spatial from s (per-segment standardise + sigmoid, Eq. 3)
 __global__ void __launch_bounds__(kSegThreads) k_spatial_finish(const DevSeg* segs, DevParams p, const float* s, float* m_spatial) {
   __shared__ SegSmem sm;

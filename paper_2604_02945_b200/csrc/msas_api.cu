@@ -489,6 +489,32 @@ extern "C" int mas_crossmodal(const mas_plan* p, const void* X, const void* Q, f
   return launch_score_mma(p, X, Q, nullptr, nullptr, rel ? rel : p->at<float>(p->lay.rel), S_opt, st);
 }
 
+// a0-a3 in one pass (the score stage of mas_forward on its own): s, gamma, rel
+extern "C" int mas_score(const mas_plan* p, const void* X, const void* Q, float* s, float* gamma, float* rel, mas_stream_t stream) {
+  if (!p || !X || !Q || !s || !rel) return MAS_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(Q)) return MAS_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc;
+  if (p->tc.enabled) {
+    float* gb = gamma ? gamma : p->at<float>(p->lay.gamma);
+    unsigned long long* qr = p->at<unsigned long long>(p->lay.counter) + 8;
+    rc = p->tc_inline_qnorm ? tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), s, gb, rel, qr, p->N, p->nQ, p->d, true, nullptr, nullptr, nullptr, st) : 1;
+    if (rc == 1) {
+      (void)cudaGetLastError();
+      if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
+      rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), s, gb, rel, qr, p->N, p->nQ, p->d, false, nullptr, nullptr, nullptr, st);
+    }
+    if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
+    if (gamma) {
+      k_gamma_finish<<<p->n_tiles, 256, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->at<DevTile>(p->lay.tiles), s, gamma, sqrtf((float)p->d));
+      CK(cudaGetLastError());
+    }
+    return MAS_OK;
+  }
+  if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
+  return launch_score_mma(p, X, Q, s, gamma, rel, nullptr, st);
+}
+
 extern "C" int mas_fuse(const mas_plan* p, const float* s, const float* gamma, const float* rel, float* m_spatial, float* mas_tok,
                         mas_segment_out* seg_out, mas_stream_t stream) {
   if (!p || !s || !gamma || !rel || !mas_tok) return MAS_ERR_INVALID_ARG;

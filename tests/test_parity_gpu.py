@@ -82,6 +82,22 @@ def test_staged_scores(B, w):
     plan.close()
 
 
+@pytest.mark.parametrize("w", small_workloads(), ids=IDS)
+def test_score_one_pass(B, w):
+    """mas_score = the score stage of mas_forward on its own: gamma and rel identical to the fused call's, s against the oracle."""
+    segs, n = O.make_segments(w.segments)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    s, g, r = plan.score(X, Q)
+    s2, g2, r2 = plan.score(X, Q, want_gamma=False)
+    o = plan.forward(X, Q)
+    torch.cuda.synchronize()
+    assert g2 is None and torch.equal(s, s2) and torch.equal(r, r2)
+    assert torch.equal(g, o["gamma"]) and torch.equal(r, o["rel"])
+    P.assert_close(s.cpu().numpy(), O.rms(segs, w.X), "s")
+    plan.close()
+
+
 @pytest.mark.parametrize("mode", [0, 1])
 def test_staged_fuse_and_select_on_shared_scalars(B, mode):
     """mas_fuse / mas_select_compact in isolation: both sides get the same fp32 scalars, selection must be bit-exact."""
