@@ -36,7 +36,8 @@ template <int DT>
 __global__ void __launch_bounds__(256) k_qprep(const void* __restrict__ Q, float* __restrict__ qinv, int64_t n_q, int d) {
   const int lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
-  pdl_launch_dependents();   // the score kernel may start streaming X; its epilogue waits for this grid before reading qinv
+  pdl_launch_dependents();   // the score kernel's CTAs may be scheduled; they wait for this grid before touching global memory
+  pdl_wait();                // (launched behind the previous call's last kernel: that one may still read what we are about to write)
   if (row >= n_q) return;
   float acc = 0.f;
   if (DT == 1) {

@@ -302,6 +302,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = ctrl->tmem_base;
+  pdl_wait();   // plain (non-cooperative) launches are chained behind k_qprep: the set-up above overlaps its tail
 
   if (is_xprod || is_qprod) {
     // ===================================================================== TMA producers (one thread each)
@@ -849,7 +850,7 @@ struct TcHeads { float* part; float* m; float bias, tau; };   // NEXT-2 riding t
 // `hf` (NULL = off): NEXT-2, Rm = the head weight rows; same requirement; sig is ignored then.
 inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, float* qinv, float* s, float* dnorm, float* rel,
                            unsigned long long* q_ready, int64_t N, int64_t nQ, int d, bool inline_qprep, const void* Rm, unsigned long long* sig,
-                           const TcHeads* hf, cudaStream_t st) {
+                           const TcHeads* hf, cudaStream_t st, bool pdl_in = false) {
   TcMaps maps;
   for (int k = 0; k < 16; ++k)
     if (!tc_make_map(&maps.x[k], X, N, d, 16 * (k + 1))) return -1;
@@ -872,7 +873,7 @@ inline int tc_launch_score(const TcSchedule& sc, const void* X, const void* Q, f
 #endif
   if (!inline_qprep) {   // qinv is already there: no CTA waits on another one, a plain launch will do
     p.Q = nullptr;
-    if (launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, false, maps, p) != cudaSuccess) return -1;
+    if (launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl_in, maps, p) != cudaSuccess) return -1;
   } else {   // cooperative launch: the query-norm prologue makes the CTAs wait on one another once, so all must be resident
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)sc.n_ctas); cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)sc.smem_bytes; cfg.stream = st;

@@ -363,11 +363,10 @@ extern "C" int32_t mas_score_schedule(const mas_segment* h_segs, int32_t n_segs,
 // ------------------------------------------------------------------------------------------------ launches
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-static int launch_qprep(const mas_plan* p, const void* Q, cudaStream_t st) {
+static int launch_qprep(const mas_plan* p, const void* Q, cudaStream_t st, bool pdl = false) {
   const unsigned grid = (unsigned)((p->nQ + 7) / 8);
-  if (p->dtype == MAS_BF16) k_qprep<1><<<grid, 256, 0, st>>>(Q, p->at<float>(p->lay.qinv), p->nQ, p->d);
-  else k_qprep<0><<<grid, 256, 0, st>>>(Q, p->at<float>(p->lay.qinv), p->nQ, p->d);
-  CK(cudaGetLastError());
+  if (p->dtype == MAS_BF16) CK(launch_k(k_qprep<1>, dim3(grid), dim3(256), 0, st, pdl, Q, p->at<float>(p->lay.qinv), p->nQ, p->d));
+  else CK(launch_k(k_qprep<0>, dim3(grid), dim3(256), 0, st, pdl, Q, p->at<float>(p->lay.qinv), p->nQ, p->d));
   return MAS_OK;
 }
 
@@ -671,9 +670,9 @@ static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* 
   const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
   const TcSchedule& sc = (Rm != nullptr || hf != nullptr) ? p->tcx : p->tc;
   if (p->tc.enabled && !p->tc_inline_qnorm) {
-    if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
+    if ((rc = launch_qprep(p, Q, st, pdl)) != MAS_OK) return rc;
     rc = tc_launch_score(sc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, false, Rm, sig, hf, st);
+                         p->nQ, p->d, false, Rm, sig, hf, st, pdl);
     if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
   } else if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
