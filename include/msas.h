@@ -278,10 +278,17 @@ int mas_plan_set_inline_query_norms(mas_plan* plan, int32_t on);
 
 /* ---- introspection (host only, no CUDA call): the tile schedule mas_plan_create would build for the tcgen05 score
  * kernel on a device with `sm_count` SMs ("persistent CTAs over a host-built tile table; a tile
- * never straddles a segment").  Writes up to `cap_tiles` records of 8 int32 each
- * {cta, row_start, n_rows, q_row0, L, prev_delta, key_rows, 0} in per-CTA order and returns the number of tiles the
- * schedule has (which may exceed cap_tiles), 0 if the shape does not take the fast path (fp32, d % 64 != 0), or a
- * negative status (-MAS_ERR_*) for invalid descriptors.  Used by the CPU tests to check coverage and balance. */
+ * never straddles a segment").  A tile is up to 8 row blocks of one segment that share the request's query rows and are
+ * swept K-chunk by K-chunk.  Writes up to `cap_tiles` records of 12 int32 each, in per-CTA order:
+ *   {cta, row0, n_rows, n_blocks, stride, mode, prev, halo, q_row0, L, seg, part0}
+ *   mode 0 (single-frame segment): the tile scores rows [row0, row0 + n_rows) in blocks of 128 (stride = 128);
+ *   mode 1 (frames of P >= 64 rows): block b scores rows [row0 + b * stride, + n_rows), stride = prev = P, i.e. the same
+ *          n_rows <= 128 patch rows in n_blocks consecutive frames; halo = 1 if the frame before block 0 is read as well;
+ *   mode 2 (frames of P < 64 rows): the tile loads rows [row0, row0 + n_rows) in overlapping 128-row windows
+ *          (stride = 128 - P, prev = P) and scores rows [row0 + halo, row0 + n_rows), halo in {0, P}.
+ * Returns the number of tiles the schedule has (which may exceed cap_tiles), 0 if the shape does not take the fast path
+ * (fp32, d % 64 != 0), or a negative status (-MAS_ERR_*) for invalid descriptors.  Used by the CPU tests to check
+ * coverage and balance. */
 int32_t mas_score_schedule(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
                            int32_t d, int32_t dtype, int32_t sm_count, int32_t* out_tiles, int32_t cap_tiles);
 

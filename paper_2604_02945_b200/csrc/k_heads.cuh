@@ -115,8 +115,8 @@ struct HeadsArgs {
   const int32_t* req_seg_off;
   int n_segs, n_requests, tile_rows, hidden;
   DevParams prm;
-  const float* part;      // [slots, 64] per-tile partials: generic tiles (k_heads_proj) or 2 halves per tcgen05 tile (k_score_tc)
-  const int32_t* slot_rank;   // NULL: the segment's slots are its generic tiles; else [n_segs + 1] first tile rank per segment (x 2 halves)
+  const float* part;      // [slots, 64] partial column sums: one slot per generic tile (k_heads_proj) or per block of a tcgen05 tile (k_score_tc)
+  const int32_t* slot_rank;   // NULL: the segment's slots are its generic tiles; else [n_segs + 1] first slot of every segment
   const float* cq;        // [n_requests, kHeadSlabs, 64] from k_heads_q
   const float* gamma;     // [N] (may be NULL when no segment is temporal)
   const float* b1;        // [64]
@@ -137,8 +137,8 @@ __global__ void __launch_bounds__(1024) k_heads_finish(HeadsArgs a) {
   const int sidx = blockIdx.x;
   const DevSeg seg = a.segs[sidx];
   const int n = seg.n_rows;
-  const int slot_lo = a.slot_rank ? 2 * a.slot_rank[sidx] : seg.tile0;
-  const int slot_hi = a.slot_rank ? 2 * a.slot_rank[sidx + 1] : seg.tile0 + (n + a.tile_rows - 1) / a.tile_rows;
+  const int slot_lo = a.slot_rank ? a.slot_rank[sidx] : seg.tile0;
+  const int slot_hi = a.slot_rank ? a.slot_rank[sidx + 1] : seg.tile0 + (n + a.tile_rows - 1) / a.tile_rows;
   {   // column c = tid % 64; the four thread groups take every fourth slot, four loads in flight each: a fixed summation tree
     const int c = tid & 63, grp = tid >> 6;
     double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;

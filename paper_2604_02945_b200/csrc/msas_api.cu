@@ -50,7 +50,9 @@ struct mas_plan {
   size_t pinned_bytes = 0;
   int sm_count = 148;
   TcSchedule tc{};            // tcgen05 fast-path schedule (tc.enabled == false -> generic kernels)
-  TcSchedule tcx{};           // the same without tall tiles (their accumulator halves are 64 columns apart), for mas_forward_lsh / mas_forward_heads
+  TcSchedule tcx{};           // the schedule of the calls that append 64 B rows (mas_forward_lsh / mas_forward_heads; needs every L <= 64)
+  mutable TcMapCache tc_maps; // tensor maps of the last few (X, Q, R) pointer sets (a plan is used by one host thread at a time)
+  mutable bool tc_coop_ok = true;   // false once a cooperative launch was refused on this device: query norms get a launch of their own
   mutable std::vector<cudaEvent_t> prof_ev;   // profiling ring: 4 events per slot
   mutable int64_t prof_calls = 0;
   int32_t prof_slots = 0;
@@ -135,7 +137,7 @@ static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_of
   return MAS_OK;
 }
 
-static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes, size_t tc_tiles_max,
+static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes, size_t tc_parts_max,
                           int64_t n_frames) {
   Layout l{};
   size_t o = 0;
@@ -144,8 +146,8 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.tiles = take(sizeof(DevTile) * n_tiles);
   l.req = take(sizeof(int32_t) * (n_req + 1));
   l.tc_sched = take(tc_bytes);
-  l.tc_sched_x = take(tc_bytes);   // without tall tiles: the schedule of the calls that add 64 B rows (NEXT-1, NEXT-2)
-  l.tc_segrank = take(sizeof(int32_t) * (n_segs + 1));   // first tile rank of every segment (TcTile::rank), NEXT-2
+  l.tc_sched_x = take(tc_bytes);   // the schedule of the calls that add 64 B rows (NEXT-1, NEXT-2)
+  l.tc_segrank = take(sizeof(int32_t) * (n_segs + 1));   // first partial slot of every segment (TcTile::part0), NEXT-2
   l.frames = take(sizeof(DevFrame) * (size_t)n_frames);   // NEXT-3: first row and patch count of every frame
   l.tables_end = o;
   l.qinv = take(sizeof(float) * nQ);
@@ -158,7 +160,7 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.nkept = take(sizeof(int32_t) * n_segs);
   l.keptoff = take(sizeof(int64_t) * (n_segs + 1));
   l.counter = take(256);
-  l.heads_part = take(sizeof(float) * kHeadRows * std::max((size_t)n_tiles, 2 * tc_tiles_max));   // NEXT-2 scratch: per-tile column sums, per-request p-half
+  l.heads_part = take(sizeof(float) * kHeadRows * std::max((size_t)n_tiles, tc_parts_max));   // NEXT-2 scratch: per-tile / per-block column sums
   l.merge_part = take(sizeof(float) * 1024 * (size_t)kMergeCtas);   // NEXT-3 scratch: row-split partial sums of the merged tokens
   l.merge_cnt = take(sizeof(int32_t) * (size_t)kMergeCtas);
   l.gridw = take(sizeof(int32_t) * n_segs);   // NEXT-3 scratch: the caller's grid widths
@@ -179,20 +181,25 @@ extern "C" int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_seg
   int64_t N, nQ; int32_t nt, maxL;
   int st = validate(h_segs, n_segs, h_q_off, n_requests, d, dtype, nullptr, &N, &nQ, &nt, &maxL);
   if (st != MAS_OK) return st;
-  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs), tc_max_tiles(h_segs, n_segs), count_frames(h_segs, n_segs)).total;
+  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs), tc_max_parts(h_segs, n_segs), count_frames(h_segs, n_segs)).total;
   return MAS_OK;
 }
 
-static std::once_flag g_attr_once;
-static void set_kernel_attrs() {
-  cudaFuncSetAttribute(k_score_mma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
-  cudaFuncSetAttribute(k_score_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
-  cudaFuncSetAttribute(k_lsh_sig<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
-  cudaFuncSetAttribute(k_lsh_sig<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
-  cudaFuncSetAttribute(k_heads_proj<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
-  cudaFuncSetAttribute(k_heads_proj<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
-  tc_set_kernel_attrs();
-  (void)cudaGetLastError();
+// The opt-in to large dynamic shared memory applies to the device that is current when it is made: once per device.
+static std::mutex g_attr_mu;
+static bool g_attr_done[64] = {};
+static cudaError_t set_kernel_attrs(int dev) {
+  std::lock_guard<std::mutex> lk(g_attr_mu);
+  if (dev >= 0 && dev < 64 && g_attr_done[dev]) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(k_score_mma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_score_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_lsh_sig<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_lsh_sig<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_heads_proj<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_heads_proj<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
+  if (e == cudaSuccess) e = tc_set_kernel_attrs();
+  if (e == cudaSuccess && dev >= 0 && dev < 64) g_attr_done[dev] = true;
+  return e;
 }
 
 extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off,
@@ -206,7 +213,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
   if (st != MAS_OK) return st;
   if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0) return MAS_ERR_UNSUPPORTED;
   const size_t tc_bytes = tc_schedule_bytes(h_segs, n_segs);
-  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes, tc_max_tiles(h_segs, n_segs), count_frames(h_segs, n_segs));
+  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes, tc_max_parts(h_segs, n_segs), count_frames(h_segs, n_segs));
   if (workspace_bytes < lay.total) return MAS_ERR_WORKSPACE;
 
   mas_plan* p = new (std::nothrow) mas_plan();
@@ -222,8 +229,8 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
   cudaError_t e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
   if (e == cudaSuccess) { p->pinned_bytes = lay.tables_end + 256; e = cudaHostAlloc(&p->pinned, p->pinned_bytes, cudaHostAllocDefault); }
-  if (e != cudaSuccess) { g_last_cuda = (int)e; (void)cudaGetLastError(); delete p; return MAS_ERR_CUDA; }
-  std::call_once(g_attr_once, set_kernel_attrs);
+  if (e == cudaSuccess) e = set_kernel_attrs(dev);
+  if (e != cudaSuccess) { g_last_cuda = (int)e; (void)cudaGetLastError(); if (p->pinned) cudaFreeHost(p->pinned); delete p; return MAS_ERR_CUDA; }
 
   char* h = static_cast<char*>(p->pinned);
   std::memset(h, 0, p->pinned_bytes);
@@ -281,16 +288,12 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     p->seg_threads = slice <= 1024 ? 256 : slice <= 2048 ? 512 : kSegThreads;
   }
   tc_build_schedule(p->tc, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched, p->ws + lay.tc_sched);
-  tc_build_schedule(p->tcx, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched_x, p->ws + lay.tc_sched_x, false);
-  if (p->tcx.enabled) {   // per-segment range of tile ranks (slots of the learned-head partials)
+  tc_build_schedule(p->tcx, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched_x, p->ws + lay.tc_sched_x, true);
+  if (p->tcx.enabled) {   // per-segment range of partial slots (one per block of every tile; a segment's slots are contiguous)
     const TcTile* tt = reinterpret_cast<const TcTile*>(h + lay.tc_sched_x);
     int32_t* sr = reinterpret_cast<int32_t*>(h + lay.tc_segrank);
     std::vector<int32_t> cnt(n_segs + 1, 0);
-    for (int i = 0; i < p->tcx.n_tiles; ++i) {
-      int32_t lo = 0, hi = n_segs - 1;   // segment holding row_start (segments tile [0, N) in order)
-      while (lo < hi) { const int32_t mid = (lo + hi + 1) / 2; if (h_segs[mid].row0 <= tt[i].row_start) lo = mid; else hi = mid - 1; }
-      ++cnt[lo + 1];
-    }
+    for (int i = 0; i < p->tcx.n_tiles; ++i) cnt[tt[i].seg + 1] += tt[i].n_blocks;
     sr[0] = 0;
     for (int32_t k = 0; k < n_segs; ++k) sr[k + 1] = sr[k] + cnt[k + 1];
   }
@@ -354,8 +357,9 @@ extern "C" int32_t mas_score_schedule(const mas_segment* h_segs, int32_t n_segs,
   const int32_t* off = reinterpret_cast<const int32_t*>(buf.data() + (size_t)sc.n_tiles * sizeof(TcTile));
   for (int c = 0; c < sc.n_ctas; ++c)
     for (int i = off[c]; i < off[c + 1] && i < cap_tiles; ++i) {
-      int32_t* o = out_tiles + (size_t)i * 8;
-      o[0] = c; o[1] = t[i].row_start; o[2] = t[i].n_rows; o[3] = t[i].q_row0; o[4] = t[i].L; o[5] = t[i].prev_delta; o[6] = t[i].key_rows; o[7] = 0;
+      int32_t* o = out_tiles + (size_t)i * 12;
+      o[0] = c; o[1] = t[i].row0; o[2] = t[i].n_rows; o[3] = t[i].n_blocks; o[4] = t[i].stride; o[5] = t[i].mode; o[6] = t[i].prev;
+      o[7] = t[i].halo; o[8] = t[i].q_row0; o[9] = t[i].L; o[10] = t[i].seg; o[11] = t[i].part0;
     }
   return sc.n_tiles;
 }
@@ -392,6 +396,26 @@ static int launch_score_mma(const mas_plan* p, const void* X, const void* Q, flo
   if (p->dtype == MAS_BF16) k_score_mma<1><<<p->n_tiles, 256, score_mma_smem_bytes(1), st>>>(a);
   else k_score_mma<0><<<p->n_tiles, 256, score_mma_smem_bytes(0), st>>>(a);
   CK(cudaGetLastError());
+  return MAS_OK;
+}
+
+// a0-a3 on the tcgen05 path.  The query norms ride the score kernel's prologue (one cooperative launch) unless the plan asks for,
+// or the device forces, a launch of their own (k_qprep, then the plain score launch chained behind it).
+static int launch_score_tc(const mas_plan* p, const TcSchedule& sc, const void* X, const void* Q, float* s, float* dnorm, float* rel,
+                           const void* Rm, unsigned long long* sig, const TcHeads* hf, cudaStream_t st, bool pdl) {
+  unsigned long long* qr = p->at<unsigned long long>(p->lay.counter) + 8;
+  float* qinv = p->at<float>(p->lay.qinv);
+  if (p->tc_inline_qnorm && p->tc_coop_ok) {
+    const cudaError_t e = tc_launch_score(sc, p->tc_maps, X, Q, qinv, s, dnorm, rel, qr, p->N, p->nQ, p->d, true, Rm, sig, hf, st);
+    if (e == cudaSuccess) return MAS_OK;
+    if (e != cudaErrorCooperativeLaunchTooLarge && e != cudaErrorNotSupported) { g_last_cuda = (int)e; (void)cudaGetLastError(); return MAS_ERR_CUDA; }
+    (void)cudaGetLastError();     // not all CTAs can be co-resident here (e.g. an MPS partition): remembered for the plan's lifetime
+    p->tc_coop_ok = false;
+  }
+  const bool chain = pdl && !(p->tc_inline_qnorm && !p->tc_coop_ok);
+  int rc = launch_qprep(p, Q, st, chain);
+  if (rc != MAS_OK) return rc;
+  CK(tc_launch_score(sc, p->tc_maps, X, Q, qinv, s, dnorm, rel, qr, p->N, p->nQ, p->d, false, Rm, sig, hf, st, chain));
   return MAS_OK;
 }
 
@@ -496,14 +520,7 @@ extern "C" int mas_score(const mas_plan* p, const void* X, const void* Q, float*
   int rc;
   if (p->tc.enabled) {
     float* gb = gamma ? gamma : p->at<float>(p->lay.gamma);
-    unsigned long long* qr = p->at<unsigned long long>(p->lay.counter) + 8;
-    rc = p->tc_inline_qnorm ? tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), s, gb, rel, qr, p->N, p->nQ, p->d, true, nullptr, nullptr, nullptr, st) : 1;
-    if (rc == 1) {
-      (void)cudaGetLastError();
-      if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
-      rc = tc_launch_score(p->tc, X, Q, p->at<float>(p->lay.qinv), s, gb, rel, qr, p->N, p->nQ, p->d, false, nullptr, nullptr, nullptr, st);
-    }
-    if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
+    if ((rc = launch_score_tc(p, p->tc, X, Q, s, gb, rel, nullptr, nullptr, nullptr, st, false)) != MAS_OK) return rc;
     if (gamma) {
       k_gamma_finish<<<p->n_tiles, 256, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->at<DevTile>(p->lay.tiles), s, gamma, sqrtf((float)p->d));
       CK(cudaGetLastError());
@@ -669,22 +686,9 @@ static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* 
   int rc;
   const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
   const TcSchedule& sc = (Rm != nullptr || hf != nullptr) ? p->tcx : p->tc;
-  if (p->tc.enabled && !p->tc_inline_qnorm) {
-    if ((rc = launch_qprep(p, Q, st, pdl)) != MAS_OK) return rc;
-    rc = tc_launch_score(sc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, false, Rm, sig, hf, st, pdl);
-    if (rc != 0) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
-  } else if (p->tc.enabled) {
+  if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
-    rc = tc_launch_score(sc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                         p->nQ, p->d, true, Rm, sig, hf, st);
-    if (rc == 1) {   // not all CTAs can be co-resident here (e.g. an MPS partition): query norms in their own launch
-      (void)cudaGetLastError();
-      if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
-      rc = tc_launch_score(sc, X, Q, p->at<float>(p->lay.qinv), sb, gb, rb, p->at<unsigned long long>(p->lay.counter) + 8, p->N,
-                           p->nQ, p->d, false, Rm, sig, hf, st);
-    }
-    if (rc == -1) { g_last_cuda = (int)cudaGetLastError(); return MAS_ERR_CUDA; }
+    if ((rc = launch_score_tc(p, sc, X, Q, sb, gb, rb, Rm, sig, hf, st, pdl)) != MAS_OK) return rc;
   } else {
     if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
     if ((rc = launch_score_mma(p, X, Q, sb, gb, rb, nullptr, st)) != MAS_OK) return rc;
