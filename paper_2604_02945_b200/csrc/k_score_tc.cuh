@@ -40,7 +40,7 @@ struct TcTile {            // 48 bytes
   int32_t row0;            // global row id of the first row block 0 loads
   int32_t n_rows;          // mode 1: rows of every block (<= 128); modes 0, 2: rows the tile loads in total (blocks of <= 128)
   int32_t n_blocks;        // 1..8 (<= TMEM accumulator slots)
-  int32_t stride;          // rows between the first rows of consecutive blocks (mode 0: 128, mode 1: P, mode 2: 128 - P)
+  int32_t stride;          // rows between the first rows of consecutive blocks (mode 0: the block height <= 128, mode 1: P, mode 2: 128 - P)
   int32_t mode;            // see above
   int32_t prev;            // P for modes 1 and 2, else 0
   int32_t halo;            // mode 1: 1 = a halo chunk (frame t0 - 1) precedes the blocks of every K-chunk;
@@ -52,17 +52,18 @@ struct TcTile {            // 48 bytes
   int32_t pad_;
 };
 
-constexpr int kTcThreads = 512;                      // 16 warps: TMA producer, MMA issuer, TMEM allocator, spare, 4 epilogue, 8 statistics
+constexpr int kTcThreads = 448;                      // 14 warps: 4 epilogue, 8 statistics, TMA producer, MMA issuer (144 registers per thread)
 constexpr int kTcAluWarps = 8;
-constexpr int kTcMaxBlocks = 8;
-constexpr int kTcXSlotBytes = 128 * 128;             // 128 rows x 64 bf16 columns
+constexpr int kTcWarpTma = 12, kTcWarpMma = 13;
+constexpr int kTcMaxBlocks = 10;                    // blocks per tile = TMEM accumulator slots (512 columns / pad16(L), at most 10)
+constexpr int kTcSliceBytes = 128 * 128;             // 128 rows x 64 bf16 columns: one K-slice of a block
 constexpr int kTcMaxXSlots = 12;
 constexpr int kTcCtrlBytes = 4096;
 constexpr int kTcStatBytes = 2 * kTcMaxBlocks * 128 * 2 * 4;   // [buffer][block][row][n2, D]
 constexpr int kTcSmemBytes = 227 * 1024;
 
 struct TcMaps {
-  CUtensorMap x[16];   // token rows: box = 8 * (i + 1) rows x 64 columns
+  CUtensorMap x[16];   // token rows as a 3-D tensor [d / 64 slices][N rows][64 columns]: box = kw slices x 8 * (i + 1) rows x 64 columns
   CUtensorMap q[3];    // query rows: box = 64 / 32 / 16 rows x 64 columns
   CUtensorMap r;       // riders: the 64 hash / head-weight rows R[64, d] (box = 64 rows x 64 columns)
 };
@@ -70,9 +71,11 @@ struct TcMaps {
 struct TcSchedule {
   bool enabled = false;
   int n_ctas = 0, n_tiles = 0, n_parts = 0;
-  int nx = 0;              // X ring slots
-  int qslot_bytes = 0;     // bytes of one query-chunk slot (two slots)
-  int wslot = 0, ns_log2 = 0;   // TMEM: columns per accumulator slot, log2 of the slot count
+  int kw = 1;              // 64-column K-slices per chunk (2 where d % 128 == 0: half the barrier round trips per byte)
+  int nx = 0;              // X ring slots (kw * 16 KB each)
+  int qslot_bytes = 0;     // bytes of one query-chunk slot
+  int nq = 2;              // query-chunk slots (2..4: short tiles need several K-steps in flight)
+  int wslot = 0, ns = 0;        // TMEM: columns per accumulator slot (pad16 of the longest query block), number of slots
   int smem_bytes = 0;
   const TcTile* d_tiles = nullptr;
   const int32_t* d_cta_off = nullptr;
@@ -98,10 +101,12 @@ struct TcParams {
   float* rel;
   int d;
   int n_kchunks;
-  int nx, qslot_bytes, wslot, ns_log2;
+  int kw, nx, nq, qslot_bytes, wslot, ns;
 };
 
-__device__ __forceinline__ int tc_block_rows(const TcTile& t, int b) { return t.mode == 1 ? t.n_rows : min(128, t.n_rows - b * t.stride); }
+__device__ __forceinline__ int tc_block_rows(const TcTile& t, int b) {
+  return t.mode == 1 ? t.n_rows : min(t.mode == 0 ? t.stride : 128, t.n_rows - b * t.stride);
+}
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -127,9 +132,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}\n" ::"r"(bar), "r"(parity)
       : "memory");
 }
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
-               "l"(map), "r"(bar), "r"(c0), "r"(c1)
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
+               "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
                : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -191,7 +196,7 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int n) {
 struct TcCtrl {                      // lives at the (1024-aligned) start of dynamic shared memory
   uint64_t xfull[kTcMaxXSlots];      // TMA -> consumers           (1 arrival + transaction bytes)
   uint64_t xempty[kTcMaxXSlots];     // consumers -> TMA           (1 MMA commit + the statistics warps)
-  uint64_t qfull[2], qempty[2];      // the query-chunk double buffer: TMA -> MMA, MMA commit -> TMA
+  uint64_t qfull[4], qempty[4];      // the query-chunk ring: TMA -> MMA, MMA commit -> TMA
   uint64_t tfull[kTcMaxBlocks];      // accumulator slot: MMA commit -> epilogue
   uint64_t tempty[kTcMaxBlocks];     // epilogue (4 warps) -> MMA
   uint64_t sfull[2], sempty[2];      // row statistics of a tile: statistics warps -> epilogue (4 warps) -> statistics warps
@@ -200,6 +205,19 @@ struct TcCtrl {                      // lives at the (1024-aligned) start of dyn
   float hred[2][4][64];              // NEXT-2: per-warp column sums of the 64 head columns, double buffered
 };
 static_assert(sizeof(TcCtrl) <= kTcCtrlBytes, "control block too large");
+
+__device__ __forceinline__ bool elect_one() {   // one lane of a converged warp: lets the compiler keep the issuing code warp-uniform
+  uint32_t pred;
+  asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.b32 %0, 1, 0, p;\n}" : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr)); return v; }
+__device__ __forceinline__ void sts32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
 
 // one token row's half K-slice (4 x 16 bytes): sum of squares
 __device__ __forceinline__ void tc_sq4(const uint4 (&x)[4], uint64_t& a, uint64_t& b) {
@@ -221,38 +239,124 @@ __device__ __forceinline__ void tc_sq4_diff(const uint4 (&x)[4], const uint4 (&v
   }
 }
 
+// The statistics warps' sweep over one tile.  Thread = (block row `arow`, half `hh` of the row's eight 16-byte units); the
+// hardware 128-byte swizzle puts unit u of row r at unit u ^ (r & 7).  Ring position (xs, xph) is carried across tiles.
+struct TcAluCtx {
+  uint32_t xring, xslot, xfull0, xempty0, stat;   // shared-space addresses; stat = this lane's accumulator of block 0 in this tile's buffer
+  int nx, nk, lane, arow;
+  uint32_t hh;
+};
+__device__ __forceinline__ void tc_alu_load(uint32_t base, uint32_t ro, uint32_t uoff, uint32_t swz, uint4 (&x)[4]) {
+#pragma unroll
+  for (int u = 0; u < 4; ++u) x[u] = lds128(base + ro + (((uoff + (uint32_t)u) ^ swz) << 4));
+}
+__device__ __forceinline__ void tc_alu_release(const TcAluCtx& c, uint32_t& xs, uint32_t& xph) {
+  __syncwarp();
+  if (c.lane == 0) mbar_arrive(c.xempty0 + xs * 8u);
+  if (++xs == (uint32_t)c.nx) { xs = 0; xph ^= 1u; }
+}
+template <int KW>
+__device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_rows, int n_blocks, int stride, int prev, bool halo,
+                                            uint32_t& xs, uint32_t& xph) {
+  const uint32_t roff = (uint32_t)c.arow * 128u, sw = (uint32_t)(c.arow & 7);
+  const uint32_t uoff = c.hh << 2;
+  const int prow = c.arow - prev;                                        // mode 2: the previous frame's row in the same chunk
+  const uint32_t proff = (uint32_t)prow * 128u, psw = (uint32_t)(prow & 7);
+  const bool inchunk = mode == 2 && prow >= 0;
+  const int hcap = mode == 0 ? stride : 128;
+  for (int kc = 0; kc < c.nk; kc += KW) {
+    uint4 pv[KW][4];                  // this thread's K-slices of the previous frame's row (mode 1: carried from block to block)
+    bool have_prev = false;
+    if (halo) {
+      mbar_wait(c.xfull0 + xs * 8u, xph);
+      if (c.arow < n_rows) {
+        const uint32_t slice = (uint32_t)((n_rows + 7) >> 3) * 1024u;
+#pragma unroll
+        for (int j = 0; j < KW; ++j) tc_alu_load(c.xring + xs * c.xslot + (uint32_t)j * slice, roff, uoff, sw, pv[j]);
+      }
+      have_prev = true;
+      tc_alu_release(c, xs, xph);
+    }
+    for (int b = 0; b < n_blocks; ++b) {
+      const int hb = mode == 1 ? n_rows : min(hcap, n_rows - b * stride);
+      const uint32_t slice = (uint32_t)((hb + 7) >> 3) * 1024u;
+      const bool act = c.arow < hb;
+      uint64_t n2a = 0, n2b = 0, Da = 0, Db = 0;     // packed fp32 pairs, all zero bits = (0.f, 0.f)
+      uint4 x[KW][4];
+      mbar_wait(c.xfull0 + xs * 8u, xph);
+      if (act) {
+#pragma unroll
+        for (int j = 0; j < KW; ++j) {
+          const uint32_t base = c.xring + xs * c.xslot + (uint32_t)j * slice;
+          tc_alu_load(base, roff, uoff, sw, x[j]);
+          if (inchunk) tc_alu_load(base, proff, uoff, psw, pv[j]);
+        }
+      }
+      tc_alu_release(c, xs, xph);   // the slot is free as soon as its bytes are in registers
+      if (act) {
+        const bool diff = inchunk || (mode == 1 && have_prev);
+#pragma unroll
+        for (int j = 0; j < KW; ++j) {
+          if (diff) tc_sq4_diff(x[j], pv[j], n2a, n2b, Da, Db); else tc_sq4(x[j], n2a, n2b);
+          if (mode == 1) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) pv[j][u] = x[j][u];
+          }
+        }
+      }
+      have_prev = true;
+      // the chunk's partial sums of a row (two lanes) join block b's accumulators in shared memory
+      float n2 = sum_f32x2(n2a) + sum_f32x2(n2b), D = sum_f32x2(Da) + sum_f32x2(Db);
+      n2 += __shfl_xor_sync(0xffffffffu, n2, 1);
+      D += __shfl_xor_sync(0xffffffffu, D, 1);
+      if (act) {   // lane pair (row): the even lane keeps sum x^2, the odd lane sum (x - x_prev)^2
+        const float mine = c.hh ? D : n2;
+        const uint32_t a = c.stat + (uint32_t)b * 1024u;
+        sts32(a, kc == 0 ? mine : lds32(a) + mine);
+      }
+    }
+  }
+}
+
+template <int KW>   // 64-column K-slices per chunk
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   TcCtrl* ctrl = reinterpret_cast<TcCtrl*>(smem);
   float* stat = reinterpret_cast<float*>(smem + kTcCtrlBytes);
-  unsigned char* qring = smem + kTcCtrlBytes + kTcStatBytes;
-  unsigned char* xring = qring + 2 * p.qslot_bytes;
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t qring = sbase + kTcCtrlBytes + kTcStatBytes;
+  const uint32_t xring = qring + (uint32_t)p.nq * (uint32_t)p.qslot_bytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  // roles: warp 0 TMA producer, 1 MMA issuer, 2 TMEM allocation, 3 spare, 4-7 epilogue (TMEM lane quarter = warp % 4),
-  // 8-15 statistics: two statistics warps and one epilogue warp on every scheduler partition
+  // roles: warps 0-3 epilogue (TMEM lane quarter = warp % 4), 4-11 statistics, 12 TMA producer, 13 MMA issuer (+ TMEM allocation):
+  // two statistics warps and one epilogue warp on every scheduler partition
   const int tile_lo = p.cta_off[blockIdx.x], tile_hi = p.cta_off[blockIdx.x + 1];
   const int nk = p.n_kchunks;
   const int nx = p.nx;
+  constexpr int kw = KW;
+  const uint32_t xslot = (uint32_t)kw * (uint32_t)kTcSliceBytes;
   const bool rider = p.sig != nullptr || p.heads_part != nullptr;   // 64 more B rows after the query rows (hash rows or head weights)
-  const uint32_t ns_mask = (1u << p.ns_log2) - 1u;
+  const uint32_t ns = (uint32_t)p.ns;                    // accumulator slots, used round-robin block after block
+  const uint32_t xfull0 = smem_u32(&ctrl->xfull[0]), xempty0 = smem_u32(&ctrl->xempty[0]);
+  const uint32_t qfull0 = smem_u32(&ctrl->qfull[0]), qempty0 = smem_u32(&ctrl->qempty[0]);
+  const uint32_t tfull0 = smem_u32(&ctrl->tfull[0]), tempty0 = smem_u32(&ctrl->tempty[0]);
 
   pdl_launch_dependents();   // the segment kernel may be scheduled as SMs free up; it waits for this grid to complete
-  if (warp == 1 && lane == 0) {
-    for (int i = 0; i < kTcMaxXSlots; ++i) { mbar_init(smem_u32(&ctrl->xfull[i]), 1); mbar_init(smem_u32(&ctrl->xempty[i]), 1 + kTcAluWarps); }
+  if (warp == kTcWarpMma && lane == 0) {
+    for (int i = 0; i < kTcMaxXSlots; ++i) { mbar_init(xfull0 + 8u * i, 1); mbar_init(xempty0 + 8u * i, 1 + kTcAluWarps); }
+    for (int i = 0; i < 4; ++i) { mbar_init(qfull0 + 8u * i, 1); mbar_init(qempty0 + 8u * i, 1); }
     for (int i = 0; i < 2; ++i) {
-      mbar_init(smem_u32(&ctrl->qfull[i]), 1); mbar_init(smem_u32(&ctrl->qempty[i]), 1);
       mbar_init(smem_u32(&ctrl->sfull[i]), kTcAluWarps); mbar_init(smem_u32(&ctrl->sempty[i]), 4);
     }
-    for (int i = 0; i < kTcMaxBlocks; ++i) { mbar_init(smem_u32(&ctrl->tfull[i]), 1); mbar_init(smem_u32(&ctrl->tempty[i]), 4); }
+    for (int i = 0; i < kTcMaxBlocks; ++i) { mbar_init(tfull0 + 8u * i, 1); mbar_init(tempty0 + 8u * i, 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 2) {   // TMEM: all 512 columns (one CTA per SM): 4 or 8 accumulator slots of 128 / 64 columns
+  if (warp == kTcWarpMma) {   // TMEM: all 512 columns (one CTA per SM): 4 to 10 accumulator slots of pad16(L) columns
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctrl->tmem_base)), "r"(512) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  if (warp == 0 && lane == 0) {
+  if (warp == kTcWarpTma && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.x[15]) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.q[0]) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.q[2]) : "memory");
@@ -263,86 +367,96 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   const uint32_t tmem_base = ctrl->tmem_base;
   pdl_wait();   // plain (non-cooperative) launches are chained behind k_qprep: the set-up above overlaps its tail
 
-  if (warp == 0) {
-    // ===================================================================== TMA producer (one thread)
-    if (lane == 0) {
-      uint32_t xs = 0, xph = 0, qk = 0;
-      for (int t = tile_lo; t < tile_hi; ++t) {
-        const TcTile tile = p.tiles[t];
-        const int nqu = (tile.L + 15) >> 4;
-        const uint32_t qbytes = (uint32_t)(nqu + (rider ? 4 : 0)) * 2048u;
-        const int b_lo = (tile.mode == 1 && tile.halo) ? -1 : 0;      // block -1 = the halo chunk (frame t0 - 1)
-        for (int kc = 0; kc < nk; ++kc) {
-          const int c0 = kc * 64;
-          {   // the request's query rows of this K-chunk (+ the rider rows): one B tile
-            const uint32_t qs = qk & 1u;
-            mbar_wait(smem_u32(&ctrl->qempty[qs]), ((qk >> 1) & 1u) ^ 1u);
-            const uint32_t bar = smem_u32(&ctrl->qfull[qs]);
+  if (warp == kTcWarpTma) {
+    // ===================================================================== TMA producer (the whole warp walks the list, one lane issues)
+    uint32_t xs = 0, xph = 0, qs = 0, qph = 0;
+    for (int t = tile_lo; t < tile_hi; ++t) {
+      const TcTile tile = p.tiles[t];
+      const int nqu = (tile.L + 15) >> 4;
+      const uint32_t qbytes = (uint32_t)(nqu + (rider ? 4 : 0)) * 2048u * (uint32_t)kw;
+      const int b_lo = (tile.mode == 1 && tile.halo) ? -1 : 0;      // block -1 = the halo chunk (frame t0 - 1)
+      for (int kc = 0; kc < nk; kc += kw) {
+        {   // the request's query rows of these K-slices (+ the rider rows): one B tile per slice
+          mbar_wait(qempty0 + 8u * qs, qph ^ 1u);
+          if (elect_one()) {
+            const uint32_t bar = qfull0 + 8u * qs;
             mbar_expect_tx(bar, qbytes);
-            uint32_t sq = smem_u32(qring + qs * (uint32_t)p.qslot_bytes);
-            int qr = tile.q_row0;
-            for (int i = 0; i < (nqu >> 2); ++i) { tma_load_2d(sq, &maps.q[0], bar, c0, qr); sq += 8192; qr += 64; }
-            if (nqu & 2) { tma_load_2d(sq, &maps.q[1], bar, c0, qr); sq += 4096; qr += 32; }
-            if (nqu & 1) { tma_load_2d(sq, &maps.q[2], bar, c0, qr); sq += 2048; }
-            if (rider) tma_load_2d(sq, &maps.r, bar, c0, 0);
-            ++qk;
-          }
-          for (int b = b_lo; b < tile.n_blocks; ++b) {
-            const int h = b < 0 ? tile.n_rows : tc_block_rows(tile, b);
-            const int h8 = (h + 7) >> 3;                               // box height in 8-row swizzle atoms
-            mbar_wait(smem_u32(&ctrl->xempty[xs]), xph ^ 1u);
-            const uint32_t bar = smem_u32(&ctrl->xfull[xs]);
-            mbar_expect_tx(bar, (uint32_t)h8 * 1024u);
-            // rows past the end of X are zero-filled by the TMA unit; rows past the block are never used
-            tma_load_2d(smem_u32(xring + xs * (uint32_t)kTcXSlotBytes), &maps.x[h8 - 1], bar, c0, tile.row0 + b * tile.stride);
-            if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
-          }
-        }
-      }
-    }
-  } else if (warp == 1) {
-    // ===================================================================== MMA issuer (one thread)
-    if (lane == 0) {
-      uint32_t xs = 0, xph = 0, qk = 0, g = 0;
-      for (int t = tile_lo; t < tile_hi; ++t) {
-        const TcTile tile = p.tiles[t];
-        const int nqb = ((tile.L + 15) >> 4) + (rider ? 4 : 0);
-        const uint32_t idesc = umma_idesc_bf16(nqb << 4);   // N = pad16(L) (+ 64 rider rows)
-        const bool halo = tile.mode == 1 && tile.halo;
-        for (int kc = 0; kc < nk; ++kc) {
-          const uint32_t qs = qk & 1u;
-          mbar_wait(smem_u32(&ctrl->qfull[qs]), (qk >> 1) & 1u);
-          tc_fence_after();
-          const uint64_t bdesc = umma_desc_sw128(smem_u32(qring + qs * (uint32_t)p.qslot_bytes));
-          if (halo) {   // not an MMA operand: release our share of the slot (behind the MMAs issued so far, which keeps the order)
-            tc_commit(smem_u32(&ctrl->xempty[xs]));
-            if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
-          }
-          for (int b = 0; b < tile.n_blocks; ++b) {
-            const uint32_t ts = (g + (uint32_t)b) & ns_mask;
-            if (kc == 0) {   // the accumulator slot must have been drained by the epilogue of its previous use
-              mbar_wait(smem_u32(&ctrl->tempty[ts]), (((g + (uint32_t)b) >> p.ns_log2) & 1u) ^ 1u);
-              tc_fence_after();
+            uint32_t sq = qring + qs * (uint32_t)p.qslot_bytes;
+            for (int j = 0; j < kw; ++j) {
+              int qr = tile.q_row0;
+              for (int i = 0; i < (nqu >> 2); ++i) { tma_load_3d(sq, &maps.q[0], bar, 0, qr, kc + j); sq += 8192; qr += 64; }
+              if (nqu & 2) { tma_load_3d(sq, &maps.q[1], bar, 0, qr, kc + j); sq += 4096; qr += 32; }
+              if (nqu & 1) { tma_load_3d(sq, &maps.q[2], bar, 0, qr, kc + j); sq += 2048; }
+              if (rider) { tma_load_3d(sq, &maps.r, bar, 0, 0, kc + j); sq += 8192; }
             }
-            mbar_wait(smem_u32(&ctrl->xfull[xs]), xph);
-            tc_fence_after();
-            // M = 128: rows past the block read whatever the slot held before (their accumulator rows are never used)
-            const uint64_t adesc = umma_desc_sw128(smem_u32(xring + xs * (uint32_t)kTcXSlotBytes));
-            const uint32_t d_tmem = tmem_base + ts * (uint32_t)p.wslot;
-#pragma unroll
-            for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
-              tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(kc | k));
-            tc_commit(smem_u32(&ctrl->xempty[xs]));
-            if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
           }
-          tc_commit(smem_u32(&ctrl->qempty[qs]));
-          ++qk;
+          if (++qs == (uint32_t)p.nq) { qs = 0; qph ^= 1u; }
         }
-        for (int b = 0; b < tile.n_blocks; ++b) tc_commit(smem_u32(&ctrl->tfull[(g + (uint32_t)b) & ns_mask]));
-        g += (uint32_t)tile.n_blocks;
+        for (int b = b_lo; b < tile.n_blocks; ++b) {
+          const int h = b < 0 ? tile.n_rows : tc_block_rows(tile, b);
+          const int h8 = (h + 7) >> 3;                               // box height in 8-row swizzle atoms
+          mbar_wait(xempty0 + 8u * xs, xph ^ 1u);
+          if (elect_one()) {
+            const uint32_t bar = xfull0 + 8u * xs;
+            mbar_expect_tx(bar, (uint32_t)h8 * 1024u * (uint32_t)kw);
+            // one box = kw slices of h8 * 8 rows, slice after slice; rows past the end of X are zero-filled by the TMA unit,
+            // rows past the block are never used
+            tma_load_3d(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc);
+          }
+          if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
+        }
       }
     }
-  } else if (warp >= 4 && warp < 8) {
+  } else if (warp == kTcWarpMma) {
+    // ===================================================================== MMA issuer (the whole warp walks the list, one lane issues)
+    uint32_t xs = 0, xph = 0, qs = 0, qph = 0, ts0 = 0, tp0 = 0;   // ts0 / tp0: accumulator slot and phase of the tile's block 0
+    for (int t = tile_lo; t < tile_hi; ++t) {
+      const TcTile tile = p.tiles[t];
+      const int nqb = ((tile.L + 15) >> 4) + (rider ? 4 : 0);
+      const uint32_t idesc = umma_idesc_bf16(nqb << 4);   // N = pad16(L) (+ 64 rider rows)
+      const bool halo = tile.mode == 1 && tile.halo;
+      for (int kc = 0; kc < nk; kc += kw) {
+        mbar_wait(qfull0 + 8u * qs, qph);
+        tc_fence_after();
+        const uint32_t qbase = qring + qs * (uint32_t)p.qslot_bytes;
+        if (halo) {   // not an MMA operand: release our share of the slot (behind the MMAs issued so far, which keeps the order)
+          if (elect_one()) tc_commit(xempty0 + 8u * xs);
+          if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
+        }
+        for (int b = 0; b < tile.n_blocks; ++b) {
+          uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
+          if (ts >= ns) { ts -= ns; tp ^= 1u; }
+          if (kc == 0) {   // the accumulator slot must have been drained by the epilogue of its previous use
+            mbar_wait(tempty0 + 8u * ts, tp ^ 1u);
+            tc_fence_after();
+          }
+          mbar_wait(xfull0 + 8u * xs, xph);
+          tc_fence_after();
+          const uint32_t slice = (uint32_t)((tc_block_rows(tile, b) + 7) >> 3) * 1024u;   // bytes between the K-slices of this chunk
+          const uint32_t xbase = xring + xs * xslot;
+          const uint32_t d_tmem = tmem_base + ts * (uint32_t)p.wslot;
+          if (elect_one()) {
+            for (int j = 0; j < kw; ++j) {
+              // M = 128: rows past the block read whatever follows in the slot (their accumulator rows are never used)
+              const uint64_t adesc = umma_desc_sw128(xbase + (uint32_t)j * slice);
+              const uint64_t bdesc = umma_desc_sw128(qbase + (uint32_t)j * (uint32_t)nqb * 2048u);
+#pragma unroll
+              for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
+                tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(kc | j | k));
+            }
+            tc_commit(xempty0 + 8u * xs);
+          }
+          if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
+        }
+        if (elect_one()) tc_commit(qempty0 + 8u * qs);
+        if (++qs == (uint32_t)p.nq) { qs = 0; qph ^= 1u; }
+      }
+      if (elect_one())
+        for (int b = 0; b < tile.n_blocks; ++b) { const uint32_t ts = ts0 + (uint32_t)b; tc_commit(tfull0 + 8u * (ts >= ns ? ts - ns : ts)); }
+      ts0 += (uint32_t)tile.n_blocks;
+      if (ts0 >= ns) { ts0 -= ns; tp0 ^= 1u; }
+    }
+  } else if (warp < 4) {
     // ===================================================================== epilogue: one accumulator row per thread
     const int q = warp & 3;                  // TMEM lane quarter this warp may access (warp % 4)
     const int r = q * 32 + lane;             // block row
@@ -369,7 +483,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       if (q == 0 && lane == 0) atomicAdd(p.q_ready, 1ull);
     }
     bool q_ok = p.Q == nullptr;
-    uint32_t g = 0, hcnt = 0;
+    uint32_t ts0 = 0, tp0 = 0, hcnt = 0;
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
@@ -378,9 +492,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const float* qinv = p.qinv + tile.q_row0;
       const float2* st2 = reinterpret_cast<const float2*>(stat) + (size_t)buf * kTcMaxBlocks * 128;
       for (int b = 0; b < tile.n_blocks; ++b) {
-        const uint32_t ts = (g + (uint32_t)b) & ns_mask;
+        uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
+        if (ts >= ns) { ts -= ns; tp ^= 1u; }
         const uint32_t tcol = tmem_base + ts * (uint32_t)p.wslot + ((uint32_t)(q * 32) << 16);
-        mbar_wait(smem_u32(&ctrl->tfull[ts]), ((g + (uint32_t)b) >> p.ns_log2) & 1u);
+        mbar_wait(smem_u32(&ctrl->tfull[ts]), tp);
         tc_fence_after();
         if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
           unsigned long long seen;
@@ -467,74 +582,24 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->sempty[buf]));
-      g += (uint32_t)tile.n_blocks;
+      ts0 += (uint32_t)tile.n_blocks;
+      if (ts0 >= ns) { ts0 -= ns; tp0 ^= 1u; }
     }
-  } else if (warp >= 8) {
+  } else {
     // ===================================================================== CUDA-core statistics: two threads per block row
-    const int arow = ((warp - 8) << 4) + (lane >> 1);     // block row
-    const uint32_t hh = (uint32_t)lane & 1u;              // which half of the row's eight 16-byte units
-    // hardware 128-byte swizzle: 16-byte unit u of row r sits at unit u ^ (r & 7)
-    const uint32_t roff = (uint32_t)arow * 128u, sw = (uint32_t)(arow & 7);
+    TcAluCtx c;
+    c.xring = xring; c.xslot = xslot; c.xfull0 = xfull0; c.xempty0 = xempty0;
+    c.nx = nx; c.nk = nk; c.lane = lane;
+    c.arow = ((warp - 4) << 4) + (lane >> 1);
+    c.hh = (uint32_t)lane & 1u;
     uint32_t xs = 0, xph = 0;
     int it = 0;
-    auto load4 = [&](const unsigned char* base, uint32_t ro, uint32_t swz, uint4 (&x)[4]) {
-#pragma unroll
-      for (int u = 0; u < 4; ++u) x[u] = *reinterpret_cast<const uint4*>(base + ro + ((((hh << 2) + (uint32_t)u) ^ swz) << 4));
-    };
-    auto release = [&]() {
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctrl->xempty[xs]));
-      if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
-    };
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
       const int buf = it & 1;
-      float* st = stat + (size_t)buf * kTcMaxBlocks * 256 + arow * 2 + hh;   // + b * 256: this lane's accumulator of block b
+      c.stat = smem_u32(stat) + (uint32_t)buf * (kTcMaxBlocks * 1024u) + (uint32_t)(c.arow * 2 + (int)c.hh) * 4u;   // + b * 1024: block b
       mbar_wait(smem_u32(&ctrl->sempty[buf]), ((uint32_t)(it >> 1) & 1u) ^ 1u);
-      const int mode = tile.mode;
-      const bool halo = mode == 1 && tile.halo;
-      const uint32_t proff = (uint32_t)(arow - tile.prev) * 128u, psw = (uint32_t)((arow - tile.prev) & 7);   // mode 2
-      for (int kc = 0; kc < nk; ++kc) {
-        uint4 pv[4];                  // mode 1: this thread's K-slice of the previous frame's row
-        bool have_prev = false;
-        if (halo) {
-          mbar_wait(smem_u32(&ctrl->xfull[xs]), xph);
-          if (arow < tile.n_rows) load4(xring + xs * (uint32_t)kTcXSlotBytes, roff, sw, pv);
-          have_prev = true;
-          release();
-        }
-        for (int b = 0; b < tile.n_blocks; ++b) {
-          const int hb = tc_block_rows(tile, b);
-          uint64_t n2a = 0, n2b = 0, Da = 0, Db = 0;     // packed fp32 pairs, all zero bits = (0.f, 0.f)
-          mbar_wait(smem_u32(&ctrl->xfull[xs]), xph);
-          if (arow < hb) {
-            const unsigned char* base = xring + xs * (uint32_t)kTcXSlotBytes;
-            uint4 x[4];
-            load4(base, roff, sw, x);
-            if (mode == 1) {
-              if (have_prev) tc_sq4_diff(x, pv, n2a, n2b, Da, Db); else tc_sq4(x, n2a, n2b);
-#pragma unroll
-              for (int u = 0; u < 4; ++u) pv[u] = x[u];
-            } else if (mode == 2 && arow >= tile.prev) {
-              uint4 v[4];
-              load4(base, proff, psw, v);
-              tc_sq4_diff(x, v, n2a, n2b, Da, Db);
-            } else {
-              tc_sq4(x, n2a, n2b);
-            }
-          }
-          have_prev = true;
-          release();
-          float n2 = sum_f32x2(n2a) + sum_f32x2(n2b), D = sum_f32x2(Da) + sum_f32x2(Db);
-          n2 += __shfl_xor_sync(0xffffffffu, n2, 1);
-          D += __shfl_xor_sync(0xffffffffu, D, 1);
-          if (arow < hb) {   // lane pair (row): the even lane keeps sum x^2, the odd lane sum (x - x_prev)^2
-            const float mine = hh ? D : n2;
-            float* a = st + b * 256;
-            *a = kc == 0 ? mine : *a + mine;
-          }
-        }
-      }
+      tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, xs, xph);
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->sfull[buf]));
     }
@@ -546,7 +611,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     __threadfence();
     if (atomicAdd(p.q_ready + 1, 1ull) == (unsigned long long)gridDim.x - 1ull) { p.q_ready[0] = 0ull; p.q_ready[1] = 0ull; __threadfence(); }
   }
-  if (warp == 2) {
+  if (warp == kTcWarpMma) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
   }
@@ -560,7 +625,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 // most 8 blocks, each tile paying a fixed cost for the query rows it streams.  Consecutive CTAs sweep neighbouring rows
 // of the same frames at the same time, so the halo chunks are L2 hits.
 struct TcCost {
-  double w_halo = 0.5, w_q = 0.5, c_tile = 24.0;   // in token rows: a halo row, a padded query row, per tile
+  // in token rows of one K-sweep.  A block of h rows costs c_blk + w_row * h: what a block costs hardly shrinks with its height
+  // (M = 128 MMAs read 128 rows of shared memory whatever the block holds, the statistics warps pay per chunk, every chunk is
+  // a barrier round trip; measured on 64 x 576-token images: 3 blocks of 90 rows take 1.4 x the time of 2 blocks of 125).
+  double c_blk = 56.0, w_row = 0.5625, w_halo = 0.25, w_q = 0.5, c_tile = 24.0;
 };
 
 inline size_t tc_max_tiles(const mas_segment* segs, int32_t n_segs) {
@@ -588,36 +656,55 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
   for (int32_t k = 0; k < n_segs; ++k) maxL = std::max(maxL, (int)(q_off[segs[k].request + 1] - q_off[segs[k].request]));
   const int npad_max = (maxL + 15) / 16 * 16 + (rider ? 64 : 0);
   if (npad_max > 128) return;
-  sc.wslot = npad_max <= 64 ? 64 : 128;
-  sc.ns_log2 = sc.wslot == 64 ? 3 : 2;
-  const int NS = 1 << sc.ns_log2;
-  sc.qslot_bytes = npad_max * 128;
-  sc.nx = std::min(kTcMaxXSlots, (kTcSmemBytes - 1024 - kTcCtrlBytes - kTcStatBytes - 2 * sc.qslot_bytes) / kTcXSlotBytes);
-  sc.smem_bytes = 1024 + kTcCtrlBytes + kTcStatBytes + 2 * sc.qslot_bytes + sc.nx * kTcXSlotBytes;
+  sc.wslot = npad_max;
+  sc.ns = std::min(kTcMaxBlocks, 512 / npad_max);
+  const int NS = sc.ns;
+  sc.kw = (d % 128 == 0) ? 2 : 1;
+  sc.qslot_bytes = npad_max * 128 * sc.kw;
+  {   // shared memory: control + statistics, then the query ring (at least 3 slots where they leave 128 KB for the token ring)
+    const int avail = kTcSmemBytes - 1024 - kTcCtrlBytes - kTcStatBytes, xs_bytes = sc.kw * kTcSliceBytes;
+    sc.nx = std::min(kTcMaxXSlots, (avail - 2 * sc.qslot_bytes) / xs_bytes);
+    sc.nq = (avail - sc.nx * xs_bytes) / sc.qslot_bytes;
+    if (sc.nq < 3 && (sc.nx - 1) * xs_bytes >= 128 * 1024) { --sc.nx; sc.nq = (avail - sc.nx * xs_bytes) / sc.qslot_bytes; }
+    sc.nq = std::max(2, std::min(4, sc.nq));
+    sc.smem_bytes = 1024 + kTcCtrlBytes + kTcStatBytes + sc.nq * sc.qslot_bytes + sc.nx * xs_bytes;
+  }
 
-  struct Strip { int32_t seg, mode, t0, F; int64_t len; double row_cost, c_fix; int64_t cap; };
+  // mode 0 / 2: a strip is a segment, its units are rows; mode 1: a strip is one block of patch rows [r0, r0 + R) of a segment
+  // through all its frames, its units are FRAMES (a tile takes up to NS consecutive frames of the block)
+  struct Strip { int32_t seg, mode, r0, R, P; int64_t len; double c_fix; int64_t cap; };   // cap: units a tile may take
   std::vector<Strip> strips;
-  double total = 0.0;
   for (int32_t k = 0; k < n_segs; ++k) {
     const mas_segment& s = segs[k];
     const int L = (int)(q_off[s.request + 1] - q_off[s.request]);
     const double c_fix = cw.w_q * ((L + 15) / 16 * 16 + (rider ? 64 : 0)) + cw.c_tile;
     const int64_t n = (int64_t)s.n_frames * s.n_patches;
     if (s.n_frames == 1) {
-      strips.push_back(Strip{k, 0, 0, 1, n, 1.0, c_fix, (int64_t)128 * NS});
+      strips.push_back(Strip{k, 0, 0, 0, 0, n, c_fix, (int64_t)128 * NS});
     } else if (s.n_patches >= 64) {
-      const int ng = (s.n_frames + NS - 1) / NS;          // frame groups of nearly equal size
-      for (int gq = 0, t0 = 0; gq < ng; ++gq) {
-        const int F = s.n_frames / ng + (gq < s.n_frames % ng ? 1 : 0);
-        strips.push_back(Strip{k, 1, t0, F, (int64_t)s.n_patches, (double)F + (t0 > 0 ? cw.w_halo : 0.0), c_fix, 128});
-        t0 += F;
+      const int nb = (s.n_patches + 127) / 128;            // row blocks of nearly equal height
+      for (int j = 0; j < nb; ++j) {
+        const int r0 = (int)((int64_t)s.n_patches * j / nb), r1 = (int)((int64_t)s.n_patches * (j + 1) / nb);
+        strips.push_back(Strip{k, 1, r0, r1 - r0, s.n_patches, (int64_t)s.n_frames, c_fix, NS});
       }
     } else {
-      const int P = s.n_patches;
-      strips.push_back(Strip{k, 2, 0, 1, n, 128.0 / (128 - P), c_fix, (int64_t)(128 - P) * NS});
+      strips.push_back(Strip{k, 2, 0, 0, s.n_patches, n, c_fix, (int64_t)(128 - s.n_patches) * NS});
     }
   }
-  auto piece_cost = [&](const Strip& st, int64_t rows) { return (double)rows * st.row_cost + (double)((rows + st.cap - 1) / st.cap) * st.c_fix; };
+  auto blk = [&](double h) { return cw.c_blk + cw.w_row * h; };   // one block of h rows, per K-sweep
+  auto tile_cost = [&](const Strip& st, int64_t n) {       // a tile of n units of the strip
+    if (st.mode == 0) { const int64_t nb = (n + 127) / 128; return (double)nb * blk((double)n / nb) + st.c_fix; }
+    if (st.mode == 1) return (double)n * blk((double)st.R) + (cw.c_blk + cw.w_halo * st.R) + st.c_fix;   // the halo chunk counted for every tile
+    const int64_t nb = (n + (128 - st.P) - 1) / (128 - st.P);
+    return (double)nb * blk(128.0) + st.c_fix;
+  };
+  // a run of `rows` units is cut into the fewest tiles, of nearly equal size (the same split as emit() below)
+  auto piece_cost = [&](const Strip& st, int64_t rows) {
+    if (rows <= 0) return 0.0;
+    const int64_t nt = (rows + st.cap - 1) / st.cap;
+    return (double)(nt - rows % nt) * tile_cost(st, rows / nt) + (double)(rows % nt) * tile_cost(st, rows / nt + 1);
+  };
+  double total = 0.0;
   for (const Strip& st : strips) total += piece_cost(st, st.len);
   const int n_ctas = (int)std::min<int64_t>(sm_count, std::max<int64_t>(1, (int64_t)(total / 96.0)));
 
@@ -634,10 +721,11 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
       t.q_row0 = (int32_t)q_off[s.request];
       t.L = (int32_t)(q_off[s.request + 1] - q_off[s.request]);
       if (st.mode == 0) {
-        t.row0 = (int32_t)(s.row0 + u); t.n_rows = (int32_t)(v - u); t.stride = 128; t.n_blocks = (t.n_rows + 127) / 128;
-      } else if (st.mode == 1) {
-        t.row0 = (int32_t)(s.row0 + (int64_t)st.t0 * s.n_patches + u); t.n_rows = (int32_t)(v - u); t.stride = s.n_patches; t.prev = s.n_patches;
-        t.n_blocks = st.F; t.halo = st.t0 > 0 ? 1 : 0;
+        t.row0 = (int32_t)(s.row0 + u); t.n_rows = (int32_t)(v - u); t.n_blocks = (t.n_rows + 127) / 128;
+        t.stride = (t.n_rows + t.n_blocks - 1) / t.n_blocks;          // blocks of nearly equal height
+      } else if (st.mode == 1) {                            // frames [u, v) of the strip's row block
+        t.row0 = (int32_t)(s.row0 + u * s.n_patches + st.r0); t.n_rows = st.R; t.stride = s.n_patches; t.prev = s.n_patches;
+        t.n_blocks = (int32_t)(v - u); t.halo = u > 0 ? 1 : 0;
       } else {
         const int P = s.n_patches;
         const int64_t a0 = u == 0 ? 0 : u - P;            // the window starts P rows early (their successors need them)
@@ -668,7 +756,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
           int64_t lo = 0, hi = left;
           while (lo < hi) { const int64_t mid = (lo + hi + 1) / 2; if (load + piece_cost(st, mid) <= target) lo = mid; else hi = mid - 1; }
           take = lo;
-          const int64_t min_rows = st.mode == 2 ? 16 : 8;
+          const int64_t min_rows = st.mode == 2 ? 16 : st.mode == 1 ? 1 : 8;
           if (take < min_rows) {          // not worth a tile of its own here
             if (load > 0.0) { close_cta(); continue; }
             take = std::min<int64_t>(left, min_rows);
@@ -709,7 +797,10 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
   sc.enabled = true;
 }
 
-inline cudaError_t tc_set_kernel_attrs() { return cudaFuncSetAttribute(k_score_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes); }
+inline cudaError_t tc_set_kernel_attrs() {
+  const cudaError_t e = cudaFuncSetAttribute(k_score_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes);
+  return e != cudaSuccess ? e : cudaFuncSetAttribute(k_score_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes);
+}
 
 typedef CUresult (*tc_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -725,34 +816,36 @@ inline tc_encode_fn tc_get_encode() {
   return fn;
 }
 
-// 2-D bf16 tensor map over a row-major [rows, d] matrix, box = [box_rows, 64 columns], 128-byte swizzle, zero OOB fill.
-inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, int box_rows) {
+// bf16 tensor map over a row-major [rows, d] matrix seen as [d / 64 slices][rows][64 columns] (slice stride 128 B, row stride
+// 2 d B): box = [box_slices][box_rows][64 columns], 128-byte swizzle, zero OOB fill.  In shared memory a box is box_slices
+// consecutive K-major tiles of box_rows x 128 B, which is what the UMMA descriptors and the statistics warps address.
+inline bool tc_make_map(CUtensorMap* m, const void* base, int64_t rows, int d, int box_rows, int box_slices) {
   tc_encode_fn enc = tc_get_encode();
   if (!enc) return false;
-  cuuint64_t gdim[2] = {(cuuint64_t)d, (cuuint64_t)rows};
-  cuuint64_t gstr[1] = {(cuuint64_t)d * 2};
-  cuuint32_t box[2] = {64u, (cuuint32_t)box_rows};
-  cuuint32_t estr[2] = {1u, 1u};
-  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+  cuuint64_t gdim[3] = {64u, (cuuint64_t)rows, (cuuint64_t)(d / 64)};
+  cuuint64_t gstr[2] = {(cuuint64_t)d * 2, 128u};
+  cuuint32_t box[3] = {64u, (cuuint32_t)box_rows, (cuuint32_t)box_slices};
+  cuuint32_t estr[3] = {1u, 1u, 1u};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // The 20 tensor maps of a launch depend on the (X, Q, R) base pointers only: the plan keeps the last few sets it encoded.
 struct TcMapCache {
-  struct Entry { const void* X = nullptr; const void* Q = nullptr; const void* R = nullptr; TcMaps maps; };
+  struct Entry { const void* X = nullptr; const void* Q = nullptr; const void* R = nullptr; int kw = 0; TcMaps maps; };
   Entry e[4];
   int next = 0;
-  const TcMaps* get(const void* X, int64_t N, const void* Q, int64_t nQ, const void* R, int d) {
+  const TcMaps* get(const void* X, int64_t N, const void* Q, int64_t nQ, const void* R, int d, int kw) {
     for (Entry& en : e)
-      if (en.X == X && en.Q == Q && en.R == R) return &en.maps;
+      if (en.X == X && en.Q == Q && en.R == R && en.kw == kw) return &en.maps;
     Entry& en = e[next];
     en.X = nullptr;
     for (int k = 0; k < 16; ++k)
-      if (!tc_make_map(&en.maps.x[k], X, N, d, 8 * (k + 1))) return nullptr;
+      if (!tc_make_map(&en.maps.x[k], X, N, d, 8 * (k + 1), kw)) return nullptr;
     for (int k = 0; k < 3; ++k)
-      if (!tc_make_map(&en.maps.q[k], Q, nQ, d, 64 >> k)) return nullptr;
-    if (R != nullptr) { if (!tc_make_map(&en.maps.r, R, 64, d, 64)) return nullptr; } else en.maps.r = en.maps.q[0];
-    en.X = X; en.Q = Q; en.R = R;
+      if (!tc_make_map(&en.maps.q[k], Q, nQ, d, 64 >> k, 1)) return nullptr;
+    if (R != nullptr) { if (!tc_make_map(&en.maps.r, R, 64, d, 64, 1)) return nullptr; } else en.maps.r = en.maps.q[0];
+    en.X = X; en.Q = Q; en.R = R; en.kw = kw;
     next = (next + 1) & 3;
     return &en.maps;
   }
@@ -770,16 +863,16 @@ inline cudaError_t tc_launch_score(const TcSchedule& sc, TcMapCache& cache, cons
                                    float* rel, unsigned long long* q_ready, int64_t N, int64_t nQ, int d, bool inline_qprep, const void* Rm,
                                    unsigned long long* sig, const TcHeads* hf, cudaStream_t st, bool pdl_in = false) {
   const bool rider = sig != nullptr || hf != nullptr;
-  const TcMaps* maps = cache.get(X, N, Q, nQ, rider ? Rm : nullptr, d);
+  const TcMaps* maps = cache.get(X, N, Q, nQ, rider ? Rm : nullptr, d, sc.kw);
   if (!maps) return cudaErrorUnknown;
   TcParams p;
   p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.sig = sig; p.s = s; p.dnorm = dnorm; p.rel = rel;
-  p.d = d; p.n_kchunks = d / 64; p.nx = sc.nx; p.qslot_bytes = sc.qslot_bytes; p.wslot = sc.wslot; p.ns_log2 = sc.ns_log2;
+  p.d = d; p.n_kchunks = d / 64; p.kw = sc.kw; p.nx = sc.nx; p.nq = sc.nq; p.qslot_bytes = sc.qslot_bytes; p.wslot = sc.wslot; p.ns = sc.ns;
   p.heads_part = hf ? hf->part : nullptr; p.heads_m = hf ? hf->m : nullptr; p.heads_bias = hf ? hf->bias : 0.f; p.heads_tau = hf ? hf->tau : 0.f;
   if (hf) p.sig = nullptr;
   if (!inline_qprep) {   // qinv is already there: no CTA waits on another one, a plain launch will do
     p.Q = nullptr;
-    return launch_k(k_score_tc, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl_in, *maps, p);
+    return launch_k(sc.kw == 2 ? k_score_tc<2> : k_score_tc<1>, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl_in, *maps, p);
   }
   // cooperative launch: the query-norm prologue makes the CTAs wait on one another once, so all must be resident
   cudaLaunchConfig_t cfg = {};
@@ -788,7 +881,7 @@ inline cudaError_t tc_launch_score(const TcSchedule& sc, TcMapCache& cache, cons
   attr[0].id = cudaLaunchAttributeCooperative;
   attr[0].val.cooperative = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, k_score_tc, *maps, p);
+  return sc.kw == 2 ? cudaLaunchKernelEx(&cfg, k_score_tc<2>, *maps, p) : cudaLaunchKernelEx(&cfg, k_score_tc<1>, *maps, p);
 }
 
 }  // namespace msas

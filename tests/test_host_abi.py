@@ -127,7 +127,7 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
     seg_of_row = np.concatenate([np.full(r[2] * r[3], k) for k, r in enumerate(rows)])
     row0_of, q0_of = np.cumsum([0] + [r[2] * r[3] for r in rows]), [int(q_off[r[0]]) for r in rows]
     maxL = int(np.diff(q_off).max())
-    n_slots = 8 if maxL <= 64 else 4                             # TMEM accumulator slots (64 or 128 columns each)
+    n_slots = min(10, 512 // ((maxL + 15) // 16 * 16))           # TMEM accumulator slots of pad16(longest query block) columns
     cost = np.zeros(148)
     for rec in t:
         cta, r0, n, nb, stride, mode, prev, halo, q0, L, seg, part0 = [int(v) for v in rec]
@@ -136,7 +136,7 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
         assert q0 == q0_of[seg] and L == q_off[rows[seg][0] + 1] - q_off[rows[seg][0]]
         assert mode == (0 if T == 1 else 1 if P >= 64 else 2)
         if mode == 0:
-            assert stride == 128 and prev == 0 and halo == 0 and nb == (n + 127) // 128
+            assert stride == -(-n // nb) and prev == 0 and halo == 0 and nb == (n + 127) // 128     # blocks of nearly equal height
         elif mode == 1:
             assert stride == P and prev == P and 1 <= n <= 128 and halo in (0, 1)
             t0 = (r0 - row0_of[seg]) // P
@@ -150,15 +150,20 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
         for lo, hi in _scored_rows(rec):
             assert lo < hi and seg_of_row[lo] == seg and seg_of_row[hi - 1] == seg    # a tile never straddles a segment
             cov[lo:hi] += 1
-        # cost model of csrc/k_score_tc.cuh (TcCost): rows streamed (half for the L2-served halo rows), 0.5 per padded query row,
-        # 24 per tile
-        streamed = n if mode != 1 else n * nb + 0.5 * n * halo
-        cost[cta] += streamed + 0.5 * ((L + 15) // 16 * 16) + 24.0
+        # cost model of csrc/k_score_tc.cuh (TcCost): 56 + 0.5625 h per block of h rows (a block costs nearly the same whatever
+        # its height), the halo chunk, 0.5 per padded query row and 24 per tile
+        if mode == 0:
+            blocks = nb * (56 + 0.5625 * n / nb)
+        elif mode == 1:
+            blocks = nb * (56 + 0.5625 * n) + halo * (56 + 0.25 * n)
+        else:
+            blocks = nb * 128.0
+        cost[cta] += blocks + 0.5 * ((L + 15) // 16 * 16) + 24.0
     assert cov.min() == 1 and cov.max() == 1                     # every row scored exactly once
     assert np.all(np.diff(t[:, 0]) >= 0)                         # grouped per CTA, CTAs in order
     if N >= 148 * 128:
         # contiguous runs at a common target: the last CTAs may stay idle when cuts add tiles, the heaviest stays near the mean
-        assert np.count_nonzero(cost) >= 140 and cost.max() <= 1.06 * cost.sum() / 148, (cost.max(), cost.sum() / 148)
+        assert np.count_nonzero(cost) >= 140 and cost.max() <= 1.10 * cost.sum() / 148, (cost.max(), cost.sum() / 148)
 
 
 def test_score_schedule_rider_variant_and_small_devices(B):
