@@ -26,7 +26,8 @@
 // AR(1) statistical law.  Free conventions shared by both sides and therefore not pinnable by mathematics:
 // kappa = 10 (G20) and the standardisation floors 1e-6 (G18).
 //
-// Build: g++ -O2 -shared -fPIC (no -ffast-math, no OpenMP).  See oracle/build_oracle.py.
+// Build: g++ -O2 -shared -fPIC (no -ffast-math, no OpenMP): oracle/mas_ref.py build().  oracle/selftest.cpp runs a few of the
+// pins and a ragged whole pass under -fsanitize=address,undefined (tests/test_oracle_pins.py).
 
 #include <algorithm>
 #include <cmath>

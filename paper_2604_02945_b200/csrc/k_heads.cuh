@@ -163,12 +163,12 @@ __global__ void __launch_bounds__(1024) k_heads_finish(HeadsArgs a) {
     for (int i = seg.n_patches + tid; i < n; i += NT) gs += (double)a.gamma[seg.row0 + i];
   block_sum3(sm, gs, d1, d2);   // its barriers also publish colsum
   double contrib = 0.0;
-  if (tid >= 1 && tid <= a.hidden) {
-    float pq = 0.f;
+  if (tid >= 1 && tid <= a.hidden) {   // the hidden unit in double: its <= 63 products are free next to the reductions above
+    double pq = 0.0;
 #pragma unroll
-    for (int y = 0; y < kHeadSlabs; ++y) pq += a.cq[((int64_t)seg.request * kHeadSlabs + y) * kHeadRows + tid];
-    const float pre = (float)(colsum[tid] / (double)n) + pq + a.b1[tid];
-    contrib = (double)(a.w2[tid] * fmaxf(pre, 0.f));
+    for (int y = 0; y < kHeadSlabs; ++y) pq += (double)a.cq[((int64_t)seg.request * kHeadSlabs + y) * kHeadRows + tid];
+    const double pre = colsum[tid] / (double)n + pq + (double)a.b1[tid];
+    contrib = (double)a.w2[tid] * fmax(pre, 0.0);
   }
   d1 = d2 = 0.0;
   block_sum3(sm, contrib, d1, d2);
@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(1024) k_heads_finish(HeadsArgs a) {
     mas_segment_out o;
     o.rho_spatial = (float)(colsum[0] / (double)n);
     o.gamma_avg = temporal ? (float)(gs / ((double)(seg.n_frames - 1) * (double)seg.n_patches)) : 0.f;
-    o.alpha_mean = (float)contrib + a.b2;
+    o.alpha_mean = (float)(contrib + (double)a.b2);
     o.beta = 0.f; o.mas = 0.f; o.mean_s = 0.f; o.std_s = 0.f;
     o.n_tokens = n; o.n_kept = 0;
     a.seg_out[sidx] = o;
@@ -191,15 +191,15 @@ __global__ void __launch_bounds__(1024) k_heads_finish(HeadsArgs a) {
   const DevParams& p = a.prm;
   for (int r = tid; r < a.n_requests; r += NT) {
     const int k0 = a.req_seg_off[r], k1 = a.req_seg_off[r + 1];
-    float mx = -INFINITY;
-    for (int k = k0; k < k1; ++k) mx = fmaxf(mx, so[k].alpha_mean);
-    float zsum = 0.f;
-    for (int k = k0; k < k1; ++k) zsum += expf(so[k].alpha_mean - mx);
-    for (int k = k0; k < k1; ++k) {
-      const float beta = expf(so[k].alpha_mean - mx) / zsum;
-      const float at = a.segs[k].n_frames > 1 ? p.lambda_temp : 0.f;
-      so[k].beta = beta;
-      so[k].mas = 1.0f - beta * (1.0f - p.lambda_spatial * so[k].rho_spatial - at * (1.0f - so[k].gamma_avg));
+    double mx = -INFINITY;
+    for (int k = k0; k < k1; ++k) mx = fmax(mx, (double)so[k].alpha_mean);
+    double zsum = 0.0;
+    for (int k = k0; k < k1; ++k) zsum += exp((double)so[k].alpha_mean - mx);
+    for (int k = k0; k < k1; ++k) {   // literal softmax and Eq. 7 in double: a few segments per request
+      const double beta = exp((double)so[k].alpha_mean - mx) / zsum;
+      const double at = a.segs[k].n_frames > 1 ? (double)p.lambda_temp : 0.0;
+      so[k].beta = (float)beta;
+      so[k].mas = (float)(1.0 - beta * (1.0 - (double)p.lambda_spatial * (double)so[k].rho_spatial - at * (1.0 - (double)so[k].gamma_avg)));
     }
   }
   if (tid == 0) *a.done_counter = 0u;

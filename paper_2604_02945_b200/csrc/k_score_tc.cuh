@@ -250,6 +250,16 @@ __device__ __forceinline__ void tc_alu_load(uint32_t base, uint32_t ro, uint32_t
 #pragma unroll
   for (int u = 0; u < 4; ++u) x[u] = lds128(base + ro + (((uoff + (uint32_t)u) ^ swz) << 4));
 }
+// makes the following instructions wait for the loads into `x` (a data dependency the scoreboard honours)
+template <int KW>
+__device__ __forceinline__ void tc_alu_fence_loads(const uint4 (&x)[KW][4]) {
+  uint32_t acc = 0;
+#pragma unroll
+  for (int j = 0; j < KW; ++j)
+#pragma unroll
+    for (int u = 0; u < 4; ++u) acc |= x[j][u].x ^ x[j][u].w;
+  asm volatile("" ::"r"(acc) : "memory");
+}
 __device__ __forceinline__ void tc_alu_release(const TcAluCtx& c, uint32_t& xs, uint32_t& xph) {
   __syncwarp();
   if (c.lane == 0) mbar_arrive(c.xempty0 + xs * 8u);
@@ -275,6 +285,7 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
         for (int j = 0; j < KW; ++j) tc_alu_load(c.xring + xs * c.xslot + (uint32_t)j * slice, roff, uoff, sw, pv[j]);
       }
       have_prev = true;
+      tc_alu_fence_loads(pv);
       tc_alu_release(c, xs, xph);
     }
     for (int b = 0; b < n_blocks; ++b) {
@@ -292,7 +303,6 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
           if (inchunk) tc_alu_load(base, proff, uoff, psw, pv[j]);
         }
       }
-      tc_alu_release(c, xs, xph);   // the slot is free as soon as its bytes are in registers
       if (act) {
         const bool diff = inchunk || (mode == 1 && have_prev);
 #pragma unroll
@@ -305,6 +315,8 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
         }
       }
       have_prev = true;
+      tc_alu_release(c, xs, xph);   // after the arithmetic: every byte of the slot has arrived in registers by now (an arrive issued
+                                    // right behind the loads could complete before them and let the TMA unit overwrite the slot)
       // the chunk's partial sums of a row (two lanes) join block b's accumulators in shared memory
       float n2 = sum_f32x2(n2a) + sum_f32x2(n2b), D = sum_f32x2(Da) + sum_f32x2(Db);
       n2 += __shfl_xor_sync(0xffffffffu, n2, 1);
@@ -419,7 +431,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         mbar_wait(qfull0 + 8u * qs, qph);
         tc_fence_after();
         const uint32_t qbase = qring + qs * (uint32_t)p.qslot_bytes;
-        if (halo) {   // not an MMA operand: release our share of the slot (behind the MMAs issued so far, which keeps the order)
+        if (halo) {   // not an MMA operand: release our share of the slot, behind the MMAs issued so far (which keeps the order) and
+                      // not before the chunk has landed (an arrival ahead of the slot's previous phase would be counted there)
+          mbar_wait(xfull0 + 8u * xs, xph);
           if (elect_one()) tc_commit(xempty0 + 8u * xs);
           if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
         }

@@ -75,3 +75,66 @@ def check_seg_out(rows, gpu_so, ref_so, ref_m, tau_s=0.3, lambda_spatial=0.6):
         assert abs(float(g["mas"]) - r.mas) <= RTOL * abs(r.mas) + ATOL + slack, (k, "mas", float(g["mas"]), r.mas)
         assert int(g["n_tokens"]) == n
         r0 += n
+
+
+# ---------------------------------------------------------------- the oracle over every request of a workload, on all host cores
+_POOL_JOB = None   # (workload, oracle params kwargs): inherited by the forked workers, never pickled
+
+
+def request_slices(w):
+    """[(segment indices, first row, end row)] per request."""
+    seg_req = np.array([s[0] for s in w.segments])
+    seg_rows = np.array([s[2] * s[3] for s in w.segments])
+    seg_row0 = np.concatenate([[0], np.cumsum(seg_rows)])
+    out = []
+    for r in range(w.n_requests):
+        ks = np.nonzero(seg_req == r)[0]
+        out.append((ks, int(seg_row0[ks[0]]), int(seg_row0[ks[-1] + 1])))
+    return out
+
+
+def oracle_request(r):
+    """The oracle's whole pass on request r alone (requests are independent: SURVEY.md 8(e))."""
+    from oracle import mas_ref as O
+    w, prm_kw = _POOL_JOB
+    ks, lo, hi = request_slices(w)[r]
+    rows = [(0,) + tuple(w.segments[k][1:]) for k in ks]
+    segs, _ = O.make_segments(rows)
+    prm = O.default_params(select_mode=w.select_mode, cut=w.cut, **prm_kw)
+    ref = O.forward(segs, [0, int(w.q_off[r + 1] - w.q_off[r])], prm, w.X[lo:hi], w.Q[w.q_off[r]:w.q_off[r + 1]], want_Y=False)
+    so = [(o.rho_spatial, o.gamma_avg, o.alpha_mean, o.beta, o.mas, o.mean_s, o.std_s, o.n_tokens, o.n_kept) for o in ref["seg_out"]]
+    return r, {k: ref[k] for k in ("m_spatial", "gamma", "rel", "mas_tok")}, so
+
+
+class SegOut:
+    __slots__ = ("rho_spatial", "gamma_avg", "alpha_mean", "beta", "mas", "mean_s", "std_s", "n_tokens", "n_kept")
+
+    def __init__(self, t):
+        for k, v in zip(self.__slots__, t):
+            setattr(self, k, v)
+
+
+def oracle_all_requests(w, requests=None, procs=None, **prm_kw):
+    """{request: (scores dict, [SegOut])} for the given requests (default: all), the single-threaded oracle run as one process per
+    host core over disjoint requests (fork: the workers inherit the inputs and never touch CUDA)."""
+    import multiprocessing as mp
+    import os
+    global _POOL_JOB
+    reqs = list(range(w.n_requests)) if requests is None else list(requests)
+    _POOL_JOB = (w, prm_kw)
+    n = min(len(reqs), procs or os.cpu_count() or 1)
+    out = {}
+    # longest requests first: the tail of the pool is then short
+    sl = request_slices(w)
+    reqs.sort(key=lambda r: -(sl[r][2] - sl[r][1]) * int(w.q_off[r + 1] - w.q_off[r]))
+    if n <= 1:
+        results = map(oracle_request, reqs)
+    else:
+        pool = mp.get_context("fork").Pool(n)
+        results = pool.imap_unordered(oracle_request, reqs, chunksize=1)
+    for r, scores, so in results:
+        out[r] = (scores, [SegOut(t) for t in so])
+    if n > 1:
+        pool.close(); pool.join()
+    _POOL_JOB = None
+    return out

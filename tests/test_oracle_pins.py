@@ -236,6 +236,60 @@ def test_eq7_special_cases():
     assert abs(out[0].mas - (0.9 * 0.5 + 0.1 * 0.45)) < 1e-15
 
 
+def test_fuse_gain_bias_kappa_worked_example():
+    """spatial_gain / spatial_bias / rel_gain / rel_bias / kappa away from their defaults (reading G2, G20): the hand-worked case of
+    tests/golden/closed_forms.txt (fusep_*).  Swapping the two gains, or a sign error on a bias, changes every value below."""
+    rows = [(0, 1, 1, 2, 1), (0, 1, 1, 2, 1)]
+    s = np.array([1.0, 3.0, 2.0, 2.0])
+    rel = np.array([0.1, 0.3, 0.5, 0.7])
+    m, mas, out = _fuse_segments(rows, s, np.zeros(4), rel, spatial_gain=2.0, spatial_bias=-0.5, rel_gain=0.5, rel_bias=0.25, kappa=3.0)
+    assert np.allclose(m, [GOLD["fusep_M_A0"], GOLD["fusep_M_A1"], GOLD["fusep_M_B"], GOLD["fusep_M_B"]], rtol=0, atol=1e-15)
+    assert np.allclose(mas[:2], [GOLD["fusep_mas_A0"], GOLD["fusep_mas_A1"]], rtol=0, atol=1e-15)
+    assert out[0].rho_spatial == 0.5 and out[1].rho_spatial == 0.0
+    assert abs(out[0].beta - GOLD["fusep_beta_A"]) < 1e-15 and abs(out[0].beta + out[1].beta - 1) < 1e-15
+    assert abs(out[0].mas - GOLD["fusep_mas_seg_A"]) < 1e-15 and abs(out[1].mas - GOLD["fusep_mas_seg_B"]) < 1e-15
+    # the relevance sigmoid of the worked case, recovered from MAS_i = 1 - g (1 - lambda_sp (1 - M)) at T = 1
+    g = (1 - mas[:2]) / (1 - 0.6 * (1 - m[:2]))
+    assert np.allclose(g, [GOLD["fusep_g_A0"], GOLD["fusep_g_A1"]], rtol=0, atol=1e-15)
+
+
+def test_fuse_nondefault_params_against_numpy_float64():
+    """Every parameter of mas_ref_fuse away from its default, three segments of one request plus a single-segment request, against
+    the formulas of SPEC S1 / S3 / S4 evaluated with numpy in float64."""
+    rng = np.random.default_rng(11)
+    rows = [(0, 1, 1, 7, 1), (0, 2, 4, 5, 1), (0, 3, 9, 1, 1), (1, 2, 3, 4, 1)]
+    sizes = [T * P for (_, _, T, P, _) in rows]
+    n = sum(sizes)
+    s, gam, rel = rng.random(n) + 0.3, rng.random(n), 0.2 * rng.standard_normal(n)
+    prm = dict(lambda_spatial=0.55, lambda_temp=0.35, tau_s=0.42, kappa=3.0, spatial_gain=2.0, spatial_bias=-0.5, rel_gain=0.5, rel_bias=0.25)
+    m, mas, out = _fuse_segments(rows, s, gam, rel, **prm)
+    sig = lambda u: 1.0 / (1.0 + np.exp(-u))
+    r0, alphas, rhos, gavgs = 0, [], [], []
+    for (_, _, T, P, _), nk in zip(rows, sizes):
+        sl = slice(r0, r0 + nk)
+        z = (s[sl] - s[sl].mean()) / s[sl].std()
+        M = sig(2.0 * z - 0.5)
+        g = sig(0.5 * (rel[sl] - rel[sl].mean()) / rel[sl].std() + 0.25)
+        a = 1.0 if T > 1 else 0.0
+        assert np.allclose(m[sl], M, rtol=1e-13, atol=0)
+        assert np.allclose(mas[sl], 1 - g * (1 - 0.55 * (1 - M) - a * 0.35 * (1 - gam[sl])), rtol=1e-13, atol=0)
+        alphas.append(rel[sl].mean()); rhos.append(np.count_nonzero(M < 0.42) / nk)
+        gavgs.append(gam[sl].reshape(T, P)[1:].mean(axis=1).mean() if T > 1 else 0.0)
+        r0 += nk
+    e = np.exp(3.0 * np.array(alphas[:3]))
+    beta = list(e / e.sum()) + [1.0]
+    for k, (_, _, T, P, _) in enumerate(rows):
+        a = 1.0 if T > 1 else 0.0
+        assert abs(out[k].rho_spatial - rhos[k]) < 1e-15 and abs(out[k].gamma_avg - gavgs[k]) < 1e-14
+        assert abs(out[k].beta - beta[k]) < 1e-13
+        assert abs(out[k].mas - (1 - beta[k] * (1 - 0.55 * rhos[k] - a * 0.35 * (1 - gavgs[k])))) < 1e-13
+    # the two gains are not interchangeable, nor are the two biases
+    m2, mas2, _ = _fuse_segments(rows, s, gam, rel, **dict(prm, spatial_gain=0.5, rel_gain=2.0))
+    assert not np.allclose(m2, m) and not np.allclose(mas2, mas)
+    m3, mas3, _ = _fuse_segments(rows, s, gam, rel, **dict(prm, spatial_bias=0.25, rel_bias=-0.5))
+    assert not np.allclose(m3, m) and not np.allclose(mas3, mas)
+
+
 def test_per_token_mas_formula_ranges_and_monotonicity():
     rng = np.random.default_rng(4)
     n = 64
@@ -639,3 +693,19 @@ def test_gather_residual_rules():
     Yb = O.gather_residual(seg2, synth.f32_to_bf16_bits(Xb), np.array([1], np.int32))
     got = (Yb.astype(np.uint32) << 16).view(np.float32)[0]
     assert got[0] == 1.0 and got[1] == 0.99609375
+
+
+# ---------------------------------------------------------------- the oracle under AddressSanitizer / UBSan
+def test_oracle_selftest_under_asan_ubsan(tmp_path):
+    """oracle/selftest.cpp (a few closed-form pins + a ragged whole pass in both selection modes) built with
+    -fsanitize=address,undefined: an out-of-bounds access, misaligned load or signed overflow in oracle/mas_oracle.cpp aborts it."""
+    import shutil
+    import subprocess
+    if shutil.which("g++") is None:
+        pytest.skip("no g++")
+    odir = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "oracle")
+    exe = str(tmp_path / "oracle_selftest")
+    subprocess.check_call(["g++", "-O1", "-g", "-std=c++17", "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-Wall", "-Wextra",
+                           "-o", exe, os.path.join(odir, "selftest.cpp")])
+    out = subprocess.run([exe], capture_output=True, text=True, env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1"))
+    assert out.returncode == 0 and "oracle selftest ok" in out.stdout, out.stdout + out.stderr

@@ -142,13 +142,13 @@ def _forward_and_compare(B, w, sample_requests=None, **prm):
     seg_rows = np.array([s[2] * s[3] for s in w.segments])
     seg_row0 = np.concatenate([[0], np.cumsum(seg_rows)])
     reqs = range(w.n_requests) if sample_requests is None else sample_requests
-    oprm = _oracle_params(w, **prm)
+    refs = P.oracle_all_requests(w, reqs, **prm)          # one oracle process per host core over disjoint requests
     for r in reqs:
         ks = np.nonzero(seg_req == r)[0]
         rows = [(0,) + tuple(w.segments[k][1:]) for k in ks]
         lo, hi = int(seg_row0[ks[0]]), int(seg_row0[ks[-1] + 1])
-        segs, n = O.make_segments(rows)
-        ref = O.forward(segs, [0, int(w.q_off[r + 1] - w.q_off[r])], oprm, w.X[lo:hi], w.Q[w.q_off[r]:w.q_off[r + 1]], want_Y=False)
+        ref, ref_so = refs[r]
+        ref = dict(ref, seg_out=ref_so)
         for name in ("m_spatial", "gamma", "rel", "mas_tok"):
             P.assert_close(host[name][lo:hi], ref[name], "%s[req %d]" % (name, r))
         assert np.array_equal(host["gamma"][lo:hi] == 0.0, ref["gamma"] == 0.0)
@@ -312,13 +312,17 @@ def test_unsupported_inputs_fail_loudly(B):
 
 
 # ---------------------------------------------------------------- full BASELINE.json sizes, bench launch configuration
+import os
+
 FULL = [("batched_images", {}, [0, 31, 63]), ("video", {}, [5]), ("audio_vision", {}, [7]), ("ragged", {}, [3, 100, 255])]
 
 
 @pytest.mark.parametrize("name,kw,sample", FULL, ids=[f[0] for f in FULL])
-def test_forward_full_size_sampled(B, name, kw, sample):
+def test_forward_full_size(B, name, kw, sample):
+    """BASELINE.json configs 2-5 at full size, in the launch configuration bench.py times: EVERY request against the oracle (the
+    oracle sharded over the host cores, one request per process at a time).  MSAS_PARITY_QUICK=1 compares the sampled requests only."""
     w = synth.make(name, **kw)
-    _forward_and_compare(B, w, sample_requests=sample)
+    _forward_and_compare(B, w, sample_requests=sample if os.environ.get("MSAS_PARITY_QUICK") else None)
 
 
 # ---------------------------------------------------------------- segment sizes around every internal boundary
@@ -598,11 +602,12 @@ def test_learned_heads(B, w, hidden):
         nk = T * Pn
         near = np.count_nonzero(np.abs(ref_m[r0:r0 + nk] - 0.3) <= 1e-3 * 0.3)
         assert abs(float(g["rho_spatial"][k]) - ref[k].rho_spatial) <= near / nk + 1e-6
-        # alpha: fp32 accumulation of O(1) pre-activations over `hidden` units
-        assert abs(float(g["alpha_mean"][k]) - ref[k].alpha_mean) <= 1e-3 * abs(ref[k].alpha_mean) + 2e-4 * np.sum(np.abs(w2)), (k, float(g["alpha_mean"][k]), ref[k].alpha_mean)
+        # alpha = w2 . relu(pre) + b2 may cancel to any small value: the absolute term is the pre-activations' error (fp32 tensor-core
+        # column sums, ~1e-6 of their O(1) scale; hidden layer and softmax in double) times sum |w2|
+        assert abs(float(g["alpha_mean"][k]) - ref[k].alpha_mean) <= P.RTOL * abs(ref[k].alpha_mean) + 1e-5 * np.sum(np.abs(w2)), (k, float(g["alpha_mean"][k]), ref[k].alpha_mean)
         assert abs(float(g["gamma_avg"][k]) - ref[k].gamma_avg) <= 1e-5
-        assert abs(float(g["beta"][k]) - ref[k].beta) <= 2e-3
-        assert abs(float(g["mas"][k]) - ref[k].mas) <= 2e-3 + 0.6 * near / nk
+        assert abs(float(g["beta"][k]) - ref[k].beta) <= P.RTOL * abs(ref[k].beta) + P.ATOL, (k, float(g["beta"][k]), ref[k].beta)
+        assert abs(float(g["mas"][k]) - ref[k].mas) <= P.RTOL * abs(ref[k].mas) + P.ATOL + 0.6 * near / nk
         assert int(g["n_tokens"][k]) == nk
         r0 += nk
     # softmax identity per request on the GPU's own numbers
@@ -622,10 +627,10 @@ def _check_learned(B, w, m, so, gamma_np, W, Wp, b1, w2, b_sp, b2, hidden):
         nk = T * Pn
         near = np.count_nonzero(np.abs(ref_m[r0:r0 + nk] - 0.3) <= 1e-3 * 0.3)
         assert abs(float(g["rho_spatial"][k]) - ref[k].rho_spatial) <= near / nk + 1e-6
-        assert abs(float(g["alpha_mean"][k]) - ref[k].alpha_mean) <= 1e-3 * abs(ref[k].alpha_mean) + 2e-4 * np.sum(np.abs(w2)), (k, float(g["alpha_mean"][k]), ref[k].alpha_mean)
+        assert abs(float(g["alpha_mean"][k]) - ref[k].alpha_mean) <= P.RTOL * abs(ref[k].alpha_mean) + 1e-5 * np.sum(np.abs(w2)), (k, float(g["alpha_mean"][k]), ref[k].alpha_mean)
         assert abs(float(g["gamma_avg"][k]) - ref[k].gamma_avg) <= 1e-5
-        assert abs(float(g["beta"][k]) - ref[k].beta) <= 2e-3
-        assert abs(float(g["mas"][k]) - ref[k].mas) <= 2e-3 + 0.6 * near / nk
+        assert abs(float(g["beta"][k]) - ref[k].beta) <= P.RTOL * abs(ref[k].beta) + P.ATOL, (k, float(g["beta"][k]), ref[k].beta)
+        assert abs(float(g["mas"][k]) - ref[k].mas) <= P.RTOL * abs(ref[k].mas) + P.ATOL + 0.6 * near / nk
         assert int(g["n_tokens"][k]) == nk
         r0 += nk
 
