@@ -109,9 +109,12 @@ int32_t     mas_keep_count(int64_t n, double ratio);     /* SPEC S5/G16: min(n, 
 /* ---- plan: validates the tables, lays out the device workspace, builds the tile schedule ----
  * h_segs[n_segs], h_q_off[n_requests+1] are host arrays read during the call only.
  * mas_plan_workspace_bytes: bytes of device workspace the plan needs (256-byte aligned base expected).
- * mas_plan_create: copies the tables into d_workspace asynchronously on `stream` (from a pinned staging area owned
- * by the plan) and returns a host object; the workspace must stay alive and untouched until mas_plan_destroy.
- * One plan may be used by one stream at a time (the workspace holds per-call scratch).
+ * mas_plan_create: copies the tables into d_workspace on `stream` (from a pinned staging area owned by the plan), waits
+ * for that copy (plan creation is set-up: it is the one call besides mas_forward_host that synchronises) and returns a
+ * host object, which may then be used on any stream; the workspace must stay alive and untouched until mas_plan_destroy.
+ * One plan may be used by one stream and one host thread at a time (the workspace holds per-call scratch, the plan
+ * caches the tensor maps of the last few (X, Q) pointer sets).  The kernels' shared-memory opt-in is made once per device,
+ * at the first plan created on it.
  * Errors: INVALID_ARG (NULL, negative sizes, tables not tiling / not ordered, keep_k out of range in top-k mode,
  * bad params), UNSUPPORTED (limits above), WORKSPACE (too small), CUDA. */
 int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_segs, const int64_t* h_q_off, int32_t n_requests,
@@ -278,10 +281,10 @@ int mas_plan_set_inline_query_norms(mas_plan* plan, int32_t on);
 
 /* ---- introspection (host only, no CUDA call): the tile schedule mas_plan_create would build for the tcgen05 score
  * kernel on a device with `sm_count` SMs ("persistent CTAs over a host-built tile table; a tile
- * never straddles a segment").  A tile is up to 8 row blocks of one segment that share the request's query rows and are
- * swept K-chunk by K-chunk.  Writes up to `cap_tiles` records of 12 int32 each, in per-CTA order:
+ * never straddles a segment").  A tile is up to 10 row blocks (one TMEM accumulator slot each: 512 columns / pad16 of the
+ * longest query block) of one segment that share the request's query rows and are swept K-chunk by K-chunk.  Writes up to `cap_tiles` records of 12 int32 each, in per-CTA order:
  *   {cta, row0, n_rows, n_blocks, stride, mode, prev, halo, q_row0, L, seg, part0}
- *   mode 0 (single-frame segment): the tile scores rows [row0, row0 + n_rows) in blocks of 128 (stride = 128);
+ *   mode 0 (single-frame segment): the tile scores rows [row0, row0 + n_rows) in blocks of `stride` <= 128 rows;
  *   mode 1 (frames of P >= 64 rows): block b scores rows [row0 + b * stride, + n_rows), stride = prev = P, i.e. the same
  *          n_rows <= 128 patch rows in n_blocks consecutive frames; halo = 1 if the frame before block 0 is read as well;
  *   mode 2 (frames of P < 64 rows): the tile loads rows [row0, row0 + n_rows) in overlapping 128-row windows

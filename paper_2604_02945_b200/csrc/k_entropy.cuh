@@ -41,7 +41,12 @@ __device__ __forceinline__ void ent_fold(EntTriple& acc, const float (&x)[N], in
   }
 #pragma unroll
   for (int k = 0; k < N; ++k)
-    if (FULL || k < n_valid) { const float u = fmaf(x[k], kLog2e, -acc.m), e = ex2f(u); acc.z += e; acc.t = fmaf(u, e, acc.t); }
+    if (FULL || k < n_valid) {
+      // masked logits (-inf, e.g. after top-k filtering) contribute 0 (0 ln 0 = 0): the clamp turns -inf, and the NaN of
+      // -inf + inf while nothing finite has been seen yet, into an exponent whose 2^u flushes to exactly 0
+      const float u = fmaxf(fmaf(x[k], kLog2e, -acc.m), -200.f), e = ex2f(u);
+      acc.z += e; acc.t = fmaf(u, e, acc.t);
+    }
 }
 
 template <int DT>   // 0: fp32, 1: bf16

@@ -298,8 +298,11 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     for (int32_t k = 0; k < n_segs; ++k) sr[k + 1] = sr[k] + cnt[k + 1];
   }
 
+  // plan creation is set-up, not the hot path: it returns when the tables are on the device, so that the plan may be used on
+  // any stream afterwards without further ordering (the entry points themselves never synchronise)
   e = cudaMemcpyAsync(p->ws, p->pinned, lay.tables_end, cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(p->ws + lay.counter, 0, 256, stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess) { g_last_cuda = (int)e; (void)cudaGetLastError(); cudaFreeHost(p->pinned); delete p; return MAS_ERR_CUDA; }
   *out = p;
   return MAS_OK;
@@ -563,7 +566,10 @@ extern "C" int mas_spatial_pool(const mas_plan* p, const int32_t* h_grid_w, int3
   for (int32_t q = 0; q < p->n_segs; ++q)
     if (h_grid_w[q] < 1 || hs[q].n_patches % h_grid_w[q] != 0) return MAS_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  CK(cudaMemcpyAsync(p->at<int32_t>(p->lay.gridw), h_grid_w, sizeof(int32_t) * p->n_segs, cudaMemcpyHostToDevice, st));
+  // the caller's array is read during this call only, whatever memory it lives in: a copy from PAGEABLE memory is staged by the
+  // runtime before cudaMemcpyAsync returns (a pinned source would be read when the copy executes)
+  const std::vector<int32_t> gw(h_grid_w, h_grid_w + p->n_segs);
+  CK(cudaMemcpyAsync(p->at<int32_t>(p->lay.gridw), gw.data(), sizeof(int32_t) * p->n_segs, cudaMemcpyHostToDevice, st));
   k_spatial_pool<<<p->n_tiles, 256, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->at<DevTile>(p->lay.tiles), p->at<int32_t>(p->lay.gridw), k, s, s_pooled);
   CK(cudaGetLastError());
   return MAS_OK;

@@ -504,6 +504,19 @@ def test_entropy_closed_forms():
     assert list(flag) == [0, 1, int(H[2] <= 1.0)]              # Eq. 10: speculate iff H <= theta
 
 
+def test_entropy_of_masked_logits():
+    """-inf logits (filtered drafts) carry no probability: 0 ln 0 = 0 (SPEC NEXT-4).  k survivors at equal logits -> ln k; one -> 0."""
+    L = np.full((3, 300), -np.inf, np.float32)
+    L[0, 10:14] = 1.5
+    L[1, 299] = -3.0
+    L[2, ::3] = 0.25
+    H, flag = O.draft_entropy(L, 1.0)
+    assert abs(H[0] - math.log(4)) < 1e-15 and H[1] == 0.0 and abs(H[2] - math.log(100)) < 1e-13
+    assert list(flag) == [0, 1, 0]
+    Hb, _ = O.draft_entropy(synth.f32_to_bf16_bits(L), 1.0)
+    assert np.allclose(Hb, H, rtol=0, atol=1e-14)
+
+
 def test_entropy_matches_scipy_and_is_shift_invariant():
     from scipy.special import softmax
     from scipy.stats import entropy

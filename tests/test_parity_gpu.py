@@ -561,6 +561,28 @@ def test_draft_entropy_matches_oracle(B, n, V, dtype):
     assert H.min() >= -1e-4 and H.max() <= np.log(V) + 1e-3
 
 
+def test_draft_entropy_with_masked_logits(B):
+    """Logits of -inf (top-k / top-p filtered drafts) contribute nothing (0 ln 0 = 0, SPEC NEXT-4); a row with one finite logit has H = 0."""
+    rng = np.random.default_rng(77)
+    n, V = 6, 5000
+    L = (3.0 * rng.standard_normal((n, V))).astype(np.float32)
+    L[0, 50:] = -np.inf                                   # 50 candidates survive
+    L[1, :] = -np.inf; L[1, 4321] = 2.5                   # one survivor: H = 0
+    L[2, ::2] = -np.inf                                   # every other logit masked (whole 16-byte groups stay mixed)
+    L[3, :4096] = -np.inf                                 # the leading groups are entirely masked
+    L[4, 8:16] = -np.inf                                  # one whole 16-byte group of a bf16 row
+    for dtype in ("f32", "bf16"):
+        Lh = L if dtype == "f32" else synth.f32_to_bf16_bits(L)
+        H, sp = B.draft_entropy(B.to_device(Lh), 2.0)
+        torch.cuda.synchronize()
+        H_r, f_r = O.draft_entropy(Lh, 2.0)
+        Hg = H.cpu().numpy().astype(np.float64)
+        assert np.all(np.isfinite(Hg)) and abs(Hg[1]) < 1e-6
+        assert np.all(np.abs(Hg - H_r) <= 2e-4 * H_r + 2e-4), (dtype, Hg, H_r)
+        decided = np.abs(H_r - 2.0) > 1e-3
+        assert np.array_equal(sp.cpu().numpy()[decided], f_r[decided])
+
+
 # ---------------------------------------------------------------- NEXT-2: learned heads (Eq. 3, Eq. 6 with supplied weights)
 def _head_weights(rng, d, hidden, dtype):
     W = np.zeros((64, d), np.float32)
