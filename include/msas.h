@@ -282,8 +282,12 @@ int mas_plan_set_inline_query_norms(mas_plan* plan, int32_t on);
 /* ---- introspection (host only, no CUDA call): the tile schedule mas_plan_create would build for the tcgen05 score
  * kernel on a device with `sm_count` SMs ("persistent CTAs over a host-built tile table; a tile
  * never straddles a segment").  A tile is up to 10 row blocks (one TMEM accumulator slot each: 512 columns / pad16 of the
- * longest query block) of one segment that share the request's query rows and are swept K-chunk by K-chunk.  Writes up to `cap_tiles` records of 12 int32 each, in per-CTA order:
- *   {cta, row0, n_rows, n_blocks, stride, mode, prev, halo, q_row0, L, seg, part0}
+ * longest query block) of one segment that share the request's query rows and are swept K-chunk by K-chunk.  Writes up to `cap_tiles` records of 16 int32 each, in per-CTA order:
+ *   {cta, row0, n_rows, n_blocks, stride, mode, prev, halo, q_row0, L, seg, part0, k0, k1, n_wait, peer}
+ *   k0, k1: the tile sweeps the 64-column K-chunks [k0, k1) (all d / 64 of them unless the block is K-SPLIT: a single-block
+ *          tile whose chunks are shared by consecutive CTAs so that every CTA carries the same cost; the part with k0 = 0
+ *          owns the block: n_wait = number of other parts, peer = CTA of the first of them; the other parts have n_wait = 0 and
+ *          peer = their own CTA: they hand their partial sums over through an exchange slot); peer = -1 for ordinary tiles;
  *   mode 0 (single-frame segment): the tile scores rows [row0, row0 + n_rows) in blocks of `stride` <= 128 rows;
  *   mode 1 (frames of P >= 64 rows): block b scores rows [row0 + b * stride, + n_rows), stride = prev = P, i.e. the same
  *          n_rows <= 128 patch rows in n_blocks consecutive frames; halo = 1 if the frame before block 0 is read as well;

@@ -164,16 +164,16 @@ def make_segments(rows):
 
 
 def score_schedule(rows, q_off, d, dtype, sm_count=148):
-    """Host-only: the tile schedule of the tcgen05 score kernel as an int32 array [n_tiles, 12]
-    (cta, row0, n_rows, n_blocks, stride, mode, prev, halo, q_row0, L, seg, part0; see include/msas.h); empty if the shape
-    takes the generic path."""
+    """Host-only: the tile schedule of the tcgen05 score kernel as an int32 array [n_tiles, 16]
+    (cta, row0, n_rows, n_blocks, stride, mode, prev, halo, q_row0, L, seg, part0, k0, k1, n_wait, peer; see include/msas.h);
+    empty if the shape takes the generic path."""
     segs, _ = make_segments(rows)
     q = np.ascontiguousarray(q_off, np.int64)
     qp = q.ctypes.data_as(C.POINTER(C.c_int64))
     n = lib.mas_score_schedule(segs, len(list(rows)), qp, len(q) - 1, d, dtype, sm_count, None, 0)
     if n < 0:
         raise MasError(-n, "mas_score_schedule")
-    out = np.zeros((max(n, 1), 12), np.int32)
+    out = np.zeros((max(n, 1), 16), np.int32)
     lib.mas_score_schedule(segs, len(list(rows)), qp, len(q) - 1, d, dtype, sm_count, out.ctypes.data_as(C.POINTER(C.c_int32)), n)
     return out[:n]
 

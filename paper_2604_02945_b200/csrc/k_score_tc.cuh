@@ -36,7 +36,7 @@
 
 namespace msas {
 
-struct TcTile {            // 48 bytes
+struct TcTile {            // 64 bytes
   int32_t row0;            // global row id of the first row block 0 loads
   int32_t n_rows;          // mode 1: rows of every block (<= 128); modes 0, 2: rows the tile loads in total (blocks of <= 128)
   int32_t n_blocks;        // 1..8 (<= TMEM accumulator slots)
@@ -49,12 +49,19 @@ struct TcTile {            // 48 bytes
   int32_t L;               // query tokens of the request
   int32_t part0;           // NEXT-2: slot of block 0's column sums (block b -> part0 + b); slots of a segment are contiguous
   int32_t seg;
+  // K-split (single-block tiles only): the tile covers K-chunks [k0, k1) of the row block.  The part that starts at chunk 0 OWNS
+  // the block: it adds the partial accumulators and row sums the other parts dumped and writes the results.
+  int32_t k0, k1;          // in 64-column chunks, multiples of the slices per chunk
+  int32_t n_wait;          // owner: number of foreign parts to add (they live in the exchange slots peer .. peer + n_wait - 1)
+  int32_t peer;            // dumping part: its exchange slot (= its CTA), -1 for ordinary tiles and owners; owner: first slot to read
   int32_t pad_;
 };
+static_assert(sizeof(TcTile) == 64, "TcTile is 64 bytes");
 
 constexpr int kTcThreads = 448;                      // 14 warps: 4 epilogue, 8 statistics, TMA producer, MMA issuer (144 registers per thread)
 constexpr int kTcAluWarps = 8;
 constexpr int kTcWarpTma = 12, kTcWarpMma = 13;
+constexpr int kTcMaxCtas = 160;                     // CTAs of a launch (one per SM) = K-split exchange slots
 constexpr int kTcMaxBlocks = 10;                    // blocks per tile = TMEM accumulator slots (512 columns / pad16(L), at most 10)
 constexpr int kTcSliceBytes = 128 * 128;             // 128 rows x 64 bf16 columns: one K-slice of a block
 constexpr int kTcMaxXSlots = 12;
@@ -77,6 +84,7 @@ struct TcSchedule {
   int nq = 2;              // query-chunk slots (2..4: short tiles need several K-steps in flight)
   int wslot = 0, ns = 0;        // TMEM: columns per accumulator slot (pad16 of the longest query block), number of slots
   int smem_bytes = 0;
+  int xchg_cols = 0;       // floats per row of a K-split exchange slot: pad16(longest query block) (+ 64) + 2
   const TcTile* d_tiles = nullptr;
   const int32_t* d_cta_off = nullptr;
 };
@@ -102,6 +110,9 @@ struct TcParams {
   int d;
   int n_kchunks;
   int kw, nx, nq, qslot_bytes, wslot, ns;
+  float* xchg;            // K-split exchange: slot c = [xchg_cols][128] floats (accumulator columns, then sum x^2, sum (x - x_prev)^2)
+  unsigned int* xflag;    // [n_ctas] 1 = slot c is filled; zero between launches (the owner re-arms it)
+  int xchg_cols;
 };
 
 __device__ __forceinline__ int tc_block_rows(const TcTile& t, int b) {
@@ -267,14 +278,14 @@ __device__ __forceinline__ void tc_alu_release(const TcAluCtx& c, uint32_t& xs, 
 }
 template <int KW>
 __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_rows, int n_blocks, int stride, int prev, bool halo,
-                                            uint32_t& xs, uint32_t& xph) {
+                                            int k0, int k1, uint32_t& xs, uint32_t& xph) {
   const uint32_t roff = (uint32_t)c.arow * 128u, sw = (uint32_t)(c.arow & 7);
   const uint32_t uoff = c.hh << 2;
   const int prow = c.arow - prev;                                        // mode 2: the previous frame's row in the same chunk
   const uint32_t proff = (uint32_t)prow * 128u, psw = (uint32_t)(prow & 7);
   const bool inchunk = mode == 2 && prow >= 0;
   const int hcap = mode == 0 ? stride : 128;
-  for (int kc = 0; kc < c.nk; kc += KW) {
+  for (int kc = k0; kc < k1; kc += KW) {
     uint4 pv[KW][4];                  // this thread's K-slices of the previous frame's row (mode 1: carried from block to block)
     bool have_prev = false;
     if (halo) {
@@ -288,12 +299,12 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
       tc_alu_fence_loads(pv);
       tc_alu_release(c, xs, xph);
     }
-    for (int b = 0; b < n_blocks; ++b) {
+    // one block's chunk: `x` receives this thread's K-slices of the row, `pv` holds those of the previous frame's row
+    auto step = [&](int b, uint4 (&x)[KW][4], uint4 (&pv)[KW][4]) __attribute__((always_inline)) {
       const int hb = mode == 1 ? n_rows : min(hcap, n_rows - b * stride);
       const uint32_t slice = (uint32_t)((hb + 7) >> 3) * 1024u;
       const bool act = c.arow < hb;
       uint64_t n2a = 0, n2b = 0, Da = 0, Db = 0;     // packed fp32 pairs, all zero bits = (0.f, 0.f)
-      uint4 x[KW][4];
       mbar_wait(c.xfull0 + xs * 8u, xph);
       if (act) {
 #pragma unroll
@@ -308,10 +319,6 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
 #pragma unroll
         for (int j = 0; j < KW; ++j) {
           if (diff) tc_sq4_diff(x[j], pv[j], n2a, n2b, Da, Db); else tc_sq4(x[j], n2a, n2b);
-          if (mode == 1) {
-#pragma unroll
-            for (int u = 0; u < 4; ++u) pv[j][u] = x[j][u];
-          }
         }
       }
       have_prev = true;
@@ -324,8 +331,17 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
       if (act) {   // lane pair (row): the even lane keeps sum x^2, the odd lane sum (x - x_prev)^2
         const float mine = c.hh ? D : n2;
         const uint32_t a = c.stat + (uint32_t)b * 1024u;
-        sts32(a, kc == 0 ? mine : lds32(a) + mine);
+        sts32(a, kc == k0 ? mine : lds32(a) + mine);
       }
+    };
+    uint4 xb[KW][4];
+    if (mode == 1) {   // frame walk: the two register sets alternate between "this frame" and "previous frame" (no copies)
+      for (int b = 0; b < n_blocks; b += 2) {
+        step(b, xb, pv);
+        if (b + 1 < n_blocks) step(b + 1, pv, xb);
+      }
+    } else {
+      for (int b = 0; b < n_blocks; ++b) step(b, xb, pv);
     }
   }
 }
@@ -387,7 +403,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int nqu = (tile.L + 15) >> 4;
       const uint32_t qbytes = (uint32_t)(nqu + (rider ? 4 : 0)) * 2048u * (uint32_t)kw;
       const int b_lo = (tile.mode == 1 && tile.halo) ? -1 : 0;      // block -1 = the halo chunk (frame t0 - 1)
-      for (int kc = 0; kc < nk; kc += kw) {
+      for (int kc = tile.k0; kc < tile.k1; kc += kw) {
         {   // the request's query rows of these K-slices (+ the rider rows): one B tile per slice
           mbar_wait(qempty0 + 8u * qs, qph ^ 1u);
           if (elect_one()) {
@@ -427,7 +443,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int nqb = ((tile.L + 15) >> 4) + (rider ? 4 : 0);
       const uint32_t idesc = umma_idesc_bf16(nqb << 4);   // N = pad16(L) (+ 64 rider rows)
       const bool halo = tile.mode == 1 && tile.halo;
-      for (int kc = 0; kc < nk; kc += kw) {
+      for (int kc = tile.k0; kc < tile.k1; kc += kw) {
         mbar_wait(qfull0 + 8u * qs, qph);
         tc_fence_after();
         const uint32_t qbase = qring + qs * (uint32_t)p.qslot_bytes;
@@ -440,7 +456,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         for (int b = 0; b < tile.n_blocks; ++b) {
           uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
           if (ts >= ns) { ts -= ns; tp ^= 1u; }
-          if (kc == 0) {   // the accumulator slot must have been drained by the epilogue of its previous use
+          if (kc == tile.k0) {   // the accumulator slot must have been drained by the epilogue of its previous use
             mbar_wait(tempty0 + 8u * ts, tp ^ 1u);
             tc_fence_after();
           }
@@ -456,7 +472,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
               const uint64_t bdesc = umma_desc_sw128(qbase + (uint32_t)j * (uint32_t)nqb * 2048u);
 #pragma unroll
               for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
-                tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)(kc | j | k));
+                tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kc - tile.k0) | j | k));
             }
             tc_commit(xempty0 + 8u * xs);
           }
@@ -505,30 +521,74 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int nqu = (tile.L + 15) >> 4;
       const float* qinv = p.qinv + tile.q_row0;
       const float2* st2 = reinterpret_cast<const float2*>(stat) + (size_t)buf * kTcMaxBlocks * 128;
+      const bool dump = tile.peer >= 0 && tile.n_wait == 0;          // K-split: this part hands its partial sums to the block's owner
+      const int n_wait = tile.n_wait;
+      const size_t xslot_f = (size_t)p.xchg_cols * 128;              // floats per exchange slot
       for (int b = 0; b < tile.n_blocks; ++b) {
         uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
         if (ts >= ns) { ts -= ns; tp ^= 1u; }
         const uint32_t tcol = tmem_base + ts * (uint32_t)p.wslot + ((uint32_t)(q * 32) << 16);
         mbar_wait(smem_u32(&ctrl->tfull[ts]), tp);
         tc_fence_after();
+        if (dump) {   // accumulator columns (column-major: lanes = rows, coalesced), then the two row sums, then the flag
+          float* xo = p.xchg + (size_t)tile.peer * xslot_f + r;
+          const int ncb = nqu + (rider ? 4 : 0);
+          for (int cb = 0; cb < ncb; ++cb) {
+            uint32_t v[16];
+            tc_ld16(tcol + (uint32_t)cb * 16u, v);
+            tc_wait_ld();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) xo[(size_t)(cb * 16 + j) * 128] = __uint_as_float(v[j]);
+          }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
+          mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
+          const float2 nd = st2[b * 128 + r];
+          xo[(size_t)(p.xchg_cols - 2) * 128] = nd.x;
+          xo[(size_t)(p.xchg_cols - 1) * 128] = nd.y;
+          __threadfence();
+          asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
+          if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + tile.peer), "r"(1u) : "memory");
+          continue;
+        }
         if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
           unsigned long long seen;
           do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
           q_ok = true;
         }
+        if (n_wait > 0) {   // owner of a split block: the other parts were swept first by the CTAs that follow this one
+          if (lane == 0)
+            for (int i = 0; i < n_wait; ++i) {
+              unsigned int f;
+              do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.xflag + tile.peer + i) : "memory"); } while (f == 0u);
+            }
+          __syncwarp();
+        }
+        const float* xi = p.xchg + (size_t)tile.peer * xslot_f + r;      // owner: the parts' slots follow one another
+        // 16 accumulator columns of this thread's row, the foreign parts added in slot order (a fixed order: bit-reproducible)
+        auto ld16 = [&](int cbi, float (&f)[16]) {
+          uint32_t v[16];
+          tc_ld16(tcol + (uint32_t)cbi * 16u, v);
+          tc_wait_ld();
+#pragma unroll
+          for (int j = 0; j < 16; ++j) f[j] = __uint_as_float(v[j]);
+          for (int i = 0; i < n_wait; ++i)
+#pragma unroll
+            for (int j = 0; j < 16; ++j) f[j] += xi[(size_t)i * xslot_f + (size_t)(cbi * 16 + j) * 128];
+        };
         const int hb = tc_block_rows(tile, b);
         const int out_lo = tile.mode == 2 ? (b == 0 ? tile.halo : tile.prev) : 0;
         const bool valid = r < hb && r >= out_lo;
         const int64_t row = (int64_t)tile.row0 + (int64_t)b * tile.stride + r;
         float m = -INFINITY;
         for (int cb = 0; cb < nqu; ++cb) {
-          uint32_t v[16];
-          tc_ld16(tcol + (uint32_t)cb * 16u, v);
-          tc_wait_ld();
+          float v[16];
+          ld16(cb, v);
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
             const int col = cb * 16 + j;
-            if (col < tile.L) m = fmaxf(m, __uint_as_float(v[j]) * qinv[col]);
+            if (col < tile.L) m = fmaxf(m, v[j] * qinv[col]);
           }
         }
         if (p.heads_part != nullptr) {   // NEXT-2: column 0 -> the learned spatial map, all 64 -> per-block column sums (fixed order)
@@ -538,11 +598,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             float x[32];
 #pragma unroll
             for (int cb = 0; cb < 2; ++cb) {
-              uint32_t v[16];
-              tc_ld16(tcol + (uint32_t)(nqu + grp * 2 + cb) * 16u, v);
-              tc_wait_ld();
+              float v[16];
+              ld16(nqu + grp * 2 + cb, v);
 #pragma unroll
-              for (int j = 0; j < 16; ++j) x[cb * 16 + j] = valid ? __uint_as_float(v[j]) : 0.f;
+              for (int j = 0; j < 16; ++j) x[cb * 16 + j] = valid ? v[j] : 0.f;
             }
             if (grp == 0) {
               float below = 0.f;
@@ -575,11 +634,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           unsigned long long bits = 0ull;
 #pragma unroll
           for (int cb = 0; cb < 4; ++cb) {
-            uint32_t v[16];
-            tc_ld16(tcol + (uint32_t)(nqu + cb) * 16u, v);
-            tc_wait_ld();
+            float v[16];
+            ld16(nqu + cb, v);
 #pragma unroll
-            for (int j = 0; j < 16; ++j) bits |= (unsigned long long)(__uint_as_float(v[j]) >= 0.f) << (cb * 16 + j);
+            for (int j = 0; j < 16; ++j) bits |= (unsigned long long)(v[j] >= 0.f) << (cb * 16 + j);
           }
           if (valid) p.sig[row] = bits;
         }
@@ -587,11 +645,19 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
         if (b == 0) mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
-        const float2 nd = st2[b * 128 + r];
+        float2 nd = st2[b * 128 + r];
+        for (int i = 0; i < n_wait; ++i) {
+          nd.x += xi[(size_t)i * xslot_f + (size_t)(p.xchg_cols - 2) * 128];
+          nd.y += xi[(size_t)i * xslot_f + (size_t)(p.xchg_cols - 1) * 128];
+        }
         if (valid) {
           p.s[row] = sqrtf(nd.x * inv_d);
           p.dnorm[row] = sqrtf(nd.y);
           p.rel[row] = nd.x > 0.f ? m / sqrtf(nd.x) : 0.f;
+        }
+        if (n_wait > 0) {   // every warp has read the slots: re-arm their flags for the next launch
+          asm volatile("bar.sync 1, 128;" ::: "memory");
+          if (q == 0 && lane < n_wait) p.xflag[tile.peer + lane] = 0u;
         }
       }
       __syncwarp();
@@ -613,7 +679,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int buf = it & 1;
       c.stat = smem_u32(stat) + (uint32_t)buf * (kTcMaxBlocks * 1024u) + (uint32_t)(c.arow * 2 + (int)c.hh) * 4u;   // + b * 1024: block b
       mbar_wait(smem_u32(&ctrl->sempty[buf]), ((uint32_t)(it >> 1) & 1u) ^ 1u);
-      tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, xs, xph);
+      tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, tile.k0, tile.k1, xs, xph);
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->sfull[buf]));
     }
@@ -639,10 +705,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 // most 8 blocks, each tile paying a fixed cost for the query rows it streams.  Consecutive CTAs sweep neighbouring rows
 // of the same frames at the same time, so the halo chunks are L2 hits.
 struct TcCost {
-  // in token rows of one K-sweep.  A block of h rows costs c_blk + w_row * h: what a block costs hardly shrinks with its height
-  // (M = 128 MMAs read 128 rows of shared memory whatever the block holds, the statistics warps pay per chunk, every chunk is
-  // a barrier round trip; measured on 64 x 576-token images: 3 blocks of 90 rows take 1.4 x the time of 2 blocks of 125).
-  double c_blk = 56.0, w_row = 0.5625, w_halo = 0.25, w_q = 0.5, c_tile = 24.0;
+  // in token rows of one K-sweep.  A block of h rows costs c_blk + w_row * h (its bytes, plus what does not shrink with its height:
+  // M = 128 MMAs read 128 rows of shared memory whatever the block holds, every chunk is a barrier round trip); a tile pays for
+  // the query rows it streams (by its share of K) and a constant.  With all CTAs running the machine is HBM-bound, so bytes
+  // dominate: constants from A/B runs on the images / video configs (profiles/r02_schedule.md).
+  double c_blk = 16.0, w_row = 0.875, w_halo = 0.25, w_q = 0.2, c_tile = 6.0;
 };
 
 inline size_t tc_max_tiles(const mas_segment* segs, int32_t n_segs) {
@@ -655,14 +722,16 @@ inline size_t tc_max_parts(const mas_segment* segs, int32_t n_segs) {   // block
   for (int32_t k = 0; k < n_segs; ++k) blocks += (size_t)(((int64_t)segs[k].n_frames * segs[k].n_patches) / 32) + 2 * (size_t)segs[k].n_frames + 8;
   return blocks + 8 * 2048;
 }
+inline size_t tc_xchg_bytes() { return (size_t)kTcMaxCtas * (kMaxL + 2) * 128 * sizeof(float); }   // K-split exchange slots, worst case
 inline size_t tc_schedule_bytes(const mas_segment* segs, int32_t n_segs) {
   return tc_max_tiles(segs, n_segs) * sizeof(TcTile) + 1024 * sizeof(int32_t) + 256;
 }
 
 // Builds the tile list (grouped per CTA) and the per-CTA offsets into `h_dst`; `d_dst` is where the image will live.
 // `rider`: the launch appends 64 B rows (NEXT-1 / NEXT-2), which needs every L <= 64.
+// `ksplit`: CTAs may share a row block along K (needs all CTAs co-resident: the owner of a block waits for the other parts).
 inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n_segs, const int64_t* q_off, int32_t d, int32_t dtype,
-                              int sm_count, char* h_dst, char* d_dst, bool rider = false) {
+                              int sm_count, char* h_dst, char* d_dst, bool rider = false, bool ksplit = true) {
   sc = TcSchedule();
   if (dtype != MAS_BF16 || d % 64 != 0 || sm_count < 1 || sm_count > 1000) return;
   const TcCost cw;
@@ -671,6 +740,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
   const int npad_max = (maxL + 15) / 16 * 16 + (rider ? 64 : 0);
   if (npad_max > 128) return;
   sc.wslot = npad_max;
+  sc.xchg_cols = npad_max + 2;
   sc.ns = std::min(kTcMaxBlocks, 512 / npad_max);
   const int NS = sc.ns;
   sc.kw = (d % 128 == 0) ? 2 : 1;
@@ -684,111 +754,145 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     sc.smem_bytes = 1024 + kTcCtrlBytes + kTcStatBytes + sc.nq * sc.qslot_bytes + sc.nx * xs_bytes;
   }
 
-  // mode 0 / 2: a strip is a segment, its units are rows; mode 1: a strip is one block of patch rows [r0, r0 + R) of a segment
-  // through all its frames, its units are FRAMES (a tile takes up to NS consecutive frames of the block)
-  struct Strip { int32_t seg, mode, r0, R, P; int64_t len; double c_fix; int64_t cap; };   // cap: units a tile may take
+  // The batch as STRIPS of row blocks that may share a tile: the blocks of a single-frame segment (nearly equal heights <= 128);
+  // one block of patch rows [r0, r0 + R) of a video segment through all its frames (block i = frame i); the overlapping windows
+  // of a short-frame segment (128 - P scored rows each).  A tile takes up to NS consecutive blocks of a strip.
+  struct Strip { int32_t seg, mode, r0, R, P; int64_t n, nblk; double cb, c_q, c_halo; };
   std::vector<Strip> strips;
   for (int32_t k = 0; k < n_segs; ++k) {
     const mas_segment& s = segs[k];
     const int L = (int)(q_off[s.request + 1] - q_off[s.request]);
-    const double c_fix = cw.w_q * ((L + 15) / 16 * 16 + (rider ? 64 : 0)) + cw.c_tile;
+    const double c_q = cw.w_q * ((L + 15) / 16 * 16 + (rider ? 64 : 0));   // the query rows a tile streams (scaled by its share of K)
     const int64_t n = (int64_t)s.n_frames * s.n_patches;
+    auto blk = [&](double h) { return cw.c_blk + cw.w_row * h; };            // one block of h rows, per K-sweep
     if (s.n_frames == 1) {
-      strips.push_back(Strip{k, 0, 0, 0, 0, n, c_fix, (int64_t)128 * NS});
+      const int64_t nb = (n + 127) / 128;
+      strips.push_back(Strip{k, 0, 0, 0, 0, n, nb, blk((double)n / nb), c_q, 0.0});
     } else if (s.n_patches >= 64) {
       const int nb = (s.n_patches + 127) / 128;            // row blocks of nearly equal height
       for (int j = 0; j < nb; ++j) {
         const int r0 = (int)((int64_t)s.n_patches * j / nb), r1 = (int)((int64_t)s.n_patches * (j + 1) / nb);
-        strips.push_back(Strip{k, 1, r0, r1 - r0, s.n_patches, (int64_t)s.n_frames, c_fix, NS});
+        strips.push_back(Strip{k, 1, r0, r1 - r0, s.n_patches, n, (int64_t)s.n_frames, blk((double)(r1 - r0)), c_q, cw.c_blk + cw.w_halo * (r1 - r0)});
       }
     } else {
-      strips.push_back(Strip{k, 2, 0, 0, s.n_patches, n, c_fix, (int64_t)(128 - s.n_patches) * NS});
+      const int64_t sdt = 128 - s.n_patches;
+      strips.push_back(Strip{k, 2, 0, 0, s.n_patches, n, (n + sdt - 1) / sdt, blk(128.0), c_q, 0.0});
     }
   }
-  auto blk = [&](double h) { return cw.c_blk + cw.w_row * h; };   // one block of h rows, per K-sweep
-  auto tile_cost = [&](const Strip& st, int64_t n) {       // a tile of n units of the strip
-    if (st.mode == 0) { const int64_t nb = (n + 127) / 128; return (double)nb * blk((double)n / nb) + st.c_fix; }
-    if (st.mode == 1) return (double)n * blk((double)st.R) + (cw.c_blk + cw.w_halo * st.R) + st.c_fix;   // the halo chunk counted for every tile
-    const int64_t nb = (n + (128 - st.P) - 1) / (128 - st.P);
-    return (double)nb * blk(128.0) + st.c_fix;
+  const int S = (d / 64) / sc.kw;                          // K-steps of a full sweep
+  const bool can_split = ksplit && S >= 4;
+  // cost of m whole consecutive blocks of a strip, cut into the fewest tiles (halo counted for every video tile)
+  auto whole_cost = [&](const Strip& st, int64_t m) {
+    if (m <= 0) return 0.0;
+    const int64_t nt = (m + NS - 1) / NS;
+    return (double)m * st.cb + (double)nt * (st.c_q + cw.c_tile + st.c_halo);
   };
-  // a run of `rows` units is cut into the fewest tiles, of nearly equal size (the same split as emit() below)
-  auto piece_cost = [&](const Strip& st, int64_t rows) {
-    if (rows <= 0) return 0.0;
-    const int64_t nt = (rows + st.cap - 1) / st.cap;
-    return (double)(nt - rows % nt) * tile_cost(st, rows / nt) + (double)(rows % nt) * tile_cost(st, rows / nt + 1);
-  };
+  // cost of K-steps [0, steps) of ONE block as a tile of its own
+  auto part_cost = [&](const Strip& st, int steps) { return (st.cb + st.c_q + st.c_halo) * (double)steps / S + cw.c_tile; };
   double total = 0.0;
-  for (const Strip& st : strips) total += piece_cost(st, st.len);
-  const int n_ctas = (int)std::min<int64_t>(sm_count, std::max<int64_t>(1, (int64_t)(total / 96.0)));
+  for (const Strip& st : strips) total += whole_cost(st, st.nblk);
+  const int n_ctas = (int)std::min<int64_t>(std::min(sm_count, kTcMaxCtas), std::max<int64_t>(1, (int64_t)(total / 96.0)));
 
   std::vector<TcTile> tiles;
   std::vector<int> cta_first(n_ctas + 1, 0);
-  auto emit = [&](const Strip& st, int64_t a, int64_t take) {   // strip rows [a, a + take) -> tiles of nearly equal size
+  // blocks [i0, i1) of a strip, K-steps [s0, s1), as one tile
+  auto emit = [&](const Strip& st, int64_t i0, int64_t i1, int s0, int s1) {
     const mas_segment& s = segs[st.seg];
-    const int64_t nt = (take + st.cap - 1) / st.cap;
-    int64_t u = a;
-    for (int64_t i = 0; i < nt; ++i) {
-      const int64_t v = a + take * (i + 1) / nt;
-      TcTile t{};
-      t.mode = st.mode; t.seg = st.seg;
-      t.q_row0 = (int32_t)q_off[s.request];
-      t.L = (int32_t)(q_off[s.request + 1] - q_off[s.request]);
-      if (st.mode == 0) {
-        t.row0 = (int32_t)(s.row0 + u); t.n_rows = (int32_t)(v - u); t.n_blocks = (t.n_rows + 127) / 128;
-        t.stride = (t.n_rows + t.n_blocks - 1) / t.n_blocks;          // blocks of nearly equal height
-      } else if (st.mode == 1) {                            // frames [u, v) of the strip's row block
-        t.row0 = (int32_t)(s.row0 + u * s.n_patches + st.r0); t.n_rows = st.R; t.stride = s.n_patches; t.prev = s.n_patches;
-        t.n_blocks = (int32_t)(v - u); t.halo = u > 0 ? 1 : 0;
-      } else {
-        const int P = s.n_patches;
-        const int64_t a0 = u == 0 ? 0 : u - P;            // the window starts P rows early (their successors need them)
-        t.row0 = (int32_t)(s.row0 + a0); t.n_rows = (int32_t)(v - a0); t.stride = 128 - P; t.prev = P; t.halo = (int32_t)(u - a0);
-        t.n_blocks = t.n_rows <= 128 ? 1 : (t.n_rows - 128 + t.stride - 1) / t.stride + 1;
-      }
-      tiles.push_back(t);
-      u = v;
+    TcTile t{};
+    t.mode = st.mode; t.seg = st.seg;
+    t.q_row0 = (int32_t)q_off[s.request];
+    t.L = (int32_t)(q_off[s.request + 1] - q_off[s.request]);
+    t.k0 = s0 * sc.kw; t.k1 = s1 * sc.kw; t.peer = -1;
+    if (st.mode == 0) {
+      const int64_t u = st.n * i0 / st.nblk, v = st.n * i1 / st.nblk;
+      t.row0 = (int32_t)(s.row0 + u); t.n_rows = (int32_t)(v - u); t.n_blocks = (int32_t)(i1 - i0);
+      t.stride = (t.n_rows + t.n_blocks - 1) / t.n_blocks;            // blocks of nearly equal height
+      t.n_blocks = (t.n_rows + t.stride - 1) / t.stride;
+    } else if (st.mode == 1) {                              // frames [i0, i1) of the strip's row block
+      t.row0 = (int32_t)(s.row0 + i0 * s.n_patches + st.r0); t.n_rows = st.R; t.stride = s.n_patches; t.prev = s.n_patches;
+      t.n_blocks = (int32_t)(i1 - i0); t.halo = i0 > 0 ? 1 : 0;
+    } else {
+      const int P = s.n_patches;
+      const int64_t u = i0 * (128 - P), v = std::min<int64_t>(st.n, i1 * (128 - P));
+      const int64_t a0 = u == 0 ? 0 : u - P;              // the window starts P rows early (their successors need them)
+      t.row0 = (int32_t)(s.row0 + a0); t.n_rows = (int32_t)(v - a0); t.stride = 128 - P; t.prev = P; t.halo = (int32_t)(u - a0);
+      t.n_blocks = t.n_rows <= 128 ? 1 : (t.n_rows - 128 + t.stride - 1) / t.stride + 1;
     }
+    tiles.push_back(t);
   };
-  // One pass with a fixed per-CTA target: CTAs fill up to the target in strip order, the last one takes what is left.
-  // Returns the last CTA's load.  Every cut may add a tile's fixed cost, which no closed form anticipates: the smallest target
-  // whose last CTA does not overshoot is found by bisection.
+  auto emit_whole = [&](const Strip& st, int64_t i0, int64_t m) {   // m blocks -> the fewest tiles, of nearly equal size
+    const int64_t nt = (m + NS - 1) / NS;
+    for (int64_t i = 0; i < nt; ++i) emit(st, i0 + m * i / nt, i0 + m * (i + 1) / nt, 0, S);
+  };
+  // One pass with a fixed per-CTA target: CTAs fill up to the target in strip order; what is left of the target after the last
+  // whole block that fits is filled with the first K-steps of the next block (K-split: that CTA owns the block, the CTA(s) that
+  // follow sweep the remaining K-steps first thing and hand their partial sums over); the last CTA takes what is left.
+  // Returns the last CTA's load.  The smallest target whose last CTA does not overshoot is found by bisection.
   auto assign = [&](double target, bool commit) {
     int c = 0;
     double load = 0.0;
+    int owner = -1;                                     // index of the tile that owns the block being split
     if (commit) { tiles.clear(); std::fill(cta_first.begin(), cta_first.end(), 0); }
     auto close_cta = [&]() {
       if (c + 1 < n_ctas) { load = 0.0; ++c; if (commit) cta_first[c] = (int)tiles.size(); }
     };
     for (const Strip& st : strips) {
-      int64_t a = 0;
-      while (a < st.len) {
-        const int64_t left = st.len - a;
-        int64_t take = left;
-        if (c + 1 < n_ctas && load + piece_cost(st, left) > target) {
-          // the largest run whose cost still fits the gap (the cost is monotone in the rows)
-          int64_t lo = 0, hi = left;
-          while (lo < hi) { const int64_t mid = (lo + hi + 1) / 2; if (load + piece_cost(st, mid) <= target) lo = mid; else hi = mid - 1; }
-          take = lo;
-          const int64_t min_rows = st.mode == 2 ? 16 : st.mode == 1 ? 1 : 8;
-          if (take < min_rows) {          // not worth a tile of its own here
-            if (load > 0.0) { close_cta(); continue; }
-            take = std::min<int64_t>(left, min_rows);
+      int64_t i = 0;
+      int ks = 0;                                       // K-steps of block i already handed out
+      while (i < st.nblk) {
+        const bool last_cta = c + 1 >= n_ctas;
+        if (ks > 0) {                                   // the rest of a split block comes first in this CTA
+          int take = S - ks;
+          if (!last_cta && load + part_cost(st, take) > target) {
+            const int fit = (int)std::floor((target - load - cw.c_tile) / ((st.cb + st.c_q + st.c_halo) / S));
+            if (fit >= 2 && take - fit >= 2) take = fit;
           }
-          if (left - take < min_rows) take = left;
+          if (commit) {
+            emit(st, i, i + 1, ks, ks + take);
+            tiles.back().peer = c;
+            tiles[owner].n_wait += 1;
+            if (tiles[owner].peer < 0) tiles[owner].peer = c;
+          }
+          load += part_cost(st, take);
+          ks += take;
+          if (ks < S) { close_cta(); continue; }
+          ks = 0; ++i; owner = -1;
+          continue;
         }
-        if (commit) emit(st, a, take);
-        load += piece_cost(st, take);
-        a += take;
-        if (a < st.len) close_cta();
+        int64_t m = st.nblk - i;
+        if (!last_cta && load + whole_cost(st, m) > target) {
+          int64_t lo = 0, hi = m;
+          while (lo < hi) { const int64_t mid = (lo + hi + 1) / 2; if (load + whole_cost(st, mid) <= target) lo = mid; else hi = mid - 1; }
+          m = lo;
+          if (commit && m > 0) emit_whole(st, i, m);
+          load += whole_cost(st, m);
+          i += m;
+          // (not in a frame walk: a split frame would be two more single-frame tiles, each with its own halo and query stream)
+          int fit = can_split && st.mode != 1 ? (int)std::floor((target - load - cw.c_tile) / ((st.cb + st.c_q + st.c_halo) / S)) : 0;
+          if (fit > S - 2) fit = S - 2;
+          if (fit >= 2) {                               // the first K-steps of the next block: this CTA owns it
+            if (commit) { emit(st, i, i + 1, 0, fit); owner = (int)tiles.size() - 1; }
+            load += part_cost(st, fit);
+            ks = fit;
+          } else if (m == 0 && load == 0.0) {           // a target below one block: take it whole
+            if (commit) emit_whole(st, i, 1);
+            load += whole_cost(st, 1);
+            ++i;
+          }
+          close_cta();
+          continue;
+        }
+        if (commit) emit_whole(st, i, m);
+        load += whole_cost(st, m);
+        i += m;
       }
     }
-    if (commit) for (int i = c + 1; i <= n_ctas; ++i) cta_first[i] = (int)tiles.size();
+    if (commit) for (int k2 = c + 1; k2 <= n_ctas; ++k2) cta_first[k2] = (int)tiles.size();
     return load;
   };
   {
-    double lo = total / n_ctas, hi = 2.0 * total / n_ctas + 2048.0;   // assign(hi) never overshoots hi by more than a tile
-    for (int i = 0; i < 40; ++i) {
+    double lo = total / n_ctas, hi = 2.0 * total / n_ctas + 4096.0;   // assign(hi) never overshoots hi by more than a tile
+    for (int it = 0; it < 40; ++it) {
       const double mid = 0.5 * (lo + hi);
       if (assign(mid, false) <= mid + 1e-9) hi = mid; else lo = mid;
     }
@@ -797,7 +901,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
   const int n_tiles = (int)tiles.size();
   {   // NEXT-2 partial slots: one per block, contiguous per segment (tiles are in row order of their segment already)
     int part = 0;
-    for (TcTile& t : tiles) { t.part0 = part; part += t.n_blocks; }
+    for (TcTile& t : tiles) { t.part0 = part; if (!(t.peer >= 0 && t.n_wait == 0)) part += t.n_blocks; }
     sc.n_parts = part;
   }
   TcTile* ht = reinterpret_cast<TcTile*>(h_dst);
@@ -874,7 +978,7 @@ struct TcHeads { float* part; float* m; float bias, tau; };   // NEXT-2 riding t
 // `Rm` / `sig` (both NULL = off): NEXT-1, hash rows R[64, d] and the per-token signatures; requires every L <= 64.
 // `hf` (NULL = off): NEXT-2, Rm = the head weight rows; same requirement; sig is ignored then.
 inline cudaError_t tc_launch_score(const TcSchedule& sc, TcMapCache& cache, const void* X, const void* Q, float* qinv, float* s, float* dnorm,
-                                   float* rel, unsigned long long* q_ready, int64_t N, int64_t nQ, int d, bool inline_qprep, const void* Rm,
+                                   float* rel, unsigned long long* q_ready, float* xchg, unsigned int* xflag, int64_t N, int64_t nQ, int d, bool inline_qprep, const void* Rm,
                                    unsigned long long* sig, const TcHeads* hf, cudaStream_t st, bool pdl_in = false) {
   const bool rider = sig != nullptr || hf != nullptr;
   const TcMaps* maps = cache.get(X, N, Q, nQ, rider ? Rm : nullptr, d, sc.kw);
@@ -882,6 +986,7 @@ inline cudaError_t tc_launch_score(const TcSchedule& sc, TcMapCache& cache, cons
   TcParams p;
   p.tiles = sc.d_tiles; p.cta_off = sc.d_cta_off; p.qinv = qinv; p.Q = Q; p.nQ = nQ; p.q_ready = q_ready; p.sig = sig; p.s = s; p.dnorm = dnorm; p.rel = rel;
   p.d = d; p.n_kchunks = d / 64; p.kw = sc.kw; p.nx = sc.nx; p.nq = sc.nq; p.qslot_bytes = sc.qslot_bytes; p.wslot = sc.wslot; p.ns = sc.ns;
+  p.xchg = xchg; p.xflag = xflag; p.xchg_cols = sc.xchg_cols;
   p.heads_part = hf ? hf->part : nullptr; p.heads_m = hf ? hf->m : nullptr; p.heads_bias = hf ? hf->bias : 0.f; p.heads_tau = hf ? hf->tau : 0.f;
   if (hf) p.sig = nullptr;
   if (!inline_qprep) {   // qinv is already there: no CTA waits on another one, a plain launch will do

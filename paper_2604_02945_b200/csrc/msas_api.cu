@@ -29,8 +29,8 @@ static thread_local int g_last_cuda = 0;
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-  size_t segs, tiles, req, tc_sched, tc_sched_x, tc_segrank, frames, tables_end;   // uploaded tables (contiguous from 0)
-  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, heads_part, gridw, heads_cq, merge_part, merge_cnt, total;
+  size_t segs, tiles, req, tc_sched, tc_sched_x, tc_sched_u, tc_sched_xu, tc_segrank, tc_segrank_u, frames, tables_end;   // uploaded tables (contiguous from 0)
+  size_t qinv, s, gamma, rel, mas, mask, segout, nkept, keptoff, counter, tc_xflag, tc_xchg, heads_part, gridw, heads_cq, merge_part, merge_cnt, total;
 };
 
 struct mas_plan {
@@ -50,6 +50,7 @@ struct mas_plan {
   size_t pinned_bytes = 0;
   int sm_count = 148;
   TcSchedule tc{};            // tcgen05 fast-path schedule (tc.enabled == false -> generic kernels)
+  TcSchedule tcu{}, tcxu{};   // tc / tcx without K-split (no CTA waits for another one): used once a cooperative launch was refused
   TcSchedule tcx{};           // the schedule of the calls that append 64 B rows (mas_forward_lsh / mas_forward_heads; needs every L <= 64)
   mutable TcMapCache tc_maps; // tensor maps of the last few (X, Q, R) pointer sets (a plan is used by one host thread at a time)
   mutable bool tc_coop_ok = true;   // false once a cooperative launch was refused on this device: query norms get a launch of their own
@@ -147,6 +148,9 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.req = take(sizeof(int32_t) * (n_req + 1));
   l.tc_sched = take(tc_bytes);
   l.tc_sched_x = take(tc_bytes);   // the schedule of the calls that add 64 B rows (NEXT-1, NEXT-2)
+  l.tc_sched_u = take(tc_bytes);   // the same two schedules without K-split, for devices that refuse the cooperative launch
+  l.tc_sched_xu = take(tc_bytes);
+  l.tc_segrank_u = take(sizeof(int32_t) * (n_segs + 1));
   l.tc_segrank = take(sizeof(int32_t) * (n_segs + 1));   // first partial slot of every segment (TcTile::part0), NEXT-2
   l.frames = take(sizeof(DevFrame) * (size_t)n_frames);   // NEXT-3: first row and patch count of every frame
   l.tables_end = o;
@@ -160,6 +164,8 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.nkept = take(sizeof(int32_t) * n_segs);
   l.keptoff = take(sizeof(int64_t) * (n_segs + 1));
   l.counter = take(256);
+  l.tc_xflag = take(sizeof(unsigned int) * kTcMaxCtas);   // K-split: one flag and one exchange slot per CTA of the score kernel
+  l.tc_xchg = take(tc_xchg_bytes());
   l.heads_part = take(sizeof(float) * kHeadRows * std::max((size_t)n_tiles, tc_parts_max));   // NEXT-2 scratch: per-tile / per-block column sums
   l.merge_part = take(sizeof(float) * 1024 * (size_t)kMergeCtas);   // NEXT-3 scratch: row-split partial sums of the merged tokens
   l.merge_cnt = take(sizeof(int32_t) * (size_t)kMergeCtas);
@@ -289,19 +295,27 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
   }
   tc_build_schedule(p->tc, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched, p->ws + lay.tc_sched);
   tc_build_schedule(p->tcx, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched_x, p->ws + lay.tc_sched_x, true);
-  if (p->tcx.enabled) {   // per-segment range of partial slots (one per block of every tile; a segment's slots are contiguous)
-    const TcTile* tt = reinterpret_cast<const TcTile*>(h + lay.tc_sched_x);
-    int32_t* sr = reinterpret_cast<int32_t*>(h + lay.tc_segrank);
+  tc_build_schedule(p->tcu, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched_u, p->ws + lay.tc_sched_u, false, false);
+  tc_build_schedule(p->tcxu, h_segs, n_segs, h_q_off, d, dtype, p->sm_count, h + lay.tc_sched_xu, p->ws + lay.tc_sched_xu, true, false);
+  // per-segment range of partial slots (one per block of every tile that writes results; a segment's slots are contiguous)
+  auto seg_ranks = [&](const TcSchedule& sc, size_t sched_off, size_t rank_off) {
+    if (!sc.enabled) return;
+    const TcTile* tt = reinterpret_cast<const TcTile*>(h + sched_off);
+    int32_t* sr = reinterpret_cast<int32_t*>(h + rank_off);
     std::vector<int32_t> cnt(n_segs + 1, 0);
-    for (int i = 0; i < p->tcx.n_tiles; ++i) cnt[tt[i].seg + 1] += tt[i].n_blocks;
+    for (int i = 0; i < sc.n_tiles; ++i)
+      if (!(tt[i].peer >= 0 && tt[i].n_wait == 0)) cnt[tt[i].seg + 1] += tt[i].n_blocks;
     sr[0] = 0;
     for (int32_t k = 0; k < n_segs; ++k) sr[k + 1] = sr[k] + cnt[k + 1];
-  }
+  };
+  seg_ranks(p->tcx, lay.tc_sched_x, lay.tc_segrank);
+  seg_ranks(p->tcxu, lay.tc_sched_xu, lay.tc_segrank_u);
 
   // plan creation is set-up, not the hot path: it returns when the tables are on the device, so that the plan may be used on
   // any stream afterwards without further ordering (the entry points themselves never synchronise)
   e = cudaMemcpyAsync(p->ws, p->pinned, lay.tables_end, cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(p->ws + lay.counter, 0, 256, stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(p->ws + lay.tc_xflag, 0, sizeof(unsigned int) * kTcMaxCtas, stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess) { g_last_cuda = (int)e; (void)cudaGetLastError(); cudaFreeHost(p->pinned); delete p; return MAS_ERR_CUDA; }
   *out = p;
@@ -360,9 +374,10 @@ extern "C" int32_t mas_score_schedule(const mas_segment* h_segs, int32_t n_segs,
   const int32_t* off = reinterpret_cast<const int32_t*>(buf.data() + (size_t)sc.n_tiles * sizeof(TcTile));
   for (int c = 0; c < sc.n_ctas; ++c)
     for (int i = off[c]; i < off[c + 1] && i < cap_tiles; ++i) {
-      int32_t* o = out_tiles + (size_t)i * 12;
+      int32_t* o = out_tiles + (size_t)i * 16;
       o[0] = c; o[1] = t[i].row0; o[2] = t[i].n_rows; o[3] = t[i].n_blocks; o[4] = t[i].stride; o[5] = t[i].mode; o[6] = t[i].prev;
       o[7] = t[i].halo; o[8] = t[i].q_row0; o[9] = t[i].L; o[10] = t[i].seg; o[11] = t[i].part0;
+      o[12] = t[i].k0; o[13] = t[i].k1; o[14] = t[i].n_wait; o[15] = t[i].peer;
     }
   return sc.n_tiles;
 }
@@ -404,12 +419,19 @@ static int launch_score_mma(const mas_plan* p, const void* X, const void* Q, flo
 
 // a0-a3 on the tcgen05 path.  The query norms ride the score kernel's prologue (one cooperative launch) unless the plan asks for,
 // or the device forces, a launch of their own (k_qprep, then the plain score launch chained behind it).
-static int launch_score_tc(const mas_plan* p, const TcSchedule& sc, const void* X, const void* Q, float* s, float* dnorm, float* rel,
+static const TcSchedule& score_schedule_of(const mas_plan* p, bool rider) {
+  // K-split tiles make CTAs wait for one another: only where the launch can be cooperative (all CTAs co-resident)
+  return p->tc_coop_ok ? (rider ? p->tcx : p->tc) : (rider ? p->tcxu : p->tcu);
+}
+static int launch_score_tc(const mas_plan* p, bool rider, const void* X, const void* Q, float* s, float* dnorm, float* rel,
                            const void* Rm, unsigned long long* sig, const TcHeads* hf, cudaStream_t st, bool pdl) {
   unsigned long long* qr = p->at<unsigned long long>(p->lay.counter) + 8;
   float* qinv = p->at<float>(p->lay.qinv);
+  float* xchg = p->at<float>(p->lay.tc_xchg);
+  unsigned int* xflag = p->at<unsigned int>(p->lay.tc_xflag);
   if (p->tc_inline_qnorm && p->tc_coop_ok) {
-    const cudaError_t e = tc_launch_score(sc, p->tc_maps, X, Q, qinv, s, dnorm, rel, qr, p->N, p->nQ, p->d, true, Rm, sig, hf, st);
+    const cudaError_t e = tc_launch_score(score_schedule_of(p, rider), p->tc_maps, X, Q, qinv, s, dnorm, rel, qr, xchg, xflag, p->N, p->nQ, p->d, true,
+                                          Rm, sig, hf, st);
     if (e == cudaSuccess) return MAS_OK;
     if (e != cudaErrorCooperativeLaunchTooLarge && e != cudaErrorNotSupported) { g_last_cuda = (int)e; (void)cudaGetLastError(); return MAS_ERR_CUDA; }
     (void)cudaGetLastError();     // not all CTAs can be co-resident here (e.g. an MPS partition): remembered for the plan's lifetime
@@ -418,7 +440,7 @@ static int launch_score_tc(const mas_plan* p, const TcSchedule& sc, const void* 
   const bool chain = pdl && !(p->tc_inline_qnorm && !p->tc_coop_ok);
   int rc = launch_qprep(p, Q, st, chain);
   if (rc != MAS_OK) return rc;
-  CK(tc_launch_score(sc, p->tc_maps, X, Q, qinv, s, dnorm, rel, qr, p->N, p->nQ, p->d, false, Rm, sig, hf, st, chain));
+  CK(tc_launch_score(score_schedule_of(p, rider), p->tc_maps, X, Q, qinv, s, dnorm, rel, qr, xchg, xflag, p->N, p->nQ, p->d, false, Rm, sig, hf, st, chain));
   return MAS_OK;
 }
 
@@ -523,7 +545,7 @@ extern "C" int mas_score(const mas_plan* p, const void* X, const void* Q, float*
   int rc;
   if (p->tc.enabled) {
     float* gb = gamma ? gamma : p->at<float>(p->lay.gamma);
-    if ((rc = launch_score_tc(p, p->tc, X, Q, s, gb, rel, nullptr, nullptr, nullptr, st, false)) != MAS_OK) return rc;
+    if ((rc = launch_score_tc(p, false, X, Q, s, gb, rel, nullptr, nullptr, nullptr, st, false)) != MAS_OK) return rc;
     if (gamma) {
       k_gamma_finish<<<p->n_tiles, 256, 0, st>>>(p->at<DevSeg>(p->lay.segs), p->at<DevTile>(p->lay.tiles), s, gamma, sqrtf((float)p->d));
       CK(cudaGetLastError());
@@ -649,7 +671,7 @@ static int heads_finish(const mas_plan* p, const float* gamma, const mas_heads* 
   HeadsArgs h;
   h.segs = p->at<DevSeg>(p->lay.segs); h.req_seg_off = p->at<int32_t>(p->lay.req);
   h.n_segs = p->n_segs; h.n_requests = p->n_requests; h.tile_rows = generic_tile_rows(p->N); h.hidden = hd->hidden;
-  h.prm = p->prm; h.part = p->at<float>(p->lay.heads_part); h.slot_rank = tc_slots ? p->at<int32_t>(p->lay.tc_segrank) : nullptr;
+  h.prm = p->prm; h.part = p->at<float>(p->lay.heads_part); h.slot_rank = tc_slots ? p->at<int32_t>(p->tc_coop_ok ? p->lay.tc_segrank : p->lay.tc_segrank_u) : nullptr;
   h.cq = cq; h.gamma = gamma; h.b1 = hd->b1; h.w2 = hd->w2; h.b2 = hd->b2;
   h.seg_out = seg_out; h.done_counter = p->at<unsigned int>(p->lay.counter);
   CK(launch_k(k_heads_finish, dim3((unsigned)p->n_segs), dim3(p->seg_cluster * p->seg_threads > 1024 ? 1024u : 256u), 0, st, pdl, h));
@@ -691,10 +713,9 @@ static int forward_impl(const mas_plan* p, const void* X, const void* Q, float* 
   if (pev) CK(cudaEventRecord(pev[0], st));
   int rc;
   const bool pdl = pev == nullptr;   // stage events between the kernels would serialise them anyway
-  const TcSchedule& sc = (Rm != nullptr || hf != nullptr) ? p->tcx : p->tc;
   if (p->tc.enabled) {
     // a0-a3 in one launch: TMA + tcgen05, query norms in its prologue; gb receives sqrt(D), finished into gamma by the segment kernel
-    if ((rc = launch_score_tc(p, sc, X, Q, sb, gb, rb, Rm, sig, hf, st, pdl)) != MAS_OK) return rc;
+    if ((rc = launch_score_tc(p, Rm != nullptr || hf != nullptr, X, Q, sb, gb, rb, Rm, sig, hf, st, pdl)) != MAS_OK) return rc;
   } else {
     if ((rc = launch_qprep(p, Q, st)) != MAS_OK) return rc;
     if ((rc = launch_score_mma(p, X, Q, sb, gb, rb, nullptr, st)) != MAS_OK) return rc;

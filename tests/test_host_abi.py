@@ -120,21 +120,26 @@ def _scored_rows(t):
 def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
     rng = np.random.default_rng(7)
     rows, q_off = _segments_of(kind, rng)
-    t = B.score_schedule(rows, q_off, 4096, B.MAS_BF16, 148)
+    d = 4096
+    t = B.score_schedule(rows, q_off, d, B.MAS_BF16, 148)
     N = sum(r[2] * r[3] for r in rows)
     assert len(t) > 0
-    cov = np.zeros(N, np.int32)
+    nk = d // 64
+    cov = np.zeros(N, np.int32)                                  # K-chunks swept per row: every row needs all nk of them, once
+    owned = np.zeros(N, np.int32)                                # tiles that WRITE the row's results
     seg_of_row = np.concatenate([np.full(r[2] * r[3], k) for k, r in enumerate(rows)])
     row0_of, q0_of = np.cumsum([0] + [r[2] * r[3] for r in rows]), [int(q_off[r[0]]) for r in rows]
     maxL = int(np.diff(q_off).max())
     n_slots = min(10, 512 // ((maxL + 15) // 16 * 16))           # TMEM accumulator slots of pad16(longest query block) columns
     cost = np.zeros(148)
+    split_open = None                                            # (rows, next k0, owner record) of a block being shared along K
     for rec in t:
-        cta, r0, n, nb, stride, mode, prev, halo, q0, L, seg, part0 = [int(v) for v in rec]
+        cta, r0, n, nb, stride, mode, prev, halo, q0, L, seg, part0, k0, k1, n_wait, peer = [int(v) for v in rec]
         T, P = rows[seg][2], rows[seg][3]
         assert 0 <= cta < 148 and 1 <= nb <= n_slots
         assert q0 == q0_of[seg] and L == q_off[rows[seg][0] + 1] - q_off[rows[seg][0]]
         assert mode == (0 if T == 1 else 1 if P >= 64 else 2)
+        assert 0 <= k0 < k1 <= nk and k0 % 2 == 0 and k1 % 2 == 0   # two K-slices per chunk at d % 128 == 0
         if mode == 0:
             assert stride == -(-n // nb) and prev == 0 and halo == 0 and nb == (n + 127) // 128     # blocks of nearly equal height
         elif mode == 1:
@@ -147,27 +152,51 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
             assert halo == (0 if r0 == row0_of[seg] else P)               # only a segment's first window starts without predecessors
             assert nb == (1 if n <= 128 else -(-(n - 128) // stride) + 1)
             assert n - (nb - 1) * stride > P                               # the last window scores at least one row
-        for lo, hi in _scored_rows(rec):
+        ranges = _scored_rows(rec)
+        for lo, hi in ranges:
             assert lo < hi and seg_of_row[lo] == seg and seg_of_row[hi - 1] == seg    # a tile never straddles a segment
-            cov[lo:hi] += 1
-        # cost model of csrc/k_score_tc.cuh (TcCost): 56 + 0.5625 h per block of h rows (a block costs nearly the same whatever
-        # its height), the halo chunk, 0.5 per padded query row and 24 per tile
+            cov[lo:hi] += k1 - k0
+        # K-split: only single-block tiles; the owner (k0 = 0) comes last in its CTA, the other parts first in the CTAs that follow
+        if (k0, k1) != (0, nk):
+            assert nb == 1
+            if k0 == 0:
+                assert split_open is None and n_wait >= 1 and peer == cta + 1
+                assert rec is t[t[:, 0] == cta][-1] or np.array_equal(rec, t[t[:, 0] == cta][-1])
+                split_open = [ranges, k1, cta, n_wait]
+            else:
+                assert split_open is not None and ranges == split_open[0] and k0 == split_open[1]
+                assert n_wait == 0 and peer == cta and np.array_equal(rec, t[t[:, 0] == cta][0])
+                assert cta == split_open[2] + 1
+                split_open[1], split_open[2], split_open[3] = k1, cta, split_open[3] - 1
+                if k1 == nk:
+                    assert split_open[3] == 0
+                    split_open = None
+        else:
+            assert n_wait == 0 and peer == -1
+        if k0 == 0:
+            for lo, hi in ranges:
+                owned[lo:hi] += 1
+        # cost model of csrc/k_score_tc.cuh (TcCost): 16 + 0.875 h per block of h rows, the halo chunk, 0.2 per padded query row
+        # (all scaled by the share of K) and 6 per tile
+        frac = (k1 - k0) / nk
         if mode == 0:
-            blocks = nb * (56 + 0.5625 * n / nb)
+            blocks = nb * (16 + 0.875 * n / nb)
         elif mode == 1:
-            blocks = nb * (56 + 0.5625 * n) + halo * (56 + 0.25 * n)
+            blocks = nb * (16 + 0.875 * n) + halo * (16 + 0.25 * n)
         else:
             blocks = nb * 128.0
-        cost[cta] += blocks + 0.5 * ((L + 15) // 16 * 16) + 24.0
-    assert cov.min() == 1 and cov.max() == 1                     # every row scored exactly once
+        cost[cta] += frac * (blocks + 0.2 * ((L + 15) // 16 * 16)) + 6.0
+    assert split_open is None
+    assert cov.min() == nk and cov.max() == nk                   # every K-chunk of every row swept exactly once
+    assert owned.min() == 1 and owned.max() == 1                 # and its results written by exactly one tile
     assert np.all(np.diff(t[:, 0]) >= 0)                         # grouped per CTA, CTAs in order
     if N >= 148 * 128:
-        # contiguous runs at a common target: the last CTAs may stay idle when cuts add tiles, the heaviest stays near the mean
+        # equal cost per CTA: K-split fills every CTA to the common target
         assert np.count_nonzero(cost) >= 140 and cost.max() <= 1.10 * cost.sum() / 148, (cost.max(), cost.sum() / 148)
 
 
 def test_score_schedule_rider_variant_and_small_devices(B):
-    """Few SMs, and a long single-frame segment: tiles of up to 8 blocks, every row once."""
+    """Few SMs, and a long single-frame segment: tiles of up to 4 blocks (L = 128), every K-chunk of every row once."""
     rows, q_off = [(0, 1, 1, 5000, 10), (1, 2, 9, 100, 10), (2, 3, 700, 1, 10)], np.array([0, 64, 70, 198], np.int64)
     for sms in (1, 3, 148):
         t = B.score_schedule(rows, q_off, 128, B.MAS_BF16, sms)
@@ -175,8 +204,8 @@ def test_score_schedule_rider_variant_and_small_devices(B):
         for rec in t:
             assert int(rec[3]) <= 4                              # L = 128 somewhere: four 128-column accumulator slots
             for lo, hi in _scored_rows(rec):
-                cov[lo:hi] += 1
-        assert cov.min() == 1 and cov.max() == 1 and t[:, 0].max() < sms
+                cov[lo:hi] += int(rec[13]) - int(rec[12])
+        assert cov.min() == 2 and cov.max() == 2 and t[:, 0].max() < sms      # d = 128: two K-chunks
 
 
 def test_score_schedule_rejects_bad_descriptors_and_generic_shapes(B):
