@@ -214,6 +214,7 @@ struct TcCtrl {                      // lives at the (1024-aligned) start of dyn
   uint32_t tmem_base;
   uint32_t pad_[31];
   float hred[2][4][64];              // NEXT-2: per-warp column sums of the 64 head columns, double buffered
+  float qinv_s[kMaxL];               // 1 / |q_j| of the tile the epilogue is working on
 };
 static_assert(sizeof(TcCtrl) <= kTcCtrlBytes, "control block too large");
 
@@ -519,9 +520,19 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const TcTile tile = p.tiles[t];
       const int buf = it & 1;
       const int nqu = (tile.L + 15) >> 4;
-      const float* qinv = p.qinv + tile.q_row0;
       const float2* st2 = reinterpret_cast<const float2*>(stat) + (size_t)buf * kTcMaxBlocks * 128;
       const bool dump = tile.peer >= 0 && tile.n_wait == 0;          // K-split: this part hands its partial sums to the block's owner
+      if (!dump) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
+        if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
+          unsigned long long seen;
+          do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
+          q_ok = true;
+        }
+        asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps are done with the previous tile's values
+        if (r < tile.L) ctrl->qinv_s[r] = p.qinv[tile.q_row0 + r];
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+      }
+      const float* qinv = ctrl->qinv_s;
       const int n_wait = tile.n_wait;
       const size_t xslot_f = (size_t)p.xchg_cols * 128;              // floats per exchange slot
       for (int b = 0; b < tile.n_blocks; ++b) {
@@ -552,11 +563,6 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + tile.peer), "r"(1u) : "memory");
           continue;
         }
-        if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
-          unsigned long long seen;
-          do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
-          q_ok = true;
-        }
         if (n_wait > 0) {   // owner of a split block: the other parts were swept first by the CTAs that follow this one
           if (lane == 0)
             for (int i = 0; i < n_wait; ++i) {
@@ -582,13 +588,34 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         const bool valid = r < hb && r >= out_lo;
         const int64_t row = (int64_t)tile.row0 + (int64_t)b * tile.stride + r;
         float m = -INFINITY;
-        for (int cb = 0; cb < nqu; ++cb) {
-          float v[16];
-          ld16(cb, v);
+        if (n_wait == 0) {   // the common case: two column groups in flight per wait
+          for (int cb = 0; cb < nqu; cb += 2) {
+            uint32_t v0[16], v1[16];
+            tc_ld16(tcol + (uint32_t)cb * 16u, v0);
+            if (cb + 1 < nqu) tc_ld16(tcol + (uint32_t)(cb + 1) * 16u, v1);
+            tc_wait_ld();
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const int col = cb * 16 + j;
-            if (col < tile.L) m = fmaxf(m, v[j] * qinv[col]);
+            for (int j = 0; j < 16; ++j) {
+              const int col = cb * 16 + j;
+              if (col < tile.L) m = fmaxf(m, __uint_as_float(v0[j]) * qinv[col]);
+            }
+            if (cb + 1 < nqu) {
+#pragma unroll
+              for (int j = 0; j < 16; ++j) {
+                const int col = cb * 16 + 16 + j;
+                if (col < tile.L) m = fmaxf(m, __uint_as_float(v1[j]) * qinv[col]);
+              }
+            }
+          }
+        } else {
+          for (int cb = 0; cb < nqu; ++cb) {
+            float v[16];
+            ld16(cb, v);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+              const int col = cb * 16 + j;
+              if (col < tile.L) m = fmaxf(m, v[j] * qinv[col]);
+            }
           }
         }
         if (p.heads_part != nullptr) {   // NEXT-2: column 0 -> the learned spatial map, all 64 -> per-block column sums (fixed order)
