@@ -798,7 +798,9 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     } else if (s.n_patches >= 64) {
       const int nb = (s.n_patches + 127) / 128;            // row blocks of nearly equal height
       for (int j = 0; j < nb; ++j) {
-        const int r0 = (int)((int64_t)s.n_patches * j / nb), r1 = (int)((int64_t)s.n_patches * (j + 1) / nb);
+        // nearly equal heights in whole 8-row swizzle atoms (a TMA box is a whole number of them): no row is fetched by two CTAs
+        const int oct = (s.n_patches + 7) / 8;
+        const int r0 = 8 * (int)((int64_t)j * oct / nb), r1 = j + 1 == nb ? s.n_patches : 8 * (int)((int64_t)(j + 1) * oct / nb);
         strips.push_back(Strip{k, 1, r0, r1 - r0, s.n_patches, n, (int64_t)s.n_frames, blk((double)(r1 - r0)), c_q, cw.c_blk + cw.w_halo * (r1 - r0)});
       }
     } else {
@@ -831,9 +833,13 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     t.L = (int32_t)(q_off[s.request + 1] - q_off[s.request]);
     t.k0 = s0 * sc.kw; t.k1 = s1 * sc.kw; t.peer = -1;
     if (st.mode == 0) {
-      const int64_t u = st.n * i0 / st.nblk, v = st.n * i1 / st.nblk;
-      t.row0 = (int32_t)(s.row0 + u); t.n_rows = (int32_t)(v - u); t.n_blocks = (int32_t)(i1 - i0);
-      t.stride = (t.n_rows + t.n_blocks - 1) / t.n_blocks;            // blocks of nearly equal height
+      // nearly equal blocks cut at whole 8-row swizzle atoms (no row is fetched by two CTAs); inside the tile the kernel walks
+      // blocks of `stride` rows
+      const int64_t oct = (st.n + 7) / 8;
+      auto cut = [&](int64_t i) { return i >= st.nblk ? st.n : 8 * (i * oct / st.nblk); };
+      const int64_t u = cut(i0), v = cut(i1);
+      t.row0 = (int32_t)(s.row0 + u); t.n_rows = (int32_t)(v - u);
+      t.stride = (int32_t)(((t.n_rows + (i1 - i0) - 1) / (i1 - i0) + 7) / 8 * 8);
       t.n_blocks = (t.n_rows + t.stride - 1) / t.stride;
     } else if (st.mode == 1) {                              // frames [i0, i1) of the strip's row block
       t.row0 = (int32_t)(s.row0 + i0 * s.n_patches + st.r0); t.n_rows = st.R; t.stride = s.n_patches; t.prev = s.n_patches;

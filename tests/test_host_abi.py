@@ -141,7 +141,8 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
         assert mode == (0 if T == 1 else 1 if P >= 64 else 2)
         assert 0 <= k0 < k1 <= nk and k0 % 2 == 0 and k1 % 2 == 0   # two K-slices per chunk at d % 128 == 0
         if mode == 0:
-            assert stride == -(-n // nb) and prev == 0 and halo == 0 and nb == (n + 127) // 128     # blocks of nearly equal height
+            assert stride % 8 == 0 and stride <= 128 and prev == 0 and halo == 0 and nb == -(-n // stride)   # blocks of nearly equal height
+            assert (r0 - row0_of[seg]) % 8 == 0                                                   # cut at whole 8-row swizzle atoms
         elif mode == 1:
             assert stride == P and prev == P and 1 <= n <= 128 and halo in (0, 1)
             t0 = (r0 - row0_of[seg]) // P
