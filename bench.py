@@ -263,7 +263,7 @@ def bench_workload(name, args, rank, local_rank, world, sampler, want_e2e):
     # at each end.  The stage events above sit BETWEEN the kernels of a step and serialise them, so their score figure also
     # holds one launch latency; this loop is the kernel's average launch duration in a stream of its own launches.
     sbuf = (torch.empty(w.n_tokens, dtype=torch.float32, device="cuda"), None, torch.empty(w.n_tokens, dtype=torch.float32, device="cuda"))
-    n_alone = min(max(args.steps, 20), 200)
+    n_alone = min(max(args.steps, 20), 50)      # a short burst: the kernel timed alone (MEASURED_PEAKS' copy figure is a burst figure too)
     for i in range(3):
         plan.score(Xs[i % 2], Qs[i % 2], want_gamma=False, out=sbuf)
     torch.cuda.synchronize()
