@@ -148,6 +148,13 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
                "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
                : "memory");
 }
+// the same with an L2 eviction-priority hint (createpolicy): the bulk of X is read once and should not push the query rows,
+// the halo frames and the exchange slots out of L2
+__device__ __forceinline__ void tma_load_3d_hint(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5}], [%2], %6;" ::"r"(dst),
+               "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "l"(pol)
+               : "memory");
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
@@ -399,6 +406,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   if (warp == kTcWarpTma) {
     // ===================================================================== TMA producer (the whole warp walks the list, one lane issues)
     uint32_t xs = 0, xph = 0, qs = 0, qph = 0;
+    uint64_t pol_stream, pol_keep;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
     for (int t = tile_lo; t < tile_hi; ++t) {
       const TcTile tile = p.tiles[t];
       const int nqu = (tile.L + 15) >> 4;
@@ -413,10 +423,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             uint32_t sq = qring + qs * (uint32_t)p.qslot_bytes;
             for (int j = 0; j < kw; ++j) {
               int qr = tile.q_row0;
-              for (int i = 0; i < (nqu >> 2); ++i) { tma_load_3d(sq, &maps.q[0], bar, 0, qr, kc + j); sq += 8192; qr += 64; }
-              if (nqu & 2) { tma_load_3d(sq, &maps.q[1], bar, 0, qr, kc + j); sq += 4096; qr += 32; }
-              if (nqu & 1) { tma_load_3d(sq, &maps.q[2], bar, 0, qr, kc + j); sq += 2048; }
-              if (rider) { tma_load_3d(sq, &maps.r, bar, 0, 0, kc + j); sq += 8192; }
+              for (int i = 0; i < (nqu >> 2); ++i) { tma_load_3d_hint(sq, &maps.q[0], bar, 0, qr, kc + j, pol_keep); sq += 8192; qr += 64; }
+              if (nqu & 2) { tma_load_3d_hint(sq, &maps.q[1], bar, 0, qr, kc + j, pol_keep); sq += 4096; qr += 32; }
+              if (nqu & 1) { tma_load_3d_hint(sq, &maps.q[2], bar, 0, qr, kc + j, pol_keep); sq += 2048; }
+              if (rider) { tma_load_3d_hint(sq, &maps.r, bar, 0, 0, kc + j, pol_keep); sq += 8192; }
             }
           }
           if (++qs == (uint32_t)p.nq) { qs = 0; qph ^= 1u; }
@@ -430,7 +440,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             mbar_expect_tx(bar, (uint32_t)h8 * 1024u * (uint32_t)kw);
             // one box = kw slices of h8 * 8 rows, slice after slice; rows past the end of X are zero-filled by the TMA unit,
             // rows past the block are never used
-            tma_load_3d(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc);
+            // a video tile's halo and last frame are read by two CTAs (as halo and as a block): ordinary priority; the rest of X
+            // is read once: evict first
+            if (tile.mode == 1 && (b < 0 || b == tile.n_blocks - 1)) tma_load_3d(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc);
+            else tma_load_3d_hint(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc, pol_stream);
           }
           if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
         }
