@@ -750,6 +750,7 @@ struct TcCost {
   // the query rows it streams (by its share of K) and a constant.  With all CTAs running the machine is HBM-bound, so bytes
   // dominate: constants from A/B runs on the images / video configs (profiles/r02_schedule.md).
   double c_blk = 16.0, w_row = 0.875, w_halo = 0.25, w_q = 0.2, c_tile = 6.0;
+  double f_short = 1.3;   // a window of a short-frame segment reads every row twice from shared memory and differences all of them
 };
 
 inline size_t tc_max_tiles(const mas_segment* segs, int32_t n_segs) {
@@ -804,7 +805,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     const int L = (int)(q_off[s.request + 1] - q_off[s.request]);
     const double c_q = cw.w_q * ((L + 15) / 16 * 16 + (rider ? 64 : 0));   // the query rows a tile streams (scaled by its share of K)
     const int64_t n = (int64_t)s.n_frames * s.n_patches;
-    auto blk = [&](double h) { return cw.c_blk + cw.w_row * h; };            // one block of h rows, per K-sweep
+    auto blk = [&](double h) { return (s.n_frames > 1 && s.n_patches < 64 ? cw.f_short : 1.0) * (cw.c_blk + cw.w_row * h); };            // one block of h rows, per K-sweep
     if (s.n_frames == 1) {
       const int64_t nb = (n + 127) / 128;
       strips.push_back(Strip{k, 0, 0, 0, 0, n, nb, blk((double)n / nb), c_q, 0.0});
