@@ -177,15 +177,15 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
         if k0 == 0:
             for lo, hi in ranges:
                 owned[lo:hi] += 1
-        # cost model of csrc/k_score_tc.cuh (TcCost): 16 + 0.875 h per block of h rows, the halo chunk, 0.2 per padded query row
-        # (all scaled by the share of K) and 6 per tile
+        # cost model of csrc/k_score_tc.cuh (TcCost): 16 + 0.875 h per block of h rows, the halo chunk, 0.2 per padded query row,
+        # a window of a short-frame segment 1.3 x a full block (all scaled by the share of K) and 6 per tile
         frac = (k1 - k0) / nk
         if mode == 0:
             blocks = nb * (16 + 0.875 * n / nb)
         elif mode == 1:
             blocks = nb * (16 + 0.875 * n) + halo * (16 + 0.25 * n)
         else:
-            blocks = nb * 128.0
+            blocks = nb * 1.3 * 128.0                              # a short-frame window: 1.3 x a full block
         cost[cta] += frac * (blocks + 0.2 * ((L + 15) // 16 * 16)) + 6.0
     assert split_open is None
     assert cov.min() == nk and cov.max() == nk                   # every K-chunk of every row swept exactly once
