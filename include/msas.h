@@ -259,6 +259,21 @@ int mas_draft_entropy_workspace_bytes(int64_t n_rows, int64_t V, size_t* out_byt
 int mas_draft_entropy(const void* logits, int64_t n_rows, int64_t V, int64_t row_stride, int32_t dtype, float theta_conf,
                       float* H, uint8_t* speculate, void* d_workspace, size_t workspace_bytes, mas_stream_t stream);
 
+/* The same for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): no workspace argument, and the call allocates nothing -- no cudaMalloc / cudaFree, no allocating library
+ * routine.  The per-row partial sums (one {max, sum, sum of l e^l} triple per slice of a row) live in a static device array of
+ * MAS_DRAFT_ENTROPY_STATIC_MAX_PARTIALS triples (12 bytes each: 192 KiB) that every GPU which loads the library holds until the
+ * process exits.  Arguments, results and arithmetic are those of mas_draft_entropy (bit-identical H and speculate).
+ * Returns MAS_ERR_WORKSPACE when n_rows x (slices per row, at most ceil(V / 8192) and about 4 x SM count / n_rows) exceeds
+ * MAS_DRAFT_ENTROPY_STATIC_MAX_PARTIALS -- nothing is launched then (a row has one slice from 4 x SM count rows on: any
+ * n_rows <= 16384 fits).  Every call on a device
+ * shares the one array, which keeps the last call's contents (every triple a call reads it has written first, so nothing needs
+ * clearing): calls that overlap on the GPU -- two streams, or two threads -- race; order them on one stream or with events.
+ * The array's device address is looked up once per device (cudaGetSymbolAddress, the device current) on the first call there. */
+#define MAS_DRAFT_ENTROPY_STATIC_MAX_PARTIALS 16384
+int mas_draft_entropy_static(const void* logits, int64_t n_rows, int64_t V, int64_t row_stride, int32_t dtype, float theta_conf,
+                             float* H, uint8_t* speculate, mas_stream_t stream);
+
 /* ---- end-to-end convenience: HOST inputs -> HOST outputs.
  * Copies h_X -> d_X and h_Q -> d_Q (cudaMemcpyAsync; pinned host memory recommended), runs mas_forward into d_out,
  * copies every non-NULL member of h_out back (Y/kept_idx: only the rows actually kept) and SYNCHRONISES the stream

@@ -21,7 +21,7 @@ MAS_MAX_QUERY_TOKENS = 128
 EXPORTS = ["mas_version", "mas_last_cuda_error", "mas_status_string", "mas_params_default", "mas_keep_count",
            "mas_plan_workspace_bytes", "mas_plan_create", "mas_plan_destroy", "mas_plan_n_tokens", "mas_plan_n_queries",
            "mas_plan_kept_capacity", "mas_plan_forward_launches", "mas_plan_enable_profiling", "mas_plan_stage_times", "mas_spatial", "mas_temporal", "mas_crossmodal", "mas_fuse",
-           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_forward_host_async", "mas_score", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_learned_heads", "mas_forward_heads", "mas_plan_n_frames", "mas_spatial_pool", "mas_merge_dropped",
+           "mas_select_compact", "mas_forward", "mas_forward_host", "mas_forward_host_async", "mas_score", "mas_score_schedule", "mas_plan_set_inline_query_norms", "mas_temporal_lsh", "mas_forward_lsh", "mas_draft_entropy_workspace_bytes", "mas_draft_entropy", "mas_draft_entropy_static", "mas_learned_heads", "mas_forward_heads", "mas_plan_n_frames", "mas_spatial_pool", "mas_merge_dropped",
            "mas_gather_residual"]
 
 
@@ -103,6 +103,8 @@ def _load():
     lib.mas_draft_entropy_workspace_bytes.restype = C.c_int
     lib.mas_draft_entropy.argtypes = [vp, i64, i64, i64, i32, C.c_float, vp, vp, vp, C.c_size_t, vp]
     lib.mas_draft_entropy.restype = C.c_int
+    lib.mas_draft_entropy_static.argtypes = [vp, i64, i64, i64, i32, C.c_float, vp, vp, vp]
+    lib.mas_draft_entropy_static.restype = C.c_int
     lib.mas_learned_heads.argtypes = [vp, vp, vp, vp, C.POINTER(mas_heads), vp, vp, vp]
     lib.mas_learned_heads.restype = C.c_int
     lib.mas_forward_heads.argtypes = [vp, vp, vp, C.POINTER(mas_heads), vp, vp, C.POINTER(mas_outputs), vp]
@@ -391,6 +393,19 @@ def draft_entropy(logits, theta_conf, workspace=None, H=None, speculate=None, st
     _check(lib.mas_draft_entropy(_ptr(logits), n, V, logits.stride(0), dt, float(theta_conf), _ptr(H), _ptr(sp), _ptr(ws), ws.numel(),
                                  _stream_ptr(stream)), "mas_draft_entropy")
     return H, sp
+
+
+DRAFT_ENTROPY_STATIC_MAX_PARTIALS = 16384   # include/msas.h, MAS_DRAFT_ENTROPY_STATIC_MAX_PARTIALS
+
+
+def draft_entropy_static(logits, theta_conf, H, speculate, stream=None):
+    """As draft_entropy, through the entry point that allocates nothing: the caller passes the outputs (H float32 [n_rows],
+    speculate uint8 [n_rows]; either may be None), the partial sums live in the library's static device array."""
+    n, V = logits.shape
+    dt = MAS_BF16 if logits.dtype == torch.bfloat16 else MAS_F32
+    _check(lib.mas_draft_entropy_static(_ptr(logits), n, V, logits.stride(0), dt, float(theta_conf), _ptr(H), _ptr(speculate),
+                                        _stream_ptr(stream)), "mas_draft_entropy_static")
+    return H, speculate
 
 
 def seg_out_numpy(t):

@@ -820,6 +820,49 @@ extern "C" int mas_draft_entropy(const void* logits, int64_t n_rows, int64_t V, 
   return MAS_OK;
 }
 
+// The same with the partial sums in a static device array: the call allocates nothing (include/msas.h).  In host code the array's
+// name is only a host-side stand-in: the kernels get its device address, looked up once per device with that device current.
+static __device__ __align__(256) EntTriple g_ent_static[MAS_DRAFT_ENTROPY_STATIC_MAX_PARTIALS];
+
+static int ent_static_address(EntTriple** out) {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static EntTriple* addr[kMaxDev] = {};
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDev) return MAS_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!addr[dev]) {
+    void* ptr = nullptr;
+    CK(cudaGetSymbolAddress(&ptr, g_ent_static));
+    addr[dev] = static_cast<EntTriple*>(ptr);
+  }
+  *out = addr[dev];
+  return MAS_OK;
+}
+
+extern "C" int mas_draft_entropy_static(const void* logits, int64_t n_rows, int64_t V, int64_t row_stride, int32_t dtype, float theta_conf,
+                                        float* H, uint8_t* speculate, mas_stream_t stream) {
+  if (!logits || n_rows < 1 || V < 1 || row_stride < V || (!H && !speculate)) return MAS_ERR_INVALID_ARG;
+  if (dtype != MAS_F32 && dtype != MAS_BF16) return MAS_ERR_INVALID_ARG;
+  const int esz = dtype == MAS_BF16 ? 2 : 4;
+  if (!aligned16(logits) || (row_stride * esz) % 16 != 0 || n_rows > 65535) return MAS_ERR_UNSUPPORTED;
+  int splits; int64_t chunk;
+  entropy_geometry(n_rows, V, &splits, &chunk);
+  if (n_rows * (int64_t)splits > (int64_t)MAS_DRAFT_ENTROPY_STATIC_MAX_PARTIALS) return MAS_ERR_WORKSPACE;   // beyond the static array
+  EntTriple* part = nullptr;
+  const int rc = ent_static_address(&part);
+  if (rc != MAS_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const dim3 grid((unsigned)splits, (unsigned)n_rows);
+  if (dtype == MAS_BF16) k_entropy_partial<1><<<grid, 256, 0, st>>>(logits, V, row_stride, chunk, part);
+  else k_entropy_partial<0><<<grid, 256, 0, st>>>(logits, V, row_stride, chunk, part);
+  CK(cudaGetLastError());
+  CK(launch_k(k_entropy_finish, dim3((unsigned)((n_rows + 3) / 4)), dim3(128), 0, st, true, (const EntTriple*)part, splits, n_rows, theta_conf,
+              H, speculate));
+  return MAS_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ host-buffer convenience
 static int forward_host_impl(const mas_plan* p, const void* h_X, const void* h_Q, void* d_X, void* d_Q, const mas_outputs* d_out,
                              const mas_outputs* h_out, mas_stream_t stream, bool final_sync) {
