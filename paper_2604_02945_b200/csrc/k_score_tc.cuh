@@ -49,11 +49,13 @@ struct TcTile {            // 64 bytes
   int32_t L;               // query tokens of the request
   int32_t part0;           // NEXT-2: slot of block 0's column sums (block b -> part0 + b); slots of a segment are contiguous
   int32_t seg;
-  // K-split (single-block tiles only): the tile covers K-chunks [k0, k1) of the row block.  The part that starts at chunk 0 OWNS
-  // the block: it adds the partial accumulators and row sums the other parts dumped and writes the results.
-  int32_t k0, k1;          // in 64-column chunks, multiples of the slices per chunk
-  int32_t n_wait;          // owner: number of foreign parts to add (they live in the exchange slots peer .. peer + n_wait - 1)
-  int32_t peer;            // dumping part: its exchange slot (= its CTA), -1 for ordinary tiles and owners; owner: first slot to read
+  // K-split: CTAs may share a row block along K.  The tile's FIRST block is swept over the K-chunks [k0, nk) only and its LAST
+  // block over [0, k1) only (a one-block tile: [k0, k1)); the blocks in between over all of K.  The part of a block that starts
+  // at chunk 0 OWNS it: it adds the partial accumulators and row sums the other parts dumped and writes the results.  A part
+  // with k0 > 0 dumps into the exchange slot of its CTA (a CTA holds at most one: the first block of its first tile).
+  int32_t k0, k1;          // in 64-column chunks, multiples of the slices per chunk; 0 and nk where the tile is not split
+  int32_t n_wait;          // owner (k1 < nk): number of foreign parts of the last block (exchange slots peer .. peer + n_wait - 1)
+  int32_t peer;            // owner: first exchange slot to read (the CTA after this one); -1 otherwise
   int32_t pad_;
 };
 static_assert(sizeof(TcTile) == 64, "TcTile is 64 bytes");
@@ -118,6 +120,11 @@ struct TcParams {
 __device__ __forceinline__ int tc_block_rows(const TcTile& t, int b) {
   return t.mode == 1 ? t.n_rows : min(t.mode == 0 ? t.stride : 128, t.n_rows - b * t.stride);
 }
+// K-chunks a tile walks, and the blocks that take part in chunk kc: block 0 joins at k0, the last block leaves at k1
+__device__ __forceinline__ int tc_k_lo(int n_blocks, int k0) { return n_blocks == 1 ? k0 : 0; }
+__device__ __forceinline__ int tc_k_hi(int n_blocks, int k1, int nk) { return n_blocks == 1 ? k1 : nk; }
+__device__ __forceinline__ int tc_b_first(int kc, int k0) { return kc < k0 ? 1 : 0; }
+__device__ __forceinline__ int tc_b_end(int kc, int k1, int n_blocks) { return kc >= k1 ? n_blocks - 1 : n_blocks; }
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -286,17 +293,19 @@ __device__ __forceinline__ void tc_alu_release(const TcAluCtx& c, uint32_t& xs, 
 }
 template <int KW>
 __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_rows, int n_blocks, int stride, int prev, bool halo,
-                                            int k0, int k1, uint32_t& xs, uint32_t& xph) {
+                                            int k0, int k1, int nk, uint32_t& xs, uint32_t& xph) {
   const uint32_t roff = (uint32_t)c.arow * 128u, sw = (uint32_t)(c.arow & 7);
   const uint32_t uoff = c.hh << 2;
   const int prow = c.arow - prev;                                        // mode 2: the previous frame's row in the same chunk
   const uint32_t proff = (uint32_t)prow * 128u, psw = (uint32_t)(prow & 7);
   const bool inchunk = mode == 2 && prow >= 0;
   const int hcap = mode == 0 ? stride : 128;
-  for (int kc = k0; kc < k1; kc += KW) {
+  for (int kc = tc_k_lo(n_blocks, k0); kc < tc_k_hi(n_blocks, k1, nk); kc += KW) {
+    const int bf = tc_b_first(kc, k0), be = tc_b_end(kc, k1, n_blocks);
+    if (bf >= be) continue;
     uint4 pv[KW][4];                  // this thread's K-slices of the previous frame's row (mode 1: carried from block to block)
     bool have_prev = false;
-    if (halo) {
+    if (mode == 1 && (halo || bf)) {  // frame t0 - 1, or frame t0 itself while block 0 has not joined yet
       mbar_wait(c.xfull0 + xs * 8u, xph);
       if (c.arow < n_rows) {
         const uint32_t slice = (uint32_t)((n_rows + 7) >> 3) * 1024u;
@@ -339,17 +348,17 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
       if (act) {   // lane pair (row): the even lane keeps sum x^2, the odd lane sum (x - x_prev)^2
         const float mine = c.hh ? D : n2;
         const uint32_t a = c.stat + (uint32_t)b * 1024u;
-        sts32(a, kc == k0 ? mine : lds32(a) + mine);
+        sts32(a, kc == (b == 0 ? k0 : 0) ? mine : lds32(a) + mine);
       }
     };
     uint4 xb[KW][4];
     if (mode == 1) {   // frame walk: the two register sets alternate between "this frame" and "previous frame" (no copies)
-      for (int b = 0; b < n_blocks; b += 2) {
+      for (int b = bf; b < be; b += 2) {
         step(b, xb, pv);
-        if (b + 1 < n_blocks) step(b + 1, pv, xb);
+        if (b + 1 < be) step(b + 1, pv, xb);
       }
     } else {
-      for (int b = 0; b < n_blocks; ++b) step(b, xb, pv);
+      for (int b = bf; b < be; ++b) step(b, xb, pv);
     }
   }
 }
@@ -413,8 +422,12 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const TcTile tile = p.tiles[t];
       const int nqu = (tile.L + 15) >> 4;
       const uint32_t qbytes = (uint32_t)(nqu + (rider ? 4 : 0)) * 2048u * (uint32_t)kw;
-      const int b_lo = (tile.mode == 1 && tile.halo) ? -1 : 0;      // block -1 = the halo chunk (frame t0 - 1)
-      for (int kc = tile.k0; kc < tile.k1; kc += kw) {
+      for (int kc = tc_k_lo(tile.n_blocks, tile.k0); kc < tc_k_hi(tile.n_blocks, tile.k1, nk); kc += kw) {
+        const int bf = tc_b_first(kc, tile.k0), be = tc_b_end(kc, tile.k1, tile.n_blocks);
+        if (bf >= be) continue;
+        // frame walk: the chunk of the frame before the first block taking part rides along for the statistics warps only (block -1 =
+        // frame t0 - 1, the halo; block 0 itself while it has not joined yet)
+        const int b_lo = tile.mode == 1 ? (bf ? 0 : (tile.halo ? -1 : 0)) : bf;
         {   // the request's query rows of these K-slices (+ the rider rows): one B tile per slice
           mbar_wait(qempty0 + 8u * qs, qph ^ 1u);
           if (elect_one()) {
@@ -431,7 +444,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           }
           if (++qs == (uint32_t)p.nq) { qs = 0; qph ^= 1u; }
         }
-        for (int b = b_lo; b < tile.n_blocks; ++b) {
+        for (int b = b_lo; b < be; ++b) {
           const int h = b < 0 ? tile.n_rows : tc_block_rows(tile, b);
           const int h8 = (h + 7) >> 3;                               // box height in 8-row swizzle atoms
           mbar_wait(xempty0 + 8u * xs, xph ^ 1u);
@@ -440,9 +453,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             mbar_expect_tx(bar, (uint32_t)h8 * 1024u * (uint32_t)kw);
             // one box = kw slices of h8 * 8 rows, slice after slice; rows past the end of X are zero-filled by the TMA unit,
             // rows past the block are never used
-            // a video tile's halo and last frame are read by two CTAs (as halo and as a block): ordinary priority; the rest of X
-            // is read once: evict first
-            if (tile.mode == 1 && (b < 0 || b == tile.n_blocks - 1)) tma_load_3d(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc);
+            // a video tile's halo and last frame are read by two CTAs (as halo and as a block), and so is the frame before a
+            // split last frame: ordinary priority; the rest of X is read once: evict first
+            if (tile.mode == 1 && (b < bf || b == tile.n_blocks - 1 || (b == tile.n_blocks - 2 && tile.k1 < nk))) tma_load_3d(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc);
             else tma_load_3d_hint(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc, pol_stream);
           }
           if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
@@ -456,8 +469,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const TcTile tile = p.tiles[t];
       const int nqb = ((tile.L + 15) >> 4) + (rider ? 4 : 0);
       const uint32_t idesc = umma_idesc_bf16(nqb << 4);   // N = pad16(L) (+ 64 rider rows)
-      const bool halo = tile.mode == 1 && tile.halo;
-      for (int kc = tile.k0; kc < tile.k1; kc += kw) {
+      for (int kc = tc_k_lo(tile.n_blocks, tile.k0); kc < tc_k_hi(tile.n_blocks, tile.k1, nk); kc += kw) {
+        const int bf = tc_b_first(kc, tile.k0), be = tc_b_end(kc, tile.k1, tile.n_blocks);
+        if (bf >= be) continue;
+        const bool halo = tile.mode == 1 && (tile.halo || bf);
         mbar_wait(qfull0 + 8u * qs, qph);
         tc_fence_after();
         const uint32_t qbase = qring + qs * (uint32_t)p.qslot_bytes;
@@ -467,10 +482,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           if (elect_one()) tc_commit(xempty0 + 8u * xs);
           if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
         }
-        for (int b = 0; b < tile.n_blocks; ++b) {
+        for (int b = bf; b < be; ++b) {
           uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
           if (ts >= ns) { ts -= ns; tp ^= 1u; }
-          if (kc == tile.k0) {   // the accumulator slot must have been drained by the epilogue of its previous use
+          const int kstart = b == 0 ? tile.k0 : 0;   // the block's first K-chunk
+          if (kc == kstart) {   // the accumulator slot must have been drained by the epilogue of its previous use
             mbar_wait(tempty0 + 8u * ts, tp ^ 1u);
             tc_fence_after();
           }
@@ -486,7 +502,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
               const uint64_t bdesc = umma_desc_sw128(qbase + (uint32_t)j * (uint32_t)nqb * 2048u);
 #pragma unroll
               for (int k = 0; k < 4; ++k)   // 4 x K=16 inside the 128-byte swizzle atom: +32 B = +2 in the 16-byte address field
-                tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kc - tile.k0) | j | k));
+                tc_mma_bf16(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kc - kstart) | j | k));
             }
             tc_commit(xempty0 + 8u * xs);
           }
@@ -534,8 +550,8 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int buf = it & 1;
       const int nqu = (tile.L + 15) >> 4;
       const float2* st2 = reinterpret_cast<const float2*>(stat) + (size_t)buf * kTcMaxBlocks * 128;
-      const bool dump = tile.peer >= 0 && tile.n_wait == 0;          // K-split: this part hands its partial sums to the block's owner
-      if (!dump) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
+      const bool dump0 = tile.k0 > 0;                                // K-split: block 0 is a part that hands its partial sums to the block's owner
+      if (!(dump0 && tile.n_blocks == 1)) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
         if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
           unsigned long long seen;
           do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
@@ -546,7 +562,6 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         asm volatile("bar.sync 1, 128;" ::: "memory");
       }
       const float* qinv = ctrl->qinv_s;
-      const int n_wait = tile.n_wait;
       const size_t xslot_f = (size_t)p.xchg_cols * 128;              // floats per exchange slot
       for (int b = 0; b < tile.n_blocks; ++b) {
         uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
@@ -554,8 +569,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         const uint32_t tcol = tmem_base + ts * (uint32_t)p.wslot + ((uint32_t)(q * 32) << 16);
         mbar_wait(smem_u32(&ctrl->tfull[ts]), tp);
         tc_fence_after();
-        if (dump) {   // accumulator columns (column-major: lanes = rows, coalesced), then the two row sums, then the flag
-          float* xo = p.xchg + (size_t)tile.peer * xslot_f + r;
+        const int n_wait = b == tile.n_blocks - 1 ? tile.n_wait : 0;   // > 0: this CTA owns a split last block
+        if (dump0 && b == 0) {   // accumulator columns (column-major: lanes = rows, coalesced), then the two row sums, then the flag
+          float* xo = p.xchg + (size_t)blockIdx.x * xslot_f + r;
           const int ncb = nqu + (rider ? 4 : 0);
           for (int cb = 0; cb < ncb; ++cb) {
             uint32_t v[16];
@@ -573,7 +589,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           xo[(size_t)(p.xchg_cols - 1) * 128] = nd.y;
           __threadfence();
           asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
-          if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + tile.peer), "r"(1u) : "memory");
+          if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + blockIdx.x), "r"(1u) : "memory");
           continue;
         }
         if (n_wait > 0) {   // owner of a split block: the other parts were swept first by the CTAs that follow this one
@@ -719,7 +735,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int buf = it & 1;
       c.stat = smem_u32(stat) + (uint32_t)buf * (kTcMaxBlocks * 1024u) + (uint32_t)(c.arow * 2 + (int)c.hh) * 4u;   // + b * 1024: block b
       mbar_wait(smem_u32(&ctrl->sempty[buf]), ((uint32_t)(it >> 1) & 1u) ^ 1u);
-      tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, tile.k0, tile.k1, xs, xph);
+      tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, tile.k0, tile.k1, nk, xs, xph);
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->sfull[buf]));
     }
@@ -745,12 +761,18 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
 // most 8 blocks, each tile paying a fixed cost for the query rows it streams.  Consecutive CTAs sweep neighbouring rows
 // of the same frames at the same time, so the halo chunks are L2 hits.
 struct TcCost {
-  // in token rows of one K-sweep.  A block of h rows costs c_blk + w_row * h (its bytes, plus what does not shrink with its height:
-  // M = 128 MMAs read 128 rows of shared memory whatever the block holds, every chunk is a barrier round trip); a tile pays for
-  // the query rows it streams (by its share of K) and a constant.  With all CTAs running the machine is HBM-bound, so bytes
-  // dominate: constants from A/B runs on the images / video configs (profiles/r02_schedule.md).
-  double c_blk = 16.0, w_row = 0.875, w_halo = 0.25, w_q = 0.2, c_tile = 6.0;
-  double f_short = 1.3;   // a window of a short-frame segment reads every row twice from shared memory and differences all of them
+  // Roughly microseconds of one CTA with the whole machine streaming (fitted to per-CTA sweep times on the five workloads,
+  // profiles/r02_schedule.md).  A block costs almost the same whatever its height (M = 128 MMAs read 128 rows of shared memory, every
+  // chunk is a barrier round trip and a dependent chain in the statistics warps); a frame-walk block differences every row, a window
+  // of a short-frame segment also reads every row twice.  A tile pays for the query rows it streams and for its halo chunks (by its
+  // share of K), a constant for the refill of the pipeline, and for the accumulator slots it has to wait for: the epilogue of the
+  // tile before it drains one slot in about t_epi.
+  double c_blk = 14.0, w_row = 0.025;
+  double f_walk = 1.28, f_short = 1.7;
+  double w_halo = 0.077;   // per row of a halo chunk
+  double w_q = 0.055;      // per (padded) query row
+  double c_tile = 1.5;
+  double epi0 = 0.35, epi_col = 0.013;   // t_epi = epi0 + epi_col * accumulator columns
 };
 
 inline size_t tc_max_tiles(const mas_segment* segs, int32_t n_segs) {
@@ -795,50 +817,58 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     sc.smem_bytes = 1024 + kTcCtrlBytes + kTcStatBytes + sc.nq * sc.qslot_bytes + sc.nx * xs_bytes;
   }
 
-  // The batch as STRIPS of row blocks that may share a tile: the blocks of a single-frame segment (nearly equal heights <= 128);
-  // one block of patch rows [r0, r0 + R) of a video segment through all its frames (block i = frame i); the overlapping windows
-  // of a short-frame segment (128 - P scored rows each).  A tile takes up to NS consecutive blocks of a strip.
-  struct Strip { int32_t seg, mode, r0, R, P; int64_t n, nblk; double cb, c_q, c_halo; };
+  // The batch as STRIPS of row blocks that may share a tile: the blocks of a single-frame segment (one height, a multiple of 8
+  // rows: a TMA box is a whole number of 8-row swizzle atoms, so no row is fetched by two CTAs); one block of patch rows
+  // [r0, r0 + R) of a video segment through all its frames (block i = frame i); the overlapping windows of a short-frame segment
+  // (window i starts at row i (128 - P) and scores its rows from P on, window 0 all of them).  A tile takes up to NS consecutive
+  // blocks of a strip.
+  struct Strip { int32_t seg, mode, r0, R, P, stride; int64_t n, nblk; double cb, c_q, c_halo, t_epi; };
   std::vector<Strip> strips;
   for (int32_t k = 0; k < n_segs; ++k) {
     const mas_segment& s = segs[k];
     const int L = (int)(q_off[s.request + 1] - q_off[s.request]);
-    const double c_q = cw.w_q * ((L + 15) / 16 * 16 + (rider ? 64 : 0));   // the query rows a tile streams (scaled by its share of K)
+    const int ncol = (L + 15) / 16 * 16 + (rider ? 64 : 0);
+    const double c_q = cw.w_q * ncol;                      // the query rows a tile streams (scaled by its share of K)
+    const double t_epi = cw.epi0 + cw.epi_col * ncol;
     const int64_t n = (int64_t)s.n_frames * s.n_patches;
-    auto blk = [&](double h) { return (s.n_frames > 1 && s.n_patches < 64 ? cw.f_short : 1.0) * (cw.c_blk + cw.w_row * h); };            // one block of h rows, per K-sweep
     if (s.n_frames == 1) {
       const int64_t nb = (n + 127) / 128;
-      strips.push_back(Strip{k, 0, 0, 0, 0, n, nb, blk((double)n / nb), c_q, 0.0});
+      const int stride = (int)(((n + nb - 1) / nb + 7) / 8 * 8);
+      strips.push_back(Strip{k, 0, 0, 0, 0, stride, n, nb, cw.c_blk + cw.w_row * ((double)n / nb), c_q, 0.0, t_epi});
     } else if (s.n_patches >= 64) {
-      const int nb = (s.n_patches + 127) / 128;            // row blocks of nearly equal height
+      const int nb = (s.n_patches + 127) / 128;            // row blocks of nearly equal height, in whole 8-row swizzle atoms
       for (int j = 0; j < nb; ++j) {
-        // nearly equal heights in whole 8-row swizzle atoms (a TMA box is a whole number of them): no row is fetched by two CTAs
         const int oct = (s.n_patches + 7) / 8;
         const int r0 = 8 * (int)((int64_t)j * oct / nb), r1 = j + 1 == nb ? s.n_patches : 8 * (int)((int64_t)(j + 1) * oct / nb);
-        strips.push_back(Strip{k, 1, r0, r1 - r0, s.n_patches, n, (int64_t)s.n_frames, blk((double)(r1 - r0)), c_q, cw.c_blk + cw.w_halo * (r1 - r0)});
+        strips.push_back(Strip{k, 1, r0, r1 - r0, s.n_patches, s.n_patches, n, (int64_t)s.n_frames, cw.f_walk * (cw.c_blk + cw.w_row * (r1 - r0)), c_q,
+                               cw.w_halo * (r1 - r0), t_epi});
       }
     } else {
       const int64_t sdt = 128 - s.n_patches;
-      strips.push_back(Strip{k, 2, 0, 0, s.n_patches, n, (n + sdt - 1) / sdt, blk(128.0), c_q, 0.0});
+      strips.push_back(Strip{k, 2, 0, 0, s.n_patches, (int32_t)sdt, n, n <= 128 ? 1 : (n - 128 + sdt - 1) / sdt + 1, cw.f_short * (cw.c_blk + cw.w_row * 128.0), c_q, 0.0,
+                             t_epi});
     }
   }
   const int S = (d / 64) / sc.kw;                          // K-steps of a full sweep
   const bool can_split = ksplit && S >= 4;
-  // cost of m whole consecutive blocks of a strip, cut into the fewest tiles (halo counted for every video tile)
-  auto whole_cost = [&](const Strip& st, int64_t m) {
-    if (m <= 0) return 0.0;
-    const int64_t nt = (m + NS - 1) / NS;
-    return (double)m * st.cb + (double)nt * (st.c_q + cw.c_tile + st.c_halo);
+  // Cost of a run of nb consecutive blocks of a strip, cut into the fewest tiles, whose first block is swept for the share `a` of K
+  // and whose last block for the share `b` (a one-block run: the share a + b - 1).  `at0`: the run starts with the strip's first
+  // block and all of its K (no halo for the first tile).  `prev_nb`, `prev_epi`: blocks and t_epi of the CTA's previous tile.
+  auto run_cost = [&](const Strip& st, int64_t nb, double a, double b, bool at0, int prev_nb, double prev_epi) {
+    if (nb <= 0) return 0.0;
+    const int64_t nt = (nb + NS - 1) / NS;
+    const double per = (double)nb / nt;                  // blocks per tile
+    const double wait0 = prev_epi * std::max(0.0, prev_nb + per - NS), wait = st.t_epi * std::max(0.0, 2.0 * per - NS);
+    if (nb == 1) return (st.cb + st.c_q + (at0 ? 0.0 : st.c_halo)) * (a + b - 1.0) + cw.c_tile + wait0;
+    return st.cb * ((double)(nb - 2) + a + b) + (double)nt * (st.c_q + cw.c_tile) + (double)(nt - (at0 ? 1 : 0)) * st.c_halo + wait0 + (double)(nt - 1) * wait;
   };
-  // cost of K-steps [0, steps) of ONE block as a tile of its own
-  auto part_cost = [&](const Strip& st, int steps) { return (st.cb + st.c_q + st.c_halo) * (double)steps / S + cw.c_tile; };
   double total = 0.0;
-  for (const Strip& st : strips) total += whole_cost(st, st.nblk);
-  const int n_ctas = (int)std::min<int64_t>(std::min(sm_count, kTcMaxCtas), std::max<int64_t>(1, (int64_t)(total / 96.0)));
+  for (const Strip& st : strips) total += run_cost(st, st.nblk, 1.0, 1.0, true, 0, 0.0);
+  const int n_ctas = (int)std::min<int64_t>(std::min(sm_count, kTcMaxCtas), std::max<int64_t>(1, (int64_t)(total / 12.0)));
 
   std::vector<TcTile> tiles;
   std::vector<int> cta_first(n_ctas + 1, 0);
-  // blocks [i0, i1) of a strip, K-steps [s0, s1), as one tile
+  // blocks [i0, i1) of a strip as one tile: block i0 from K-step s0 on, block i1 - 1 up to K-step s1
   auto emit = [&](const Strip& st, int64_t i0, int64_t i1, int s0, int s1) {
     const mas_segment& s = segs[st.seg];
     TcTile t{};
@@ -846,109 +876,111 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     t.q_row0 = (int32_t)q_off[s.request];
     t.L = (int32_t)(q_off[s.request + 1] - q_off[s.request]);
     t.k0 = s0 * sc.kw; t.k1 = s1 * sc.kw; t.peer = -1;
+    t.n_blocks = (int32_t)(i1 - i0); t.stride = st.stride;
     if (st.mode == 0) {
-      // nearly equal blocks cut at whole 8-row swizzle atoms (no row is fetched by two CTAs); inside the tile the kernel walks
-      // blocks of `stride` rows
-      const int64_t oct = (st.n + 7) / 8;
-      auto cut = [&](int64_t i) { return i >= st.nblk ? st.n : 8 * (i * oct / st.nblk); };
-      const int64_t u = cut(i0), v = cut(i1);
-      t.row0 = (int32_t)(s.row0 + u); t.n_rows = (int32_t)(v - u);
-      t.stride = (int32_t)(((t.n_rows + (i1 - i0) - 1) / (i1 - i0) + 7) / 8 * 8);
-      t.n_blocks = (t.n_rows + t.stride - 1) / t.stride;
+      t.row0 = (int32_t)(s.row0 + i0 * st.stride); t.n_rows = (int32_t)(std::min<int64_t>(st.n, i1 * st.stride) - i0 * st.stride);
     } else if (st.mode == 1) {                              // frames [i0, i1) of the strip's row block
-      t.row0 = (int32_t)(s.row0 + i0 * s.n_patches + st.r0); t.n_rows = st.R; t.stride = s.n_patches; t.prev = s.n_patches;
-      t.n_blocks = (int32_t)(i1 - i0); t.halo = i0 > 0 ? 1 : 0;
+      t.row0 = (int32_t)(s.row0 + i0 * s.n_patches + st.r0); t.n_rows = st.R; t.prev = s.n_patches; t.halo = i0 > 0 ? 1 : 0;
     } else {
-      const int P = s.n_patches;
-      const int64_t u = i0 * (128 - P), v = std::min<int64_t>(st.n, i1 * (128 - P));
-      const int64_t a0 = u == 0 ? 0 : u - P;              // the window starts P rows early (their successors need them)
-      t.row0 = (int32_t)(s.row0 + a0); t.n_rows = (int32_t)(v - a0); t.stride = 128 - P; t.prev = P; t.halo = (int32_t)(u - a0);
-      t.n_blocks = t.n_rows <= 128 ? 1 : (t.n_rows - 128 + t.stride - 1) / t.stride + 1;
+      t.row0 = (int32_t)(s.row0 + i0 * st.stride); t.n_rows = (int32_t)(std::min<int64_t>(st.n, (i1 - 1) * st.stride + 128) - i0 * st.stride);
+      t.prev = st.P; t.halo = i0 > 0 ? st.P : 0;            // leading rows of the first window that are loaded for their successors only
     }
     tiles.push_back(t);
   };
-  auto emit_whole = [&](const Strip& st, int64_t i0, int64_t m) {   // m blocks -> the fewest tiles, of nearly equal size
-    const int64_t nt = (m + NS - 1) / NS;
-    for (int64_t i = 0; i < nt; ++i) emit(st, i0 + m * i / nt, i0 + m * (i + 1) / nt, 0, S);
-  };
-  // One pass with a fixed per-CTA target: CTAs fill up to the target in strip order; what is left of the target after the last
-  // whole block that fits is filled with the first K-steps of the next block (K-split: that CTA owns the block, the CTA(s) that
-  // follow sweep the remaining K-steps first thing and hand their partial sums over); the last CTA takes what is left.
-  // Returns the last CTA's load.  The smallest target whose last CTA does not overshoot is found by bisection.
+  // One pass with a fixed per-CTA target: CTAs fill up to the target in strip order, first with whole blocks, then with the first
+  // K-steps of the next block (K-split: that CTA owns the block; the CTA that follows starts with its remaining K-steps and hands
+  // the partial sums over); the last CTA takes what is left.  Returns the last CTA's load.
   auto assign = [&](double target, bool commit) {
     int c = 0;
     double load = 0.0;
     int owner = -1;                                     // index of the tile that owns the block being split
+    int prev_nb = 0;                                    // the CTA's previous tile
+    double prev_epi = 0.0;
     if (commit) { tiles.clear(); std::fill(cta_first.begin(), cta_first.end(), 0); }
     auto close_cta = [&]() {
-      if (c + 1 < n_ctas) { load = 0.0; ++c; if (commit) cta_first[c] = (int)tiles.size(); }
+      if (c + 1 < n_ctas) { load = 0.0; prev_nb = 0; ++c; if (commit) cta_first[c] = (int)tiles.size(); }
+    };
+    auto took = [&](const Strip& st, int64_t nb) {      // a run of nb blocks joined the CTA: its last tile is the previous one now
+      const int64_t nt = (nb + NS - 1) / NS;
+      prev_nb = (int)(nb - nb * (nt - 1) / nt); prev_epi = st.t_epi;
+    };
+    auto cost = [&](const Strip& st, int64_t i, int ks, int64_t nb, double b) {
+      return run_cost(st, nb, (double)(S - ks) / S, b, i == 0 && ks == 0, prev_nb, prev_epi);
+    };
+    // the run of blocks [i, i + nb) with block i from K-step ks on and the last block up to K-step s1, as the fewest tiles
+    auto emit_run = [&](const Strip& st, int64_t i, int64_t nb, int ks, int s1) {
+      const int64_t nt = (nb + NS - 1) / NS;
+      for (int64_t j = 0; j < nt; ++j) {
+        const int64_t b0 = i + nb * j / nt, b1 = i + nb * (j + 1) / nt;
+        emit(st, b0, b1, j == 0 ? ks : 0, j + 1 == nt ? s1 : S);
+        const int me = (int)tiles.size() - 1;
+        if (j == 0 && ks > 0) {                         // a dumping part: slot c, read by the owner
+          tiles[owner].n_wait += 1;
+          if (tiles[owner].peer < 0) tiles[owner].peer = c;
+        }
+        if (j + 1 == nt && s1 < S && !(nb == 1 && ks > 0)) owner = me;
+      }
     };
     for (const Strip& st : strips) {
       int64_t i = 0;
       int ks = 0;                                       // K-steps of block i already handed out
       while (i < st.nblk) {
-        const bool last_cta = c + 1 >= n_ctas;
-        if (ks > 0) {                                   // the rest of a split block comes first in this CTA
-          int take = S - ks;
-          if (!last_cta && load + part_cost(st, take) > target) {
-            const int fit = (int)std::floor((target - load - cw.c_tile) / ((st.cb + st.c_q + st.c_halo) / S));
-            if (fit >= 2 && take - fit >= 2) take = fit;
-          }
-          if (commit) {
-            emit(st, i, i + 1, ks, ks + take);
-            tiles.back().peer = c;
-            tiles[owner].n_wait += 1;
-            if (tiles[owner].peer < 0) tiles[owner].peer = c;
-          }
-          load += part_cost(st, take);
-          ks += take;
-          if (ks < S) { close_cta(); continue; }
-          ks = 0; ++i; owner = -1;
-          continue;
+        const int64_t m_all = st.nblk - i;
+        if (c + 1 >= n_ctas || load + cost(st, i, ks, m_all, 1.0) <= target) {   // the rest of the strip
+          if (commit) emit_run(st, i, m_all, ks, S);
+          load += cost(st, i, ks, m_all, 1.0);
+          took(st, m_all);
+          break;
         }
-        int64_t m = st.nblk - i;
-        if (!last_cta && load + whole_cost(st, m) > target) {
-          int64_t lo = 0, hi = m;
-          while (lo < hi) { const int64_t mid = (lo + hi + 1) / 2; if (load + whole_cost(st, mid) <= target) lo = mid; else hi = mid - 1; }
-          m = lo;
-          if (commit && m > 0) emit_whole(st, i, m);
-          load += whole_cost(st, m);
-          i += m;
-          // (not in a frame walk: a split frame would be two more single-frame tiles, each with its own halo and query stream)
-          int fit = can_split && st.mode != 1 ? (int)std::floor((target - load - cw.c_tile) / ((st.cb + st.c_q + st.c_halo) / S)) : 0;
-          if (fit > S - 2) fit = S - 2;
-          if (fit >= 2) {                               // the first K-steps of the next block: this CTA owns it
-            if (commit) { emit(st, i, i + 1, 0, fit); owner = (int)tiles.size() - 1; }
-            load += part_cost(st, fit);
-            ks = fit;
-          } else if (m == 0 && load == 0.0) {           // a target below one block: take it whole
-            if (commit) emit_whole(st, i, 1);
-            load += whole_cost(st, 1);
-            ++i;
-          }
-          close_cta();
-          continue;
+        int64_t lo = 0, hi = m_all - 1;                 // whole blocks that fit
+        while (lo < hi) { const int64_t mid = (lo + hi + 1) / 2; if (load + cost(st, i, ks, mid, 1.0) <= target) lo = mid; else hi = mid - 1; }
+        int64_t nb = lo;
+        int fit = 0;                                    // K-steps of block i + nb on top
+        if (can_split) {
+          const double base = cost(st, i, ks, nb + 1, nb == 0 ? (double)ks / S : 0.0);   // with none of the K-steps of block i + nb
+          const double per = cost(st, i, ks, nb + 1, (nb == 0 ? (double)ks / S : 0.0) + 1.0 / S) - base;
+          const int avail = nb == 0 ? S - ks : S;
+          fit = (int)std::floor((target - load - base) / per);
+          if (fit > avail - 2) fit = avail - 2;
+          if (fit < 2) fit = 0;
         }
-        if (commit) emit_whole(st, i, m);
-        load += whole_cost(st, m);
-        i += m;
+        if (nb == 0 && fit == 0) {
+          if (load > 0.0) { close_cta(); continue; }
+          nb = 1;                                       // a target below one block: take it (or what is left of it) whole
+        }
+        const int s1 = fit > 0 ? (nb == 0 ? ks + fit : fit) : S;
+        const int64_t n_run = nb + (fit > 0 ? 1 : 0);
+        if (commit) emit_run(st, i, n_run, ks, s1);
+        load += cost(st, i, ks, n_run, (double)s1 / S);
+        took(st, n_run);
+        i += nb;
+        ks = fit > 0 ? s1 : 0;
+        close_cta();
       }
     }
     if (commit) for (int k2 = c + 1; k2 <= n_ctas; ++k2) cta_first[k2] = (int)tiles.size();
     return load;
   };
   {
-    double lo = total / n_ctas, hi = 2.0 * total / n_ctas + 4096.0;   // assign(hi) never overshoots hi by more than a tile
+    // feasible = the last CTA does not overshoot.  Feasibility is not quite monotonic in the target (tiles come and go), so after
+    // the bisection a scan upwards from a little below looks for a smaller feasible target.
+    double lo = 0.5 * total / n_ctas, hi = 2.0 * total / n_ctas + 4096.0;   // assign(hi) never overshoots hi by more than a tile
     for (int it = 0; it < 40; ++it) {
       const double mid = 0.5 * (lo + hi);
       if (assign(mid, false) <= mid + 1e-9) hi = mid; else lo = mid;
+    }
+    const double from = 0.97 * hi;
+    for (int k = 0; k < 120; ++k) {
+      const double t = from * (1.0 + 0.00025 * k);
+      if (t >= hi) break;
+      if (assign(t, false) <= t + 1e-9) { hi = t; break; }
     }
     assign(hi, true);
   }
   const int n_tiles = (int)tiles.size();
   {   // NEXT-2 partial slots: one per block, contiguous per segment (tiles are in row order of their segment already)
     int part = 0;
-    for (TcTile& t : tiles) { t.part0 = part; if (!(t.peer >= 0 && t.n_wait == 0)) part += t.n_blocks; }
+    for (TcTile& t : tiles) { const int dumped = t.k0 > 0 ? 1 : 0; t.part0 = part - dumped; part += t.n_blocks - dumped; }   // (a dumped block 0 writes no results)
     sc.n_parts = part;
   }
   TcTile* ht = reinterpret_cast<TcTile*>(h_dst);

@@ -106,14 +106,21 @@ def _segments_of(kind, rng):
     return rows, np.concatenate([[0], np.cumsum(L)]).astype(np.int64)
 
 
-def _scored_rows(t):
-    """Row ranges a schedule record scores (include/msas.h, mas_score_schedule)."""
+def _block_sweeps(t, nk):
+    """(scored row range, first K-chunk, end K-chunk) of every block of a schedule record (include/msas.h, mas_score_schedule):
+    block 0 joins at k0, the last block leaves at k1, the blocks in between are swept over all of K."""
     cta, row0, n, nb, stride, mode, prev, halo = [int(v) for v in t[:8]]
-    if mode == 0:
-        return [(row0, row0 + n)]
-    if mode == 1:
-        return [(row0 + b * stride, row0 + b * stride + n) for b in range(nb)]
-    return [(row0 + halo, row0 + n)]
+    k0, k1 = int(t[12]), int(t[13])
+    out = []
+    for b in range(nb):
+        if mode == 0:
+            lo, hi = row0 + b * stride, row0 + min(n, (b + 1) * stride)
+        elif mode == 1:
+            lo, hi = row0 + b * stride, row0 + b * stride + n
+        else:   # window b: 128 rows from row0 + b * stride on, scored from `prev` on (the record's first window: from `halo` on)
+            lo, hi = row0 + b * stride + (halo if b == 0 else prev), row0 + min(n, b * stride + 128)
+        out.append(((lo, hi), k0 if b == 0 else 0, k1 if b == nb - 1 else nk))
+    return out
 
 
 @pytest.mark.parametrize("kind", ["images", "video", "audio", "ragged", "tiny"])
@@ -133,15 +140,16 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
     n_slots = min(10, 512 // ((maxL + 15) // 16 * 16))           # TMEM accumulator slots of pad16(longest query block) columns
     cost = np.zeros(148)
     split_open = None                                            # (rows, next k0, owner record) of a block being shared along K
+    prev_nb, prev_epi = 0, 0.0
     for rec in t:
         cta, r0, n, nb, stride, mode, prev, halo, q0, L, seg, part0, k0, k1, n_wait, peer = [int(v) for v in rec]
         T, P = rows[seg][2], rows[seg][3]
         assert 0 <= cta < 148 and 1 <= nb <= n_slots
         assert q0 == q0_of[seg] and L == q_off[rows[seg][0] + 1] - q_off[rows[seg][0]]
         assert mode == (0 if T == 1 else 1 if P >= 64 else 2)
-        assert 0 <= k0 < k1 <= nk and k0 % 2 == 0 and k1 % 2 == 0   # two K-slices per chunk at d % 128 == 0
+        assert 0 <= k0 < nk and 0 < k1 <= nk and k0 % 2 == 0 and k1 % 2 == 0   # two K-slices per chunk at d % 128 == 0
         if mode == 0:
-            assert stride % 8 == 0 and stride <= 128 and prev == 0 and halo == 0 and nb == -(-n // stride)   # blocks of nearly equal height
+            assert stride % 8 == 0 and stride <= 128 and prev == 0 and halo == 0 and nb == -(-n // stride)   # blocks of one height
             assert (r0 - row0_of[seg]) % 8 == 0                                                   # cut at whole 8-row swizzle atoms
         elif mode == 1:
             assert stride == P and prev == P and 1 <= n <= 128 and halo in (0, 1)
@@ -153,40 +161,40 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
             assert halo == (0 if r0 == row0_of[seg] else P)               # only a segment's first window starts without predecessors
             assert nb == (1 if n <= 128 else -(-(n - 128) // stride) + 1)
             assert n - (nb - 1) * stride > P                               # the last window scores at least one row
-        ranges = _scored_rows(rec)
-        for lo, hi in ranges:
+        sweeps = _block_sweeps(rec, nk)
+        for (lo, hi), ka, kb in sweeps:
             assert lo < hi and seg_of_row[lo] == seg and seg_of_row[hi - 1] == seg    # a tile never straddles a segment
-            cov[lo:hi] += k1 - k0
-        # K-split: only single-block tiles; the owner (k0 = 0) comes last in its CTA, the other parts first in the CTAs that follow
-        if (k0, k1) != (0, nk):
-            assert nb == 1
-            if k0 == 0:
-                assert split_open is None and n_wait >= 1 and peer == cta + 1
-                assert rec is t[t[:, 0] == cta][-1] or np.array_equal(rec, t[t[:, 0] == cta][-1])
-                split_open = [ranges, k1, cta, n_wait]
-            else:
-                assert split_open is not None and ranges == split_open[0] and k0 == split_open[1]
-                assert n_wait == 0 and peer == cta and np.array_equal(rec, t[t[:, 0] == cta][0])
-                assert cta == split_open[2] + 1
-                split_open[1], split_open[2], split_open[3] = k1, cta, split_open[3] - 1
-                if k1 == nk:
-                    assert split_open[3] == 0
-                    split_open = None
+            assert 0 <= ka < kb <= nk
+            cov[lo:hi] += kb - ka
+            if ka == 0:
+                owned[lo:hi] += 1
+        mine = t[t[:, 0] == cta]
+        # K-split: a block shared along K is the last block of its owner (the part from chunk 0; last tile of its CTA) and the first
+        # block of the first tile of every CTA that follows, until chunk nk is reached
+        if k0 > 0:
+            assert split_open is not None and sweeps[0][0] == split_open[0] and k0 == split_open[1] and cta == split_open[2] + 1
+            assert np.array_equal(rec, mine[0])
+            split_open[1], split_open[2], split_open[3] = sweeps[0][2], cta, split_open[3] - 1
+            if sweeps[0][2] == nk:
+                assert split_open[3] == 0
+                split_open = None
+        if k1 < nk and (nb > 1 or k0 == 0):
+            assert split_open is None and n_wait >= 1 and peer == cta + 1 and np.array_equal(rec, mine[-1])
+            split_open = [sweeps[-1][0], k1, cta, n_wait]
         else:
             assert n_wait == 0 and peer == -1
-        if k0 == 0:
-            for lo, hi in ranges:
-                owned[lo:hi] += 1
-        # cost model of csrc/k_score_tc.cuh (TcCost): 16 + 0.875 h per block of h rows, the halo chunk, 0.2 per padded query row,
-        # a window of a short-frame segment 1.3 x a full block (all scaled by the share of K) and 6 per tile
-        frac = (k1 - k0) / nk
-        if mode == 0:
-            blocks = nb * (16 + 0.875 * n / nb)
-        elif mode == 1:
-            blocks = nb * (16 + 0.875 * n) + halo * (16 + 0.25 * n)
-        else:
-            blocks = nb * 1.3 * 128.0                              # a short-frame window: 1.3 x a full block
-        cost[cta] += frac * (blocks + 0.2 * ((L + 15) // 16 * 16)) + 6.0
+        # cost model of csrc/k_score_tc.cuh (TcCost), about microseconds: a block 14 + 0.025 h (x 1.28 in a frame walk, x 1.7 for a window
+        # of a short-frame segment) by its share of K; per tile (by its share of K) 0.055 per padded query row and 0.077 per row of a
+        # halo chunk; 1.5 per tile; and the wait for accumulator slots the CTA's previous tile still holds (0.35 + 0.013 columns each)
+        share = sum(kb - ka for _, ka, kb in sweeps) / nk          # in blocks
+        h = rows[seg][3] / -(-rows[seg][3] // 128) if mode == 0 else n if mode == 1 else 128
+        blocks = share * (1.0, 1.28, 1.7)[mode] * (14 + 0.025 * h)
+        tile_share = share if nb == 1 else 1.0
+        Lpad = (L + 15) // 16 * 16
+        first_of_cta = np.array_equal(rec, mine[0])
+        wait = 0.0 if first_of_cta else prev_epi * max(0, prev_nb + nb - n_slots)
+        cost[cta] += blocks + tile_share * (0.055 * Lpad + (0.077 * n if mode == 1 and (halo or k0 > 0) else 0)) + 1.5 + wait
+        prev_nb, prev_epi = nb, 0.35 + 0.013 * Lpad
     assert split_open is None
     assert cov.min() == nk and cov.max() == nk                   # every K-chunk of every row swept exactly once
     assert owned.min() == 1 and owned.max() == 1                 # and its results written by exactly one tile
@@ -204,8 +212,8 @@ def test_score_schedule_rider_variant_and_small_devices(B):
         cov = np.zeros(5000 + 900 + 700, np.int32)
         for rec in t:
             assert int(rec[3]) <= 4                              # L = 128 somewhere: four 128-column accumulator slots
-            for lo, hi in _scored_rows(rec):
-                cov[lo:hi] += int(rec[13]) - int(rec[12])
+            for (lo, hi), ka, kb in _block_sweeps(rec, 2):
+                cov[lo:hi] += kb - ka
         assert cov.min() == 2 and cov.max() == 2 and t[:, 0].max() < sms      # d = 128: two K-chunks
 
 
