@@ -299,12 +299,13 @@ int mas_plan_set_inline_query_norms(mas_plan* plan, int32_t on);
  * never straddles a segment").  A tile is up to 10 row blocks (one TMEM accumulator slot each: 512 columns / pad16 of the
  * longest query block) of one segment that share the request's query rows and are swept K-chunk by K-chunk.  Writes up to `cap_tiles` records of 16 int32 each, in per-CTA order:
  *   {cta, row0, n_rows, n_blocks, stride, mode, prev, halo, q_row0, L, seg, part0, k0, k1, n_wait, peer}
- *   k0, k1: K-SPLIT.  CTAs may share a row block along K so that every CTA carries the same cost: the tile's FIRST block is swept
- *          over the 64-column K-chunks [k0, d / 64) only and its LAST block over [0, k1) only (a one-block tile: [k0, k1)); the
+ *   k0, k1: K-SPLIT.  CTAs may share a row block along K so that every CTA carries the same cost: the tile's LAST block is swept
+ *          over the 64-column K-chunks [k0, d / 64) only and its FIRST block over [0, k1) only (a one-block tile: [k0, k1)); the
  *          blocks in between, and every block of an unsplit tile (k0 = 0, k1 = d / 64), over all of K.  The part of a block
- *          that starts at chunk 0 owns it and writes its results: n_wait = number of other parts of the tile's last block,
- *          peer = CTA of the first of them (the CTAs that follow, each starting with its part and handing its partial sums
- *          over through the exchange slot of its CTA); n_wait = 0 and peer = -1 for every other tile;
+ *          that ends at chunk d / 64 owns it and writes its results (it is the last thing its CTA does): n_wait = number of
+ *          other parts of the tile's last block, peer = CTA of the first of them (the CTAs that follow, each STARTING with its
+ *          part, in descending K, and handing its partial sums over through the exchange slot of its CTA early in its sweep);
+ *          n_wait = 0 and peer = -1 for every other tile;
  *   mode 0 (single-frame segment): the tile scores rows [row0, row0 + n_rows) in blocks of `stride` <= 128 rows (a multiple of 8);
  *   mode 1 (frames of P >= 64 rows): block b scores rows [row0 + b * stride, + n_rows), stride = prev = P, i.e. the same
  *          n_rows <= 128 patch rows in n_blocks consecutive frames; halo = 1 if the frame before block 0 is read as well;

@@ -49,12 +49,13 @@ struct TcTile {            // 64 bytes
   int32_t L;               // query tokens of the request
   int32_t part0;           // NEXT-2: slot of block 0's column sums (block b -> part0 + b); slots of a segment are contiguous
   int32_t seg;
-  // K-split: CTAs may share a row block along K.  The tile's FIRST block is swept over the K-chunks [k0, nk) only and its LAST
-  // block over [0, k1) only (a one-block tile: [k0, k1)); the blocks in between over all of K.  The part of a block that starts
-  // at chunk 0 OWNS it: it adds the partial accumulators and row sums the other parts dumped and writes the results.  A part
-  // with k0 > 0 dumps into the exchange slot of its CTA (a CTA holds at most one: the first block of its first tile).
+  // K-split: CTAs may share a row block along K.  The tile's LAST block is swept over the K-chunks [k0, nk) only and its FIRST
+  // block over [0, k1) only (a one-block tile: [k0, k1)); the blocks in between over all of K.  The part of a block that ends
+  // at chunk nk OWNS it: it is the last thing its CTA does, and it adds the partial accumulators and row sums the other parts
+  // dumped and writes the results.  A part with k1 < nk is the first block of its CTA's first tile: it is complete early in
+  // that CTA's sweep and dumped into the exchange slot of the CTA right away, long before the owner asks for it.
   int32_t k0, k1;          // in 64-column chunks, multiples of the slices per chunk; 0 and nk where the tile is not split
-  int32_t n_wait;          // owner (k1 < nk): number of foreign parts of the last block (exchange slots peer .. peer + n_wait - 1)
+  int32_t n_wait;          // owner (last block with k0 > 0, k1 = nk if it is the only one): number of foreign parts (exchange slots peer .. peer + n_wait - 1)
   int32_t peer;            // owner: first exchange slot to read (the CTA after this one); -1 otherwise
   int32_t pad_;
 };
@@ -120,11 +121,11 @@ struct TcParams {
 __device__ __forceinline__ int tc_block_rows(const TcTile& t, int b) {
   return t.mode == 1 ? t.n_rows : min(t.mode == 0 ? t.stride : 128, t.n_rows - b * t.stride);
 }
-// K-chunks a tile walks, and the blocks that take part in chunk kc: block 0 joins at k0, the last block leaves at k1
+// K-chunks a tile walks, and the blocks that take part in chunk kc: block 0 leaves at k1, the last block joins at k0
 __device__ __forceinline__ int tc_k_lo(int n_blocks, int k0) { return n_blocks == 1 ? k0 : 0; }
 __device__ __forceinline__ int tc_k_hi(int n_blocks, int k1, int nk) { return n_blocks == 1 ? k1 : nk; }
-__device__ __forceinline__ int tc_b_first(int kc, int k0) { return kc < k0 ? 1 : 0; }
-__device__ __forceinline__ int tc_b_end(int kc, int k1, int n_blocks) { return kc >= k1 ? n_blocks - 1 : n_blocks; }
+__device__ __forceinline__ int tc_b_first(int kc, int k1, int n_blocks) { return n_blocks > 1 && kc >= k1 ? 1 : 0; }
+__device__ __forceinline__ int tc_b_end(int kc, int k0, int n_blocks) { return n_blocks > 1 && kc < k0 ? n_blocks - 1 : n_blocks; }
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -225,8 +226,9 @@ struct TcCtrl {                      // lives at the (1024-aligned) start of dyn
   uint64_t tfull[kTcMaxBlocks];      // accumulator slot: MMA commit -> epilogue
   uint64_t tempty[kTcMaxBlocks];     // epilogue (4 warps) -> MMA
   uint64_t sfull[2], sempty[2];      // row statistics of a tile: statistics warps -> epilogue (4 warps) -> statistics warps
+  uint64_t s0full;                   // row statistics of a dumped first block (at most one per CTA: single use)
   uint32_t tmem_base;
-  uint32_t pad_[31];
+  uint32_t pad_[29];
   float hred[2][4][64];              // NEXT-2: per-warp column sums of the 64 head columns, double buffered
   float qinv_s[kMaxL];               // 1 / |q_j| of the tile the epilogue is working on
 };
@@ -269,6 +271,7 @@ __device__ __forceinline__ void tc_sq4_diff(const uint4 (&x)[4], const uint4 (&v
 // hardware 128-byte swizzle puts unit u of row r at unit u ^ (r & 7).  Ring position (xs, xph) is carried across tiles.
 struct TcAluCtx {
   uint32_t xring, xslot, xfull0, xempty0, stat;   // shared-space addresses; stat = this lane's accumulator of block 0 in this tile's buffer
+  uint32_t s0full;                                // barrier: block 0 of a tile whose first block is a dumped part is complete
   int nx, nk, lane, arow;
   uint32_t hh;
 };
@@ -301,11 +304,11 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
   const bool inchunk = mode == 2 && prow >= 0;
   const int hcap = mode == 0 ? stride : 128;
   for (int kc = tc_k_lo(n_blocks, k0); kc < tc_k_hi(n_blocks, k1, nk); kc += KW) {
-    const int bf = tc_b_first(kc, k0), be = tc_b_end(kc, k1, n_blocks);
+    const int bf = tc_b_first(kc, k1, n_blocks), be = tc_b_end(kc, k0, n_blocks);
     if (bf >= be) continue;
     uint4 pv[KW][4];                  // this thread's K-slices of the previous frame's row (mode 1: carried from block to block)
     bool have_prev = false;
-    if (mode == 1 && (halo || bf)) {  // frame t0 - 1, or frame t0 itself while block 0 has not joined yet
+    if (mode == 1 && (halo || bf)) {  // frame t0 - 1, or frame t0 itself once block 0 has left
       mbar_wait(c.xfull0 + xs * 8u, xph);
       if (c.arow < n_rows) {
         const uint32_t slice = (uint32_t)((n_rows + 7) >> 3) * 1024u;
@@ -348,7 +351,7 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
       if (act) {   // lane pair (row): the even lane keeps sum x^2, the odd lane sum (x - x_prev)^2
         const float mine = c.hh ? D : n2;
         const uint32_t a = c.stat + (uint32_t)b * 1024u;
-        sts32(a, kc == (b == 0 ? k0 : 0) ? mine : lds32(a) + mine);
+        sts32(a, kc == (b == n_blocks - 1 ? k0 : 0) ? mine : lds32(a) + mine);
       }
     };
     uint4 xb[KW][4];
@@ -359,6 +362,10 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
       }
     } else {
       for (int b = bf; b < be; ++b) step(b, xb, pv);
+    }
+    if (n_blocks > 1 && k1 < nk && kc + KW == k1) {   // block 0 has left the sweep: its row sums are complete (the epilogue dumps them early)
+      __syncwarp();
+      if (c.lane == 0) mbar_arrive(c.s0full);
     }
   }
 }
@@ -395,6 +402,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       mbar_init(smem_u32(&ctrl->sfull[i]), kTcAluWarps); mbar_init(smem_u32(&ctrl->sempty[i]), 4);
     }
     for (int i = 0; i < kTcMaxBlocks; ++i) { mbar_init(tfull0 + 8u * i, 1); mbar_init(tempty0 + 8u * i, 4); }
+    mbar_init(smem_u32(&ctrl->s0full), kTcAluWarps);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kTcWarpMma) {   // TMEM: all 512 columns (one CTA per SM): 4 to 10 accumulator slots of pad16(L) columns
@@ -423,10 +431,10 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int nqu = (tile.L + 15) >> 4;
       const uint32_t qbytes = (uint32_t)(nqu + (rider ? 4 : 0)) * 2048u * (uint32_t)kw;
       for (int kc = tc_k_lo(tile.n_blocks, tile.k0); kc < tc_k_hi(tile.n_blocks, tile.k1, nk); kc += kw) {
-        const int bf = tc_b_first(kc, tile.k0), be = tc_b_end(kc, tile.k1, tile.n_blocks);
+        const int bf = tc_b_first(kc, tile.k1, tile.n_blocks), be = tc_b_end(kc, tile.k0, tile.n_blocks);
         if (bf >= be) continue;
         // frame walk: the chunk of the frame before the first block taking part rides along for the statistics warps only (block -1 =
-        // frame t0 - 1, the halo; block 0 itself while it has not joined yet)
+        // frame t0 - 1, the halo; block 0 itself once it has left)
         const int b_lo = tile.mode == 1 ? (bf ? 0 : (tile.halo ? -1 : 0)) : bf;
         {   // the request's query rows of these K-slices (+ the rider rows): one B tile per slice
           mbar_wait(qempty0 + 8u * qs, qph ^ 1u);
@@ -455,7 +463,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
             // rows past the block are never used
             // a video tile's halo and last frame are read by two CTAs (as halo and as a block), and so is the frame before a
             // split last frame: ordinary priority; the rest of X is read once: evict first
-            if (tile.mode == 1 && (b < bf || b == tile.n_blocks - 1 || (b == tile.n_blocks - 2 && tile.k1 < nk))) tma_load_3d(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc);
+            if (tile.mode == 1 && (b < bf || b == tile.n_blocks - 1 || (b == tile.n_blocks - 2 && tile.k0 > 0))) tma_load_3d(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc);
             else tma_load_3d_hint(xring + xs * xslot, &maps.x[h8 - 1], bar, 0, tile.row0 + b * tile.stride, kc, pol_stream);
           }
           if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
@@ -469,8 +477,9 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const TcTile tile = p.tiles[t];
       const int nqb = ((tile.L + 15) >> 4) + (rider ? 4 : 0);
       const uint32_t idesc = umma_idesc_bf16(nqb << 4);   // N = pad16(L) (+ 64 rider rows)
+      const bool early0 = tile.n_blocks > 1 && tile.k1 < nk;   // the first block is a dumped part that leaves the sweep at k1
       for (int kc = tc_k_lo(tile.n_blocks, tile.k0); kc < tc_k_hi(tile.n_blocks, tile.k1, nk); kc += kw) {
-        const int bf = tc_b_first(kc, tile.k0), be = tc_b_end(kc, tile.k1, tile.n_blocks);
+        const int bf = tc_b_first(kc, tile.k1, tile.n_blocks), be = tc_b_end(kc, tile.k0, tile.n_blocks);
         if (bf >= be) continue;
         const bool halo = tile.mode == 1 && (tile.halo || bf);
         mbar_wait(qfull0 + 8u * qs, qph);
@@ -485,7 +494,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         for (int b = bf; b < be; ++b) {
           uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
           if (ts >= ns) { ts -= ns; tp ^= 1u; }
-          const int kstart = b == 0 ? tile.k0 : 0;   // the block's first K-chunk
+          const int kstart = b == tile.n_blocks - 1 ? tile.k0 : 0;   // the block's first K-chunk
           if (kc == kstart) {   // the accumulator slot must have been drained by the epilogue of its previous use
             mbar_wait(tempty0 + 8u * ts, tp ^ 1u);
             tc_fence_after();
@@ -508,11 +517,14 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           }
           if (++xs == (uint32_t)nx) { xs = 0; xph ^= 1u; }
         }
-        if (elect_one()) tc_commit(qempty0 + 8u * qs);
+        if (elect_one()) {
+          tc_commit(qempty0 + 8u * qs);
+          if (early0 && kc + kw == tile.k1) tc_commit(tfull0 + 8u * ts0);   // block 0 has left the sweep: the epilogue may dump it now
+        }
         if (++qs == (uint32_t)p.nq) { qs = 0; qph ^= 1u; }
       }
       if (elect_one())
-        for (int b = 0; b < tile.n_blocks; ++b) { const uint32_t ts = ts0 + (uint32_t)b; tc_commit(tfull0 + 8u * (ts >= ns ? ts - ns : ts)); }
+        for (int b = early0 ? 1 : 0; b < tile.n_blocks; ++b) { const uint32_t ts = ts0 + (uint32_t)b; tc_commit(tfull0 + 8u * (ts >= ns ? ts - ns : ts)); }
       ts0 += (uint32_t)tile.n_blocks;
       if (ts0 >= ns) { ts0 -= ns; tp0 ^= 1u; }
     }
@@ -550,7 +562,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       const int buf = it & 1;
       const int nqu = (tile.L + 15) >> 4;
       const float2* st2 = reinterpret_cast<const float2*>(stat) + (size_t)buf * kTcMaxBlocks * 128;
-      const bool dump0 = tile.k0 > 0;                                // K-split: block 0 is a part that hands its partial sums to the block's owner
+      const bool dump0 = tile.k1 < nk;                               // K-split: block 0 is a part that hands its partial sums to the block's owner
       if (!(dump0 && tile.n_blocks == 1)) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
         if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
           unsigned long long seen;
@@ -583,7 +595,8 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
-          mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
+          if (tile.n_blocks > 1) mbar_wait(smem_u32(&ctrl->s0full), 0u);   // (complete long before the tile's other blocks)
+          else mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
           const float2 nd = st2[b * 128 + r];
           xo[(size_t)(p.xchg_cols - 2) * 128] = nd.x;
           xo[(size_t)(p.xchg_cols - 1) * 128] = nd.y;
@@ -592,7 +605,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
           if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + blockIdx.x), "r"(1u) : "memory");
           continue;
         }
-        if (n_wait > 0) {   // owner of a split block: the other parts were swept first by the CTAs that follow this one
+        if (n_wait > 0) {   // owner of a split block: the other parts were the first thing the CTAs that follow this one swept
           if (lane == 0)
             for (int i = 0; i < n_wait; ++i) {
               unsigned int f;
@@ -700,7 +713,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
-        if (b == 0) mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
+        if (b == (dump0 ? 1 : 0)) mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
         float2 nd = st2[b * 128 + r];
         for (int i = 0; i < n_wait; ++i) {
           nd.x += xi[(size_t)i * xslot_f + (size_t)(p.xchg_cols - 2) * 128];
@@ -724,7 +737,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
   } else {
     // ===================================================================== CUDA-core statistics: two threads per block row
     TcAluCtx c;
-    c.xring = xring; c.xslot = xslot; c.xfull0 = xfull0; c.xempty0 = xempty0;
+    c.xring = xring; c.xslot = xslot; c.xfull0 = xfull0; c.xempty0 = xempty0; c.s0full = smem_u32(&ctrl->s0full);
     c.nx = nx; c.nk = nk; c.lane = lane;
     c.arow = ((warp - 4) << 4) + (lane >> 1);
     c.hh = (uint32_t)lane & 1u;
@@ -868,7 +881,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
 
   std::vector<TcTile> tiles;
   std::vector<int> cta_first(n_ctas + 1, 0);
-  // blocks [i0, i1) of a strip as one tile: block i0 from K-step s0 on, block i1 - 1 up to K-step s1
+  // blocks [i0, i1) of a strip as one tile: block i1 - 1 from K-step s0 on, block i0 up to K-step s1 (one block: [s0, s1))
   auto emit = [&](const Strip& st, int64_t i0, int64_t i1, int s0, int s1) {
     const mas_segment& s = segs[st.seg];
     TcTile t{};
@@ -887,9 +900,10 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     }
     tiles.push_back(t);
   };
-  // One pass with a fixed per-CTA target: CTAs fill up to the target in strip order, first with whole blocks, then with the first
-  // K-steps of the next block (K-split: that CTA owns the block; the CTA that follows starts with its remaining K-steps and hands
-  // the partial sums over); the last CTA takes what is left.  Returns the last CTA's load.
+  // One pass with a fixed per-CTA target: CTAs fill up to the target in strip order, first with whole blocks, then with the LAST
+  // K-steps of the next block (K-split: that CTA owns the block and sweeps its part at the very end; the CTA that follows starts
+  // with the block's remaining K-steps, which are complete and dumped early in its sweep); the last CTA takes what is left.
+  // Returns the last CTA's load.
   auto assign = [&](double target, bool commit) {
     int c = 0;
     double load = 0.0;
@@ -904,21 +918,24 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
       const int64_t nt = (nb + NS - 1) / NS;
       prev_nb = (int)(nb - nb * (nt - 1) / nt); prev_epi = st.t_epi;
     };
+    // cost of the run of nb blocks from block i on, `ks` K-steps of block i already handed out (from the top), the last block
+    // taking the share b of K
     auto cost = [&](const Strip& st, int64_t i, int ks, int64_t nb, double b) {
       return run_cost(st, nb, (double)(S - ks) / S, b, i == 0 && ks == 0, prev_nb, prev_epi);
     };
-    // the run of blocks [i, i + nb) with block i from K-step ks on and the last block up to K-step s1, as the fewest tiles
-    auto emit_run = [&](const Strip& st, int64_t i, int64_t nb, int ks, int s1) {
+    // the run of blocks [i, i + nb): block i up to K-step e0 (a dumped part if e0 < S), the last block from K-step s_last on (the
+    // owner's part if s_last > 0), as the fewest tiles
+    auto emit_run = [&](const Strip& st, int64_t i, int64_t nb, int e0, int s_last) {
       const int64_t nt = (nb + NS - 1) / NS;
       for (int64_t j = 0; j < nt; ++j) {
         const int64_t b0 = i + nb * j / nt, b1 = i + nb * (j + 1) / nt;
-        emit(st, b0, b1, j == 0 ? ks : 0, j + 1 == nt ? s1 : S);
+        emit(st, b0, b1, j + 1 == nt ? s_last : 0, j == 0 ? e0 : S);
         const int me = (int)tiles.size() - 1;
-        if (j == 0 && ks > 0) {                         // a dumping part: slot c, read by the owner
+        if (j == 0 && e0 < S) {                         // a dumping part: slot c, read by the owner
           tiles[owner].n_wait += 1;
           if (tiles[owner].peer < 0) tiles[owner].peer = c;
         }
-        if (j + 1 == nt && s1 < S && !(nb == 1 && ks > 0)) owner = me;
+        if (j + 1 == nt && s_last > 0 && !(nb == 1 && e0 < S)) owner = me;
       }
     };
     for (const Strip& st : strips) {
@@ -927,7 +944,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
       while (i < st.nblk) {
         const int64_t m_all = st.nblk - i;
         if (c + 1 >= n_ctas || load + cost(st, i, ks, m_all, 1.0) <= target) {   // the rest of the strip
-          if (commit) emit_run(st, i, m_all, ks, S);
+          if (commit) emit_run(st, i, m_all, S - ks, 0);
           load += cost(st, i, ks, m_all, 1.0);
           took(st, m_all);
           break;
@@ -937,8 +954,9 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
         int64_t nb = lo;
         int fit = 0;                                    // K-steps of block i + nb on top
         if (can_split) {
-          const double base = cost(st, i, ks, nb + 1, nb == 0 ? (double)ks / S : 0.0);   // with none of the K-steps of block i + nb
-          const double per = cost(st, i, ks, nb + 1, (nb == 0 ? (double)ks / S : 0.0) + 1.0 / S) - base;
+          const double b_none = nb == 0 ? (double)ks / S : 0.0;                          // (a one-block run's share is a + b - 1)
+          const double base = cost(st, i, ks, nb + 1, b_none);                           // with none of the K-steps of block i + nb
+          const double per = cost(st, i, ks, nb + 1, b_none + 1.0 / S) - base;
           const int avail = nb == 0 ? S - ks : S;
           fit = (int)std::floor((target - load - base) / per);
           if (fit > avail - 2) fit = avail - 2;
@@ -948,13 +966,20 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
           if (load > 0.0) { close_cta(); continue; }
           nb = 1;                                       // a target below one block: take it (or what is left of it) whole
         }
-        const int s1 = fit > 0 ? (nb == 0 ? ks + fit : fit) : S;
-        const int64_t n_run = nb + (fit > 0 ? 1 : 0);
-        if (commit) emit_run(st, i, n_run, ks, s1);
-        load += cost(st, i, ks, n_run, (double)s1 / S);
-        took(st, n_run);
-        i += nb;
-        ks = fit > 0 ? s1 : 0;
+        const int e0 = S - ks;                          // block i is still to be swept over K-steps [0, e0)
+        if (nb == 0) {                                  // K-steps [e0 - fit, e0) of block i: a middle part
+          if (commit) emit_run(st, i, 1, e0, e0 - fit);
+          load += cost(st, i, ks, 1, (double)(ks + fit) / S);
+          took(st, 1);
+          ks += fit;
+        } else {
+          const int64_t n_run = nb + (fit > 0 ? 1 : 0);
+          if (commit) emit_run(st, i, n_run, e0, fit > 0 ? S - fit : 0);
+          load += cost(st, i, ks, n_run, fit > 0 ? (double)fit / S : 1.0);
+          took(st, n_run);
+          i += nb;
+          ks = fit;
+        }
         close_cta();
       }
     }
@@ -980,7 +1005,7 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
   const int n_tiles = (int)tiles.size();
   {   // NEXT-2 partial slots: one per block, contiguous per segment (tiles are in row order of their segment already)
     int part = 0;
-    for (TcTile& t : tiles) { const int dumped = t.k0 > 0 ? 1 : 0; t.part0 = part - dumped; part += t.n_blocks - dumped; }   // (a dumped block 0 writes no results)
+    for (TcTile& t : tiles) { const int dumped = t.k1 < S * sc.kw ? 1 : 0; t.part0 = part - dumped; part += t.n_blocks - dumped; }   // (a dumped block 0 writes no results)
     sc.n_parts = part;
   }
   TcTile* ht = reinterpret_cast<TcTile*>(h_dst);

@@ -304,7 +304,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
     int32_t* sr = reinterpret_cast<int32_t*>(h + rank_off);
     std::vector<int32_t> cnt(n_segs + 1, 0);
     for (int i = 0; i < sc.n_tiles; ++i)
-      cnt[tt[i].seg + 1] += tt[i].n_blocks - (tt[i].k0 > 0 ? 1 : 0);   // a dumped first block writes no results
+      cnt[tt[i].seg + 1] += tt[i].n_blocks - (tt[i].k1 < d / 64 ? 1 : 0);   // a dumped first block writes no results
     sr[0] = 0;
     for (int32_t k = 0; k < n_segs; ++k) sr[k + 1] = sr[k] + cnt[k + 1];
   };

@@ -108,7 +108,7 @@ def _segments_of(kind, rng):
 
 def _block_sweeps(t, nk):
     """(scored row range, first K-chunk, end K-chunk) of every block of a schedule record (include/msas.h, mas_score_schedule):
-    block 0 joins at k0, the last block leaves at k1, the blocks in between are swept over all of K."""
+    the last block joins at k0, block 0 leaves at k1 (a one-block record: [k0, k1)), the blocks in between are swept over all of K."""
     cta, row0, n, nb, stride, mode, prev, halo = [int(v) for v in t[:8]]
     k0, k1 = int(t[12]), int(t[13])
     out = []
@@ -119,7 +119,7 @@ def _block_sweeps(t, nk):
             lo, hi = row0 + b * stride, row0 + b * stride + n
         else:   # window b: 128 rows from row0 + b * stride on, scored from `prev` on (the record's first window: from `halo` on)
             lo, hi = row0 + b * stride + (halo if b == 0 else prev), row0 + min(n, b * stride + 128)
-        out.append(((lo, hi), k0 if b == 0 else 0, k1 if b == nb - 1 else nk))
+        out.append(((lo, hi), k0 if b == nb - 1 else 0, k1 if b == 0 else nk))
     return out
 
 
@@ -166,21 +166,21 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
             assert lo < hi and seg_of_row[lo] == seg and seg_of_row[hi - 1] == seg    # a tile never straddles a segment
             assert 0 <= ka < kb <= nk
             cov[lo:hi] += kb - ka
-            if ka == 0:
+            if kb == nk:
                 owned[lo:hi] += 1
         mine = t[t[:, 0] == cta]
-        # K-split: a block shared along K is the last block of its owner (the part from chunk 0; last tile of its CTA) and the first
-        # block of the first tile of every CTA that follows, until chunk nk is reached
-        if k0 > 0:
-            assert split_open is not None and sweeps[0][0] == split_open[0] and k0 == split_open[1] and cta == split_open[2] + 1
+        # K-split: a block shared along K is the last block of its owner (the part that ends at chunk nk; last tile of its CTA) and
+        # the first block of the first tile of every CTA that follows, in descending K, until chunk 0 is reached
+        if k1 < nk:
+            assert split_open is not None and sweeps[0][0] == split_open[0] and k1 == split_open[1] and cta == split_open[2] + 1
             assert np.array_equal(rec, mine[0])
-            split_open[1], split_open[2], split_open[3] = sweeps[0][2], cta, split_open[3] - 1
-            if sweeps[0][2] == nk:
+            split_open[1], split_open[2], split_open[3] = sweeps[0][1], cta, split_open[3] - 1
+            if sweeps[0][1] == 0:
                 assert split_open[3] == 0
                 split_open = None
-        if k1 < nk and (nb > 1 or k0 == 0):
+        if k0 > 0 and (nb > 1 or k1 == nk):
             assert split_open is None and n_wait >= 1 and peer == cta + 1 and np.array_equal(rec, mine[-1])
-            split_open = [sweeps[-1][0], k1, cta, n_wait]
+            split_open = [sweeps[-1][0], k0, cta, n_wait]
         else:
             assert n_wait == 0 and peer == -1
         # cost model of csrc/k_score_tc.cuh (TcCost), about microseconds: a block 14 + 0.025 h (x 1.28 in a frame walk, x 1.7 for a window
@@ -193,7 +193,7 @@ def test_score_schedule_covers_every_row_once_and_is_balanced(B, kind):
         Lpad = (L + 15) // 16 * 16
         first_of_cta = np.array_equal(rec, mine[0])
         wait = 0.0 if first_of_cta else prev_epi * max(0, prev_nb + nb - n_slots)
-        cost[cta] += blocks + tile_share * (0.055 * Lpad + (0.077 * n if mode == 1 and (halo or k0 > 0) else 0)) + 1.5 + wait
+        cost[cta] += blocks + tile_share * (0.055 * Lpad + (0.077 * n if mode == 1 and (halo or k1 < nk) else 0)) + 1.5 + wait
         prev_nb, prev_epi = nb, 0.35 + 0.013 * Lpad
     assert split_open is None
     assert cov.min() == nk and cov.max() == nk                   # every K-chunk of every row swept exactly once
