@@ -88,6 +88,7 @@ struct TcSchedule {
   int wslot = 0, ns = 0;        // TMEM: columns per accumulator slot (pad16 of the longest query block), number of slots
   int smem_bytes = 0;
   int xchg_cols = 0;       // floats per row of a K-split exchange slot: pad16(longest query block) (+ 64) + 2
+  int help = 0;            // the CTAs' last tiles are long (>= 6 blocks on average): the HELP instantiation of the kernel is launched
   const TcTile* d_tiles = nullptr;
   const int32_t* d_cta_off = nullptr;
 };
@@ -370,9 +371,191 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
   }
 }
 
-template <int KW>   // 64-column K-slices per chunk
+// One block of a tile's epilogue, by four warps that cover the four TMEM lane quarters (q = warp % 4, r = the thread's block row).
+// BAR: a named barrier of their own.
+template <int BAR>
+__device__ __forceinline__ void tc_epi_block(const TcParams& p, TcCtrl* ctrl, const float* stat, uint32_t tmem_base, const TcTile& tile, int b,
+                                             uint32_t ts0, uint32_t tp0, int buf, int it, int q, int lane, uint32_t& hcnt) {
+  const int r = q * 32 + lane;
+  const int nk = p.n_kchunks;
+  const uint32_t ns = (uint32_t)p.ns;
+  const bool rider = p.sig != nullptr || p.heads_part != nullptr;
+  const int nqu = (tile.L + 15) >> 4;
+  const float inv_d = 1.0f / (float)p.d;
+  const float2* st2 = reinterpret_cast<const float2*>(stat) + (size_t)buf * kTcMaxBlocks * 128;
+  const bool dump0 = tile.k1 < nk;                               // K-split: block 0 is a part that hands its partial sums to the block's owner
+  const float* qinv = ctrl->qinv_s;
+  const size_t xslot_f = (size_t)p.xchg_cols * 128;              // floats per exchange slot
+  uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
+  if (ts >= ns) { ts -= ns; tp ^= 1u; }
+  const uint32_t tcol = tmem_base + ts * (uint32_t)p.wslot + ((uint32_t)(q * 32) << 16);
+  mbar_wait(smem_u32(&ctrl->tfull[ts]), tp);
+  tc_fence_after();
+  const int n_wait = b == tile.n_blocks - 1 ? tile.n_wait : 0;   // > 0: this CTA owns a split last block
+  if (dump0 && b == 0) {   // accumulator columns (column-major: lanes = rows, coalesced), then the two row sums, then the flag
+    float* xo = p.xchg + (size_t)blockIdx.x * xslot_f + r;
+    const int ncb = nqu + (rider ? 4 : 0);
+    for (int cb = 0; cb < ncb; ++cb) {
+      uint32_t v[16];
+      tc_ld16(tcol + (uint32_t)cb * 16u, v);
+      tc_wait_ld();
+#pragma unroll
+      for (int j = 0; j < 16; ++j) xo[(size_t)(cb * 16 + j) * 128] = __uint_as_float(v[j]);
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
+    if (tile.n_blocks > 1) mbar_wait(smem_u32(&ctrl->s0full), 0u);   // (complete long before the tile's other blocks)
+    else mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
+    const float2 nd = st2[b * 128 + r];
+    xo[(size_t)(p.xchg_cols - 2) * 128] = nd.x;
+    xo[(size_t)(p.xchg_cols - 1) * 128] = nd.y;
+    __threadfence();
+    asm volatile("bar.sync %0, 128;" ::"n"(BAR) : "memory");       // the four epilogue warps
+    if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + blockIdx.x), "r"(1u) : "memory");
+    return;
+  }
+  if (n_wait > 0) {   // owner of a split block: the other parts were the first thing the CTAs that follow this one swept
+    if (lane == 0)
+      for (int i = 0; i < n_wait; ++i) {
+        unsigned int f;
+        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.xflag + tile.peer + i) : "memory"); } while (f == 0u);
+      }
+    __syncwarp();
+  }
+  const float* xi = p.xchg + (size_t)tile.peer * xslot_f + r;      // owner: the parts' slots follow one another
+  // 16 accumulator columns of this thread's row, the foreign parts added in slot order (a fixed order: bit-reproducible)
+  auto ld16 = [&](int cbi, float (&f)[16]) {
+    uint32_t v[16];
+    tc_ld16(tcol + (uint32_t)cbi * 16u, v);
+    tc_wait_ld();
+#pragma unroll
+    for (int j = 0; j < 16; ++j) f[j] = __uint_as_float(v[j]);
+    for (int i = 0; i < n_wait; ++i)
+#pragma unroll
+      for (int j = 0; j < 16; ++j) f[j] += xi[(size_t)i * xslot_f + (size_t)(cbi * 16 + j) * 128];
+  };
+  const int hb = tc_block_rows(tile, b);
+  const int out_lo = tile.mode == 2 ? (b == 0 ? tile.halo : tile.prev) : 0;
+  const bool valid = r < hb && r >= out_lo;
+  const int64_t row = (int64_t)tile.row0 + (int64_t)b * tile.stride + r;
+  float m = -INFINITY;
+  if (n_wait == 0) {   // the common case: two column groups in flight per wait
+    for (int cb = 0; cb < nqu; cb += 2) {
+      uint32_t v0[16], v1[16];
+      tc_ld16(tcol + (uint32_t)cb * 16u, v0);
+      if (cb + 1 < nqu) tc_ld16(tcol + (uint32_t)(cb + 1) * 16u, v1);
+      tc_wait_ld();
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const int col = cb * 16 + j;
+        if (col < tile.L) m = fmaxf(m, __uint_as_float(v0[j]) * qinv[col]);
+      }
+      if (cb + 1 < nqu) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          const int col = cb * 16 + 16 + j;
+          if (col < tile.L) m = fmaxf(m, __uint_as_float(v1[j]) * qinv[col]);
+        }
+      }
+    }
+  } else {
+    for (int cb = 0; cb < nqu; ++cb) {
+      float v[16];
+      ld16(cb, v);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const int col = cb * 16 + j;
+        if (col < tile.L) m = fmaxf(m, v[j] * qinv[col]);
+      }
+    }
+  }
+  if (p.heads_part != nullptr) {   // NEXT-2: column 0 -> the learned spatial map, all 64 -> per-block column sums (fixed order)
+    float tot[2];
+#pragma unroll
+    for (int grp = 0; grp < 2; ++grp) {
+      float x[32];
+#pragma unroll
+      for (int cb = 0; cb < 2; ++cb) {
+        float v[16];
+        ld16(nqu + grp * 2 + cb, v);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) x[cb * 16 + j] = valid ? v[j] : 0.f;
+      }
+      if (grp == 0) {
+        float below = 0.f;
+        if (valid) {
+          const float M = sigmoidf_acc(x[0] + p.heads_bias);
+          p.heads_m[row] = M;
+          below = M < p.heads_tau ? 1.f : 0.f;
+        }
+        x[0] = below;
+      }
+      // transpose-reduce over the warp: 31 shuffles leave the total of column `lane` in lane `lane`
+#pragma unroll
+      for (int w = 16; w >= 1; w >>= 1) {
+        const bool up = (lane & w) != 0;
+#pragma unroll
+        for (int i = 0; i < w; ++i) {
+          const float send = up ? x[i] : x[i + w], keep = up ? x[i + w] : x[i];
+          x[i] = keep + __shfl_xor_sync(0xffffffffu, send, w);
+        }
+      }
+      tot[grp] = x[0];
+    }
+    const int hbuf = (int)(hcnt++ & 1u);
+    ctrl->hred[hbuf][q][lane] = tot[0];
+    ctrl->hred[hbuf][q][32 + lane] = tot[1];
+    asm volatile("bar.sync %0, 128;" ::"n"(BAR) : "memory");       // the four epilogue warps
+    if (r < 64)
+      p.heads_part[((int64_t)tile.part0 + b) * 64 + r] = (ctrl->hred[hbuf][0][r] + ctrl->hred[hbuf][1][r]) + (ctrl->hred[hbuf][2][r] + ctrl->hred[hbuf][3][r]);
+  } else if (rider) {   // NEXT-1: the 64 accumulator columns after the query columns are r_k . x: their signs are the hash bits
+    unsigned long long bits = 0ull;
+#pragma unroll
+    for (int cb = 0; cb < 4; ++cb) {
+      float v[16];
+      ld16(nqu + cb, v);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) bits |= (unsigned long long)(v[j] >= 0.f) << (cb * 16 + j);
+    }
+    if (valid) p.sig[row] = bits;
+  }
+  tc_fence_before();
+  __syncwarp();
+  if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
+  mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);   // (true at once after the tile's first wait)
+  float2 nd = st2[b * 128 + r];
+  for (int i = 0; i < n_wait; ++i) {
+    nd.x += xi[(size_t)i * xslot_f + (size_t)(p.xchg_cols - 2) * 128];
+    nd.y += xi[(size_t)i * xslot_f + (size_t)(p.xchg_cols - 1) * 128];
+  }
+  if (valid) {
+    p.s[row] = sqrtf(nd.x * inv_d);
+    p.dnorm[row] = sqrtf(nd.y);
+    p.rel[row] = nd.x > 0.f ? m / sqrtf(nd.x) : 0.f;
+  }
+  if (n_wait > 0) {   // every warp has read the slots: re-arm their flags for the next launch
+    asm volatile("bar.sync %0, 128;" ::"n"(BAR) : "memory");
+    if (q == 0 && lane < n_wait) p.xflag[tile.peer + lane] = 0u;
+  }
+}
+
+// The epilogue of a CTA's last tile has nothing to hide behind: where that tile is long (a frame walk) the eight statistics warps,
+// done with their sweep, take two blocks in three (group G = 1: warps 4-7, G = 2: warps 8-11; blocks b % 3 == G).  Not inlined: the
+// sweep must not pay for it in registers.  Only in the HELP instantiation of the kernel: the mere presence of the call costs the
+// short-tile workloads more than it saves them.
+template <int G>
+__device__ __noinline__ void tc_epi_help(const TcParams& p, TcCtrl* ctrl, const float* stat, uint32_t tmem_base, const TcTile* tile_g,
+                                         uint32_t ts0, uint32_t tp0, int buf, int it) {
+  const TcTile tile = *tile_g;
+  const int lane = threadIdx.x & 31, q = (threadIdx.x >> 5) & 3;
+  uint32_t hcnt = 0;
+  for (int b = G; b < tile.n_blocks; b += 3) tc_epi_block<1 + G>(p, ctrl, stat, tmem_base, tile, b, ts0, tp0, buf, it, q, lane, hcnt);
+}
+
+template <int KW, bool HELP>   // 64-column K-slices per chunk; the statistics warps join the epilogue of the CTA's last tile
 __global__ void __launch_bounds__(kTcThreads, 1)
-k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
+k_score_tc(const __grid_constant__ TcMaps maps, const __grid_constant__ TcParams p) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   TcCtrl* ctrl = reinterpret_cast<TcCtrl*>(smem);
@@ -532,7 +715,6 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     // ===================================================================== epilogue: one accumulator row per thread
     const int q = warp & 3;                  // TMEM lane quarter this warp may access (warp % 4)
     const int r = q * 32 + lane;             // block row
-    const float inv_d = 1.0f / (float)p.d;
     // a0 inside the same launch: while the first chunks stream in, these four warps compute 1 / |q_j| for this CTA's
     // share of the query rows (row j belongs to CTA j % gridDim.x).  Every CTA of the grid is co-resident (cooperative
     // launch), so the first epilogue may wait on the grid-wide counter for the other CTAs' shares.
@@ -560,10 +742,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
       const int buf = it & 1;
-      const int nqu = (tile.L + 15) >> 4;
-      const float2* st2 = reinterpret_cast<const float2*>(stat) + (size_t)buf * kTcMaxBlocks * 128;
-      const bool dump0 = tile.k1 < nk;                               // K-split: block 0 is a part that hands its partial sums to the block's owner
-      if (!(dump0 && tile.n_blocks == 1)) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
+      if (!(tile.k1 < nk && tile.n_blocks == 1)) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
         if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
           unsigned long long seen;
           do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
@@ -573,161 +752,11 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
         if (r < tile.L) ctrl->qinv_s[r] = p.qinv[tile.q_row0 + r];
         asm volatile("bar.sync 1, 128;" ::: "memory");
       }
-      const float* qinv = ctrl->qinv_s;
-      const size_t xslot_f = (size_t)p.xchg_cols * 128;              // floats per exchange slot
+      const bool helped = HELP && t == tile_hi - 1;                  // the CTA's last tile: the statistics warps take two blocks in three
+      if (helped) asm volatile("bar.arrive 4, 384;" ::: "memory");   // qinv_s is staged
       for (int b = 0; b < tile.n_blocks; ++b) {
-        uint32_t ts = ts0 + (uint32_t)b, tp = tp0;
-        if (ts >= ns) { ts -= ns; tp ^= 1u; }
-        const uint32_t tcol = tmem_base + ts * (uint32_t)p.wslot + ((uint32_t)(q * 32) << 16);
-        mbar_wait(smem_u32(&ctrl->tfull[ts]), tp);
-        tc_fence_after();
-        const int n_wait = b == tile.n_blocks - 1 ? tile.n_wait : 0;   // > 0: this CTA owns a split last block
-        if (dump0 && b == 0) {   // accumulator columns (column-major: lanes = rows, coalesced), then the two row sums, then the flag
-          float* xo = p.xchg + (size_t)blockIdx.x * xslot_f + r;
-          const int ncb = nqu + (rider ? 4 : 0);
-          for (int cb = 0; cb < ncb; ++cb) {
-            uint32_t v[16];
-            tc_ld16(tcol + (uint32_t)cb * 16u, v);
-            tc_wait_ld();
-#pragma unroll
-            for (int j = 0; j < 16; ++j) xo[(size_t)(cb * 16 + j) * 128] = __uint_as_float(v[j]);
-          }
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
-          if (tile.n_blocks > 1) mbar_wait(smem_u32(&ctrl->s0full), 0u);   // (complete long before the tile's other blocks)
-          else mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
-          const float2 nd = st2[b * 128 + r];
-          xo[(size_t)(p.xchg_cols - 2) * 128] = nd.x;
-          xo[(size_t)(p.xchg_cols - 1) * 128] = nd.y;
-          __threadfence();
-          asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
-          if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + blockIdx.x), "r"(1u) : "memory");
-          continue;
-        }
-        if (n_wait > 0) {   // owner of a split block: the other parts were the first thing the CTAs that follow this one swept
-          if (lane == 0)
-            for (int i = 0; i < n_wait; ++i) {
-              unsigned int f;
-              do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(p.xflag + tile.peer + i) : "memory"); } while (f == 0u);
-            }
-          __syncwarp();
-        }
-        const float* xi = p.xchg + (size_t)tile.peer * xslot_f + r;      // owner: the parts' slots follow one another
-        // 16 accumulator columns of this thread's row, the foreign parts added in slot order (a fixed order: bit-reproducible)
-        auto ld16 = [&](int cbi, float (&f)[16]) {
-          uint32_t v[16];
-          tc_ld16(tcol + (uint32_t)cbi * 16u, v);
-          tc_wait_ld();
-#pragma unroll
-          for (int j = 0; j < 16; ++j) f[j] = __uint_as_float(v[j]);
-          for (int i = 0; i < n_wait; ++i)
-#pragma unroll
-            for (int j = 0; j < 16; ++j) f[j] += xi[(size_t)i * xslot_f + (size_t)(cbi * 16 + j) * 128];
-        };
-        const int hb = tc_block_rows(tile, b);
-        const int out_lo = tile.mode == 2 ? (b == 0 ? tile.halo : tile.prev) : 0;
-        const bool valid = r < hb && r >= out_lo;
-        const int64_t row = (int64_t)tile.row0 + (int64_t)b * tile.stride + r;
-        float m = -INFINITY;
-        if (n_wait == 0) {   // the common case: two column groups in flight per wait
-          for (int cb = 0; cb < nqu; cb += 2) {
-            uint32_t v0[16], v1[16];
-            tc_ld16(tcol + (uint32_t)cb * 16u, v0);
-            if (cb + 1 < nqu) tc_ld16(tcol + (uint32_t)(cb + 1) * 16u, v1);
-            tc_wait_ld();
-#pragma unroll
-            for (int j = 0; j < 16; ++j) {
-              const int col = cb * 16 + j;
-              if (col < tile.L) m = fmaxf(m, __uint_as_float(v0[j]) * qinv[col]);
-            }
-            if (cb + 1 < nqu) {
-#pragma unroll
-              for (int j = 0; j < 16; ++j) {
-                const int col = cb * 16 + 16 + j;
-                if (col < tile.L) m = fmaxf(m, __uint_as_float(v1[j]) * qinv[col]);
-              }
-            }
-          }
-        } else {
-          for (int cb = 0; cb < nqu; ++cb) {
-            float v[16];
-            ld16(cb, v);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) {
-              const int col = cb * 16 + j;
-              if (col < tile.L) m = fmaxf(m, v[j] * qinv[col]);
-            }
-          }
-        }
-        if (p.heads_part != nullptr) {   // NEXT-2: column 0 -> the learned spatial map, all 64 -> per-block column sums (fixed order)
-          float tot[2];
-#pragma unroll
-          for (int grp = 0; grp < 2; ++grp) {
-            float x[32];
-#pragma unroll
-            for (int cb = 0; cb < 2; ++cb) {
-              float v[16];
-              ld16(nqu + grp * 2 + cb, v);
-#pragma unroll
-              for (int j = 0; j < 16; ++j) x[cb * 16 + j] = valid ? v[j] : 0.f;
-            }
-            if (grp == 0) {
-              float below = 0.f;
-              if (valid) {
-                const float M = sigmoidf_acc(x[0] + p.heads_bias);
-                p.heads_m[row] = M;
-                below = M < p.heads_tau ? 1.f : 0.f;
-              }
-              x[0] = below;
-            }
-            // transpose-reduce over the warp: 31 shuffles leave the total of column `lane` in lane `lane`
-#pragma unroll
-            for (int w = 16; w >= 1; w >>= 1) {
-              const bool up = (lane & w) != 0;
-#pragma unroll
-              for (int i = 0; i < w; ++i) {
-                const float send = up ? x[i] : x[i + w], keep = up ? x[i + w] : x[i];
-                x[i] = keep + __shfl_xor_sync(0xffffffffu, send, w);
-              }
-            }
-            tot[grp] = x[0];
-          }
-          const int hbuf = (int)(hcnt++ & 1u);
-          ctrl->hred[hbuf][q][lane] = tot[0];
-          ctrl->hred[hbuf][q][32 + lane] = tot[1];
-          asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
-          if (r < 64)
-            p.heads_part[((int64_t)tile.part0 + b) * 64 + r] = (ctrl->hred[hbuf][0][r] + ctrl->hred[hbuf][1][r]) + (ctrl->hred[hbuf][2][r] + ctrl->hred[hbuf][3][r]);
-        } else if (rider) {   // NEXT-1: the 64 accumulator columns after the query columns are r_k . x: their signs are the hash bits
-          unsigned long long bits = 0ull;
-#pragma unroll
-          for (int cb = 0; cb < 4; ++cb) {
-            float v[16];
-            ld16(nqu + cb, v);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) bits |= (unsigned long long)(v[j] >= 0.f) << (cb * 16 + j);
-          }
-          if (valid) p.sig[row] = bits;
-        }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctrl->tempty[ts]));
-        if (b == (dump0 ? 1 : 0)) mbar_wait(smem_u32(&ctrl->sfull[buf]), (uint32_t)(it >> 1) & 1u);
-        float2 nd = st2[b * 128 + r];
-        for (int i = 0; i < n_wait; ++i) {
-          nd.x += xi[(size_t)i * xslot_f + (size_t)(p.xchg_cols - 2) * 128];
-          nd.y += xi[(size_t)i * xslot_f + (size_t)(p.xchg_cols - 1) * 128];
-        }
-        if (valid) {
-          p.s[row] = sqrtf(nd.x * inv_d);
-          p.dnorm[row] = sqrtf(nd.y);
-          p.rel[row] = nd.x > 0.f ? m / sqrtf(nd.x) : 0.f;
-        }
-        if (n_wait > 0) {   // every warp has read the slots: re-arm their flags for the next launch
-          asm volatile("bar.sync 1, 128;" ::: "memory");
-          if (q == 0 && lane < n_wait) p.xflag[tile.peer + lane] = 0u;
-        }
+        if (helped && b % 3 != 0) continue;
+        tc_epi_block<1>(p, ctrl, stat, tmem_base, tile, b, ts0, tp0, buf, it, q, lane, hcnt);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->sempty[buf]));
@@ -741,7 +770,7 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
     c.nx = nx; c.nk = nk; c.lane = lane;
     c.arow = ((warp - 4) << 4) + (lane >> 1);
     c.hh = (uint32_t)lane & 1u;
-    uint32_t xs = 0, xph = 0;
+    uint32_t xs = 0, xph = 0, nbsum = 0;
     int it = 0;
     for (int t = tile_lo; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
@@ -751,6 +780,13 @@ k_score_tc(const __grid_constant__ TcMaps maps, const TcParams p) {
       tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, tile.k0, tile.k1, nk, xs, xph);
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->sfull[buf]));
+      if (HELP && t + 1 < tile_hi) nbsum += (uint32_t)tile.n_blocks;   // accumulator slots are handed out round-robin, block after block
+    }
+    if (HELP && tile_hi > tile_lo) {   // the last tile's epilogue: see tc_epi_help
+      const int itl = tile_hi - 1 - tile_lo;
+      asm volatile("bar.sync 4, 384;" ::: "memory");     // the epilogue warps have staged the tile's 1 / |q_j|
+      if (warp < 8) tc_epi_help<1>(p, ctrl, stat, tmem_base, p.tiles + tile_hi - 1, nbsum % ns, (nbsum / ns) & 1u, itl & 1, itl);
+      else tc_epi_help<2>(p, ctrl, stat, tmem_base, p.tiles + tile_hi - 1, nbsum % ns, (nbsum / ns) & 1u, itl & 1, itl);
     }
   }
 
@@ -1003,6 +1039,12 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     assign(hi, true);
   }
   const int n_tiles = (int)tiles.size();
+  {   // long last tiles (a frame walk): the epilogue of a CTA's last tile, which nothing hides, is worth sharing
+    int64_t last_blocks = 0, busy = 0;
+    for (int c = 0; c < n_ctas; ++c)
+      if (cta_first[c + 1] > cta_first[c]) { last_blocks += tiles[cta_first[c + 1] - 1].n_blocks; ++busy; }
+    sc.help = busy > 0 && last_blocks >= 6 * busy ? 1 : 0;
+  }
   {   // NEXT-2 partial slots: one per block, contiguous per segment (tiles are in row order of their segment already)
     int part = 0;
     for (TcTile& t : tiles) { const int dumped = t.k1 < S * sc.kw ? 1 : 0; t.part0 = part - dumped; part += t.n_blocks - dumped; }   // (a dumped block 0 writes no results)
@@ -1020,8 +1062,12 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
 }
 
 inline cudaError_t tc_set_kernel_attrs() {
-  const cudaError_t e = cudaFuncSetAttribute(k_score_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes);
-  return e != cudaSuccess ? e : cudaFuncSetAttribute(k_score_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes);
+  void (*const ks[4])(const TcMaps, const TcParams) = {k_score_tc<1, false>, k_score_tc<2, false>, k_score_tc<1, true>, k_score_tc<2, true>};
+  for (auto k : ks) {
+    const cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 typedef CUresult (*tc_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
@@ -1093,9 +1139,12 @@ inline cudaError_t tc_launch_score(const TcSchedule& sc, TcMapCache& cache, cons
   p.xchg = xchg; p.xflag = xflag; p.xchg_cols = sc.xchg_cols;
   p.heads_part = hf ? hf->part : nullptr; p.heads_m = hf ? hf->m : nullptr; p.heads_bias = hf ? hf->bias : 0.f; p.heads_tau = hf ? hf->tau : 0.f;
   if (hf) p.sig = nullptr;
+  // (no helpers with the NEXT-2 rider: its column sums go through one staging buffer)
+  const bool help = sc.help != 0 && hf == nullptr;
+  void (*const kern)(const TcMaps, const TcParams) = sc.kw == 2 ? (help ? k_score_tc<2, true> : k_score_tc<2, false>) : (help ? k_score_tc<1, true> : k_score_tc<1, false>);
   if (!inline_qprep) {   // qinv is already there: no CTA waits on another one, a plain launch will do
     p.Q = nullptr;
-    return launch_k(sc.kw == 2 ? k_score_tc<2> : k_score_tc<1>, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl_in, *maps, p);
+    return launch_k(kern, dim3((unsigned)sc.n_ctas), dim3(kTcThreads), (size_t)sc.smem_bytes, st, pdl_in, *maps, p);
   }
   // cooperative launch: the query-norm prologue makes the CTAs wait on one another once, so all must be resident
   cudaLaunchConfig_t cfg = {};
@@ -1104,7 +1153,7 @@ inline cudaError_t tc_launch_score(const TcSchedule& sc, TcMapCache& cache, cons
   attr[0].id = cudaLaunchAttributeCooperative;
   attr[0].val.cooperative = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  return sc.kw == 2 ? cudaLaunchKernelEx(&cfg, k_score_tc<2>, *maps, p) : cudaLaunchKernelEx(&cfg, k_score_tc<1>, *maps, p);
+  return cudaLaunchKernelEx(&cfg, kern, *maps, p);
 }
 
 }  // namespace msas
