@@ -33,27 +33,33 @@ __global__ void __launch_bounds__(256) k_spatial_pool(const DevSeg* __restrict__
   }
 }
 
-// (b) mean of a frame's dropped rows.  One CTA per (frame, slab of 128 16-byte column vectors, row split): each warp takes
-// every 8th row of its row range, four rows at a time (mask bytes first, then 16 predicated vector loads per lane), lanes cover
-// the slab's vectors; fp32 sums in a fixed order.  With one row split the CTA writes the mean; with several (few frames: a
-// batch of images) it writes partial sums and k_merge_finish adds them in split order.
+// (b) mean of a frame's dropped rows.  One CTA of four warps per (frame, slab of 128 16-byte column vectors, row split); consecutive
+// CTAs take the slabs of one frame.  Each warp takes every 4th row of its row range: the mask bytes of 32 rows at once, then only the
+// dropped rows, four at a time (16 vector loads per lane), lanes cover the slab's vectors; fp32 sums in a fixed order.  With one row
+// split the CTA writes the mean; with several (few frames: a batch of images) it writes partial sums and k_merge_finish adds them in
+// split order.
 constexpr int kMergeCtas = 1184;                 // CTAs aimed at when a batch has few frames (8 per SM); also the scratch slabs
 constexpr int kMergeVPL = 4;                     // vectors per lane: a slab is 32 lanes x 4 vectors
+constexpr int kMergeWarps = 4;                   // warps per CTA: small CTAs, so that a video batch's (frame, slab) units are all resident at once
 template <int DT>
-__global__ void __launch_bounds__(256) k_merge_dropped(const DevFrame* __restrict__ frames, const void* __restrict__ X,
+__global__ void __launch_bounds__(32 * kMergeWarps) k_merge_dropped(const DevFrame* __restrict__ frames, const void* __restrict__ X,
                                                        const uint8_t* __restrict__ keep_mask, float* __restrict__ Ymerge,
                                                        int32_t* __restrict__ n_dropped, float* __restrict__ part,
                                                        int32_t* __restrict__ cnt_part, int d) {
   constexpr int VE = DT == 1 ? 8 : 4;            // elements per 16-byte vector
   constexpr int VPL = kMergeVPL;
   constexpr int SLAB = 32 * VPL * VE;            // columns per slab
-  __shared__ float red[8][32 * VE];              // [warp][one vector index of the slab]
-  __shared__ int cnt_s[8];
-  const DevFrame fr = frames[blockIdx.x];
+  constexpr int NW = kMergeWarps;
+  __shared__ float red[NW][32 * VE];              // [warp][one vector index of the slab]
+  __shared__ int cnt_s[NW];
+  // consecutive CTAs take the slabs of ONE frame (the CTAs that run side by side read neighbouring pieces of the same rows)
+  const unsigned lin = blockIdx.x + gridDim.x * blockIdx.y;
+  const int fidx = (int)(lin / gridDim.y), sidx = (int)(lin % gridDim.y);
+  const DevFrame fr = frames[fidx];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int RS = gridDim.z, rs = blockIdx.z;
   const int per = (fr.n_patches + RS - 1) / RS, p_lo = min(fr.n_patches, rs * per), p_hi = min(fr.n_patches, p_lo + per);
-  const int c0 = blockIdx.y * SLAB;
+  const int c0 = sidx * SLAB;
   const int esz = DT == 1 ? 2 : 4;
   float acc[VPL][VE];
 #pragma unroll
@@ -61,32 +67,42 @@ __global__ void __launch_bounds__(256) k_merge_dropped(const DevFrame* __restric
 #pragma unroll
     for (int e = 0; e < VE; ++e) acc[v][e] = 0.f;
   int cnt = 0;
-  for (int p0 = p_lo + warp; p0 < p_hi; p0 += 32) {   // rows p0, p0 + 8, p0 + 16, p0 + 24
-    bool drop[4];
+  // This warp's rows are p_lo + warp + NW j.  The mask bytes of 32 of them are read at once (one per lane) and turned into a bit mask
+  // of the DROPPED ones; the loads then visit only those, four rows (16 vector loads per lane) at a time, in ascending order: the
+  // mask latency is off the load chain and kept rows take no load slots.  (Same summation order as a plain row loop.)
+  const int nj = p_hi > p_lo + warp ? (p_hi - p_lo - warp + NW - 1) / NW : 0;
+  for (int j0 = 0; j0 < nj; j0 += 32) {
+    const int prl = p_lo + warp + NW * (j0 + lane);
+    unsigned m = __ballot_sync(0xffffffffu, prl < p_hi && keep_mask[fr.row0 + prl] == 0);
+    cnt += __popc(m);
+    while (m) {
+      int pr[4];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) { const int pr = p0 + 8 * q; drop[q] = pr < p_hi && keep_mask[fr.row0 + pr] == 0; }
-    uint4 u[4][VPL];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const char* src = static_cast<const char*>(X) + (fr.row0 + p0 + 8 * q) * (int64_t)d * esz;
-#pragma unroll
-      for (int v = 0; v < VPL; ++v) {
-        const int col = c0 + (v * 32 + lane) * VE;
-        u[q][v] = (drop[q] && col < d) ? ld_nc16(src + (int64_t)col * esz) : make_uint4(0, 0, 0, 0);
+      for (int q = 0; q < 4; ++q) {
+        if (m) { const int b = __ffs(m) - 1; m &= m - 1; pr[q] = p_lo + warp + NW * (j0 + b); } else pr[q] = -1;
       }
-    }
+      uint4 u[4][VPL];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      cnt += drop[q] ? 1 : 0;
+      for (int q = 0; q < 4; ++q) {
+        const char* src = static_cast<const char*>(X) + (fr.row0 + (pr[q] < 0 ? 0 : pr[q])) * (int64_t)d * esz;
 #pragma unroll
-      for (int v = 0; v < VPL; ++v) {
-        if (DT == 1) {
-          const uint32_t w[4] = {u[q][v].x, u[q][v].y, u[q][v].z, u[q][v].w};
+        for (int v = 0; v < VPL; ++v) {
+          const int col = c0 + (v * 32 + lane) * VE;
+          u[q][v] = (pr[q] >= 0 && col < d) ? ld_nc16(src + (int64_t)col * esz) : make_uint4(0, 0, 0, 0);
+        }
+      }
 #pragma unroll
-          for (int k = 0; k < 4; ++k) { acc[v][(2 * k) % VE] += bf_lo(w[k]); acc[v][(2 * k + 1) % VE] += bf_hi(w[k]); }
-        } else {
-          acc[v][0] += __uint_as_float(u[q][v].x); acc[v][1] += __uint_as_float(u[q][v].y);
-          acc[v][2 % VE] += __uint_as_float(u[q][v].z); acc[v][3 % VE] += __uint_as_float(u[q][v].w);
+      for (int q = 0; q < 4; ++q) {
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) {
+          if (DT == 1) {
+            const uint32_t w[4] = {u[q][v].x, u[q][v].y, u[q][v].z, u[q][v].w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { acc[v][(2 * k) % VE] += bf_lo(w[k]); acc[v][(2 * k + 1) % VE] += bf_hi(w[k]); }
+          } else {
+            acc[v][0] += __uint_as_float(u[q][v].x); acc[v][1] += __uint_as_float(u[q][v].y);
+            acc[v][2 % VE] += __uint_as_float(u[q][v].z); acc[v][3 % VE] += __uint_as_float(u[q][v].w);
+          }
         }
       }
     }
@@ -95,23 +111,23 @@ __global__ void __launch_bounds__(256) k_merge_dropped(const DevFrame* __restric
   __syncthreads();
   int total = 0;
 #pragma unroll
-  for (int w = 0; w < 8; ++w) total += cnt_s[w];
+  for (int w = 0; w < NW; ++w) total += cnt_s[w];
   const bool final_ = RS == 1;
   const float scale = final_ ? (total > 0 ? 1.0f / (float)total : 0.f) : 1.0f;
-  if (blockIdx.y == 0 && threadIdx.x == 0) {
-    if (final_) n_dropped[blockIdx.x] = total; else cnt_part[blockIdx.x * RS + rs] = total;
+  if (sidx == 0 && threadIdx.x == 0) {
+    if (final_) n_dropped[fidx] = total; else cnt_part[fidx * RS + rs] = total;
   }
-  float* dst = final_ ? Ymerge + (int64_t)blockIdx.x * d : part + ((int64_t)(blockIdx.x * RS + rs) * gridDim.y + blockIdx.y) * SLAB - c0;
+  float* dst = final_ ? Ymerge + (int64_t)fidx * d : part + ((int64_t)(fidx * RS + rs) * gridDim.y + sidx) * SLAB - c0;
 #pragma unroll
   for (int v = 0; v < VPL; ++v) {
     __syncthreads();
 #pragma unroll
     for (int e = 0; e < VE; ++e) red[warp][lane * VE + e] = acc[v][e];
     __syncthreads();
-    for (int i = threadIdx.x; i < 32 * VE; i += 256) {
+    for (int i = threadIdx.x; i < 32 * VE; i += 32 * NW) {
       float t = 0.f;
 #pragma unroll
-      for (int w = 0; w < 8; ++w) t += red[w][i];
+      for (int w = 0; w < NW; ++w) t += red[w][i];
       const int col = c0 + v * 32 * VE + i;   // i = lane * VE + e
       if (col < d) dst[col] = t * scale;
     }
@@ -153,21 +169,32 @@ __global__ void __launch_bounds__(256) k_gather_residual(const DevSeg* __restric
     const uint4* src = reinterpret_cast<const uint4*>(X + row * (int64_t)d * esz);
     const uint4* prv = reinterpret_cast<const uint4*>(X + (row - sg.n_patches) * (int64_t)d * esz);
     uint4* dst = reinterpret_cast<uint4*>(Y + j * (int64_t)d * esz);
-    for (int i = lane; i < n16; i += 32) {
-      uint4 v = ld_nc16(src + i);
-      if (res) {
-        const uint4 q = ld_nc16(prv + i);
-        if (DT == 1) {   // the difference of two bf16 values is exact in fp32; cvt.rn rounds it to nearest even
-          v.x = pack_bf16x2(bf_lo(v.x) - bf_lo(q.x), bf_hi(v.x) - bf_hi(q.x));
-          v.y = pack_bf16x2(bf_lo(v.y) - bf_lo(q.y), bf_hi(v.y) - bf_hi(q.y));
-          v.z = pack_bf16x2(bf_lo(v.z) - bf_lo(q.z), bf_hi(v.z) - bf_hi(q.z));
-          v.w = pack_bf16x2(bf_lo(v.w) - bf_lo(q.w), bf_hi(v.w) - bf_hi(q.w));
-        } else {
-          v.x = __float_as_uint(__uint_as_float(v.x) - __uint_as_float(q.x)); v.y = __float_as_uint(__uint_as_float(v.y) - __uint_as_float(q.y));
-          v.z = __float_as_uint(__uint_as_float(v.z) - __uint_as_float(q.z)); v.w = __float_as_uint(__uint_as_float(v.w) - __uint_as_float(q.w));
-        }
+    auto diff = [&](uint4 v, const uint4& q) {
+      if (DT == 1) {   // the difference of two bf16 values is exact in fp32; cvt.rn rounds it to nearest even
+        v.x = pack_bf16x2(bf_lo(v.x) - bf_lo(q.x), bf_hi(v.x) - bf_hi(q.x));
+        v.y = pack_bf16x2(bf_lo(v.y) - bf_lo(q.y), bf_hi(v.y) - bf_hi(q.y));
+        v.z = pack_bf16x2(bf_lo(v.z) - bf_lo(q.z), bf_hi(v.z) - bf_hi(q.z));
+        v.w = pack_bf16x2(bf_lo(v.w) - bf_lo(q.w), bf_hi(v.w) - bf_hi(q.w));
+      } else {
+        v.x = __float_as_uint(__uint_as_float(v.x) - __uint_as_float(q.x)); v.y = __float_as_uint(__uint_as_float(v.y) - __uint_as_float(q.y));
+        v.z = __float_as_uint(__uint_as_float(v.z) - __uint_as_float(q.z)); v.w = __float_as_uint(__uint_as_float(v.w) - __uint_as_float(q.w));
       }
-      st_na16(dst + i, v);
+      return v;
+    };
+    // four vectors of the row (and of its predecessor) in flight per lane
+    for (int i0 = lane; i0 < n16; i0 += 128) {
+      uint4 v[4], q[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + 32 * u;
+        v[u] = i < n16 ? ld_nc16(src + i) : make_uint4(0, 0, 0, 0);
+        q[u] = res && i < n16 ? ld_nc16(prv + i) : make_uint4(0, 0, 0, 0);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + 32 * u;
+        if (i < n16) st_na16(dst + i, res ? diff(v[u], q[u]) : v[u]);
+      }
     }
   }
 }

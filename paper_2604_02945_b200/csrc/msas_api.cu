@@ -532,6 +532,10 @@ extern "C" int mas_crossmodal(const mas_plan* p, const void* X, const void* Q, f
   if (!p || !X || !Q || (!rel && !S_opt)) return MAS_ERR_INVALID_ARG;
   if (!aligned16(X) || !aligned16(Q)) return MAS_ERR_UNSUPPORTED;
   cudaStream_t st = (cudaStream_t)stream;
+  // without the similarity matrix this is the score sweep with two of its three outputs left in the plan's workspace: the tcgen05
+  // kernel (bf16, d % 64 == 0) instead of the generic mma.sync one
+  if (!S_opt && p->tc.enabled)
+    return launch_score_tc(p, false, X, Q, p->at<float>(p->lay.s), p->at<float>(p->lay.gamma), rel, nullptr, nullptr, nullptr, st, false);
   int rc = launch_qprep(p, Q, st);
   if (rc != MAS_OK) return rc;
   return launch_score_mma(p, X, Q, nullptr, nullptr, rel ? rel : p->at<float>(p->lay.rel), S_opt, st);
@@ -613,8 +617,8 @@ extern "C" int mas_merge_dropped(const mas_plan* p, const void* X, const uint8_t
   const dim3 grid((unsigned)p->n_frames, (unsigned)slabs, (unsigned)rs);
   float* part = p->at<float>(p->lay.merge_part);
   int32_t* cnt = p->at<int32_t>(p->lay.merge_cnt);
-  if (p->dtype == MAS_BF16) k_merge_dropped<1><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, part, cnt, p->d);
-  else k_merge_dropped<0><<<grid, 256, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, part, cnt, p->d);
+  if (p->dtype == MAS_BF16) k_merge_dropped<1><<<grid, 32 * kMergeWarps, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, part, cnt, p->d);
+  else k_merge_dropped<0><<<grid, 32 * kMergeWarps, 0, st>>>(p->at<DevFrame>(p->lay.frames), X, keep_mask, Ymerge, n_dropped, part, cnt, p->d);
   CK(cudaGetLastError());
   if (rs > 1) {
     k_merge_finish<<<dim3((unsigned)p->n_frames, (unsigned)slabs), 256, 0, st>>>(part, cnt, Ymerge, n_dropped, (int)rs, slab, p->d);

@@ -64,6 +64,9 @@ def test_staged_scores(B, w):
     P.assert_close(gam.cpu().numpy(), ref_g, "gamma")
     assert np.array_equal(gam.cpu().numpy() == 0.0, ref_g == 0.0)          # bit-identical rows give exactly 0.0f
     P.assert_close(rel.cpu().numpy(), ref_rel, "rel")
+    rel_only = plan.crossmodal(X, Q, want_S=False)                         # no S: bf16 / d % 64 == 0 plans take the tcgen05 score kernel
+    torch.cuda.synchronize()
+    P.assert_close(rel_only.cpu().numpy(), ref_rel, "rel (without S)")
     # raw dot products: error relative to |x||q| (the scale of the accumulation), not to a possibly tiny S_ij
     Sg = S.cpu().numpy()
     r0 = 0
