@@ -88,7 +88,7 @@ struct TcSchedule {
   int wslot = 0, ns = 0;        // TMEM: columns per accumulator slot (pad16 of the longest query block), number of slots
   int smem_bytes = 0;
   int xchg_cols = 0;       // floats per row of a K-split exchange slot: pad16(longest query block) (+ 64) + 2
-  int help = 0;            // the CTAs' last tiles are long (>= 6 blocks on average): the HELP instantiation of the kernel is launched
+  int help = 0;            // 1: the HELP instantiation of the kernel is launched
   const TcTile* d_tiles = nullptr;
   const int32_t* d_cta_off = nullptr;
 };
@@ -372,10 +372,9 @@ __device__ __forceinline__ void tc_alu_tile(const TcAluCtx& c, int mode, int n_r
 }
 
 // One block of a tile's epilogue, by four warps that cover the four TMEM lane quarters (q = warp % 4, r = the thread's block row).
-// BAR: a named barrier of their own.
-template <int BAR>
+// `bar_id`: a named barrier of their own.
 __device__ __forceinline__ void tc_epi_block(const TcParams& p, TcCtrl* ctrl, const float* stat, uint32_t tmem_base, const TcTile& tile, int b,
-                                             uint32_t ts0, uint32_t tp0, int buf, int it, int q, int lane, uint32_t& hcnt) {
+                                             uint32_t ts0, uint32_t tp0, int buf, int it, int q, int lane, uint32_t bar_id, uint32_t& hcnt) {
   const int r = q * 32 + lane;
   const int nk = p.n_kchunks;
   const uint32_t ns = (uint32_t)p.ns;
@@ -411,7 +410,7 @@ __device__ __forceinline__ void tc_epi_block(const TcParams& p, TcCtrl* ctrl, co
     xo[(size_t)(p.xchg_cols - 2) * 128] = nd.x;
     xo[(size_t)(p.xchg_cols - 1) * 128] = nd.y;
     __threadfence();
-    asm volatile("bar.sync %0, 128;" ::"n"(BAR) : "memory");       // the four epilogue warps
+    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");       // the four epilogue warps
     if (q == 0 && lane == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.xflag + blockIdx.x), "r"(1u) : "memory");
     return;
   }
@@ -506,7 +505,7 @@ __device__ __forceinline__ void tc_epi_block(const TcParams& p, TcCtrl* ctrl, co
     const int hbuf = (int)(hcnt++ & 1u);
     ctrl->hred[hbuf][q][lane] = tot[0];
     ctrl->hred[hbuf][q][32 + lane] = tot[1];
-    asm volatile("bar.sync %0, 128;" ::"n"(BAR) : "memory");       // the four epilogue warps
+    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");       // the four epilogue warps
     if (r < 64)
       p.heads_part[((int64_t)tile.part0 + b) * 64 + r] = (ctrl->hred[hbuf][0][r] + ctrl->hred[hbuf][1][r]) + (ctrl->hred[hbuf][2][r] + ctrl->hred[hbuf][3][r]);
   } else if (rider) {   // NEXT-1: the 64 accumulator columns after the query columns are r_k . x: their signs are the hash bits
@@ -535,22 +534,9 @@ __device__ __forceinline__ void tc_epi_block(const TcParams& p, TcCtrl* ctrl, co
     p.rel[row] = nd.x > 0.f ? m / sqrtf(nd.x) : 0.f;
   }
   if (n_wait > 0) {   // every warp has read the slots: re-arm their flags for the next launch
-    asm volatile("bar.sync %0, 128;" ::"n"(BAR) : "memory");
+    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
     if (q == 0 && lane < n_wait) p.xflag[tile.peer + lane] = 0u;
   }
-}
-
-// The epilogue of a CTA's last tile has nothing to hide behind: where that tile is long (a frame walk) the eight statistics warps,
-// done with their sweep, take two blocks in three (group G = 1: warps 4-7, G = 2: warps 8-11; blocks b % 3 == G).  Not inlined: the
-// sweep must not pay for it in registers.  Only in the HELP instantiation of the kernel: the mere presence of the call costs the
-// short-tile workloads more than it saves them.
-template <int G>
-__device__ __noinline__ void tc_epi_help(const TcParams& p, TcCtrl* ctrl, const float* stat, uint32_t tmem_base, const TcTile* tile_g,
-                                         uint32_t ts0, uint32_t tp0, int buf, int it) {
-  const TcTile tile = *tile_g;
-  const int lane = threadIdx.x & 31, q = (threadIdx.x >> 5) & 3;
-  uint32_t hcnt = 0;
-  for (int b = G; b < tile.n_blocks; b += 3) tc_epi_block<1 + G>(p, ctrl, stat, tmem_base, tile, b, ts0, tp0, buf, it, q, lane, hcnt);
 }
 
 template <int KW, bool HELP>   // 64-column K-slices per chunk; the statistics warps join the epilogue of the CTA's last tile
@@ -711,82 +697,93 @@ k_score_tc(const __grid_constant__ TcMaps maps, const __grid_constant__ TcParams
       ts0 += (uint32_t)tile.n_blocks;
       if (ts0 >= ns) { ts0 -= ns; tp0 ^= 1u; }
     }
-  } else if (warp < 4) {
-    // ===================================================================== epilogue: one accumulator row per thread
+  } else {
+    // ===================================================================== epilogue warps (0-3) and statistics warps (4-11)
+    // Both end in the same tile-epilogue loop below (one copy of its code): the epilogue warps run it over all tiles, the
+    // statistics warps (HELP) join it for the CTA's last tile, whose epilogue nothing hides, with two blocks in three.
+    const bool epi = warp < 4;
     const int q = warp & 3;                  // TMEM lane quarter this warp may access (warp % 4)
     const int r = q * 32 + lane;             // block row
-    // a0 inside the same launch: while the first chunks stream in, these four warps compute 1 / |q_j| for this CTA's
-    // share of the query rows (row j belongs to CTA j % gridDim.x).  Every CTA of the grid is co-resident (cooperative
-    // launch), so the first epilogue may wait on the grid-wide counter for the other CTAs' shares.
-    if (p.Q != nullptr) {
-      const uint4* Qv = static_cast<const uint4*>(p.Q);
-      const int n16 = p.d >> 3;              // 16-byte pieces per bf16 row
-      for (long long j = (long long)blockIdx.x + (long long)q * gridDim.x; j < p.nQ; j += 4ll * gridDim.x) {
-        float acc = 0.f;
-        for (int i = lane; i < n16; i += 32) {
-          const uint4 v = ld_nc16(Qv + j * n16 + i);
-          const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-          for (int k = 0; k < 4; ++k) { const float a0 = bf_lo(w[k]), a1 = bf_hi(w[k]); acc = fmaf(a0, a0, acc); acc = fmaf(a1, a1, acc); }
-        }
-        acc = warp_sum(acc);
-        if (lane == 0) p.qinv[j] = acc > 0.f ? 1.0f / sqrtf(acc) : 0.f;
-      }
-      __threadfence();
-      asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
-      if (q == 0 && lane == 0) atomicAdd(p.q_ready, 1ull);
-    }
-    bool q_ok = p.Q == nullptr;
     uint32_t ts0 = 0, tp0 = 0, hcnt = 0;
-    int it = 0;
-    for (int t = tile_lo; t < tile_hi; ++t, ++it) {
+    int it = 0, t_first = tile_lo, b_first = 0;
+    uint32_t bar_id = 1;                     // named barrier of this group of four warps
+    bool q_ok = p.Q == nullptr;
+    if (epi) {
+      // a0 inside the same launch: while the first chunks stream in, these four warps compute 1 / |q_j| for this CTA's
+      // share of the query rows (row j belongs to CTA j % gridDim.x).  Every CTA of the grid is co-resident (cooperative
+      // launch), so the first epilogue may wait on the grid-wide counter for the other CTAs' shares.
+      if (p.Q != nullptr) {
+        const uint4* Qv = static_cast<const uint4*>(p.Q);
+        const int n16 = p.d >> 3;              // 16-byte pieces per bf16 row
+        for (long long j = (long long)blockIdx.x + (long long)q * gridDim.x; j < p.nQ; j += 4ll * gridDim.x) {
+          float acc = 0.f;
+          for (int i = lane; i < n16; i += 32) {
+            const uint4 v = ld_nc16(Qv + j * n16 + i);
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { const float a0 = bf_lo(w[k]), a1 = bf_hi(w[k]); acc = fmaf(a0, a0, acc); acc = fmaf(a1, a1, acc); }
+          }
+          acc = warp_sum(acc);
+          if (lane == 0) p.qinv[j] = acc > 0.f ? 1.0f / sqrtf(acc) : 0.f;
+        }
+        __threadfence();
+        asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps
+        if (q == 0 && lane == 0) atomicAdd(p.q_ready, 1ull);
+      }
+    } else {
+      // CUDA-core statistics: two threads per block row
+      TcAluCtx c;
+      c.xring = xring; c.xslot = xslot; c.xfull0 = xfull0; c.xempty0 = xempty0; c.s0full = smem_u32(&ctrl->s0full);
+      c.nx = nx; c.nk = nk; c.lane = lane;
+      c.arow = ((warp - 4) << 4) + (lane >> 1);
+      c.hh = (uint32_t)lane & 1u;
+      uint32_t xs = 0, xph = 0, nbsum = 0;
+      int ia = 0;
+      for (int t = tile_lo; t < tile_hi; ++t, ++ia) {
+        const TcTile tile = p.tiles[t];
+        const int buf = ia & 1;
+        c.stat = smem_u32(stat) + (uint32_t)buf * (kTcMaxBlocks * 1024u) + (uint32_t)(c.arow * 2 + (int)c.hh) * 4u;   // + b * 1024: block b
+        mbar_wait(smem_u32(&ctrl->sempty[buf]), ((uint32_t)(ia >> 1) & 1u) ^ 1u);
+        tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, tile.k0, tile.k1, nk, xs, xph);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl->sfull[buf]));
+        if (HELP && t + 1 < tile_hi) nbsum += (uint32_t)tile.n_blocks;   // accumulator slots are handed out round-robin, block after block
+      }
+      t_first = tile_hi;
+      if (HELP && tile_hi > tile_lo) {   // join the last tile's epilogue: warps 4-7 blocks b % 3 == 1, warps 8-11 b % 3 == 2
+        t_first = tile_hi - 1;
+        it = t_first - tile_lo;
+        ts0 = nbsum % ns; tp0 = (nbsum / ns) & 1u;
+        b_first = warp < 8 ? 1 : 2;
+        bar_id = (uint32_t)(1 + b_first);
+        asm volatile("bar.sync 4, 384;" ::: "memory");     // the epilogue warps have staged the tile's 1 / |q_j|
+      }
+    }
+    for (int t = t_first; t < tile_hi; ++t, ++it) {
       const TcTile tile = p.tiles[t];
       const int buf = it & 1;
-      if (!(tile.k1 < nk && tile.n_blocks == 1)) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
-        if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
-          unsigned long long seen;
-          do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
-          q_ok = true;
+      const bool helped = HELP && t == tile_hi - 1;
+      if (epi) {
+        if (!(tile.k1 < nk && tile.n_blocks == 1)) {   // the tile's 1 / |q_j| into shared memory: the column loop below reads them as broadcasts
+          if (!q_ok) {   // all CTAs' shares of qinv are written (first tile only; normally long since true)
+            unsigned long long seen;
+            do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(p.q_ready) : "memory"); } while (seen < (unsigned long long)gridDim.x);
+            q_ok = true;
+          }
+          asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps are done with the previous tile's values
+          if (r < tile.L) ctrl->qinv_s[r] = p.qinv[tile.q_row0 + r];
+          asm volatile("bar.sync 1, 128;" ::: "memory");
         }
-        asm volatile("bar.sync 1, 128;" ::: "memory");       // the four epilogue warps are done with the previous tile's values
-        if (r < tile.L) ctrl->qinv_s[r] = p.qinv[tile.q_row0 + r];
-        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (helped) asm volatile("bar.arrive 4, 384;" ::: "memory");   // qinv_s is staged
       }
-      const bool helped = HELP && t == tile_hi - 1;                  // the CTA's last tile: the statistics warps take two blocks in three
-      if (helped) asm volatile("bar.arrive 4, 384;" ::: "memory");   // qinv_s is staged
-      for (int b = 0; b < tile.n_blocks; ++b) {
-        if (helped && b % 3 != 0) continue;
-        tc_epi_block<1>(p, ctrl, stat, tmem_base, tile, b, ts0, tp0, buf, it, q, lane, hcnt);
+      for (int b = b_first; b < tile.n_blocks; b += helped ? 3 : 1)
+        tc_epi_block(p, ctrl, stat, tmem_base, tile, b, ts0, tp0, buf, it, q, lane, bar_id, hcnt);
+      if (epi) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl->sempty[buf]));
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctrl->sempty[buf]));
       ts0 += (uint32_t)tile.n_blocks;
       if (ts0 >= ns) { ts0 -= ns; tp0 ^= 1u; }
-    }
-  } else {
-    // ===================================================================== CUDA-core statistics: two threads per block row
-    TcAluCtx c;
-    c.xring = xring; c.xslot = xslot; c.xfull0 = xfull0; c.xempty0 = xempty0; c.s0full = smem_u32(&ctrl->s0full);
-    c.nx = nx; c.nk = nk; c.lane = lane;
-    c.arow = ((warp - 4) << 4) + (lane >> 1);
-    c.hh = (uint32_t)lane & 1u;
-    uint32_t xs = 0, xph = 0, nbsum = 0;
-    int it = 0;
-    for (int t = tile_lo; t < tile_hi; ++t, ++it) {
-      const TcTile tile = p.tiles[t];
-      const int buf = it & 1;
-      c.stat = smem_u32(stat) + (uint32_t)buf * (kTcMaxBlocks * 1024u) + (uint32_t)(c.arow * 2 + (int)c.hh) * 4u;   // + b * 1024: block b
-      mbar_wait(smem_u32(&ctrl->sempty[buf]), ((uint32_t)(it >> 1) & 1u) ^ 1u);
-      tc_alu_tile<KW>(c, tile.mode, tile.n_rows, tile.n_blocks, tile.stride, tile.prev, tile.mode == 1 && tile.halo != 0, tile.k0, tile.k1, nk, xs, xph);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctrl->sfull[buf]));
-      if (HELP && t + 1 < tile_hi) nbsum += (uint32_t)tile.n_blocks;   // accumulator slots are handed out round-robin, block after block
-    }
-    if (HELP && tile_hi > tile_lo) {   // the last tile's epilogue: see tc_epi_help
-      const int itl = tile_hi - 1 - tile_lo;
-      asm volatile("bar.sync 4, 384;" ::: "memory");     // the epilogue warps have staged the tile's 1 / |q_j|
-      if (warp < 8) tc_epi_help<1>(p, ctrl, stat, tmem_base, p.tiles + tile_hi - 1, nbsum % ns, (nbsum / ns) & 1u, itl & 1, itl);
-      else tc_epi_help<2>(p, ctrl, stat, tmem_base, p.tiles + tile_hi - 1, nbsum % ns, (nbsum / ns) & 1u, itl & 1, itl);
     }
   }
 
@@ -1039,12 +1036,9 @@ inline void tc_build_schedule(TcSchedule& sc, const mas_segment* segs, int32_t n
     assign(hi, true);
   }
   const int n_tiles = (int)tiles.size();
-  {   // long last tiles (a frame walk): the epilogue of a CTA's last tile, which nothing hides, is worth sharing
-    int64_t last_blocks = 0, busy = 0;
-    for (int c = 0; c < n_ctas; ++c)
-      if (cta_first[c + 1] > cta_first[c]) { last_blocks += tiles[cta_first[c + 1] - 1].n_blocks; ++busy; }
-    sc.help = busy > 0 && last_blocks >= 6 * busy ? 1 : 0;
-  }
+  // the epilogue of a CTA's last tile, which nothing hides, is shared with the statistics warps (the HELP instantiation of the kernel;
+  // the launch turns it off for the NEXT-2 rider, whose column sums go through one staging buffer)
+  sc.help = 1;
   {   // NEXT-2 partial slots: one per block, contiguous per segment (tiles are in row order of their segment already)
     int part = 0;
     for (TcTile& t : tiles) { const int dumped = t.k1 < S * sc.kw ? 1 : 0; t.part0 = part - dumped; part += t.n_blocks - dumped; }   // (a dumped block 0 writes no results)
