@@ -263,17 +263,26 @@ def bench_workload(name, args, rank, local_rank, world, sampler, want_e2e):
     # at each end.  The stage events above sit BETWEEN the kernels of a step and serialise them, so their score figure also
     # holds one launch latency; this loop is the kernel's average launch duration in a stream of its own launches.
     sbuf = (torch.empty(w.n_tokens, dtype=torch.float32, device="cuda"), None, torch.empty(w.n_tokens, dtype=torch.float32, device="cuda"))
-    n_alone = min(max(args.steps, 20), 50)      # a short burst: the kernel timed alone (MEASURED_PEAKS' copy figure is a burst figure too)
+    # Five short bursts (MEASURED_PEAKS' copy figure is a burst figure too), the median burst reported: the nvidia-smi sampler
+    # that runs beside the whole benchmark stalls a launch now and then, which lands in one burst, not in the figure.
+    # The bursts start from a rested GPU (1.5 s idle): after a few hundred steps the board sits at its power cap (SM clock 1965 ->
+    # 1760-1920 MHz) and the same kernel takes 7-11 % longer, which is what the in-step figure (`achieved`) already shows.
+    n_alone = min(max(args.steps, 10), 20)
+    torch.cuda.synchronize()
+    time.sleep(1.5)
     for i in range(3):
         plan.score(Xs[i % 2], Qs[i % 2], want_gamma=False, out=sbuf)
     torch.cuda.synchronize()
-    ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ea.record(stream)
-    for i in range(n_alone):
-        plan.score(Xs[i % 2], Qs[i % 2], want_gamma=False, out=sbuf)
-    eb.record(stream)
-    torch.cuda.synchronize()
-    score_alone_ms = ea.elapsed_time(eb) / n_alone
+    bursts = []
+    for rep in range(5):
+        ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ea.record(stream)
+        for i in range(n_alone):
+            plan.score(Xs[i % 2], Qs[i % 2], want_gamma=False, out=sbuf)
+        eb.record(stream)
+        torch.cuda.synchronize()
+        bursts.append(ea.elapsed_time(eb) / n_alone)
+    score_alone_ms = float(np.median(bursts))
 
     # ---- end to end through the host-buffer entry point (pinned host inputs, every result read back)
     e2e = None
@@ -324,8 +333,8 @@ def bench_workload(name, args, rank, local_rank, world, sampler, want_e2e):
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": score_bytes, "avg_launch_ms": score_ms,
                      "frac_of_8000_nominal": achieved / 8000.0,
-                     "note": "achieved / avg_launch_ms: events around the score stage inside a step (they serialise the step's kernels, so one launch latency is inside); kernel_alone_*: the same kernel in a stream of its own back-to-back launches",
-                     "kernel_alone_ms": score_alone_ms, "kernel_alone_achieved": achieved_alone, "kernel_alone_frac": achieved_alone / peak,
+                     "note": "achieved / avg_launch_ms: events around the score stage inside a step (they serialise the step's kernels, so one launch latency is inside); kernel_alone_*: the same kernel in a stream of its own back-to-back launches (median of five bursts of 20 launches after 1.5 s of idle, i.e. not power-capped; kernel_alone_bursts_ms lists them)",
+                     "kernel_alone_ms": score_alone_ms, "kernel_alone_bursts_ms": [round(b, 6) for b in bursts], "kernel_alone_achieved": achieved_alone, "kernel_alone_frac": achieved_alone / peak,
                      "kernel_alone_frac_of_8000_nominal": achieved_alone / 8000.0},
         "stages_ms": {"score": score_ms, "segment_select": float(stage[:, 1].mean()), "gather": float(stage[:, 2].mean())},
         "whole_pass": {"algorithmic_bytes": total_bytes, "achieved_gbs": total_bytes / (ms_step * 1e-3) / 1e9,

@@ -328,6 +328,23 @@ def test_forward_full_size(B, name, kw, sample):
     _forward_and_compare(B, w, sample_requests=sample if os.environ.get("MSAS_PARITY_QUICK") else None)
 
 
+@pytest.mark.parametrize("name", ["batched_images", "video", "ragged"])
+def test_forward_full_size_is_bit_reproducible(B, name):
+    """Two runs of the full-size pass on the same inputs give the same bits in every output: the K-split parts of a row block are
+    added in exchange-slot order and every reduction of the segment kernel is fixed-order (no floating-point atomics anywhere)."""
+    w = synth.make(name)
+    plan = _plan(B, w)
+    X, Q = B.to_device(w.X), B.to_device(w.Q)
+    a = plan.forward(X, Q)
+    b = plan.forward(X, Q)
+    torch.cuda.synchronize()
+    for k in ("m_spatial", "gamma", "rel", "mas_tok", "keep_mask", "kept_off"):
+        assert torch.equal(a[k], b[k]), k
+    total = min(int(a["kept_off"][-1].item()), int(a["cap_rows"]))          # rows past the kept count are never written
+    assert torch.equal(a["kept_idx"][:total], b["kept_idx"][:total]) and torch.equal(a["Y"][:total], b["Y"][:total])
+    plan.close()
+
+
 # ---------------------------------------------------------------- segment sizes around every internal boundary
 def _random_workload(seed, seg_shapes, d, L_list, select_mode=0, cut=0.5, keep_ratio=0.3):
     """seg_shapes: list of (request, modality, T, P); plain random rows (no planted structure needed here)."""
