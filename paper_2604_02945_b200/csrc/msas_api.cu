@@ -688,6 +688,16 @@ extern "C" int mas_learned_heads(const mas_plan* p, const void* X, const void* Q
   int rc = heads_check(p, X, Q, gamma, false, hd);
   if (rc != MAS_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
+  if (p->tc.enabled && p->max_L <= 64) {
+    // bf16, d % 64 == 0, every L <= 64: the weight rows ride the tcgen05 score kernel's MMA as 64 more B rows, exactly as in
+    // mas_forward_heads; its own three outputs go to plan scratch (not to the gamma workspace: the caller's `gamma` may be that)
+    TcHeads hf{p->at<float>(p->lay.heads_part), m_spatial, hd->b_spatial, p->prm.tau_s};
+    if ((rc = heads_q(p, Q, hd, st)) != MAS_OK) return rc;
+    if ((rc = launch_score_tc(p, true, X, Q, p->at<float>(p->lay.s), p->at<float>(p->lay.mas), p->at<float>(p->lay.rel), hd->W, nullptr, &hf, st,
+                              false)) != MAS_OK)
+      return rc;
+    return heads_finish(p, gamma, hd, true, seg_out, st);
+  }
   ScoreArgs a = score_args(p, X, hd->W, nullptr, nullptr, nullptr, nullptr);
   a.heads_part = p->at<float>(p->lay.heads_part); a.heads_m = m_spatial; a.heads_bias = hd->b_spatial; a.heads_tau = p->prm.tau_s;
   if (p->dtype == MAS_BF16) k_heads_proj<1><<<p->n_tiles, 256, score_mma_smem_bytes(1), st>>>(a);
