@@ -150,6 +150,166 @@ __global__ void __launch_bounds__(256) k_merge_finish(const float* __restrict__ 
   }
 }
 
+// (b') the same through the TMA unit, for rows of at most 16 KB.  LSU loads stream the dropped rows at about 4 TB/s; bulk copies
+// into shared memory reach the HBM rate.  Persistent CTAs, one per SM: CTA c owns the global rows [c R, (c + 1) R) -- frames tile
+// the rows in order, so it sees a run of frames, the first and the last possibly shared with its neighbours.  One producer warp
+// reads the mask bytes of 32 rows at a time and issues one bulk copy (cp.async.bulk, mbarrier complete_tx) per DROPPED row into a
+// ring of row slots; eight consumer warps each own an eighth of the row's 16-byte vectors and add them to fp32 accumulators in
+// ascending row order (they read the same mask bytes, so they know which rows arrive).  A frame that lies inside one CTA's rows
+// is written as its mean at once; a piece of a frame shared with a neighbour goes to slot 2c (the frame began before this
+// CTA's rows) or 2c + 1 (it continues beyond them) of the scratch, and k_merge_tma_finish adds a frame's pieces in CTA order.
+constexpr int kMergeTmaWarps = 8;                // consumer warps
+constexpr int kMergeTmaVPL = 4;                  // 16-byte vectors per lane at most: rows of <= 8 * 32 * 4 * 16 B = 16 KB
+constexpr int kMergeTmaSmem = 200 * 1024;        // ring bytes at most
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void add_f32x2(uint64_t& acc, uint64_t a) { asm("add.rn.f32x2 %0, %0, %1;" : "+l"(acc) : "l"(a)); }
+template <int DT, int VPL>   // VPL: 16-byte vectors of a row per lane (1, 2 or 4)
+__global__ void __launch_bounds__(32 * (kMergeTmaWarps + 1), 1)
+k_merge_tma(const DevFrame* __restrict__ frames, int n_frames, const char* __restrict__ X, const uint8_t* __restrict__ keep_mask,
+            float* __restrict__ Ymerge, int32_t* __restrict__ n_dropped, float* __restrict__ part, int32_t* __restrict__ cnt_part, int d,
+            long long N, long long R, int n_slots) {
+  constexpr int VE = DT == 1 ? 8 : 4;
+  constexpr int NW = kMergeTmaWarps;
+  extern __shared__ unsigned char merge_smem_raw[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(merge_smem_raw) + 127) & ~(uintptr_t)127);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);          // [n_slots] producer -> consumers (1 arrival + row bytes)
+  uint64_t* empty = full + 32;                                  // [n_slots] consumers -> producer (NW arrivals)
+  const uint32_t ring = smem_u32(smem) + 512u;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t row_bytes = (uint32_t)d * (DT == 1 ? 2u : 4u);
+  const int n16 = (int)(row_bytes >> 4);                        // 16-byte vectors per row
+  const int vpw = (n16 + NW - 1) / NW;                          // vectors per consumer warp
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < n_slots; ++i) { mbar_init(smem_u32(&full[i]), 1); mbar_init(smem_u32(&empty[i]), NW); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const long long lo = (long long)blockIdx.x * R, hi = lo + R < N ? lo + R : N;
+  if (lo >= hi) return;
+  int f = 0;                                                    // the frame that holds row `lo`
+  { int a = 0, b = n_frames - 1; while (a < b) { const int m = (a + b + 1) >> 1; if (frames[m].row0 <= lo) a = m; else b = m - 1; } f = a; }
+  uint32_t slot = 0, ph = 0;
+  if (warp == NW) {
+    // ---- producer
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    for (long long r0 = lo; r0 < hi; r0 += 32) {
+      const long long r = r0 + lane;
+      unsigned m = __ballot_sync(0xffffffffu, r < hi && keep_mask[r] == 0);
+      while (m) {
+        const int b = __ffs(m) - 1; m &= m - 1;
+        mbar_wait(smem_u32(&empty[slot]), ph ^ 1u);
+        if (lane == 0) {
+          const uint32_t bar = smem_u32(&full[slot]);
+          mbar_expect_tx(bar, row_bytes);
+          bulk_load(ring + slot * row_bytes, X + (r0 + b) * (long long)row_bytes, row_bytes, bar, pol);
+        }
+        __syncwarp();
+        if (++slot == (uint32_t)n_slots) { slot = 0; ph ^= 1u; }
+      }
+    }
+    return;
+  }
+  // ---- consumers: warp w owns vectors [w vpw, (w + 1) vpw) of a row, lane l the vectors w vpw + l + 32 j
+  // bf16: packed fp32 pairs (one FADD2 per two columns); fp32: plain adds
+  uint64_t acc2[VPL][4];
+  float acc[VPL][4];
+  long long r = lo;
+  while (r < hi) {
+    const DevFrame fr = frames[f];
+    const long long f_lo = fr.row0, f_hi = fr.row0 + fr.n_patches;
+    const long long p_hi = f_hi < hi ? f_hi : hi;               // this CTA's piece of frame f: rows [r, p_hi)
+#pragma unroll
+    for (int j = 0; j < VPL; ++j)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { acc[j][e] = 0.f; acc2[j][e] = 0ull; }
+    int cnt = 0;
+    // the mask groups of the producer start at lo + 32 k: walk the piece group by group, masking off rows outside it
+    for (long long g0 = lo + ((r - lo) & ~31ll); g0 < p_hi; g0 += 32) {
+      const long long rr = g0 + lane;
+      unsigned m = __ballot_sync(0xffffffffu, rr >= r && rr < p_hi && keep_mask[rr] == 0);
+      cnt += __popc(m);
+      for (int k = __popc(m); k > 0; --k) {
+        mbar_wait(smem_u32(&full[slot]), ph);
+        const uint32_t base = ring + slot * row_bytes;
+        uint4 u[VPL];
+        uint32_t seen = 0;
+#pragma unroll
+        for (int j = 0; j < VPL; ++j) {
+          const int v = warp * vpw + lane + 32 * j;
+          u[j] = (lane + 32 * j < vpw && v < n16) ? lds128(base + (uint32_t)v * 16u) : make_uint4(0, 0, 0, 0);
+          seen |= u[j].x ^ u[j].w;
+        }
+        // the slot is released as soon as this warp's share of it is in registers (the empty asm consumes the loaded values, so
+        // the arrive cannot be issued ahead of them)
+        asm volatile("" ::"r"(seen) : "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&empty[slot]));
+#pragma unroll
+        for (int j = 0; j < VPL; ++j) {
+          if (DT == 1) {
+            add_f32x2(acc2[j][0], bf16x2_to_f32x2(u[j].x)); add_f32x2(acc2[j][1], bf16x2_to_f32x2(u[j].y));
+            add_f32x2(acc2[j][2], bf16x2_to_f32x2(u[j].z)); add_f32x2(acc2[j][3], bf16x2_to_f32x2(u[j].w));
+          } else {
+            acc[j][0] += __uint_as_float(u[j].x); acc[j][1] += __uint_as_float(u[j].y); acc[j][2] += __uint_as_float(u[j].z); acc[j][3] += __uint_as_float(u[j].w);
+          }
+        }
+        if (++slot == (uint32_t)n_slots) { slot = 0; ph ^= 1u; }
+      }
+    }
+    const bool whole = f_lo >= lo && f_hi <= hi;                // the frame lies inside this CTA's rows: write its mean
+    const float scale = whole ? (cnt > 0 ? 1.0f / (float)cnt : 0.f) : 1.0f;
+    const int pslot = 2 * (int)blockIdx.x + (f_lo < lo ? 0 : 1);
+    float* dst = whole ? Ymerge + (long long)f * d : part + (long long)pslot * d;
+    if (warp == 0 && lane == 0) { if (whole) n_dropped[f] = cnt; else cnt_part[pslot] = cnt; }
+#pragma unroll
+    for (int j = 0; j < VPL; ++j) {
+      const int v = warp * vpw + lane + 32 * j;
+      if (lane + 32 * j < vpw && v < n16) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          if (DT == 1) {
+            float lo2, hi2;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(lo2), "=f"(hi2) : "l"(acc2[j][e]));
+            dst[v * VE + 2 * e] = lo2 * scale; dst[v * VE + 2 * e + 1] = hi2 * scale;
+          } else {
+            dst[v * VE + e] = acc[j][e] * scale;
+          }
+        }
+      }
+    }
+    r = p_hi;
+    ++f;
+  }
+}
+// frames shared by several CTAs of k_merge_tma: their pieces added in CTA order; one CTA per frame (most return at once)
+__global__ void __launch_bounds__(256) k_merge_tma_finish(const DevFrame* __restrict__ frames, const float* __restrict__ part,
+                                                          const int32_t* __restrict__ cnt_part, float* __restrict__ Ymerge,
+                                                          int32_t* __restrict__ n_dropped, int d, long long R) {
+  const int f = blockIdx.x;
+  const DevFrame fr = frames[f];
+  const long long c0 = fr.row0 / R, c1 = (fr.row0 + fr.n_patches - 1) / R;
+  if (c0 == c1) return;
+  int total = 0;
+  for (long long c = c0; c <= c1; ++c) total += cnt_part[2 * c + (fr.row0 < c * R ? 0 : 1)];
+  if (threadIdx.x == 0) n_dropped[f] = total;
+  const float inv = total > 0 ? 1.0f / (float)total : 0.f;
+  // d % 4 == 0 (16-byte rows); the scratch slots are d floats apart and 16-byte aligned
+  for (int i = threadIdx.x * 4; i < d; i += 1024) {
+    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (long long c = c0; c <= c1; ++c) {
+      const float4 v = *reinterpret_cast<const float4*>(part + (2 * c + (fr.row0 < c * R ? 0 : 1)) * (long long)d + i);
+      t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
+    }
+    float* y = Ymerge + (long long)f * d + i;
+    y[0] = t.x * inv; y[1] = t.y * inv; y[2] = t.z * inv; y[3] = t.w * inv;
+  }
+}
+
 // (c) gather with residual coding: kept row j of a temporal segment's frame t >= 1 is written as x_t - x_{t-1}; one warp per row.
 template <int DT>
 __global__ void __launch_bounds__(256) k_gather_residual(const DevSeg* __restrict__ segs, int n_segs, const char* __restrict__ X,

@@ -139,7 +139,7 @@ static int validate(const mas_segment* segs, int32_t n_segs, const int64_t* q_of
 }
 
 static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, int32_t n_tiles, size_t tc_bytes, size_t tc_parts_max,
-                          int64_t n_frames) {
+                          int64_t n_frames, int d) {
   Layout l{};
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
@@ -167,7 +167,7 @@ static Layout make_layout(int32_t n_segs, int32_t n_req, int64_t N, int64_t nQ, 
   l.tc_xflag = take(sizeof(unsigned int) * kTcMaxCtas);   // K-split: one flag and one exchange slot per CTA of the score kernel
   l.tc_xchg = take(tc_xchg_bytes());
   l.heads_part = take(sizeof(float) * kHeadRows * std::max((size_t)n_tiles, tc_parts_max));   // NEXT-2 scratch: per-tile / per-block column sums
-  l.merge_part = take(sizeof(float) * 1024 * (size_t)kMergeCtas);   // NEXT-3 scratch: row-split partial sums of the merged tokens
+  l.merge_part = take(sizeof(float) * std::max<size_t>(1024 * (size_t)kMergeCtas, 2 * (size_t)kTcMaxCtas * (size_t)d));   // NEXT-3 scratch: partial sums of the merged tokens
   l.merge_cnt = take(sizeof(int32_t) * (size_t)kMergeCtas);
   l.gridw = take(sizeof(int32_t) * n_segs);   // NEXT-3 scratch: the caller's grid widths
   l.heads_cq = take(sizeof(float) * kHeadRows * kHeadSlabs * (size_t)n_req);
@@ -187,7 +187,7 @@ extern "C" int mas_plan_workspace_bytes(const mas_segment* h_segs, int32_t n_seg
   int64_t N, nQ; int32_t nt, maxL;
   int st = validate(h_segs, n_segs, h_q_off, n_requests, d, dtype, nullptr, &N, &nQ, &nt, &maxL);
   if (st != MAS_OK) return st;
-  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs), tc_max_parts(h_segs, n_segs), count_frames(h_segs, n_segs)).total;
+  *out_bytes = make_layout(n_segs, n_requests, N, nQ, nt, tc_schedule_bytes(h_segs, n_segs), tc_max_parts(h_segs, n_segs), count_frames(h_segs, n_segs), d).total;
   return MAS_OK;
 }
 
@@ -204,6 +204,12 @@ static cudaError_t set_kernel_attrs(int dev) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_heads_proj<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(0));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_heads_proj<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_mma_smem_bytes(1));
   if (e == cudaSuccess) e = tc_set_kernel_attrs();
+  {
+    typedef void (*merge_fn)(const DevFrame*, int, const char*, const uint8_t*, float*, int32_t*, float*, int32_t*, int, long long, long long, int);
+    const merge_fn mk[6] = {k_merge_tma<0, 1>, k_merge_tma<0, 2>, k_merge_tma<0, 4>, k_merge_tma<1, 1>, k_merge_tma<1, 2>, k_merge_tma<1, 4>};
+    for (merge_fn k : mk)
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kMergeTmaSmem + 1024);
+  }
   if (e == cudaSuccess && dev >= 0 && dev < 64) g_attr_done[dev] = true;
   return e;
 }
@@ -219,7 +225,7 @@ extern "C" int mas_plan_create(mas_plan** out, const mas_segment* h_segs, int32_
   if (st != MAS_OK) return st;
   if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0) return MAS_ERR_UNSUPPORTED;
   const size_t tc_bytes = tc_schedule_bytes(h_segs, n_segs);
-  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes, tc_max_parts(h_segs, n_segs), count_frames(h_segs, n_segs));
+  Layout lay = make_layout(n_segs, n_requests, N, nQ, nt, tc_bytes, tc_max_parts(h_segs, n_segs), count_frames(h_segs, n_segs), d);
   if (workspace_bytes < lay.total) return MAS_ERR_WORKSPACE;
 
   mas_plan* p = new (std::nothrow) mas_plan();
@@ -606,6 +612,30 @@ extern "C" int mas_merge_dropped(const mas_plan* p, const void* X, const uint8_t
   if (!p || !X || !keep_mask || !Ymerge || !n_dropped) return MAS_ERR_INVALID_ARG;
   if (!aligned16(X)) return MAS_ERR_UNSUPPORTED;
   cudaStream_t st = (cudaStream_t)stream;
+  {   // rows of at most 16 KB: through the TMA unit (k_merge_tma), persistent CTAs over equal runs of rows
+    const size_t row_bytes = (size_t)p->d * (p->dtype == MAS_BF16 ? 2 : 4);
+    const int n_slots = (int)std::min<size_t>(32, kMergeTmaSmem / row_bytes);
+    if (row_bytes % 16 == 0 && row_bytes / 16 <= (size_t)kMergeTmaWarps * 32 * kMergeTmaVPL && n_slots >= 4 && p->n_frames < 2147483647ll) {
+      const int n_max = std::min(p->sm_count, kTcMaxCtas);
+      const long long R = std::max<long long>(64, (p->N + n_max - 1) / n_max);
+      const unsigned grid = (unsigned)((p->N + R - 1) / R);
+      const size_t smem = 128 + 512 + (size_t)n_slots * row_bytes;
+      float* part = p->at<float>(p->lay.merge_part);
+      int32_t* cnt = p->at<int32_t>(p->lay.merge_cnt);
+      const DevFrame* fr = p->at<DevFrame>(p->lay.frames);
+      const int vpw = (int)((row_bytes / 16 + kMergeTmaWarps - 1) / kMergeTmaWarps), vpl = vpw <= 32 ? 1 : vpw <= 64 ? 2 : 4;
+      const dim3 blk(32 * (kMergeTmaWarps + 1));
+#define MSAS_MERGE_TMA(DT, VPL) \
+  k_merge_tma<DT, VPL><<<grid, blk, smem, st>>>(fr, (int)p->n_frames, static_cast<const char*>(X), keep_mask, Ymerge, n_dropped, part, cnt, p->d, (long long)p->N, R, n_slots)
+      if (p->dtype == MAS_BF16) { if (vpl == 1) MSAS_MERGE_TMA(1, 1); else if (vpl == 2) MSAS_MERGE_TMA(1, 2); else MSAS_MERGE_TMA(1, 4); }
+      else { if (vpl == 1) MSAS_MERGE_TMA(0, 1); else if (vpl == 2) MSAS_MERGE_TMA(0, 2); else MSAS_MERGE_TMA(0, 4); }
+#undef MSAS_MERGE_TMA
+      CK(cudaGetLastError());
+      k_merge_tma_finish<<<(unsigned)p->n_frames, 256, 0, st>>>(fr, part, cnt, Ymerge, n_dropped, p->d, R);
+      CK(cudaGetLastError());
+      return MAS_OK;
+    }
+  }
   const int slab = 32 * kMergeVPL * (p->dtype == MAS_BF16 ? 8 : 4);
   const int64_t slabs = (p->d + slab - 1) / slab;
   if (slabs > 65535) return MAS_ERR_UNSUPPORTED;

@@ -757,8 +757,10 @@ def test_spatial_pool(B, w, k):
 
 
 @pytest.mark.parametrize("w", [synth.batched_images(seed=74, R=5, d=512, L_lo=3, L_hi=9, P=333), synth.video(seed=75, R=2, T=4, P=300, d=2304, L=8),
-                               synth.video(seed=76, R=1, T=3, P=70, d=200, L=4, dtype="f32"), synth.audio_vision(seed=77, R=2, d=256, L=5, P_img=130, T_aud=260)],
-                         ids=["images", "video_d2304", "video_f32_d200", "audio_vision"])
+                               synth.video(seed=76, R=1, T=3, P=70, d=200, L=4, dtype="f32"), synth.audio_vision(seed=77, R=2, d=256, L=5, P_img=130, T_aud=260),
+                               synth.video(seed=78, R=1, T=3, P=70, d=6144, L=4),      # 12 KB rows: four vectors per lane in the bulk-copy merge
+                               synth.video(seed=79, R=1, T=2, P=40, d=9216, L=4)],     # 18 KB rows: beyond the bulk-copy merge, the LSU kernel
+                         ids=["images", "video_d2304", "video_f32_d200", "audio_vision", "video_d6144", "video_d9216"])
 def test_merge_dropped_and_residual_gather(B, w):
     segs, n = O.make_segments(w.segments)
     plan = _plan(B, w)
